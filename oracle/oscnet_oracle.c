@@ -1,0 +1,403 @@
+/*
+ * oscnet_oracle.c  --  TEST INFRASTRUCTURE, NOT PRODUCT CODE.
+ *
+ * Plain, slow, double-precision CPU restatement of the hot path of
+ * arXiv:2410.19075 (Sudakov & Maistrenko): fixed-step classical RK4 of N
+ * coupled oscillators whose right-hand side is "local vector field + sum over
+ * the in-neighbours the topology allows".  Only tests/, __graft_entry__.smoke()
+ * and bench.py's cpu_baseline / --impl reference legs may load this file.  It
+ * shares no code, header, table or constant generator with the CUDA library
+ * under paper_2410_19075_b200/csrc/.
+ *
+ * Decomposition = the paper's: parallel over elements, each element's neighbour
+ * sum serial, in ascending neighbour index ("The right-hand part
+ * of the differential equation for each individual oscillator is computed
+ * serially as described by Algorithm 1"; Alg. 1).
+ * No algebraic rewrites (no factorised sine, no prefix sums, no tiling).
+ *
+ * Readings of the paper that this file takes are the DESIGN.md "Readings"
+ * table (R1..R14); each function names the ones it uses.
+ *
+ * Pins (tests/test_oracle_*.py, all -m "not gpu"):
+ *   ora_topology_ring / _lattice : ball sizes 33 (P=2) and 925 (P=6) printed in
+ *       PAPER.md:337-339 (tests/golden/lattice_link_counts.txt), symmetry,
+ *       dense-matrix brute force, index map k*N1^2+j*N1+i.
+ *   ora_topology_random_indegree : exactly k distinct sources != i, sorted;
+ *       re-derived in pure Python integers on tiny cases.
+ *   ora_rhs (KS)  : K=0 closed form, in-phase invariance, sum conservation for
+ *       alpha=0, mean-field identity on all-to-all rings, dense brute force.
+ *   ora_rhs (FHN) : closed-form fixed point (-a, -a+a^3/3), vanishing coupling
+ *       on uniform states, zero-sum coupling, dense brute force.
+ *   ora_rhs (HH)  : hand-computed rate values at V=-65 mV, rest state near the
+ *       textbook -65 mV / m=0.0529 h=0.5961 n=0.3177, dense brute force.
+ *   ora_rk4       : 4th-order convergence against a 16x finer step; exactness
+ *       for constant RHS.
+ *   ora_local_order, phase maps : R=1 for identical phases, splay state R=0.
+ *   Long-run order-parameter statistics: PARITY UNPINNED in absolute terms
+ *       (the paper prints no value); they are only compared GPU-vs-oracle.
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+
+#define ORA_MODEL_KS 0
+#define ORA_MODEL_FHN 1
+#define ORA_MODEL_HH 2
+
+/* ------------------------------------------------------------------ */
+/* Topology: canonical CSR, rows = in-neighbour lists (PAPER.md:147:    */
+/* L_ij = 1 iff j influences i), sorted ascending, int64 row_ptr,       */
+/* int32 col_idx.  Row ranges [row_begin, row_begin+row_count) so that  */
+/* huge lattices can be sampled; row_ptr is relative to the range.      */
+/* ------------------------------------------------------------------ */
+
+static int cmp_i32(const void* a, const void* b) {
+    int32_t x = *(const int32_t*)a, y = *(const int32_t*)b;
+    return (x > y) - (x < y);
+}
+
+/* 1D ring: "each oscillator is coupled with its P neighbors on both sides" on
+ * a circle.  j = (i + d) mod n, d in [-P, P], d != 0 unless
+ * include_self (reading R4). */
+int ora_topology_ring(int64_t n, int32_t P, int32_t include_self, int64_t row_begin,
+                      int64_t row_count, int64_t* row_ptr, int32_t* col_idx) {
+    if (n < 1 || P < 0 || 2 * (int64_t)P >= n) return -1;
+    int64_t pos = 0;
+    for (int64_t r = 0; r < row_count; ++r) {
+        int64_t i = row_begin + r;
+        row_ptr[r] = pos;
+        int64_t start = pos;
+        for (int64_t d = -P; d <= P; ++d) {
+            if (d == 0 && !include_self) continue;
+            int64_t j = (i + d) % n;
+            if (j < 0) j += n;
+            col_idx[pos++] = (int32_t)j;
+        }
+        qsort(col_idx + start, (size_t)(pos - start), sizeof(int32_t), cmp_i32);
+    }
+    row_ptr[row_count] = pos;
+    return 0;
+}
+
+/* Number of lattice points d with |d|^2 <= P^2 (minus the centre unless
+ * include_self).  PAPER.md:309 (2D disc), :313 (3D ball). */
+int64_t ora_lattice_degree(int32_t ndim, int32_t P, int32_t include_self) {
+    int64_t c = 0;
+    int32_t Pz = ndim >= 3 ? P : 0, Py = ndim >= 2 ? P : 0;
+    for (int32_t dz = -Pz; dz <= Pz; ++dz)
+        for (int32_t dy = -Py; dy <= Py; ++dy)
+            for (int32_t dx = -P; dx <= P; ++dx)
+                if (dx * dx + dy * dy + dz * dz <= P * P) ++c;
+    return include_self ? c : c - 1;
+}
+
+/* d-dimensional periodic lattice.  Site (i,j,k) <-> index k*nx*ny + j*nx + i
+ * (PAPER.md:309 "jN1+i", :311 "kN1^2+jN1+i"); neighbours = all sites with
+ * (i-i')^2+(j-j')^2+(k-k')^2 <= P^2, coordinates taken modulo
+ * the extent ("torus"). */
+int ora_topology_lattice(int32_t ndim, const int64_t* extent, int32_t P, int32_t include_self,
+                         int64_t row_begin, int64_t row_count, int64_t* row_ptr,
+                         int32_t* col_idx) {
+    if (ndim < 1 || ndim > 3 || P < 0) return -1;
+    int64_t nx = extent[0], ny = ndim >= 2 ? extent[1] : 1, nz = ndim >= 3 ? extent[2] : 1;
+    if (2 * (int64_t)P >= nx) return -1;
+    if (ndim >= 2 && 2 * (int64_t)P >= ny) return -1;
+    if (ndim >= 3 && 2 * (int64_t)P >= nz) return -1;
+    int32_t Pz = ndim >= 3 ? P : 0, Py = ndim >= 2 ? P : 0;
+    int64_t pos = 0;
+    for (int64_t r = 0; r < row_count; ++r) {
+        int64_t idx = row_begin + r;
+        int64_t i = idx % nx, j = (idx / nx) % ny, k = idx / (nx * ny);
+        row_ptr[r] = pos;
+        int64_t start = pos;
+        for (int32_t dz = -Pz; dz <= Pz; ++dz)
+            for (int32_t dy = -Py; dy <= Py; ++dy)
+                for (int32_t dx = -P; dx <= P; ++dx) {
+                    if (dx * dx + dy * dy + dz * dz > P * P) continue;
+                    if (dx == 0 && dy == 0 && dz == 0 && !include_self) continue;
+                    int64_t ii = ((i + dx) % nx + nx) % nx;
+                    int64_t jj = ((j + dy) % ny + ny) % ny;
+                    int64_t kk = ((k + dz) % nz + nz) % nz;
+                    col_idx[pos++] = (int32_t)(kk * nx * ny + jj * nx + ii);
+                }
+        qsort(col_idx + start, (size_t)(pos - start), sizeof(int32_t), cmp_i32);
+    }
+    row_ptr[row_count] = pos;
+    return 0;
+}
+
+/* Reading R8: seeded random graph with fixed in-degree k, uniform sources, no
+ * self-loops, no multi-edges.  Integer-only and counter-based so that any
+ * other implementation of the same rule is bit-exact:
+ *   mix(z): z ^= z>>30; z *= 0xBF58476D1CE4E5B9; z ^= z>>27;
+ *           z *= 0x94D049BB133111EB; z ^= z>>31        (splitmix64 finaliser)
+ *   h(seed,i,t) = mix( mix(seed + G*(i+1)) + G*(t+1) ),  G = 0x9E3779B97F4A7C15
+ *   candidate  j = floor(h * (n-1) / 2^64);  if j >= i then j += 1
+ * for t = 0,1,2,...; a candidate already in the row is skipped; the row is the
+ * first k distinct candidates, sorted ascending. */
+uint64_t ora_mix64(uint64_t z) {
+    z ^= z >> 30;
+    z *= 0xBF58476D1CE4E5B9ULL;
+    z ^= z >> 27;
+    z *= 0x94D049BB133111EBULL;
+    z ^= z >> 31;
+    return z;
+}
+
+int ora_topology_random_indegree(int64_t n, int32_t k, uint64_t seed, int64_t row_begin,
+                                 int64_t row_count, int64_t* row_ptr, int32_t* col_idx) {
+    if (n < 2 || k < 0 || (int64_t)k > n - 1) return -1;
+    const uint64_t G = 0x9E3779B97F4A7C15ULL;
+    for (int64_t r = 0; r < row_count; ++r) {
+        int64_t i = row_begin + r;
+        int32_t* row = col_idx + r * (int64_t)k;
+        row_ptr[r] = r * (int64_t)k;
+        uint64_t hi = ora_mix64(seed + G * (uint64_t)(i + 1));
+        int32_t have = 0;
+        for (uint64_t t = 0; have < k; ++t) {
+            uint64_t h = ora_mix64(hi + G * (t + 1));
+            uint64_t j = (uint64_t)(((unsigned __int128)h * (unsigned __int128)(uint64_t)(n - 1)) >> 64);
+            if (j >= (uint64_t)i) j += 1;
+            int dup = 0;
+            for (int32_t q = 0; q < have; ++q)
+                if (row[q] == (int32_t)j) { dup = 1; break; }
+            if (!dup) row[have++] = (int32_t)j;
+        }
+        qsort(row, (size_t)k, sizeof(int32_t), cmp_i32);
+    }
+    row_ptr[row_count] = row_count * (int64_t)k;
+    return 0;
+}
+
+/* ------------------------------------------------------------------ */
+/* Network description handed to the RHS / integrator.                  */
+/* State is SoA: y[var*n + i].                                           */
+/*   KS : var 0 = phi                          elem_param = omega[n]     */
+/*   FHN: var 0 = u, 1 = v                     elem_param unused         */
+/*   HH : var 0 = V, 1 = m, 2 = h, 3 = n       elem_param = I_ext[n]     */
+/* p[] per model:                                                        */
+/*   KS : K, alpha                                                       */
+/*   FHN: eps, a, sigma, b_uu, b_uv, b_vu, b_vv                          */
+/*   HH : gNa, gK, gL, ENa, EK, EL, C, g_syn, E_syn, theta_syn, k_syn    */
+/* ------------------------------------------------------------------ */
+typedef struct {
+    int32_t model;
+    int32_t pad_;
+    int64_t n;
+    const int64_t* row_ptr; /* n+1 */
+    const int32_t* col_idx;
+    const double* elem_param;
+    double p[16];
+} ora_net;
+
+int32_t ora_nvar(int32_t model) {
+    return model == ORA_MODEL_KS ? 1 : model == ORA_MODEL_FHN ? 2 : model == ORA_MODEL_HH ? 4 : -1;
+}
+
+/* Kuramoto-Sakaguchi (eq. (3) with m=0, eps=1, mu=1/Omega, PAPER.md:79, :107;
+ * Alg. 1) with natural frequency and strength K as the
+ * north-star configs state them:
+ *   f_i = omega_i + (K/Omega_i) * sum_{j in row i} sin(phi_j - phi_i - alpha)
+ * Omega_i = number of links actually iterated; the division happens once,
+ * after the loop (reading R2 of the garbled listing). */
+static void rhs_ks(const ora_net* net, const double* y, double* f) {
+    const int64_t n = net->n;
+    const double K = net->p[0], alpha = net->p[1];
+    const double* phi = y;
+#pragma omp parallel for schedule(static)
+    for (int64_t i = 0; i < n; ++i) {
+        double der = 0.0;
+        int64_t links_amount = 0;
+        for (int64_t e = net->row_ptr[i]; e < net->row_ptr[i + 1]; ++e, ++links_amount) {
+            int32_t j = net->col_idx[e];
+            der += sin(phi[j] - phi[i] - alpha);
+        }
+        if (links_amount > 0) der /= (double)links_amount;
+        f[i] = net->elem_param[i] + K * der;
+    }
+}
+
+/* FitzHugh-Nagumo, eq. (2) PAPER.md:70-75 in the north-star variant (reading
+ * R3): rotated 2x2 diffusive coupling on (u,v), no delay, no noise, no I_app.
+ *   Cu_i = sum_j (u_j - u_i),  Cv_i = sum_j (v_j - v_i)   over row i
+ *   eps du_i/dt = u_i - u_i^3/3 - v_i + (sigma/Omega_i)(b_uu Cu_i + b_uv Cv_i)
+ *       dv_i/dt = u_i + a            + (sigma/Omega_i)(b_vu Cu_i + b_vv Cv_i) */
+static void rhs_fhn(const ora_net* net, const double* y, double* f) {
+    const int64_t n = net->n;
+    const double eps = net->p[0], a = net->p[1], sigma = net->p[2];
+    const double buu = net->p[3], buv = net->p[4], bvu = net->p[5], bvv = net->p[6];
+    const double* u = y;
+    const double* v = y + n;
+#pragma omp parallel for schedule(static)
+    for (int64_t i = 0; i < n; ++i) {
+        double Cu = 0.0, Cv = 0.0;
+        int64_t links_amount = 0;
+        for (int64_t e = net->row_ptr[i]; e < net->row_ptr[i + 1]; ++e, ++links_amount) {
+            int32_t j = net->col_idx[e];
+            Cu += u[j] - u[i];
+            Cv += v[j] - v[i];
+        }
+        double s = links_amount > 0 ? sigma / (double)links_amount : 0.0;
+        f[i] = (u[i] - u[i] * u[i] * u[i] / 3.0 - v[i] + s * (buu * Cu + buv * Cv)) / eps;
+        f[n + i] = u[i] + a + s * (bvu * Cu + bvv * Cv);
+    }
+}
+
+/* x / (1 - exp(-x/10)) with its removable singularity at x = 0 (reading R10):
+ * -x/expm1(-x/10), and the limit 10 when |x/10| < 1e-9. */
+static double hh_vtrap(double x) {
+    if (fabs(x / 10.0) < 1e-9) return 10.0;
+    return -x / expm1(-x / 10.0);
+}
+
+/* Standard squid-axon rate functions, rest near -65 mV (reading R7; mV, ms). */
+static void hh_rates(double V, double* am, double* bm, double* ah, double* bh, double* an,
+                     double* bn) {
+    *am = 0.1 * hh_vtrap(V + 40.0);
+    *bm = 4.0 * exp(-(V + 65.0) / 18.0);
+    *ah = 0.07 * exp(-(V + 65.0) / 20.0);
+    *bh = 1.0 / (1.0 + exp(-(V + 35.0) / 10.0));
+    *an = 0.01 * hh_vtrap(V + 55.0);
+    *bn = 0.125 * exp(-(V + 65.0) / 80.0);
+}
+
+/* Hodgkin-Huxley type element, eq. (1), in the north-star
+ * variant (reading R7): instantaneous sigmoidal synapse S(V_pre),
+ *   C dV_i/dt = I_ext,i - gNa m^3 h (V-ENa) - gK n^4 (V-EK) - gL (V-EL)
+ *               + (g_syn/Omega_i) (E_syn - V_i) sum_{j in row i} S(V_j)
+ *   dx/dt = alpha_x(V)(1-x) - beta_x(V) x,  x in {m,h,n}
+ *   S(V) = 1/(1+exp(-(V-theta_syn)/k_syn)). */
+static void rhs_hh(const ora_net* net, const double* y, double* f) {
+    const int64_t n = net->n;
+    const double gNa = net->p[0], gK = net->p[1], gL = net->p[2];
+    const double ENa = net->p[3], EK = net->p[4], EL = net->p[5], C = net->p[6];
+    const double gsyn = net->p[7], Esyn = net->p[8], th = net->p[9], ks = net->p[10];
+    const double *V = y, *m = y + n, *h = y + 2 * n, *g = y + 3 * n;
+#pragma omp parallel for schedule(static)
+    for (int64_t i = 0; i < n; ++i) {
+        double ssum = 0.0;
+        int64_t links_amount = 0;
+        for (int64_t e = net->row_ptr[i]; e < net->row_ptr[i + 1]; ++e, ++links_amount) {
+            int32_t j = net->col_idx[e];
+            ssum += 1.0 / (1.0 + exp(-(V[j] - th) / ks));
+        }
+        double Isyn = links_amount > 0 ? (gsyn / (double)links_amount) * (Esyn - V[i]) * ssum : 0.0;
+        double am, bm, ah, bh, an, bn;
+        hh_rates(V[i], &am, &bm, &ah, &bh, &an, &bn);
+        double INa = gNa * m[i] * m[i] * m[i] * h[i] * (V[i] - ENa);
+        double IK = gK * g[i] * g[i] * g[i] * g[i] * (V[i] - EK);
+        double IL = gL * (V[i] - EL);
+        f[i] = (net->elem_param[i] - INa - IK - IL + Isyn) / C;
+        f[n + i] = am * (1.0 - m[i]) - bm * m[i];
+        f[2 * n + i] = ah * (1.0 - h[i]) - bh * h[i];
+        f[3 * n + i] = an * (1.0 - g[i]) - bn * g[i];
+    }
+}
+
+/* One full right-hand-side evaluation f(y); y and f are nvar*n SoA. */
+int ora_rhs(const ora_net* net, const double* y, double* f) {
+    switch (net->model) {
+        case ORA_MODEL_KS: rhs_ks(net, y, f); return 0;
+        case ORA_MODEL_FHN: rhs_fhn(net, y, f); return 0;
+        case ORA_MODEL_HH: rhs_hh(net, y, f); return 0;
+    }
+    return -1;
+}
+
+/* Gate steady states x_inf(V) = alpha_x/(alpha_x+beta_x) (used to prepare the
+ * north-star HH initial condition "gates at steady state"). */
+void ora_hh_steady_gates(int64_t n, const double* V, double* m, double* h, double* g) {
+    for (int64_t i = 0; i < n; ++i) {
+        double am, bm, ah, bh, an, bn;
+        hh_rates(V[i], &am, &bm, &ah, &bh, &an, &bn);
+        m[i] = am / (am + bm);
+        h[i] = ah / (ah + bh);
+        g[i] = an / (an + bn);
+    }
+}
+
+/* Classical 4-stage Runge-Kutta, fixed step (reading R1; the north star
+ * prescribes it, the paper's own solvers are adaptive):
+ *   k1=f(y); k2=f(y+dt/2 k1); k3=f(y+dt/2 k2); k4=f(y+dt k3);
+ *   y <- y + dt/6 (k1 + 2 k2 + 2 k3 + k4).
+ * The systems are autonomous, so t is not passed to f. */
+int ora_rk4(const ora_net* net, double* y, int64_t n_steps, double dt) {
+    int32_t nv = ora_nvar(net->model);
+    if (nv < 0) return -1;
+    int64_t len = (int64_t)nv * net->n;
+    double* buf = (double*)malloc(sizeof(double) * (size_t)len * 5);
+    if (!buf) return -2;
+    double *k1 = buf, *k2 = buf + len, *k3 = buf + 2 * len, *k4 = buf + 3 * len,
+           *tmp = buf + 4 * len;
+    for (int64_t s = 0; s < n_steps; ++s) {
+        ora_rhs(net, y, k1);
+        for (int64_t q = 0; q < len; ++q) tmp[q] = y[q] + 0.5 * dt * k1[q];
+        ora_rhs(net, tmp, k2);
+        for (int64_t q = 0; q < len; ++q) tmp[q] = y[q] + 0.5 * dt * k2[q];
+        ora_rhs(net, tmp, k3);
+        for (int64_t q = 0; q < len; ++q) tmp[q] = y[q] + dt * k3[q];
+        ora_rhs(net, tmp, k4);
+        for (int64_t q = 0; q < len; ++q)
+            y[q] = y[q] + (dt / 6.0) * (k1[q] + 2.0 * k2[q] + 2.0 * k3[q] + k4[q]);
+    }
+    free(buf);
+    return 0;
+}
+
+/* ------------------------------------------------------------------ */
+/* Observables (reading R9; the paper names them - "synchronization    */
+/* analysis at each output" PAPER.md:416, average frequencies :301,    */
+/* coherent/incoherent regions :325 - but gives no formulas).          */
+/* ------------------------------------------------------------------ */
+
+/* Phase map theta_i.  KS: phi.  FHN: atan2(v,u).  HH: atan2(n - n_c,
+ * (V - V_c)/V_s); pm = {V_c, n_c, V_s}. */
+void ora_phase(int32_t model, int64_t n, const double* y, const double* pm, double* theta) {
+    for (int64_t i = 0; i < n; ++i) {
+        if (model == ORA_MODEL_KS)
+            theta[i] = y[i];
+        else if (model == ORA_MODEL_FHN)
+            theta[i] = atan2(y[n + i], y[i]);
+        else
+            theta[i] = atan2(y[3 * n + i] - pm[1], (y[i] - pm[0]) / pm[2]);
+    }
+}
+
+/* Global Kuramoto order parameter  R e^{i Psi} = (1/N) sum_j e^{i theta_j}. */
+void ora_global_order(int64_t n, const double* theta, double* R, double* Psi) {
+    double c = 0.0, s = 0.0;
+    for (int64_t j = 0; j < n; ++j) {
+        c += cos(theta[j]);
+        s += sin(theta[j]);
+    }
+    c /= (double)n;
+    s /= (double)n;
+    *R = sqrt(c * c + s * s);
+    *Psi = atan2(s, c);
+}
+
+/* Local order parameter over the coupling neighbourhood plus the element:
+ *   R_i = | ( sum_{j in row i} e^{i theta_j} + e^{i theta_i} ) / (Omega_i + 1) |
+ * (if the row already holds i, it is not added a second time). */
+void ora_local_order(int64_t n, const int64_t* row_ptr, const int32_t* col_idx,
+                     const double* theta, double* Rloc) {
+#pragma omp parallel for schedule(static)
+    for (int64_t i = 0; i < n; ++i) {
+        double c = 0.0, s = 0.0;
+        int64_t cnt = 0;
+        int has_self = 0;
+        for (int64_t e = row_ptr[i]; e < row_ptr[i + 1]; ++e, ++cnt) {
+            int32_t j = col_idx[e];
+            if (j == i) has_self = 1;
+            c += cos(theta[j]);
+            s += sin(theta[j]);
+        }
+        if (!has_self) {
+            c += cos(theta[i]);
+            s += sin(theta[i]);
+            ++cnt;
+        }
+        Rloc[i] = sqrt(c * c + s * s) / (double)cnt;
+    }
+}

@@ -1,0 +1,339 @@
+"""Pins of the oracle's right-hand sides, RK4 and observables (no GPU).
+
+Every check compares the oracle with something fixed by the mathematics or by
+a textbook / the paper, not with the oracle itself: closed forms, invariants,
+dense brute force with an explicit 0/1 matrix, hand-evaluated numbers.
+"""
+import math
+import os
+
+import numpy as np
+import pytest
+
+from oracle import oracle as ora
+
+RNG = np.random.default_rng(12345)
+
+
+def _dense(rp, ci, n):
+    L = np.zeros((n, n))
+    for i in range(n):
+        L[i, ci[rp[i]:rp[i + 1]]] = 1.0
+    return L
+
+
+def _topologies():
+    out = []
+    rp, ci = ora.topology_ring(13, 3)
+    out.append(("ring", 13, rp, ci))
+    rp, ci = ora.topology_lattice((4, 4), 1)
+    out.append(("lat2d", 16, rp, ci))
+    rp, ci = ora.topology_lattice((5, 5, 5), 2)
+    out.append(("lat3d", 125, rp, ci))
+    rp, ci = ora.topology_random_indegree(16, 5, 9)
+    out.append(("rand", 16, rp, ci))
+    return out
+
+
+TOPOS = _topologies()
+
+
+# ------------------------------------------------------------------ Kuramoto
+@pytest.mark.parametrize("name,n,rp,ci", TOPOS)
+def test_ks_dense_brute_force(name, n, rp, ci):
+    # f_i = omega_i + (K/Omega_i) sum_j L_ij sin(phi_j - phi_i - alpha), L dense 0/1, j influences i
+    phi, omega = RNG.uniform(-3, 3, n), RNG.normal(size=n)
+    K, alpha = 1.7, 0.6
+    L = _dense(rp, ci, n)
+    S = np.sin(phi[None, :] - phi[:, None] - alpha)
+    expect = omega + K * (L * S).sum(axis=1) / L.sum(axis=1)
+    got = ora.OracleNet.ks(n, rp, ci, K, alpha, omega).rhs(phi)[0]
+    np.testing.assert_allclose(got, expect, rtol=0, atol=1e-13)
+
+
+def test_ks_uncoupled_closed_form():
+    # K = 0  =>  phi(t) = phi0 + omega t; RK4 is exact for a constant RHS.
+    n = 32
+    rp, ci = ora.topology_ring(n, 5)
+    phi0, omega = RNG.uniform(-3, 3, n), RNG.normal(size=n)
+    net = ora.OracleNet.ks(n, rp, ci, 0.0, 0.3, omega)
+    y = net.rk4(phi0, 200, 0.05)[0]
+    np.testing.assert_allclose(y, phi0 + omega * 10.0, rtol=0, atol=5e-13)
+
+
+@pytest.mark.parametrize("include_self", [False, True])
+def test_ks_in_phase_state_is_invariant(include_self):
+    # identical phases and frequencies: every term is sin(-alpha), so
+    # f_i = omega - K sin(alpha) whatever the neighbourhood is (self link or not).
+    n, P, K, alpha, w = 40, 6, 1.3, 0.7, 0.25
+    rp, ci = ora.topology_ring(n, P, include_self=include_self)
+    net = ora.OracleNet.ks(n, rp, ci, K, alpha, w)
+    phi = np.full(n, 0.4)
+    np.testing.assert_allclose(net.rhs(phi)[0], w - K * math.sin(alpha), atol=1e-15)
+    y = net.rk4(phi, 100, 0.05)[0]
+    assert np.ptp(y) < 1e-13
+    np.testing.assert_allclose(y, 0.4 + (w - K * math.sin(alpha)) * 5.0, atol=1e-12)
+
+
+@pytest.mark.parametrize("builder", [lambda: ora.topology_ring(50, 7),
+                                     lambda: ora.topology_lattice((6, 6, 6), 2)])
+def test_ks_sum_conservation_alpha0(builder):
+    # alpha = 0, symmetric topology with uniform degree: sin is odd, so the pair
+    # terms cancel and sum_i f_i = sum_i omega_i.
+    rp, ci = builder()
+    n = len(rp) - 1
+    phi, omega = RNG.uniform(-3, 3, n), RNG.normal(size=n)
+    f = ora.OracleNet.ks(n, rp, ci, 2.0, 0.0, omega).rhs(phi)[0]
+    assert abs(f.sum() - omega.sum()) < 1e-12 * n
+
+
+@pytest.mark.parametrize("n", [5, 9, 15])
+def test_ks_all_to_all_mean_field_identity(n):
+    # ring with 2P = n-1 is all-to-all.  With R e^{i Psi} = (1/n) sum_j e^{i phi_j}:
+    #   sum_{j != i} sin(phi_j - phi_i - a) = n R sin(Psi - phi_i - a) + sin(a)
+    P = (n - 1) // 2
+    rp, ci = ora.topology_ring(n, P)
+    phi = RNG.uniform(-3, 3, n)
+    K, a = 0.9, 1.1
+    z = np.exp(1j * phi).mean()
+    R, Psi = abs(z), np.angle(z)
+    expect = K * (n * R * np.sin(Psi - phi - a) + math.sin(a)) / (n - 1)
+    got = ora.OracleNet.ks(n, rp, ci, K, a, 0.0).rhs(phi)[0]
+    np.testing.assert_allclose(got, expect, atol=1e-14)
+
+
+# ------------------------------------------------------------ FitzHugh-Nagumo
+@pytest.mark.parametrize("name,n,rp,ci", TOPOS)
+def test_fhn_dense_brute_force(name, n, rp, ci):
+    u, v = RNG.uniform(-2, 2, n), RNG.uniform(-2, 2, n)
+    eps, a, sigma, phi = 0.05, 0.5, 0.3, math.pi / 2 - 0.1
+    L = _dense(rp, ci, n)
+    Om = L.sum(axis=1)
+    Cu = L @ u - Om * u
+    Cv = L @ v - Om * v
+    fu = (u - u ** 3 / 3 - v + sigma / Om * (math.cos(phi) * Cu + math.sin(phi) * Cv)) / eps
+    fv = u + a + sigma / Om * (-math.sin(phi) * Cu + math.cos(phi) * Cv)
+    got = ora.OracleNet.fhn(n, rp, ci, eps, a, sigma, phi).rhs(np.stack([u, v]))
+    np.testing.assert_allclose(got[0], fu, rtol=0, atol=2e-12)
+    np.testing.assert_allclose(got[1], fv, rtol=0, atol=1e-13)
+
+
+def test_fhn_fixed_point_and_uniform_state():
+    # uncoupled fixed point (u*, v*) = (-a, -a + a^3/3): for a = 0.5 that is (-0.5, -0.458333..)
+    n, a = 30, 0.5
+    rp, ci = ora.topology_ring(n, 4)
+    net = ora.OracleNet.fhn(n, rp, ci, 0.05, a, 0.4, 1.2)
+    y = np.stack([np.full(n, -0.5), np.full(n, -0.5 + 0.125 / 3)])
+    assert abs(-0.5 + 0.125 / 3 - (-0.4583333333333333)) < 1e-15
+    assert np.abs(net.rhs(y)).max() < 1e-14
+    # a uniform state feels no coupling: same trajectory as sigma = 0
+    y0 = np.stack([np.full(n, 1.3), np.full(n, -0.2)])
+    net0 = ora.OracleNet.fhn(n, rp, ci, 0.05, a, 0.0, 1.2)
+    np.testing.assert_allclose(net.rk4(y0, 50, 0.01), net0.rk4(y0, 50, 0.01), atol=1e-12)
+    # and the hand-evaluated local field at (u,v) = (1.3, -0.2):
+    f = net.rhs(y0)
+    assert abs(f[0, 0] - (1.3 - 1.3 ** 3 / 3 + 0.2) / 0.05) < 1e-12
+    assert abs(f[1, 0] - 1.8) < 1e-15
+
+
+def test_fhn_coupling_sums_to_zero_and_phi0_is_diagonal():
+    n = 216
+    rp, ci = ora.topology_lattice((6, 6, 6), 2)
+    y = RNG.uniform(-2, 2, (2, n))
+    eps, a, sigma = 0.05, 0.5, 0.7
+    f_c = ora.OracleNet.fhn(n, rp, ci, eps, a, sigma, 0.9).rhs(y)
+    f_0 = ora.OracleNet.fhn(n, rp, ci, eps, a, 0.0, 0.9).rhs(y)
+    # sum_i Cu_i = sum_i Cv_i = 0 on a symmetric topology => coupling terms cancel in the sum
+    assert abs((f_c[0] - f_0[0]).sum() * eps) < 1e-10
+    assert abs((f_c[1] - f_0[1]).sum()) < 1e-10
+    # phi = 0: pure u->u, v->v diffusion: dv/dt must not depend on the u-differences
+    y2 = y.copy()
+    y2[0] += RNG.normal(size=n) * 0.0          # keep u
+    f_a = ora.OracleNet.fhn(n, rp, ci, eps, a, sigma, 0.0).rhs(y)
+    L = _dense(rp, ci, n)
+    np.testing.assert_allclose(f_a[1] - f_0[1], sigma / 32 * (L @ y[1] - 32 * y[1]), atol=1e-12)
+    np.testing.assert_allclose((f_a[0] - f_0[0]) * eps, sigma / 32 * (L @ y[0] - 32 * y[0]),
+                               atol=1e-12)
+
+
+# ------------------------------------------------------------- Hodgkin-Huxley
+def _golden(golden_dir, name):
+    d = {}
+    for line in open(os.path.join(golden_dir, name)):
+        if line.startswith("#") or not line.strip():
+            continue
+        k, v = line.split()
+        d[k] = float(v)
+    return d
+
+
+def _hh_single(I=0.0, **kw):
+    rp, ci = np.array([0, 0], dtype=np.int64), np.zeros(0, dtype=np.int32)
+    return ora.OracleNet.hh(1, rp, ci, I, **kw)
+
+
+def test_hh_rates_against_hand_values(golden_dir):
+    g = _golden(golden_dir, "hh_textbook_rest.txt")
+    net = _hh_single()
+    # gates all 0: dx/dt = alpha_x ; gates all 1: dx/dt = -beta_x
+    f0 = net.rhs(np.array([-65.0, 0, 0, 0]))[:, 0]
+    f1 = net.rhs(np.array([-65.0, 1, 1, 1]))[:, 0]
+    hand = dict(alpha_m=2.5 / (math.e ** 2.5 - 1), beta_m=4.0, alpha_h=0.07,
+                beta_h=1 / (1 + math.e ** 3), alpha_n=0.1 / (math.e - 1), beta_n=0.125)
+    for q, x in enumerate("mhn"):
+        assert abs(f0[1 + q] - hand["alpha_" + x]) < 1e-14
+        assert abs(-f1[1 + q] - hand["beta_" + x]) < 1e-14
+        assert abs(f0[1 + q] - g["alpha_" + x]) < 6e-5       # textbook 4-decimal values
+        assert abs(-f1[1 + q] - g["beta_" + x]) < 6e-5
+    # membrane equation, hand numbers: gates 0 -> only the leak: -0.3*(-65+54.4) = 3.18
+    assert abs(f0[0] - 3.18) < 1e-13
+    # m=h=1,n=0: -120*(-65-50) = 13800 (+3.18);  n=1, m=0: -36*(-65+77) = -432 (+3.18)
+    assert abs(net.rhs(np.array([-65.0, 1, 1, 0]))[0, 0] - 13803.18) < 1e-9
+    assert abs(net.rhs(np.array([-65.0, 0, 0, 1]))[0, 0] - (-428.82)) < 1e-10
+    assert abs(_hh_single(I=7.5).rhs(np.array([-65.0, 0, 0, 0]))[0, 0] - 10.68) < 1e-13
+
+
+def test_hh_removable_singularities():
+    net = _hh_single()
+    for V0, q, lim in [(-40.0, 1, 1.0), (-55.0, 3, 0.1)]:
+        vals = [net.rhs(np.array([V0 + d, 0, 0, 0]))[q, 0] for d in (-1e-7, -1e-11, 0.0, 1e-11, 1e-7)]
+        assert abs(vals[2] - lim) < 1e-15
+        assert max(abs(v - lim) for v in vals) < 1e-8
+        assert all(vals[i] <= vals[i + 1] + 1e-13 for i in range(4))      # smooth through it
+
+
+def test_hh_textbook_rest_state(golden_dir):
+    g = _golden(golden_dir, "hh_textbook_rest.txt")
+    m, h, n_ = ora.hh_steady_gates(np.array([-65.0]))
+    assert abs(m[0] - g["m_inf"]) < 6e-5 and abs(h[0] - g["h_inf"]) < 6e-5
+    assert abs(n_[0] - g["n_inf"]) < 6e-5
+    net = _hh_single()
+    f = net.rhs(np.array([-65.0, m[0], h[0], n_[0]]))[:, 0]
+    assert abs(f[0]) < 2e-3 and np.abs(f[1:]).max() < 1e-15       # essentially at rest
+    # relax for 200 ms: stays within 0.01 mV of the textbook -65 mV and becomes stationary
+    y = net.rk4(np.array([-65.0, m[0], h[0], n_[0]]), 20000, 0.01)
+    assert abs(y[0, 0] - g["V_rest_mV"]) < 0.01
+    assert np.abs(net.rhs(y)).max() < 1e-9
+
+
+def test_hh_fires_repetitively_at_10uA():
+    # the standard model fires periodically (several tens of Hz, spikes overshooting 0 mV)
+    # for I = 10 uA/cm^2 and is silent for I = 0
+    net = _hh_single(I=10.0)
+    m, h, n_ = ora.hh_steady_gates(np.array([-65.0]))
+    y = np.array([-65.0, m[0], h[0], n_[0]])
+    V = []
+    for _ in range(2000):
+        y = net.rk4(y, 10, 0.01)[:, 0]
+        V.append(y[0])
+    V = np.array(V)                                  # 200 ms sampled every 0.1 ms
+    ups = np.nonzero((V[:-1] < 0) & (V[1:] >= 0))[0]
+    rate = (len(ups) - 1) / ((ups[-1] - ups[0]) * 1e-4)
+    assert 55 < rate < 80 and V.max() > 20 and V.min() > -80
+
+
+def test_hh_synapse_sign_normaliser_and_dense():
+    # one edge j -> i: I_syn = g_syn (E_syn - V_i) S(V_j), S(theta_syn) = 1/2
+    rp, ci = np.array([0, 1, 1], dtype=np.int64), np.array([1], dtype=np.int32)
+    net = ora.OracleNet.hh(2, rp, ci, 0.0)
+    base = ora.OracleNet.hh(2, rp, ci, 0.0, g_syn=0.0)
+    y = np.array([[-65.0, 0.0], [0, 0], [0, 0], [0, 0]])
+    d = net.rhs(y) - base.rhs(y)
+    assert abs(d[0, 0] - 0.1 * 65.0 * 0.5) < 1e-13 and d[0, 1] == 0.0
+    # dense brute force on a random graph, in-degree 5: g_syn/k * (E-V_i) * sum_j L_ij S(V_j)
+    n, k = 16, 5
+    rp, ci = ora.topology_random_indegree(n, k, 4)
+    V = RNG.uniform(-70, 20, n)
+    y = np.stack([V, RNG.random(n), RNG.random(n), RNG.random(n)])
+    L = _dense(rp, ci, n)
+    S = 1 / (1 + np.exp(-(V - 0.0) / 2.0))
+    expect = 0.1 / k * (0.0 - V) * (L @ S)
+    I = RNG.uniform(9, 11, n)
+    got = ora.OracleNet.hh(n, rp, ci, I).rhs(y)[0] - ora.OracleNet.hh(n, rp, ci, I, g_syn=0.0).rhs(y)[0]
+    np.testing.assert_allclose(got, expect, atol=1e-12)
+
+
+# ------------------------------------------------------------------------ RK4
+def test_rk4_fourth_order():
+    # tiny net (N=8 ring, P=2); error against a 16x finer step falls by 16 per halving of dt
+    n = 8
+    rp, ci = ora.topology_ring(n, 2)
+    net = ora.OracleNet.ks(n, rp, ci, 1.0, 0.4, RNG.normal(size=n))
+    phi0 = RNG.uniform(-3, 3, n)
+    T = 2.0
+    ref = net.rk4(phi0, 16 * 160, T / (16 * 160))
+    errs = [np.abs(net.rk4(phi0, m, T / m) - ref).max() for m in (20, 40, 80)]
+    assert 13 < errs[0] / errs[1] < 19 and 13 < errs[1] / errs[2] < 19
+
+
+def test_rk4_matches_textbook_scalar_step():
+    # one step of dy/dt = -y^3+... is awkward through the models, so use FHN with sigma=0 on one
+    # element and redo the four stages by hand with the local field typed here.
+    rp, ci = np.array([0, 0], dtype=np.int64), np.zeros(0, dtype=np.int32)
+    eps, a = 0.05, 0.5
+    net = ora.OracleNet.fhn(1, rp, ci, eps, a, 0.0, 0.0)
+
+    def f(y):
+        return np.array([(y[0] - y[0] ** 3 / 3 - y[1]) / eps, y[0] + a])
+    y0, dt = np.array([0.7, -0.3]), 0.01
+    k1 = f(y0); k2 = f(y0 + dt / 2 * k1); k3 = f(y0 + dt / 2 * k2); k4 = f(y0 + dt * k3)
+    expect = y0 + dt / 6 * (k1 + 2 * k2 + 2 * k3 + k4)
+    np.testing.assert_allclose(net.rk4(y0.reshape(2, 1), 1, dt)[:, 0], expect, atol=1e-15)
+
+
+# ---------------------------------------------------------------- observables
+def test_order_parameters_closed_forms():
+    n = 24
+    rp, ci = ora.topology_ring(n, 3)
+    net = ora.OracleNet.ks(n, rp, ci, 1.0, 0.0, 0.0)
+    R, Psi = net.global_order(np.full(n, 0.7))
+    assert abs(R - 1) < 1e-15 and abs(Psi - 0.7) < 1e-15
+    assert np.abs(net.local_order(np.full(n, 0.7)) - 1).max() < 1e-15
+    splay = 2 * np.pi * np.arange(n) / n
+    assert net.global_order(splay)[0] < 1e-15
+    # splay state: local R over 2P+1 = 7 consecutive phases = |sin(7 d/2)/(7 sin(d/2))|, d = 2pi/n
+    d = 2 * np.pi / n
+    np.testing.assert_allclose(net.local_order(splay), abs(math.sin(3.5 * d) / (7 * math.sin(d / 2))),
+                               atol=1e-14)
+    # brute force with the dense matrix
+    th = RNG.uniform(-3, 3, n)
+    L = _dense(rp, ci, n) + np.eye(n)
+    np.testing.assert_allclose(net.local_order(th), np.abs(L @ np.exp(1j * th)) / 7, atol=1e-14)
+
+
+def test_phase_maps():
+    rp, ci = ora.topology_ring(4, 1)
+    y = np.array([[1.0, 0.0, -1.0, 0.0], [0.0, 2.0, 0.0, -3.0]])
+    th = ora.OracleNet.fhn(4, rp, ci, 0.05, 0.5, 0.1, 0.0).phase(y)
+    np.testing.assert_allclose(th, [0, np.pi / 2, np.pi, -np.pi / 2], atol=1e-15)
+    yh = np.zeros((4, 4)); yh[0] = [80.0, -20.0, -120.0, -20.0]; yh[3] = [0.55, 1.55, 0.55, -0.45]
+    th = ora.OracleNet.hh(4, rp, ci, 0.0).phase(yh)
+    np.testing.assert_allclose(th, [0, np.pi / 2, np.pi, -np.pi / 2], atol=1e-15)
+
+
+def test_mean_phase_velocity_uncoupled():
+    # KS, K = 0: mean phase velocity equals omega_i exactly
+    n = 16
+    rp, ci = ora.topology_ring(n, 2)
+    omega = RNG.normal(size=n)
+    st = ora.OracleNet.ks(n, rp, ci, 0.0, 0.0, omega).run_statistics(RNG.uniform(-3, 3, n), 200,
+                                                                     0.05, 10)
+    np.testing.assert_allclose(st["vel"], omega, atol=1e-12)
+    assert st["n_samples"] == 11
+    # FHN, uncoupled oscillator: 2 pi / |mean phase velocity| = period between upward zero
+    # crossings of u (measured here from the trajectory itself)
+    rp1, ci1 = np.array([0, 0], dtype=np.int64), np.zeros(0, dtype=np.int32)
+    net = ora.OracleNet.fhn(1, rp1, ci1, 0.05, 0.5, 0.0, 0.0)
+    y = np.array([[2.0], [0.0]])
+    y = net.rk4(y, 3000, 0.005)                       # discard the transient
+    us, ys = [], y
+    for _ in range(6000):
+        ys = net.rk4(ys, 1, 0.005)
+        us.append(ys[0, 0])
+    us = np.array(us)
+    up = np.nonzero((us[:-1] < 0) & (us[1:] >= 0))[0]
+    tc = up + (-us[up]) / (us[up + 1] - us[up])       # linear interpolation of the crossing
+    period = np.diff(tc).mean() * 0.005
+    k = int(round(2 * (tc[-1] - tc[0])))              # a whole number of periods, in steps
+    st = net.run_statistics(y, 2 * k, 0.005, 4)
+    assert abs(2 * np.pi / abs(st["vel"][0]) - period) < 2e-3 * period
