@@ -1,0 +1,222 @@
+/*
+ * oscnet.h -- C ABI of the B200-native coupled-oscillator RK4 hot path of
+ * arXiv:2410.19075 (Sudakov & Maistrenko, "Parallelization of Network Dynamics
+ * Computations in Heterogeneous Distributed Environment").
+ *
+ * The library integrates N coupled oscillators with fixed-step classical RK4.
+ * Each right-hand-side evaluation is "local vector field + coupling sum over the
+ * in-neighbours the topology allows" (Alg. 1),
+ * for the three model classes of Sec. II: Hodgkin-Huxley type (eq. (1),
+ * PAPER.md:48-60), FitzHugh-Nagumo (eq. (2)) and
+ * Kuramoto-Sakaguchi phase oscillators (eq. (3)), on the coupling
+ * topologies of Sec. IV: ring, 2D/3D periodic lattice with
+ * Euclidean radius P or an arbitrary runtime graph
+ * given as CSR.  "Integration ... requires the runtime
+ * specification of initial values for dynamical variables, model parameters,
+ * and the coupling topology of the network": these are exactly
+ * the arguments of net_create / net_set_state / net_set_param_array.
+ *
+ * Conventions
+ *  - Every function returns an int32_t status: NET_OK or a negative NET_ERR_*.
+ *    Nothing throws, aborts or exits.  net_last_error() gives the message of the
+ *    last failing call on that handle (or of the last failing net_create /
+ *    net_workspace_bytes when called with NULL).
+ *  - The library never allocates device memory.  All device storage (state,
+ *    RK4 stages, topology, scratch) lives in the caller's workspace, whose size
+ *    net_workspace_bytes() reports.  The handle is a small host object.
+ *  - The CUDA stream is borrowed.  Every call enqueues its work on that stream.
+ *    Calls whose source/destination is a HOST pointer synchronise the stream
+ *    before returning; calls with DEVICE pointers are stream-ordered and
+ *    asynchronous.  Asynchronous CUDA faults surface at the next synchronising
+ *    call as NET_ERR_CUDA.
+ *  - State layout: structure of arrays [nvar][n], element type = the dtype of
+ *    the net (float or double), contiguous (variable v of element i at
+ *    v*n + i).  nvar: KS 1 (phi); FHN 2 (u, v); HH 4 (V, m, h, n).
+ *  - Element numbering of lattices: site (i,j,k) is element k*nx*ny + j*nx + i
+ *    (PAPER.md:309 "jN1+i", :311 "kN1^2+jN1+i").
+ *  - CSR orientation: row i lists the elements j that influence i
+ *    (L_ij = 1 iff the j-th oscillator influences the i-th).
+ */
+#ifndef OSCNET_H
+#define OSCNET_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct net net_t;
+
+enum {
+    NET_OK = 0,
+    NET_ERR_INVALID = -1,     /* null pointer, bad enum, bad size, 2*radius >= extent, ... */
+    NET_ERR_SIZE = -2,        /* workspace too small or misaligned (needs 256-byte alignment) */
+    NET_ERR_TOPOLOGY = -3,    /* CSR not monotone / index out of range / self-loop where forbidden */
+    NET_ERR_CUDA = -4,        /* a CUDA call failed; message holds cudaGetErrorString */
+    NET_ERR_UNSUPPORTED = -5  /* valid request this build does not implement (e.g. batch > 1) */
+};
+
+enum { NET_MODEL_KS = 0, NET_MODEL_FHN = 1, NET_MODEL_HH = 2 };
+enum { NET_TOPO_RING = 0, NET_TOPO_LATTICE = 1, NET_TOPO_CSR = 2, NET_TOPO_RANDOM_INDEGREE = 3 };
+enum { NET_F32 = 0, NET_F64 = 1 };
+
+/* How the coupling sum is evaluated.  DIRECT = one term per neighbour, gathered
+ * from global memory (the formulation of Alg. 1).  FAST = the rewrite for that
+ * model/topology that is exact in real arithmetic: factorised sine + tiled
+ * window sums on lattices, prefix sums on rings, warp-per-row gathers of
+ * precomputed synaptic activations on graphs.  AUTO = FAST where one exists. */
+enum { NET_METHOD_AUTO = 0, NET_METHOD_DIRECT = 1, NET_METHOD_FAST = 2 };
+
+enum { NET_PARAM_OMEGA = 0, NET_PARAM_IEXT = 1 };
+
+enum {
+    NET_OBS_PHASE = 0,               /* theta[n] of the current state, dtype double */
+    NET_OBS_GLOBAL_ORDER = 1,        /* double[2] = {R, Psi}: R e^{i Psi} = (1/N) sum_j e^{i theta_j} */
+    NET_OBS_LOCAL_ORDER = 2,         /* double[n]: R_i over the coupling neighbourhood plus i */
+    NET_OBS_MEAN_PHASE_VELOCITY = 3, /* double[n] over the window of net_integrate_observed */
+    NET_OBS_STATS = 4                /* double[8], see net_integrate_observed */
+};
+
+/* Kuramoto-Sakaguchi, eq. (3) with m=0, eps=1, mu=K/Omega_i:
+ *   dphi_i/dt = omega_i + (K/Omega_i) sum_{j in row i} sin(phi_j - phi_i - alpha).
+ * omega_i = omega0 for all i until net_set_param_array(NET_PARAM_OMEGA). */
+typedef struct {
+    double K, alpha, omega0;
+} net_ks_params;
+
+/* FitzHugh-Nagumo, eq. (2) with rotated 2x2 diffusive coupling:
+ *   eps du_i/dt = u_i - u_i^3/3 - v_i + (sigma/Omega_i) sum_j [b_uu (u_j-u_i) + b_uv (v_j-v_i)]
+ *       dv_i/dt = u_i + a           + (sigma/Omega_i) sum_j [b_vu (u_j-u_i) + b_vv (v_j-v_i)]
+ *   (b_uu, b_uv, b_vu, b_vv) = (cos phi, sin phi, -sin phi, cos phi). */
+typedef struct {
+    double eps, a, sigma, phi;
+} net_fhn_params;
+
+/* Hodgkin-Huxley type element, eq. (1), standard squid-axon
+ * channels and an instantaneous sigmoidal synapse (mV, ms, uA/cm^2, mS/cm^2, uF/cm^2):
+ *   C dV_i/dt = I_ext,i - gNa m^3 h (V-ENa) - gK n^4 (V-EK) - gL (V-EL)
+ *               + (g_syn/Omega_i)(E_syn - V_i) sum_{j in row i} S(V_j),
+ *   S(V) = 1/(1+exp(-(V-theta_syn)/k_syn)),  dx/dt = alpha_x(V)(1-x) - beta_x(V) x.
+ * I_ext,i = I_ext0 until net_set_param_array(NET_PARAM_IEXT).
+ * (V_c, n_c, V_s) define the phase map theta = atan2(n - n_c, (V - V_c)/V_s). */
+typedef struct {
+    double gNa, gK, gL, ENa, EK, EL, C, g_syn, E_syn, theta_syn, k_syn;
+    double I_ext0;
+    double V_c, n_c, V_s;
+} net_hh_params;
+
+/* Coupling topology (static during a run).
+ *  RING:    n elements on a circle, each coupled to `radius` neighbours on both sides.
+ *  LATTICE: ndim (1..3) periodic lattice extent[0] x extent[1] x extent[2] (x fastest),
+ *           coupled to all sites with squared Euclidean distance <= radius^2.
+ *           2*radius < every used extent is required (no site may be reached twice).
+ *  CSR:     row_ptr[n+1] (int64), col_idx[nnz] (int32); host or device pointers
+ *           (ptrs_are_device); copied into the workspace by net_create.
+ *  RANDOM_INDEGREE: every row has exactly in_degree distinct sources != i, drawn by the
+ *           integer counter-based rule of DESIGN.md reading R8 from `seed`; built on the device.
+ *  include_self (ring/lattice): also count the centre as a link (then Omega = 2P+1 / 33 / 257,
+ *           the link counts the paper prints). */
+typedef struct {
+    int32_t kind;
+    int32_t ndim;
+    int64_t extent[3];
+    int32_t radius;
+    int32_t include_self;
+    const int64_t* row_ptr;
+    const int32_t* col_idx;
+    int64_t nnz;
+    int32_t ptrs_are_device;
+    int32_t in_degree;
+    uint64_t seed;
+} net_topology;
+
+typedef struct {
+    int32_t model;  /* NET_MODEL_*  */
+    int32_t dtype;  /* NET_F32 | NET_F64: storage and arithmetic type of the state */
+    int64_t n;      /* number of elements (64-bit) */
+    int32_t batch;  /* independent replicas of the net; this build supports 1 */
+    int32_t method; /* NET_METHOD_* */
+    net_topology topo;
+} net_desc;
+
+/* Bytes of device workspace net_create needs for this description (pure function). */
+int32_t net_workspace_bytes(const net_desc* desc, size_t* bytes);
+
+/* Builds the network: validates, lays out the workspace, builds the topology on the device
+ * (offset tables / CSR / random graph) and zeroes the state.  `params` points to the
+ * net_*_params struct of desc->model (params_bytes = its sizeof).  d_workspace: device memory,
+ * 256-byte aligned, >= net_workspace_bytes; owned by the caller and must outlive the handle.
+ * cuda_stream: a cudaStream_t (NULL = legacy default stream).  On failure *out is NULL. */
+int32_t net_create(const net_desc* desc, const void* params, size_t params_bytes,
+                   void* d_workspace, size_t workspace_bytes, void* cuda_stream, net_t** out);
+
+/* Frees the host handle (and its CUDA graph); the workspace stays with the caller. */
+int32_t net_destroy(net_t* net);
+
+/* Copies a full state [nvar][n] (dtype of the net) into / out of the net.  Resets nothing
+ * else; the time and step counter are kept (net_set_time changes them). */
+int32_t net_set_state(net_t* net, const void* src, int32_t src_is_device);
+int32_t net_get_state(net_t* net, void* dst, int32_t dst_is_device);
+
+/* Per-element parameter array [n] in the dtype of the net: NET_PARAM_OMEGA (KS) or
+ * NET_PARAM_IEXT (HH). */
+int32_t net_set_param_array(net_t* net, int32_t which, const void* src, int32_t src_is_device);
+
+/* HH only: sets m, h, n of every element to the steady state x_inf(V_i) of its current V
+ * (the north-star initial condition "gates at steady state"). */
+int32_t net_hh_steady_gates(net_t* net);
+
+/* Advances the state by n_steps classical RK4 steps of size dt (enqueued, asynchronous):
+ *   k1=f(y); k2=f(y+dt/2 k1); k3=f(y+dt/2 k2); k4=f(y+dt k3); y += dt/6 (k1+2k2+2k3+k4).
+ * Every stage is one fused kernel (coupled RHS + stage update); steps are replayed from a
+ * captured CUDA graph. */
+int32_t net_integrate(net_t* net, int64_t n_steps, double dt);
+
+/* net_integrate plus the long-run statistics of DESIGN.md reading R9: samples after steps
+ * obs_every, 2*obs_every, ..., n_steps (n_steps % obs_every == 0); the window is the samples
+ * with step >= n_steps/2.  Afterwards NET_OBS_STATS gives double[8] =
+ * {mean R, std R (population), mean_i R_loc,i at the last sample, mean_i and std_i of the mean
+ *  phase velocity over the window, number of samples, t_a, t_b} and
+ * NET_OBS_MEAN_PHASE_VELOCITY the per-element velocities. */
+int32_t net_integrate_observed(net_t* net, int64_t n_steps, double dt, int64_t obs_every);
+
+/* One right-hand-side evaluation f(y) at the current state, [nvar][n] in the dtype of the net
+ * (parity hook). */
+int32_t net_eval_rhs(net_t* net, void* dst, int32_t dst_is_device);
+
+/* Observables of the current state (or of the last net_integrate_observed window), always
+ * double; sizes under NET_OBS_*. */
+int32_t net_observables(net_t* net, int32_t what, void* dst, int32_t dst_is_device);
+
+/* Expands rows [row_begin, row_begin+row_count) of the topology to canonical CSR: each row
+ * sorted ascending, row_ptr[row_count+1] relative to the range (parity hook; bit-exact
+ * against the oracle). */
+int32_t net_get_topology(net_t* net, int64_t row_begin, int64_t row_count, int64_t* row_ptr,
+                         int32_t* col_idx, int32_t dst_is_device);
+
+/* nnz of the whole topology and the in-degree if every row has the same one (else -1). */
+int32_t net_get_degree(net_t* net, int64_t* nnz, int32_t* uniform_degree);
+
+int32_t net_get_time(net_t* net, double* t, int64_t* step);
+int32_t net_set_time(net_t* net, double t, int64_t step);
+
+/* Number of kernels this handle has launched (graph replays count their kernel nodes) and
+ * the method actually in use (NET_METHOD_DIRECT or NET_METHOD_FAST). */
+int32_t net_get_counters(net_t* net, int64_t* kernel_launches, int32_t* method_in_use);
+
+/* Blocks until the stream is idle; returns NET_ERR_CUDA if anything failed asynchronously. */
+int32_t net_synchronize(net_t* net);
+
+/* Message of the last error on this handle (NULL: of the last failed handle-less call).
+ * The string is owned by the library and valid until the next call on the same handle. */
+const char* net_last_error(const net_t* net);
+
+/* "oscnet <major>.<minor> sm_100a" */
+const char* net_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* OSCNET_H */

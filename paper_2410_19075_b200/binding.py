@@ -1,0 +1,377 @@
+"""Thin ctypes binding of liboscnet.so (include/oscnet.h).
+
+Argument marshalling only: every step of the hot path runs in the CUDA library.
+PyTorch supplies device memory (the workspace), streams and pinned host memory.
+The module-level ``net_*`` functions mirror the C ABI one to one; ``Net`` is a
+small convenience wrapper that owns the workspace tensor.  There is no CPU
+fallback: a missing library or a missing GPU raises.
+"""
+import ctypes as C
+import os
+
+import numpy as np
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(HERE, "liboscnet.so")
+
+NET_OK = 0
+MODEL_KS, MODEL_FHN, MODEL_HH = 0, 1, 2
+TOPO_RING, TOPO_LATTICE, TOPO_CSR, TOPO_RANDOM_INDEGREE = 0, 1, 2, 3
+F32, F64 = 0, 1
+METHOD_AUTO, METHOD_DIRECT, METHOD_FAST = 0, 1, 2
+PARAM_OMEGA, PARAM_IEXT = 0, 1
+OBS_PHASE, OBS_GLOBAL_ORDER, OBS_LOCAL_ORDER, OBS_MEAN_PHASE_VELOCITY, OBS_STATS = 0, 1, 2, 3, 4
+NVAR = {MODEL_KS: 1, MODEL_FHN: 2, MODEL_HH: 4}
+
+ABI_SYMBOLS = [
+    "net_workspace_bytes", "net_create", "net_destroy", "net_set_state", "net_get_state",
+    "net_set_param_array", "net_hh_steady_gates", "net_integrate", "net_integrate_observed",
+    "net_eval_rhs", "net_observables", "net_get_topology", "net_get_degree", "net_get_time",
+    "net_set_time", "net_get_counters", "net_synchronize", "net_last_error", "net_version",
+]
+
+
+class KSParams(C.Structure):
+    _fields_ = [("K", C.c_double), ("alpha", C.c_double), ("omega0", C.c_double)]
+
+
+class FHNParams(C.Structure):
+    _fields_ = [("eps", C.c_double), ("a", C.c_double), ("sigma", C.c_double), ("phi", C.c_double)]
+
+
+class HHParams(C.Structure):
+    _fields_ = [(k, C.c_double) for k in
+                ("gNa", "gK", "gL", "ENa", "EK", "EL", "C", "g_syn", "E_syn", "theta_syn", "k_syn",
+                 "I_ext0", "V_c", "n_c", "V_s")]
+
+
+HH_PHASE_MAP = dict(V_c=-20.0, n_c=0.55, V_s=100.0)
+
+
+class Topology(C.Structure):
+    _fields_ = [("kind", C.c_int32), ("ndim", C.c_int32), ("extent", C.c_int64 * 3),
+                ("radius", C.c_int32), ("include_self", C.c_int32), ("row_ptr", C.c_void_p),
+                ("col_idx", C.c_void_p), ("nnz", C.c_int64), ("ptrs_are_device", C.c_int32),
+                ("in_degree", C.c_int32), ("seed", C.c_uint64)]
+
+
+class Desc(C.Structure):
+    _fields_ = [("model", C.c_int32), ("dtype", C.c_int32), ("n", C.c_int64), ("batch", C.c_int32),
+                ("method", C.c_int32), ("topo", Topology)]
+
+
+class OscnetError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__("oscnet error %d: %s" % (code, msg))
+        self.code = code
+
+
+_lib = None
+
+
+def lib():
+    """Loads liboscnet.so; raises if it has not been built (no fallback)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise OSError("liboscnet.so is missing: run `python -m paper_2410_19075_b200.build` "
+                          "(the product path has no CPU fallback)")
+        L = C.CDLL(LIB_PATH)
+        L.net_last_error.restype = C.c_char_p
+        L.net_last_error.argtypes = [C.c_void_p]
+        L.net_version.restype = C.c_char_p
+        L.net_workspace_bytes.argtypes = [C.POINTER(Desc), C.POINTER(C.c_size_t)]
+        L.net_create.argtypes = [C.POINTER(Desc), C.c_void_p, C.c_size_t, C.c_void_p, C.c_size_t,
+                                 C.c_void_p, C.POINTER(C.c_void_p)]
+        L.net_destroy.argtypes = [C.c_void_p]
+        L.net_set_state.argtypes = [C.c_void_p, C.c_void_p, C.c_int32]
+        L.net_get_state.argtypes = [C.c_void_p, C.c_void_p, C.c_int32]
+        L.net_set_param_array.argtypes = [C.c_void_p, C.c_int32, C.c_void_p, C.c_int32]
+        L.net_hh_steady_gates.argtypes = [C.c_void_p]
+        L.net_integrate.argtypes = [C.c_void_p, C.c_int64, C.c_double]
+        L.net_integrate_observed.argtypes = [C.c_void_p, C.c_int64, C.c_double, C.c_int64]
+        L.net_eval_rhs.argtypes = [C.c_void_p, C.c_void_p, C.c_int32]
+        L.net_observables.argtypes = [C.c_void_p, C.c_int32, C.c_void_p, C.c_int32]
+        L.net_get_topology.argtypes = [C.c_void_p, C.c_int64, C.c_int64, C.c_void_p, C.c_void_p,
+                                       C.c_int32]
+        L.net_get_degree.argtypes = [C.c_void_p, C.POINTER(C.c_int64), C.POINTER(C.c_int32)]
+        L.net_get_time.argtypes = [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_int64)]
+        L.net_set_time.argtypes = [C.c_void_p, C.c_double, C.c_int64]
+        L.net_get_counters.argtypes = [C.c_void_p, C.POINTER(C.c_int64), C.POINTER(C.c_int32)]
+        L.net_synchronize.argtypes = [C.c_void_p]
+        for name in ABI_SYMBOLS:
+            if name not in ("net_last_error", "net_version"):
+                getattr(L, name).restype = C.c_int32
+        _lib = L
+    return _lib
+
+
+def _check(rc, handle=None):
+    if rc != NET_OK:
+        msg = lib().net_last_error(handle)
+        raise OscnetError(rc, msg.decode() if msg else "")
+
+
+# ---------------------------------------------------------------- C-ABI mirrors
+def net_version():
+    return lib().net_version().decode()
+
+
+def net_workspace_bytes(desc):
+    out = C.c_size_t()
+    _check(lib().net_workspace_bytes(C.byref(desc), C.byref(out)))
+    return out.value
+
+
+def net_create(desc, params, workspace_ptr, workspace_bytes, stream_ptr):
+    h = C.c_void_p()
+    _check(lib().net_create(C.byref(desc), C.byref(params), C.sizeof(params), workspace_ptr,
+                            workspace_bytes, stream_ptr, C.byref(h)))
+    return h
+
+
+def net_destroy(h):
+    _check(lib().net_destroy(h))
+
+
+def net_set_state(h, ptr, is_device):
+    _check(lib().net_set_state(h, ptr, int(is_device)), h)
+
+
+def net_get_state(h, ptr, is_device):
+    _check(lib().net_get_state(h, ptr, int(is_device)), h)
+
+
+def net_set_param_array(h, which, ptr, is_device):
+    _check(lib().net_set_param_array(h, which, ptr, int(is_device)), h)
+
+
+def net_hh_steady_gates(h):
+    _check(lib().net_hh_steady_gates(h), h)
+
+
+def net_integrate(h, n_steps, dt):
+    _check(lib().net_integrate(h, n_steps, dt), h)
+
+
+def net_integrate_observed(h, n_steps, dt, obs_every):
+    _check(lib().net_integrate_observed(h, n_steps, dt, obs_every), h)
+
+
+def net_eval_rhs(h, ptr, is_device):
+    _check(lib().net_eval_rhs(h, ptr, int(is_device)), h)
+
+
+def net_observables(h, what, ptr, is_device):
+    _check(lib().net_observables(h, what, ptr, int(is_device)), h)
+
+
+def net_get_topology(h, row_begin, row_count, row_ptr_ptr, col_idx_ptr, is_device):
+    _check(lib().net_get_topology(h, row_begin, row_count, row_ptr_ptr, col_idx_ptr,
+                                  int(is_device)), h)
+
+
+def net_get_degree(h):
+    nnz, deg = C.c_int64(), C.c_int32()
+    _check(lib().net_get_degree(h, C.byref(nnz), C.byref(deg)), h)
+    return nnz.value, deg.value
+
+
+def net_get_time(h):
+    t, s = C.c_double(), C.c_int64()
+    _check(lib().net_get_time(h, C.byref(t), C.byref(s)), h)
+    return t.value, s.value
+
+
+def net_set_time(h, t, step):
+    _check(lib().net_set_time(h, t, step), h)
+
+
+def net_get_counters(h):
+    k, m = C.c_int64(), C.c_int32()
+    _check(lib().net_get_counters(h, C.byref(k), C.byref(m)), h)
+    return k.value, m.value
+
+
+def net_synchronize(h):
+    _check(lib().net_synchronize(h), h)
+
+
+# ------------------------------------------------------------------ convenience
+def make_params(model, p):
+    if model == MODEL_KS:
+        return KSParams(p["K"], p["alpha"], p.get("omega0", 0.0))
+    if model == MODEL_FHN:
+        return FHNParams(p["eps"], p["a"], p["sigma"], p["phi"])
+    q = dict(HH_PHASE_MAP, I_ext0=0.0)
+    q.update(p)
+    return HHParams(*[q[k] for k, _ in HHParams._fields_])
+
+
+def _np_dtype(dtype):
+    return np.float32 if dtype == F32 else np.float64
+
+
+class Net:
+    """Owns a workspace tensor and a handle; methods mirror the C ABI."""
+
+    def __init__(self, model, dtype, n, topo, params, method=METHOD_AUTO, device="cuda:0",
+                 stream=None):
+        import torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("oscnet needs a CUDA device (no CPU fallback)")
+        self.torch = torch
+        self.device = torch.device(device)
+        self.model, self.dtype, self.n = model, dtype, int(n)
+        self.nvar = NVAR[model]
+        self.np_dtype = _np_dtype(dtype)
+        self.torch_dtype = torch.float32 if dtype == F32 else torch.float64
+        d = Desc()
+        d.model, d.dtype, d.n, d.batch, d.method = model, dtype, self.n, 1, method
+        t = d.topo
+        t.kind = topo["kind"]
+        ext = list(topo.get("extent", ())) + [1, 1, 1]
+        t.ndim = len(topo.get("extent", ())) or 1
+        for q in range(3):
+            t.extent[q] = ext[q]
+        t.radius = topo.get("radius", 0)
+        t.include_self = int(topo.get("include_self", False))
+        t.in_degree = topo.get("in_degree", 0)
+        t.seed = topo.get("seed", 0)
+        self._keep = []
+        if t.kind == TOPO_CSR:
+            rp, ci = topo["row_ptr"], topo["col_idx"]
+            if isinstance(rp, np.ndarray):
+                rp = np.ascontiguousarray(rp, dtype=np.int64)
+                ci = np.ascontiguousarray(ci, dtype=np.int32)
+                t.row_ptr, t.col_idx = rp.ctypes.data, ci.ctypes.data
+                t.nnz, t.ptrs_are_device = int(rp[-1]), 0
+            else:
+                t.row_ptr, t.col_idx = rp.data_ptr(), ci.data_ptr()
+                t.nnz, t.ptrs_are_device = int(ci.numel()), 1
+            self._keep += [rp, ci]
+        self.desc = d
+        self.params = make_params(model, params)
+        with torch.cuda.device(self.device):
+            # a stream of its own: the legacy default stream cannot be captured into a CUDA graph
+            self.stream = stream or torch.cuda.Stream(device=self.device)
+            self.stream.wait_stream(torch.cuda.current_stream())
+            self.workspace_bytes = net_workspace_bytes(d)
+            self.workspace = torch.empty(self.workspace_bytes + 256, dtype=torch.uint8,
+                                         device=self.device)
+            self.workspace.record_stream(self.stream)
+            base = (self.workspace.data_ptr() + 255) // 256 * 256
+            self.h = net_create(d, self.params, base, self.workspace_bytes,
+                                self.stream.cuda_stream)
+
+    @classmethod
+    def from_workload(cls, w, method=METHOD_AUTO, device="cuda:0", stream=None):
+        from . import configs
+        dtype = F32 if w.dtype == "f32" else F64
+        if w.topo == configs.RING:
+            topo = dict(kind=TOPO_RING, radius=w.radius)
+        elif w.topo == configs.LATTICE:
+            topo = dict(kind=TOPO_LATTICE, extent=w.extent, radius=w.radius)
+        else:
+            topo = dict(kind=TOPO_RANDOM_INDEGREE, in_degree=w.in_degree, seed=w.topo_seed)
+        return cls(w.model, dtype, w.n, topo, w.params, method=method, device=device,
+                   stream=stream)
+
+    def close(self):
+        if getattr(self, "h", None):
+            net_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # state --------------------------------------------------------------------
+    def _ptr(self, x):
+        """(pointer, is_device) of a numpy array or torch tensor (must be contiguous)."""
+        if isinstance(x, np.ndarray):
+            assert x.flags["C_CONTIGUOUS"]
+            return x.ctypes.data, False
+        assert x.is_contiguous()
+        if x.is_cuda:       # order the net's stream after the producer of the tensor
+            self.stream.wait_stream(self.torch.cuda.current_stream())
+            x.record_stream(self.stream)
+        return x.data_ptr(), x.is_cuda
+
+    def _publish(self, x):
+        """Makes torch's current stream wait for a device-side result written on the net's stream."""
+        if not isinstance(x, np.ndarray) and x.is_cuda:
+            self.torch.cuda.current_stream().wait_stream(self.stream)
+
+    def set_state(self, y):
+        if isinstance(y, np.ndarray):
+            y = np.ascontiguousarray(y, dtype=self.np_dtype).reshape(self.nvar, self.n)
+        else:
+            assert y.dtype == self.torch_dtype and y.numel() == self.nvar * self.n
+        net_set_state(self.h, *self._ptr(y))
+
+    def get_state(self, out=None):
+        if out is None:
+            out = np.empty((self.nvar, self.n), dtype=self.np_dtype)
+        net_get_state(self.h, *self._ptr(out))
+        self._publish(out)
+        return out
+
+    def set_param_array(self, which, x):
+        if isinstance(x, np.ndarray):
+            x = np.ascontiguousarray(x, dtype=self.np_dtype)
+        net_set_param_array(self.h, which, *self._ptr(x))
+
+    def hh_steady_gates(self):
+        net_hh_steady_gates(self.h)
+
+    # dynamics -----------------------------------------------------------------
+    def integrate(self, n_steps, dt):
+        net_integrate(self.h, int(n_steps), float(dt))
+
+    def integrate_observed(self, n_steps, dt, obs_every):
+        net_integrate_observed(self.h, int(n_steps), float(dt), int(obs_every))
+        st = np.empty(8)
+        net_observables(self.h, OBS_STATS, st.ctypes.data, False)
+        return dict(R_mean=st[0], R_std=st[1], Rloc_mean=st[2], vel_mean=st[3], vel_std=st[4],
+                    n_samples=int(st[5]), t_a=st[6], t_b=st[7])
+
+    def eval_rhs(self, out=None):
+        if out is None:
+            out = np.empty((self.nvar, self.n), dtype=self.np_dtype)
+        net_eval_rhs(self.h, *self._ptr(out))
+        self._publish(out)
+        return out
+
+    def observable(self, what):
+        size = 2 if what == OBS_GLOBAL_ORDER else 8 if what == OBS_STATS else self.n
+        out = np.empty(size)
+        net_observables(self.h, what, out.ctypes.data, False)
+        return out
+
+    def get_topology(self, row_begin=0, row_count=None):
+        row_count = self.n - row_begin if row_count is None else row_count
+        nnz, deg = net_get_degree(self.h)
+        rp = np.empty(row_count + 1, dtype=np.int64)
+        if deg >= 0:
+            cnt = row_count * deg
+        else:       # general CSR: ask for the pointers first
+            full = np.empty(1, dtype=np.int64)
+            cnt = nnz
+        ci = np.empty(max(cnt, 1), dtype=np.int32)
+        net_get_topology(self.h, row_begin, row_count, rp.ctypes.data, ci.ctypes.data, False)
+        return rp, ci[:rp[-1]]
+
+    def degree(self):
+        return net_get_degree(self.h)
+
+    def time(self):
+        return net_get_time(self.h)
+
+    def counters(self):
+        return net_get_counters(self.h)
+
+    def synchronize(self):
+        net_synchronize(self.h)

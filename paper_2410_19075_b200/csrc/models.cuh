@@ -1,0 +1,132 @@
+// Local vector fields of the three model classes (device functions, T = float | double).
+// Equations: include/oscnet.h (net_*_params) and PAPER.md eq. (1)-(3).
+#pragma once
+#include "oscnet_internal.cuh"
+
+namespace oscnet {
+
+template <class T> struct Math;
+template <> struct Math<double> {
+    static __device__ __forceinline__ double exp(double x) { return ::exp(x); }
+    static __device__ __forceinline__ double expm1(double x) { return ::expm1(x); }
+    static __device__ __forceinline__ double sin(double x) { return ::sin(x); }
+    static __device__ __forceinline__ void sincos(double x, double* s, double* c) { ::sincos(x, s, c); }
+    static __device__ __forceinline__ double abs(double x) { return ::fabs(x); }
+};
+template <> struct Math<float> {
+    static __device__ __forceinline__ float exp(float x) { return ::expf(x); }
+    static __device__ __forceinline__ float expm1(float x) { return ::expm1f(x); }
+    static __device__ __forceinline__ float sin(float x) { return ::sinf(x); }
+    static __device__ __forceinline__ void sincos(float x, float* s, float* c) { ::sincosf(x, s, c); }
+    static __device__ __forceinline__ float abs(float x) { return ::fabsf(x); }
+};
+
+// ----------------------------------------------------------------- Kuramoto
+// Direct form: f = omega + (K/Omega) * sum_j sin(phi_j - phi_i - alpha); `sum` is that sum.
+template <class T>
+__device__ __forceinline__ T ks_rhs_direct(const ModelParams& mp, T omega, T sum, T inv_deg) {
+    return omega + T(mp.K) * inv_deg * sum;
+}
+// Factorised form: with C = sum_j cos phi_j, S = sum_j sin phi_j and (ci, si) = (cos, sin) phi_i,
+//   sum_j sin(phi_j - phi_i - alpha) = S cos(phi_i+alpha) - C sin(phi_i+alpha).
+template <class T>
+__device__ __forceinline__ T ks_rhs_factorised(const ModelParams& mp, T omega, T C, T S, T ci,
+                                               T si, T inv_deg) {
+    T ca = T(mp.cos_a), sa = T(mp.sin_a);
+    T cia = ci * ca - si * sa;  // cos(phi_i + alpha)
+    T sia = si * ca + ci * sa;  // sin(phi_i + alpha)
+    return omega + T(mp.K) * inv_deg * (S * cia - C * sia);
+}
+
+// ---------------------------------------------------------- FitzHugh-Nagumo
+// Cu = sum_j (u_j - u_i), Cv = sum_j (v_j - v_i).
+template <class T>
+__device__ __forceinline__ void fhn_rhs(const ModelParams& mp, T u, T v, T Cu, T Cv, T inv_deg,
+                                        T* fu, T* fv) {
+    T s = T(mp.sigma) * inv_deg;
+    *fu = (u - u * u * u * T(1.0 / 3.0) - v + s * (T(mp.buu) * Cu + T(mp.buv) * Cv)) * T(mp.inv_eps);
+    *fv = u + T(mp.a) + s * (T(mp.bvu) * Cu + T(mp.bvv) * Cv);
+}
+
+// ----------------------------------------------------------- Hodgkin-Huxley
+// x/(1-exp(-x/10)) with the removable singularity at 0 (reading R10).
+template <class T>
+__device__ __forceinline__ T hh_vtrap(T x) {
+    T r = x * T(0.1);
+    if (Math<T>::abs(r) < T(1e-9)) return T(10);
+    return -x / Math<T>::expm1(-r);
+}
+
+template <class T>
+__device__ __forceinline__ void hh_rates(T V, T* am, T* bm, T* ah, T* bh, T* an, T* bn) {
+    *am = T(0.1) * hh_vtrap<T>(V + T(40));
+    *bm = T(4) * Math<T>::exp(-(V + T(65)) * T(1.0 / 18.0));
+    *ah = T(0.07) * Math<T>::exp(-(V + T(65)) * T(1.0 / 20.0));
+    *bh = T(1) / (T(1) + Math<T>::exp(-(V + T(35)) * T(0.1)));
+    *an = T(0.01) * hh_vtrap<T>(V + T(55));
+    *bn = T(0.125) * Math<T>::exp(-(V + T(65)) * T(1.0 / 80.0));
+}
+
+template <class T>
+__device__ __forceinline__ T hh_syn_activation(const ModelParams& mp, T V) {
+    return T(1) / (T(1) + Math<T>::exp(-(V - T(mp.theta_syn)) * T(mp.inv_k_syn)));
+}
+
+// ssum = sum_j S(V_j) over the in-neighbours.
+template <class T>
+__device__ __forceinline__ void hh_rhs(const ModelParams& mp, T V, T m, T h, T g, T Iext, T ssum,
+                                       T inv_deg, T* fV, T* fm, T* fh, T* fg) {
+    T am, bm, ah, bh, an, bn;
+    hh_rates<T>(V, &am, &bm, &ah, &bh, &an, &bn);
+    T INa = T(mp.gNa) * m * m * m * h * (V - T(mp.ENa));
+    T g2 = g * g;
+    T IK = T(mp.gK) * g2 * g2 * (V - T(mp.EK));
+    T IL = T(mp.gL) * (V - T(mp.EL));
+    T Isyn = T(mp.g_syn) * inv_deg * (T(mp.E_syn) - V) * ssum;
+    *fV = (Iext - INa - IK - IL + Isyn) * T(mp.inv_C);
+    *fm = am * (T(1) - m) - bm * m;
+    *fh = ah * (T(1) - h) - bh * h;
+    *fg = an * (T(1) - g) - bn * g;
+}
+
+// --------------------------------------------------------------- neighbours
+// Calls f(j) for every in-neighbour j of element i, and returns the in-degree.
+template <int TOPO, class F>
+__device__ __forceinline__ int for_each_neighbor(const TopoView& tv, int64_t n, int64_t i, F&& f) {
+    if (TOPO == NET_TOPO_RING) {
+        int P = tv.P;
+        for (int d = -P; d <= P; ++d) {
+            if (d == 0 && !tv.include_self) continue;
+            int64_t j = i + d;
+            if (j < 0) j += n;
+            if (j >= n) j -= n;
+            f(j);
+        }
+        return 2 * P + (tv.include_self ? 1 : 0);
+    } else if (TOPO == NET_TOPO_LATTICE) {
+        int nx = tv.nx, ny = tv.ny, nz = tv.nz;
+        int x = (int)(i % nx);
+        int64_t r = i / nx;
+        int y = (int)(r % ny);
+        int z = (int)(r / ny);
+        for (int q = 0; q < tv.noff; ++q) {
+            int xx = x + tv.off[3 * q], yy = y + tv.off[3 * q + 1], zz = z + tv.off[3 * q + 2];
+            xx += (xx < 0) ? nx : 0; xx -= (xx >= nx) ? nx : 0;
+            yy += (yy < 0) ? ny : 0; yy -= (yy >= ny) ? ny : 0;
+            zz += (zz < 0) ? nz : 0; zz -= (zz >= nz) ? nz : 0;
+            f(((int64_t)zz * ny + yy) * nx + xx);
+        }
+        return tv.noff;
+    } else if (TOPO == NET_TOPO_CSR) {
+        int64_t b = tv.row_ptr[i], e = tv.row_ptr[i + 1];
+        for (int64_t q = b; q < e; ++q) f((int64_t)tv.col_idx[q]);
+        return (int)(e - b);
+    } else {
+        int k = tv.k_uniform;
+        const int32_t* row = tv.col_idx + i * (int64_t)k;
+        for (int q = 0; q < k; ++q) f((int64_t)row[q]);
+        return k;
+    }
+}
+
+}  // namespace oscnet

@@ -1,0 +1,164 @@
+// Internal declarations shared by the translation units of liboscnet.so.
+// Nothing here is part of the C ABI (include/oscnet.h is).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stdio.h>
+#include <string.h>
+
+#include "../../include/oscnet.h"
+
+namespace oscnet {
+
+// ---------------------------------------------------------------- parameters
+// Model parameters as passed to kernels (always double; kernels convert to T).
+struct ModelParams {
+    // KS
+    double K, alpha, sin_a, cos_a;
+    // FHN
+    double inv_eps, a, sigma, buu, buv, bvu, bvv;
+    // HH
+    double gNa, gK, gL, ENa, EK, EL, inv_C, g_syn, E_syn, theta_syn, inv_k_syn;
+    double V_c, n_c, inv_V_s;
+};
+
+// Topology as seen by kernels.
+struct TopoView {
+    int32_t kind;          // NET_TOPO_*
+    int32_t ndim;
+    int32_t nx, ny, nz;    // lattice extents (1 for unused dims)
+    int32_t P;             // ring: neighbours per side; lattice: Euclidean radius
+    int32_t include_self;
+    int32_t noff;          // lattice: number of offsets (= Omega)
+    int32_t k_uniform;     // RANDOM_INDEGREE: in-degree; else 0
+    const int32_t* off;    // lattice: noff x (dx,dy,dz), sorted by (dz,dy,dx)
+    const int64_t* row_ptr;
+    const int32_t* col_idx;
+};
+
+// RK4 in the low-traffic form: four state-sized arrays
+// y, Y2, Y3, Y4; no separate accumulator.
+//   stage 0: Y2 = y + dt/2 f(y)      stage 1: Y3 = y + dt/2 f(Y2)
+//   stage 2: Y4 = y + dt   f(Y3)     stage 3: y  = (Y2 + 2 Y3 + Y4 - y)/3 + dt/6 f(Y4)
+//   stage 4 (RHS only): out = f(in)
+enum { STAGE_RHS_ONLY = 4 };
+
+struct StageArgs {
+    const void* in;   // array the RHS is evaluated on (stencil source)
+    const void* y;    // base state
+    const void* Y2;
+    const void* Y3;
+    void* out;
+    const void* elem_param;  // omega / I_ext, may be null
+    const void* s_in;        // HH fast path: S(V) of `in`
+    void* s_out;             // HH fast path: S(V) of `out`
+    int64_t n, ld;
+    double dt;
+    int32_t stage;
+};
+
+template <class T>
+__device__ __forceinline__ T stage_combine(int stage, T dt, T k, T y, T Y2, T Y3, T Y4in) {
+    // Y4in is the value of the stage input at this element (only used in stage 3).
+    switch (stage) {
+        case 0:
+        case 1: return y + (T(0.5) * dt) * k;
+        case 2: return y + dt * k;
+        case 3: return (Y2 + T(2) * Y3 + Y4in - y) * T(1.0 / 3.0) + (dt * T(1.0 / 6.0)) * k;
+        default: return k;
+    }
+}
+
+// ------------------------------------------------------------------- handle
+struct Buffers {
+    void *y, *Y2, *Y3, *Y4;       // nvar*ld elements each
+    void* elem_param;             // ld elements
+    void *s_y, *s_Y2, *s_Y3, *s_Y4;  // HH fast path, ld elements each (else null)
+    int32_t* off;                 // lattice offsets
+    int64_t* row_ptr;
+    int32_t* col_idx;
+    int32_t* flag;                // device error/validation flag (4 ints)
+    // observables
+    double* obs_theta_prev;       // n
+    double* obs_wind;             // n
+    double* obs_ref;              // n (KS: phi at t_a)
+    double* obs_vel;              // n
+    double* obs_tmp;              // 2n (cos/sin of theta) -- also local-order scratch
+    double* obs_loc;              // n
+    double* obs_partial;          // reduction partials (4096 doubles)
+    double* obs_acc;              // small accumulator block (16 doubles)
+    void* scratch;                // method-specific scratch
+    size_t scratch_bytes;
+};
+
+}  // namespace oscnet
+
+struct net {
+    net_desc desc;
+    int32_t nvar;
+    int32_t esize;
+    int64_t n, ld;
+    cudaStream_t stream;
+    oscnet::ModelParams mp;
+    oscnet::TopoView tv;
+    oscnet::Buffers b;
+    int32_t method;        // NET_METHOD_DIRECT or NET_METHOD_FAST actually in use
+    int32_t fast_kind;     // which fast kernel family (internal)
+    int64_t nnz;
+    int32_t degree_uniform;
+    // step driver
+    cudaGraphExec_t graph_exec;
+    cudaGraph_t graph;
+    double graph_dt;
+    int32_t graph_steps;
+    int64_t graph_kernels;
+    int64_t step;
+    double t;
+    int64_t launches;
+    // observed-run results (host copies)
+    double stats[8];
+    int stats_valid;
+    int s_valid;           // HH fast path: s_y consistent with y
+    char err[512];
+};
+
+namespace oscnet {
+
+// error helpers -------------------------------------------------------------
+int32_t set_err(net* h, int32_t code, const char* fmt, ...);
+int32_t cuda_err(net* h, cudaError_t e, const char* what);
+#define OSC_CUDA(h, call)                                            \
+    do {                                                             \
+        cudaError_t e_ = (call);                                     \
+        if (e_ != cudaSuccess) return oscnet::cuda_err(h, e_, #call); \
+    } while (0)
+
+// topology.cu ---------------------------------------------------------------
+int32_t topo_lattice_noff(int ndim, int P, int include_self);
+int32_t topo_build(net* h);   // fills workspace topology from h->desc
+int32_t topo_expand(net* h, int64_t row_begin, int64_t row_count, int64_t* d_row_ptr,
+                    int32_t* d_col_idx);  // device destinations
+
+// direct.cu -----------------------------------------------------------------
+int32_t direct_stage(net* h, const StageArgs& a);
+int32_t hh_compute_s(net* h, const void* V, void* s);     // s = S(V)
+int32_t hh_steady_gates(net* h);
+
+// csr_fast.cu / lattice_fast.cu / ring_fast.cu ------------------------------
+enum { FAST_NONE = 0, FAST_CSR_WARP = 1, FAST_LATTICE3D = 2, FAST_RING_FHN = 3, FAST_RING_KS = 4 };
+int32_t fast_select(const net_desc* d);                   // FAST_* available for this desc
+size_t fast_scratch_bytes(const net_desc* d, int32_t fast_kind);
+int32_t fast_stage(net* h, const StageArgs& a);
+int32_t fast_integrate(net* h, int64_t n_steps, double dt, bool* handled);  // persistent kernels
+
+// observables.cu ------------------------------------------------------------
+int32_t obs_phase(net* h, const void* state, double* d_theta);
+int32_t obs_global_order(net* h, const double* d_theta, double* d_out2);  // {R, Psi}
+int32_t obs_local_order(net* h, const double* d_theta, double* d_out);
+int32_t obs_window_begin(net* h);
+int32_t obs_window_sample(net* h, int first);
+int32_t obs_window_finish(net* h, double t_a, double t_b, int64_t n_samples);
+
+inline int64_t round_up(int64_t x, int64_t m) { return (x + m - 1) / m * m; }
+
+}  // namespace oscnet

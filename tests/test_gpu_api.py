@@ -1,0 +1,74 @@
+"""Edge cases and error behaviour of the C ABI on a GPU."""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+
+def _B():
+    from paper_2410_19075_b200 import binding
+    return binding
+
+
+def test_state_roundtrip_unaligned_n_and_device_pointers():
+    import torch
+    B = _B()
+    n = 1001                                     # not a multiple of the internal stride
+    net = B.Net(B.MODEL_HH, B.F32, n, dict(kind=B.TOPO_RING, radius=2), dict(
+        gNa=120.0, gK=36.0, gL=0.3, ENa=50.0, EK=-77.0, EL=-54.4, C=1.0, g_syn=0.1, E_syn=0.0,
+        theta_syn=0.0, k_syn=2.0))
+    y = np.random.default_rng(0).normal(size=(4, n)).astype(np.float32)
+    net.set_state(y)
+    assert np.array_equal(net.get_state(), y)
+    yd = torch.from_numpy(y * 2).cuda()
+    net.set_state(yd)
+    out = torch.empty_like(yd)
+    net.get_state(out)
+    torch.cuda.synchronize()
+    assert torch.equal(out, yd)
+    pinned = torch.empty((4, n), dtype=torch.float32).pin_memory()
+    net.get_state(pinned)
+    assert np.array_equal(pinned.numpy(), y * 2)
+
+
+def test_degenerate_networks():
+    B = _B()
+    # one element, no neighbours: pure local dynamics; KS: phi(t) = phi0 + omega t
+    net = B.Net(B.MODEL_KS, B.F64, 1, dict(kind=B.TOPO_RING, radius=0), dict(K=1.0, alpha=0.3, omega0=0.5))
+    net.set_state(np.array([[0.25]]))
+    net.integrate(100, 0.01)
+    assert abs(net.get_state()[0, 0] - 0.75) < 1e-13
+    # zero steps is a no-op; in-degree 0 graph
+    net.integrate(0, 0.01)
+    assert net.time() == (1.0, 100) or abs(net.time()[0] - 1.0) < 1e-12
+    g = B.Net(B.MODEL_FHN, B.F64, 50, dict(kind=B.TOPO_RANDOM_INDEGREE, in_degree=0, seed=1),
+              dict(eps=0.05, a=0.5, sigma=0.1, phi=0.2))
+    y = np.stack([np.full(50, -0.5), np.full(50, -0.5 + 0.125 / 3)])
+    g.set_state(y)
+    assert np.abs(g.eval_rhs()).max() < 1e-14          # the FHN fixed point
+
+
+def test_errors_are_reported_not_thrown():
+    B = _B()
+    with pytest.raises(B.OscnetError) as e:
+        B.Net(B.MODEL_KS, B.F64, 10, dict(kind=B.TOPO_RING, radius=5), dict(K=1.0, alpha=0.0))
+    assert e.value.code == -1
+    with pytest.raises(B.OscnetError):
+        B.Net(B.MODEL_KS, B.F64, 64, dict(kind=B.TOPO_LATTICE, extent=(4, 4, 4), radius=2), dict(K=1.0, alpha=0.0))
+    net = B.Net(B.MODEL_KS, B.F64, 10, dict(kind=B.TOPO_RING, radius=2), dict(K=1.0, alpha=0.0))
+    with pytest.raises(B.OscnetError):
+        net.set_param_array(B.PARAM_IEXT, np.zeros(10))
+    with pytest.raises(B.OscnetError):
+        net.hh_steady_gates()
+    with pytest.raises(B.OscnetError):
+        net.integrate_observed(10, 0.1, 3)
+    with pytest.raises(B.OscnetError):
+        net.observable(B.OBS_STATS)
+    # workspace too small / misaligned
+    import torch
+    ws = torch.empty(1024, dtype=torch.uint8, device="cuda")
+    with pytest.raises(B.OscnetError) as e:
+        B.net_create(net.desc, net.params, ws.data_ptr(), 1024, 0)
+    assert e.value.code == -2
+    launches, method = net.counters()
+    assert launches >= 1 and method in (B.METHOD_DIRECT, B.METHOD_FAST)
