@@ -1,0 +1,372 @@
+#!/usr/bin/env python
+"""bench.py -- oscillator-steps/s of the fused RK4 hot path on B200, against its roofline.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 5] [--impl ours|reference]
+                    [--no-per-config] [--no-cpu-baseline]
+
+One bench "step" = one output interval of the workload = `obs_every` RK4 steps (4 fused stage
+kernels each) of net_integrate over the whole network.  `value` = N x RK4 steps / s with the
+state resident in HBM; `e2e` = the same through the C ABI with HOST buffers (net_set_state from
+pinned memory + net_integrate + net_get_state to pinned memory inside the timed region).
+The headline workload is config 5 (the metric is quoted per config;
+config 5 is the largest one and has a clean HBM roofline); `per_config` carries the same
+measurement for every other north-star config.  N > 1 GPUs = independent replicas (weak
+scaling, no collective on the data path).  `--impl reference` times the CPU oracle, as it
+stands, on a bounded sample of the same workload.
+"""
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "oscillator-steps/s"
+HEADLINE = "5"
+PER_CONFIG = ("1", "2", "3a", "3b", "4", "5")
+
+
+# ------------------------------------------------------------------ inputs
+def make_inputs(w, seed=1):
+    """Seeded synthetic inputs of DESIGN.md "Input recipe" (numpy only; HH gates are set to
+    their steady state by the consumer)."""
+    import numpy as np
+    from paper_2410_19075_b200 import configs, inputs
+    dt = np.float32 if w.dtype == "f32" else np.float64
+    elem = None
+    if w.model == configs.KS:
+        y0 = inputs.ks_phases(w.n, seed).reshape(1, -1)
+        if w.extra.get("omega") == "lorentzian":
+            elem = inputs.lorentzian_omega(w.n, seed, w.extra["gamma"], w.extra["omega_max"])
+    elif w.model == configs.FHN:
+        y0 = inputs.fhn_circle(w.n, seed)
+    else:
+        V = inputs.hh_voltage(w.n, seed)
+        y0 = np.zeros((4, w.n))
+        y0[0] = V
+        elem = inputs.hh_current(w.n, seed)
+    return np.ascontiguousarray(y0.astype(dt)), None if elem is None else elem.astype(dt)
+
+
+# ------------------------------------------------------------------ clocks
+class ClockSampler:
+    """Samples SM clock and throttle reasons of one GPU through NVML while the timed region runs."""
+
+    REASONS = {0x4: "sw_power_cap", 0x8: "hw_slowdown", 0x20: "sw_thermal_slowdown",
+               0x40: "hw_thermal_slowdown", 0x80: "hw_power_brake_slowdown"}
+
+    def __init__(self, device_index):
+        self.samples, self.mask, self.max_mhz, self.ok = [], 0, None, False
+        self._stop = threading.Event()
+        try:
+            import pynvml
+            import torch
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            try:
+                uuid = "GPU-" + str(torch.cuda.get_device_properties(device_index).uuid)
+                self.h = pynvml.nvmlDeviceGetHandleByUUID(uuid)
+            except Exception:
+                self.h = pynvml.nvmlDeviceGetHandleByIndex(device_index)
+            self.max_mhz = float(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+            self.ok = True
+        except Exception as e:      # no NVML: report that, never fake a clock
+            self.err = repr(e)
+
+    def _one(self):
+        try:
+            self.samples.append(float(self.nv.nvmlDeviceGetClockInfo(self.h, self.nv.NVML_CLOCK_SM)))
+            self.mask |= int(self.nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h))
+        except Exception:
+            pass
+
+    def _run(self):
+        while not self._stop.is_set():
+            self._one()
+            self._stop.wait(0.02)
+
+    def __enter__(self):
+        if self.ok:
+            self.t = threading.Thread(target=self._run, daemon=True)
+            self.t.start()
+        return self
+
+    def __exit__(self, *a):
+        if self.ok:
+            self._stop.set()
+            self.t.join()
+            self._one()
+
+    def summary(self):
+        if not self.ok or not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": ["nvml_unavailable"]}
+        s = sorted(self.samples)
+        reasons = [n for b, n in self.REASONS.items() if self.mask & b]
+        return {"sm_mhz": s[len(s) // 2], "sm_max_mhz": self.max_mhz, "reasons": reasons,
+                "samples": len(s)}
+
+
+# ------------------------------------------------------------------ our arm
+def build_net(w, device, seed=1):
+    from paper_2410_19075_b200 import binding as B, configs
+    y0, elem = make_inputs(w, seed)
+    net = B.Net.from_workload(w, device=device)
+    net.set_state(y0)
+    if elem is not None:
+        net.set_param_array(B.PARAM_OMEGA if w.model == configs.KS else B.PARAM_IEXT, elem)
+    if w.model == configs.HH:
+        net.hh_steady_gates()
+        y0 = net.get_state()                # full initial state (gates included) for the e2e leg
+    return net, y0
+
+
+def measure(w, device, steps, warmup, e2e=True, seed=1):
+    """Times `steps` bench steps (each = w.obs_every RK4 steps) after `warmup` untimed ones.
+    Returns device-resident ms, e2e ms, launches and byte counts."""
+    import torch
+    from paper_2410_19075_b200 import replicas
+    net, y0 = build_net(w, device, seed)
+    S = w.obs_every
+    stream = net.stream
+    for _ in range(warmup):
+        net.integrate(S, w.dt)
+    net.synchronize()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    l0 = net.counters()[0]
+    with ClockSampler(torch.device(device).index or 0) as clk:
+        replicas.barrier()
+        torch.cuda.synchronize()
+        ev0.record(stream)
+        for _ in range(steps):
+            net.integrate(S, w.dt)
+        ev1.record(stream)
+        torch.cuda.synchronize()
+        replicas.barrier()
+    ms = ev0.elapsed_time(ev1)
+    launches = net.counters()[0] - l0
+    method = net.counters()[1]
+    out = dict(ms=ms, launches=launches, method=method, clocks=clk.summary(), rk4_per_step=S)
+    if e2e:
+        host_in = torch.from_numpy(y0).pin_memory()
+        host_out = torch.empty_like(host_in).pin_memory()
+        # warm-up of the host path
+        net.set_state(host_in)
+        net.integrate(S, w.dt)
+        net.get_state(host_out)
+        replicas.barrier()
+        torch.cuda.synchronize()
+        ev0.record(stream)
+        for _ in range(steps):
+            net.set_state(host_in)          # H2D from pinned memory (C ABI, host pointer)
+            net.integrate(S, w.dt)
+            net.get_state(host_out)         # D2H of the step's result
+        ev1.record(stream)
+        torch.cuda.synchronize()
+        replicas.barrier()
+        out.update(e2e_ms=ev0.elapsed_time(ev1), h2d=host_in.numel() * host_in.element_size(),
+                   d2h=host_out.numel() * host_out.element_size())
+    net.close()
+    del net
+    torch.cuda.empty_cache()
+    return out
+
+
+def roofline_object(w, m, steps):
+    """roofline of the dominant kernel (the fused RHS+RK4 stage kernel; every launch in the timed
+    region is one of its four stage instances)."""
+    from paper_2410_19075_b200 import roofline as R
+    pk = R.peaks()
+    c = R.ceiling(w, pk)
+    rk4 = steps * m["rk4_per_step"]
+    sec = m["ms"] * 1e-3
+    avg_launch_s = sec / max(1, m["launches"])
+    if c["bound"] == "hbm":
+        per_launch = R.bytes_per_osc_step(w) * w.n * rk4 / max(1, m["launches"])
+        achieved, peak, unit = per_launch / avg_launch_s / 1e9, pk["hbm_gbs"], "GB/s"
+        peak_src = "MEASURED_PEAKS.json hbm_gbs" if pk["hbm_source"] == "measured" else "guide fallback"
+    else:
+        per_launch = c["ops"] * w.n * rk4 / max(1, m["launches"])
+        achieved, peak, unit = per_launch / avg_launch_s / 1e9, pk[c["pipe"] + "_ginstr_s"], "Ginstr/s"
+        peak_src = "148 SM x %d lanes x sm_max_mhz (%s pipe)" % (R.LANES[c["pipe"]], c["pipe"])
+    return {"bound": c["bound"], "achieved": achieved, "peak": peak, "unit": unit,
+            "frac": achieved / peak, "traffic": None, "kernel": "fused RHS+RK4 stage kernel",
+            "avg_launch_us": avg_launch_s * 1e6, "peak_source": peak_src,
+            "bytes_per_osc_step": R.bytes_per_osc_step(w),
+            "survey_bytes_per_osc_step": R.survey_bytes_per_osc_step(w),
+            "ceiling_osc_steps_per_s": c["osc_steps_per_s"],
+            "frac_of_ceiling": (w.n * rk4 / sec) / c["osc_steps_per_s"]}
+
+
+# ------------------------------------------------------------------ CPU oracle arm
+SAMPLE = {"1": dict(), "2": dict(n=8192), "3a": dict(n1=64), "3b": dict(n1=64),
+          "4": dict(n=200_000), "5": dict(n1=96)}
+
+
+def oracle_sample(cfg, seed=1):
+    """The oracle, as it stands, on a bounded sample of workload `cfg`: same model, parameters,
+    radius rule, dtype rounding and step on a smaller ring / lattice / graph (SAMPLE).
+    Returns (sample workload, OracleNet, y0)."""
+    import numpy as np
+    from oracle import oracle as ora           # the one place bench.py may load oracle/
+    from paper_2410_19075_b200 import configs
+    w = configs.get(cfg, **SAMPLE[cfg])
+    y0, elem = make_inputs(w, seed)
+    y0 = y0.astype(np.float64)
+    if w.topo == configs.RING:
+        rp, ci = ora.topology_ring(w.n, w.radius)
+    elif w.topo == configs.LATTICE:
+        rp, ci = ora.topology_lattice(w.extent, w.radius)
+    else:
+        rp, ci = ora.topology_random_indegree(w.n, w.in_degree, w.topo_seed)
+    p = w.params
+    if w.model == configs.KS:
+        om = np.full(w.n, p["omega0"]) if elem is None else elem.astype(np.float64)
+        net = ora.OracleNet.ks(w.n, rp, ci, p["K"], p["alpha"], om)
+    elif w.model == configs.FHN:
+        net = ora.OracleNet.fhn(w.n, rp, ci, p["eps"], p["a"], p["sigma"], p["phi"])
+    else:
+        y0[1], y0[2], y0[3] = ora.hh_steady_gates(y0[0])
+        net = ora.OracleNet.hh(w.n, rp, ci, elem.astype(np.float64), **p)
+    return w, net, y0, ora.omp_threads()
+
+
+def time_oracle(cfg, budget_s=12.0, rk4_steps=None):
+    """oscillator-steps/s of the oracle on its sample; about budget_s of CPU work."""
+    w, net, y0, cores = oracle_sample(cfg)
+    t0 = time.perf_counter()
+    y = net.rk4(y0, 1, w.dt)
+    one = max(time.perf_counter() - t0, 1e-6)
+    if rk4_steps is None:
+        rk4_steps = int(max(1, min(w.n_steps, budget_s / one)))
+    t0 = time.perf_counter()
+    net.rk4(y, rk4_steps, w.dt)
+    sec = time.perf_counter() - t0
+    return dict(value=w.n * rk4_steps / sec, unit=METRIC, cores=cores, kind="oracle",
+                sample="%s, %d RK4 steps, %.1f s (plain C fp64, direct neighbour sums, OpenMP over "
+                       "elements)" % (w.name, rk4_steps, sec)), w, sec, rk4_steps
+
+
+def run_reference(args):
+    from paper_2410_19075_b200 import configs, replicas
+    rank, _, ws = replicas.world()
+    if rank != 0:
+        return 0
+    full = configs.get(args.config)
+    w, net, y0, cores = oracle_sample(args.config)
+    t0 = time.perf_counter()
+    y = net.rk4(y0, 1, w.dt)
+    one = max(time.perf_counter() - t0, 1e-6)
+    # each bench step = a bounded number of RK4 steps of the sample (<= obs_every, ~<= 4 s)
+    S = int(max(1, min(full.obs_every, 4.0 / one)))
+    for _ in range(args.warmup):
+        y = net.rk4(y, S, w.dt)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        y = net.rk4(y, S, w.dt)
+    sec = time.perf_counter() - t0
+    value = w.n * S * args.steps / sec
+    sample = "%s, %d RK4 steps per bench step" % (w.name, S)
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": METRIC,
+            "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": sec * 1e3 / args.steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": full.name, "cfg": full.cfg, "sample": sample},
+            "cpu_baseline": {"value": value, "unit": METRIC, "cores": cores, "kind": "oracle",
+                             "sample": sample},
+            "e2e": {"value": value, "unit": METRIC, "h2d_bytes_per_step": 0,
+                    "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+# ------------------------------------------------------------------ main
+def line_for(w, m, steps, n_gpus, units_total=None, ms_max=None):
+    """The JSON fields of one measured workload (headline or per_config entry)."""
+    rk4 = steps * m["rk4_per_step"]
+    ms = m["ms"] if ms_max is None else ms_max
+    units = w.n * rk4 * n_gpus if units_total is None else units_total
+    out = {"workload": w.name, "cfg": w.cfg, "value": units / (ms * 1e-3), "unit": METRIC,
+           "ms_per_step": ms / steps, "rk4_steps_per_step": m["rk4_per_step"],
+           "dtype": w.dtype, "method": "FAST" if m["method"] == 2 else "DIRECT",
+           "gpu_launches": m["launches"], "roofline": roofline_object(w, m, steps)}
+    if "e2e_ms" in m:
+        out["e2e"] = {"value": w.n * rk4 * n_gpus / (m["e2e_ms"] * 1e-3), "unit": METRIC,
+                      "h2d_bytes_per_step": m["h2d"], "d2h_bytes_per_step": m["d2h"]}
+    return out
+
+
+def run_ours(args):
+    import torch
+    from paper_2410_19075_b200 import binding, configs, replicas
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the product path has no CPU fallback)")
+    binding.lib()                                   # fail loudly if liboscnet.so is missing
+    rank, local_rank, ws = replicas.world()
+    torch.cuda.set_device(local_rank)
+    device = "cuda:%d" % local_rank
+    if ws > 1:
+        replicas.init("nccl")
+    w = configs.get(args.config)
+    m = measure(w, device, args.steps, args.warmup, e2e=True)
+    rk4 = args.steps * m["rk4_per_step"]
+    units, ms_max, value = replicas.aggregate(w.n * rk4, m["ms"], device)
+    _, e2e_ms_max, e2e_value = replicas.aggregate(w.n * rk4, m["e2e_ms"], device)
+    head = line_for(w, m, args.steps, ws, units, ms_max)
+    line = {"metric": METRIC, "value": value, "unit": METRIC, "n_gpus": ws, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms_max / args.steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": w.dtype, "data": "synthetic",
+            "config": {"workload": w.name, "cfg": w.cfg, "n": w.n, "dt": w.dt,
+                       "rk4_steps_per_step": m["rk4_per_step"], "method": head["method"],
+                       "parallelism": "replicas x%d (no data-path collective)" % ws,
+                       "l2": ("state arrays larger than L2 (no flush needed)"
+                              if w.n * w.nvar * (4 if w.dtype == "f32" else 8) > 126e6 else
+                              "state smaller than L2 by definition of the workload; resident by design")},
+            "clocks": m["clocks"],
+            "e2e": {"value": e2e_value, "unit": METRIC, "h2d_bytes_per_step": m["h2d"],
+                    "d2h_bytes_per_step": m["d2h"]},
+            "gpu_launches": m["launches"], "roofline": head["roofline"]}
+    if rank == 0 and ws == 1 and not args.no_per_config:
+        per = []
+        for cfg in PER_CONFIG:
+            if cfg == w.cfg:
+                continue
+            wc = configs.get(cfg)
+            k = max(3, min(args.steps, 10))
+            mc = measure(wc, device, k, max(3, args.warmup), e2e=True)
+            e = line_for(wc, mc, k, 1)
+            e["clocks"] = mc["clocks"]
+            per.append(e)
+        line["per_config"] = per
+    if rank == 0 and ws == 1 and not args.no_cpu_baseline:
+        cb, _, _, _ = time_oracle(w.cfg)
+        line["cpu_baseline"] = cb
+    if rank == 0:
+        print(json.dumps(line), flush=True)
+    if ws > 1:
+        import torch.distributed as dist
+        dist.barrier()
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", default=HEADLINE, choices=list(PER_CONFIG))
+    ap.add_argument("--no-per-config", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    return run_reference(args) if args.impl == "reference" else run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())
