@@ -312,6 +312,7 @@ int32_t net_create(const net_desc* desc, const void* params, size_t params_bytes
     rc = topo_build(h);
     h->desc.topo.row_ptr = nullptr;
     h->desc.topo.col_idx = nullptr;
+    if (rc == NET_OK) rc = fast_prepare(h);
     cudaError_t e = cudaSuccess;
     if (rc == NET_OK) {
         size_t state = (size_t)h->nvar * h->ld * h->esize;

@@ -4,10 +4,14 @@
 namespace oscnet {
 
 int32_t csr_warp_stage(net* h, const StageArgs& a);
+bool lattice3d_supported(const net_desc* d);
+int32_t lattice3d_prepare(net* h);
+int32_t lattice3d_stage(net* h, const StageArgs& a);
 
 int32_t fast_select(const net_desc* d) {
     const net_topology& t = d->topo;
     if (t.kind == NET_TOPO_CSR || t.kind == NET_TOPO_RANDOM_INDEGREE) return FAST_CSR_WARP;
+    if (lattice3d_supported(d)) return FAST_LATTICE3D;
     return FAST_NONE;
 }
 
@@ -16,9 +20,25 @@ size_t fast_scratch_bytes(const net_desc* d, int32_t fast_kind) {
     return 0;
 }
 
+// Launch geometry, shared-memory opt-in and occupancy of the selected family.  A family that
+// cannot take this shape (NET_ERR_UNSUPPORTED) falls back to DIRECT unless FAST was demanded.
+int32_t fast_prepare(net* h) {
+    int32_t rc = NET_OK;
+    if (h->fast_kind == FAST_LATTICE3D) rc = lattice3d_prepare(h);
+    if (rc == NET_ERR_UNSUPPORTED && h->desc.method != NET_METHOD_FAST) {
+        h->fast_kind = FAST_NONE;
+        h->method = NET_METHOD_DIRECT;
+        rc = NET_OK;
+    } else if (rc == NET_ERR_UNSUPPORTED) {
+        set_err(h, rc, "the FAST kernel family does not support this shape");
+    }
+    return rc;
+}
+
 int32_t fast_stage(net* h, const StageArgs& a) {
     switch (h->fast_kind) {
         case FAST_CSR_WARP: return csr_warp_stage(h, a);
+        case FAST_LATTICE3D: return lattice3d_stage(h, a);
         default: return set_err(h, NET_ERR_UNSUPPORTED, "fast kernel family %d has no stage kernel", h->fast_kind);
     }
 }

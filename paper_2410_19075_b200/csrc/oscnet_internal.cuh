@@ -91,6 +91,17 @@ struct Buffers {
     size_t scratch_bytes;
 };
 
+// launch geometry of the tiled 3D lattice kernels (lattice_fast.cu)
+struct Lat3 {
+    int32_t nx, ny, nz;
+    int32_t TX, S;            // tile: TX columns, S strips of TY rows
+    int32_t tiles_x, tiles_y;
+    int32_t Lz, nchunks;      // planes per z chunk
+    int32_t PW, PH;           // staged plane: (TX+2P) x (S*TY+2P)
+    int32_t n_ball;           // lattice points in the ball including the centre
+    int32_t include_self;
+};
+
 }  // namespace oscnet
 
 struct net {
@@ -119,6 +130,10 @@ struct net {
     double stats[8];
     int stats_valid;
     int s_valid;           // HH fast path: s_y consistent with y
+    oscnet::Lat3 lat;      // FAST_LATTICE3D launch geometry
+    unsigned lat_grid;
+    int lat_threads;
+    size_t lat_smem;
     char err[512];
 };
 
@@ -148,6 +163,7 @@ int32_t hh_steady_gates(net* h);
 enum { FAST_NONE = 0, FAST_CSR_WARP = 1, FAST_LATTICE3D = 2, FAST_RING_FHN = 3, FAST_RING_KS = 4 };
 int32_t fast_select(const net_desc* d);                   // FAST_* available for this desc
 size_t fast_scratch_bytes(const net_desc* d, int32_t fast_kind);
+int32_t fast_prepare(net* h);                             // once, at the end of net_create
 int32_t fast_stage(net* h, const StageArgs& a);
 int32_t fast_integrate(net* h, int64_t n_steps, double dt, bool* handled);  // persistent kernels
 
