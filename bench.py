@@ -4,8 +4,9 @@
     python bench.py [--gpus N] [--steps K] [--warmup W] [--config 5] [--impl ours|reference]
                     [--no-per-config] [--no-cpu-baseline]
 
-One bench "step" = one output interval of the workload = `obs_every` RK4 steps (4 fused stage
-kernels each) of net_integrate over the whole network.  `value` = N x RK4 steps / s with the
+One bench "step" = one net_integrate call of BENCH_RK4[cfg] RK4 steps over the whole network
+(the output interval `obs_every` of the workload for the large nets; the whole 1000-step run
+for the 256-oscillator ring, whose single call is one persistent kernel).  `value` = N x RK4 steps / s with the
 state resident in HBM; `e2e` = the same through the C ABI with HOST buffers (net_set_state from
 pinned memory + net_integrate + net_get_state to pinned memory inside the timed region).
 The headline workload is config 5 (DESIGN.md "Measurement": the metric is quoted per config;
@@ -28,6 +29,8 @@ if ROOT not in sys.path:
 METRIC = "oscillator-steps/s"
 HEADLINE = "5"
 PER_CONFIG = ("1", "2", "3a", "3b", "4", "5")
+# RK4 steps per bench step (= per net_integrate call)
+BENCH_RK4 = {"1": 1000, "2": 200, "3a": 10, "3b": 10, "4": 100, "5": 10}
 
 
 # ------------------------------------------------------------------ inputs
@@ -125,12 +128,12 @@ def build_net(w, device, seed=1):
 
 
 def measure(w, device, steps, warmup, e2e=True, seed=1):
-    """Times `steps` bench steps (each = w.obs_every RK4 steps) after `warmup` untimed ones.
+    """Times `steps` bench steps (each = BENCH_RK4[cfg] RK4 steps) after `warmup` untimed ones.
     Returns device-resident ms, e2e ms, launches and byte counts."""
     import torch
     from paper_2410_19075_b200 import replicas
     net, y0 = build_net(w, device, seed)
-    S = w.obs_every
+    S = BENCH_RK4[w.cfg]
     stream = net.stream
     for _ in range(warmup):
         net.integrate(S, w.dt)
@@ -260,8 +263,8 @@ def run_reference(args):
     t0 = time.perf_counter()
     y = net.rk4(y0, 1, w.dt)
     one = max(time.perf_counter() - t0, 1e-6)
-    # each bench step = a bounded number of RK4 steps of the sample (<= obs_every, ~<= 4 s)
-    S = int(max(1, min(full.obs_every, 4.0 / one)))
+    # each bench step = a bounded number of RK4 steps of the sample (<= BENCH_RK4[cfg], ~<= 4 s)
+    S = int(max(1, min(BENCH_RK4[full.cfg], 4.0 / one)))
     for _ in range(args.warmup):
         y = net.rk4(y, S, w.dt)
     t0 = time.perf_counter()

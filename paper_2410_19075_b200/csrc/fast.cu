@@ -7,16 +7,20 @@ int32_t csr_warp_stage(net* h, const StageArgs& a);
 bool lattice3d_supported(const net_desc* d);
 int32_t lattice3d_prepare(net* h);
 int32_t lattice3d_stage(net* h, const StageArgs& a);
+bool ring_supported(const net_desc* d);
+size_t ring_scratch_bytes(const net_desc* d);
+int32_t ring_run(net* h, const void* y_in, void* y_out, int64_t n_steps, double dt, int rhs_only);
 
 int32_t fast_select(const net_desc* d) {
     const net_topology& t = d->topo;
     if (t.kind == NET_TOPO_CSR || t.kind == NET_TOPO_RANDOM_INDEGREE) return FAST_CSR_WARP;
     if (lattice3d_supported(d)) return FAST_LATTICE3D;
+    if (ring_supported(d)) return d->model == NET_MODEL_KS ? FAST_RING_KS : FAST_RING_FHN;
     return FAST_NONE;
 }
 
 size_t fast_scratch_bytes(const net_desc* d, int32_t fast_kind) {
-    (void)d; (void)fast_kind;
+    if (fast_kind == FAST_RING_KS || fast_kind == FAST_RING_FHN) return ring_scratch_bytes(d);
     return 0;
 }
 
@@ -39,13 +43,28 @@ int32_t fast_stage(net* h, const StageArgs& a) {
     switch (h->fast_kind) {
         case FAST_CSR_WARP: return csr_warp_stage(h, a);
         case FAST_LATTICE3D: return lattice3d_stage(h, a);
-        default: return set_err(h, NET_ERR_UNSUPPORTED, "fast kernel family %d has no stage kernel", h->fast_kind);
+        case FAST_RING_KS:
+        case FAST_RING_FHN:
+            // the ring family integrates whole runs (fast_integrate); as a stage it only serves
+            // the RHS hook
+            if (a.stage != STAGE_RHS_ONLY) break;
+            return ring_run(h, a.in, a.out, 0, 0.0, 1);
+        default: break;
     }
+    return set_err(h, NET_ERR_UNSUPPORTED, "fast kernel family %d has no stage kernel", h->fast_kind);
 }
 
 int32_t fast_integrate(net* h, int64_t n_steps, double dt, bool* handled) {
-    (void)h; (void)n_steps; (void)dt;
     *handled = false;
+    if (h->fast_kind != FAST_RING_KS && h->fast_kind != FAST_RING_FHN) return NET_OK;
+    // one persistent launch per <= 2^20 steps (the grid-barrier counter is 32 bits wide)
+    for (int64_t left = n_steps; left > 0;) {
+        const int64_t now = left < (1 << 20) ? left : (1 << 20);
+        int32_t rc = ring_run(h, h->b.y, h->b.y, now, dt, 0);
+        if (rc) return rc;
+        left -= now;
+    }
+    *handled = true;
     return NET_OK;
 }
 

@@ -1,0 +1,327 @@
+// FAST method for rings (configs 1 and 2): one persistent cooperative kernel integrates all
+// n_steps; the coupling window sum over |j-i| <= P is a difference of
+// prefix sums, exact in real arithmetic.
+//
+// Both ring models reduce to the window sum of NF = 2 fields: FHN (eq. (2))
+// is linear, sum_j (u_j - u_i) = W_u(i) - (2P+1) u_i; for KS (eq. (3)) the sine is
+// factorised, sum_j sin(phi_j - phi_i - a) = S_i cos(phi_i + a) - C_i sin(phi_i + a) with
+// (C, S) the window sums of (cos phi, sin phi) -- one sincos per element per stage instead of
+// one sine per link.
+//
+// These nets are latency-bound (2 KB / 1 MB of state), so the whole run is one launch: every
+// thread keeps its E elements (base state, stage state, RK4 accumulator) in registers for all
+// steps.  CTA b owns the contiguous chunk [b*chunk, (b+1)*chunk).  Per stage:
+//   A. fields of the stage state -> inclusive prefix inside the chunk (thread-serial, warp
+//      shuffles, warp totals) -> Sloc[f][i] and the chunk total tot[f][b] to global memory (L2);
+//   B. ONE grid barrier (monotonic counter in L2; co-residency guaranteed by the cooperative
+//      launch); single-CTA nets (config 1) use shared memory and __syncthreads instead;
+//   C. every CTA scans the G chunk totals (double) into exclusive block offsets BT, and each
+//      element forms W(i) = Pref(i+P) - Pref(i-P-1), Pref(j) = BT[blk(j)] + Sloc[j], with the
+//      ring wrap taken as one extra full-ring term; local vector field; RK4 update in registers.
+// Sloc/tot are double-buffered over consecutive stages, so one barrier per stage suffices.
+// The cancellation of the prefix differences is bounded by (chunk length) x ulp x max|field| on
+// Sloc plus G x ulp(double) on BT; the RHS divides it by Omega (measured: tests).
+#include <cooperative_groups.h>
+
+#include "models.cuh"
+
+namespace oscnet {
+
+constexpr int RING_THREADS = 256;
+constexpr int RING_GMAX = RING_THREADS;   // the chunk totals are scanned in one pass by one CTA
+
+struct RingArgs {
+    const void* y_in;        // [nvar][ld] state the run starts from / RHS is evaluated on
+    void* y_out;             // integrate: final state (may alias y_in); rhs_only: f(y_in)
+    const void* elem_param;  // omega_i (KS)
+    void* S[2];              // 2 x [2][npad] prefix buffers (T)
+    double* tot[2];          // 2 x [2][RING_GMAX] chunk totals
+    unsigned int* bar;       // grid barrier counter (zeroed before the launch)
+    int64_t n, ld, npad;
+    int32_t P, include_self, chunk, G;
+    int64_t n_steps;
+    double dt;
+    int32_t rhs_only;
+};
+
+__device__ __forceinline__ unsigned ld_acquire_u32(const unsigned* p) {
+    unsigned v;
+    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ void red_release_add_u32(unsigned* p, unsigned v) {
+    asm volatile("red.release.gpu.global.add.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+
+// All CTAs arrive; returns when `target` arrivals have been counted.
+__device__ __forceinline__ void grid_barrier(unsigned* bar, unsigned target) {
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        red_release_add_u32(bar, 1u);
+        while (ld_acquire_u32(bar) < target) {}
+    }
+    __syncthreads();
+}
+
+template <class T> __device__ __forceinline__ T ld_l2(const T* p) { return __ldcg(p); }
+template <class T> __device__ __forceinline__ void st_l2(T* p, T v) { __stcg(p, v); }
+
+// Inclusive block scan of two values per thread (a, b); returns the block totals through
+// (ta, tb).  wsum: shared scratch [2][RING_THREADS/32].
+template <class A>
+__device__ __forceinline__ void block_scan2(A& a, A& b, A& ta, A& tb, A (*wsum)[RING_THREADS / 32]) {
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        A ua = __shfl_up_sync(0xffffffffu, a, o), ub = __shfl_up_sync(0xffffffffu, b, o);
+        if (lane >= o) { a += ua; b += ub; }
+    }
+    if (lane == 31) { wsum[0][warp] = a; wsum[1][warp] = b; }
+    __syncthreads();
+    A oa = 0, ob = 0, sa = 0, sb = 0;
+#pragma unroll
+    for (int w = 0; w < RING_THREADS / 32; ++w) {
+        const A va = wsum[0][w], vb = wsum[1][w];
+        if (w < warp) { oa += va; ob += vb; }
+        sa += va; sb += vb;
+    }
+    a += oa; b += ob;
+    ta = sa; tb = sb;
+    __syncthreads();
+}
+
+template <class T, int MODEL, int E, bool SINGLE>
+__global__ void __launch_bounds__(RING_THREADS) ring_persistent_kernel(RingArgs a, ModelParams mp) {
+    constexpr int NV = MODEL == NET_MODEL_KS ? 1 : 2;
+    extern __shared__ __align__(16) unsigned char ring_smem[];
+    __shared__ T wsumT[2][RING_THREADS / 32];
+    __shared__ double wsumD[2][RING_THREADS / 32];
+    __shared__ double BT[2][RING_GMAX + 1];
+
+    const int64_t n = a.n, ld = a.ld;
+    const int chunk = a.chunk, G = a.G, P = a.P;
+    const int b = blockIdx.x;
+    const int64_t cbeg = (int64_t)b * chunk;
+    const int64_t i0 = cbeg + (int64_t)threadIdx.x * E;      // first element of this thread
+    const T* __restrict__ yin = (const T*)a.y_in;
+    const T* __restrict__ ep = (const T*)a.elem_param;
+    const T dt = (T)a.dt;
+    const int deg = 2 * P + (a.include_self ? 1 : 0);
+    const T inv_deg = deg > 0 ? T(1) / T(deg) : T(0);
+    const T nwin = T(2 * P + 1);
+
+    T y0[E][NV], x[E][NV], acc[E][NV], om[E];
+    bool ok[E];
+#pragma unroll
+    for (int e = 0; e < E; ++e) {
+        ok[e] = i0 + e < n && threadIdx.x * E + e < chunk;
+        om[e] = (MODEL == NET_MODEL_KS && ok[e]) ? ep[i0 + e] : T(0);
+#pragma unroll
+        for (int v = 0; v < NV; ++v) {
+            y0[e][v] = ok[e] ? yin[v * ld + i0 + e] : T(0);
+            x[e][v] = y0[e][v];
+            acc[e][v] = T(0);
+        }
+    }
+
+    const int64_t n_stage = a.rhs_only ? 1 : 4 * a.n_steps;
+    for (int64_t q = 0; q < n_stage; ++q) {
+        const int stage = (int)(q & 3);
+        const int buf = (int)(q & 1);
+        T* Sg = SINGLE ? reinterpret_cast<T*>(ring_smem) : (T*)a.S[buf];
+        const int64_t sstride = SINGLE ? (int64_t)chunk : a.npad;
+        // ---- A: fields and their inclusive prefix inside the chunk
+        T f0[E], f1[E];
+#pragma unroll
+        for (int e = 0; e < E; ++e) {
+            if (MODEL == NET_MODEL_KS) {
+                T s, c;
+                Math<T>::sincos(x[e][0], &s, &c);
+                f0[e] = ok[e] ? c : T(0);
+                f1[e] = ok[e] ? s : T(0);
+            } else {
+                f0[e] = x[e][0];            // zero where !ok (state loaded as zero)
+                f1[e] = x[e][NV - 1];
+            }
+        }
+        T p0[E], p1[E];
+        p0[0] = f0[0]; p1[0] = f1[0];
+#pragma unroll
+        for (int e = 1; e < E; ++e) { p0[e] = p0[e - 1] + f0[e]; p1[e] = p1[e - 1] + f1[e]; }
+        T s0 = p0[E - 1], s1 = p1[E - 1], t0, t1;
+        block_scan2<T>(s0, s1, t0, t1, wsumT);
+        const T ex0 = s0 - p0[E - 1], ex1 = s1 - p1[E - 1];   // exclusive offset of this thread
+#pragma unroll
+        for (int e = 0; e < E; ++e) {
+            if (ok[e]) {
+                const int64_t at = SINGLE ? (int64_t)(threadIdx.x * E + e) : i0 + e;
+                if (SINGLE) { Sg[at] = ex0 + p0[e]; Sg[sstride + at] = ex1 + p1[e]; }
+                else { st_l2(Sg + at, ex0 + p0[e]); st_l2(Sg + sstride + at, ex1 + p1[e]); }
+            }
+        }
+        if (!SINGLE && threadIdx.x == 0) {
+            st_l2(a.tot[buf] + b, (double)t0);
+            st_l2(a.tot[buf] + RING_GMAX + b, (double)t1);
+        }
+        // ---- B: every chunk's prefix is visible
+        if (SINGLE) __syncthreads();
+        else grid_barrier(a.bar, (unsigned)((q + 1) * G));
+        // ---- C: block offsets
+        if (!SINGLE) {
+            double c0 = threadIdx.x < G ? ld_l2(a.tot[buf] + threadIdx.x) : 0.0;
+            double c1 = threadIdx.x < G ? ld_l2(a.tot[buf] + RING_GMAX + threadIdx.x) : 0.0;
+            const double v0 = c0, v1 = c1;
+            double u0, u1;
+            block_scan2<double>(c0, c1, u0, u1, wsumD);
+            if (threadIdx.x < G) { BT[0][threadIdx.x] = c0 - v0; BT[1][threadIdx.x] = c1 - v1; }
+            if (threadIdx.x == 0) { BT[0][G] = u0; BT[1][G] = u1; }
+            __syncthreads();
+        }
+        // window sums, local field, RK4 update
+        T k[E][NV];
+#pragma unroll
+        for (int e = 0; e < E; ++e) {
+            T W0 = T(0), W1 = T(0);
+            if (ok[e]) {
+                const int64_t i = i0 + e;
+                double bt0 = 0.0, bt1 = 0.0;
+                T sl0 = T(0), sl1 = T(0);
+                auto term = [&](int64_t j, int sign) {     // +- Pref(j)
+                    const int bj = SINGLE ? 0 : (int)(j / chunk);
+                    const int64_t at = SINGLE ? j : j;
+                    const T v0 = SINGLE ? Sg[at] : ld_l2(Sg + at);
+                    const T v1 = SINGLE ? Sg[sstride + at] : ld_l2(Sg + sstride + at);
+                    if (sign > 0) { sl0 += v0; sl1 += v1; if (!SINGLE) { bt0 += BT[0][bj]; bt1 += BT[1][bj]; } }
+                    else { sl0 -= v0; sl1 -= v1; if (!SINGLE) { bt0 -= BT[0][bj]; bt1 -= BT[1][bj]; } }
+                };
+                int64_t hi = i + P, lo = i - P - 1;
+                if (hi >= n) { term(n - 1, +1); hi -= n; }
+                term(hi, +1);
+                if (lo < -1) { term(n - 1, +1); lo += n; }
+                if (lo >= 0) term(lo, -1);
+                W0 = (T)bt0 + sl0;
+                W1 = (T)bt1 + sl1;
+            }
+            if (MODEL == NET_MODEL_KS) {
+                T C = W0, S = W1;
+                if (!a.include_self) { C -= f0[e]; S -= f1[e]; }
+                k[e][0] = ks_rhs_factorised<T>(mp, om[e], C, S, f0[e], f1[e], inv_deg);
+            } else {
+                const T Cu = W0 - nwin * f0[e], Cv = W1 - nwin * f1[e];
+                fhn_rhs<T>(mp, f0[e], f1[e], Cu, Cv, inv_deg, &k[e][0], &k[e][NV - 1]);
+            }
+        }
+        if (a.rhs_only) {
+            T* out = (T*)a.y_out;
+#pragma unroll
+            for (int e = 0; e < E; ++e)
+                if (ok[e])
+#pragma unroll
+                    for (int v = 0; v < NV; ++v) out[v * ld + i0 + e] = k[e][v];
+            return;
+        }
+        // textbook RK4 in registers: acc = k1 + 2 k2 + 2 k3 (+ k4)
+#pragma unroll
+        for (int e = 0; e < E; ++e)
+#pragma unroll
+            for (int v = 0; v < NV; ++v) {
+                const T kv = k[e][v];
+                if (stage == 0) { acc[e][v] = kv; x[e][v] = y0[e][v] + (T(0.5) * dt) * kv; }
+                else if (stage == 1) { acc[e][v] += T(2) * kv; x[e][v] = y0[e][v] + (T(0.5) * dt) * kv; }
+                else if (stage == 2) { acc[e][v] += T(2) * kv; x[e][v] = y0[e][v] + dt * kv; }
+                else { y0[e][v] += (dt * T(1.0 / 6.0)) * (acc[e][v] + kv); x[e][v] = y0[e][v]; }
+            }
+        if (SINGLE) __syncthreads();   // the shared prefix buffer is rewritten by the next stage
+    }
+    T* out = (T*)a.y_out;
+#pragma unroll
+    for (int e = 0; e < E; ++e)
+        if (ok[e])
+#pragma unroll
+            for (int v = 0; v < NV; ++v) out[v * ld + i0 + e] = y0[e][v];
+}
+
+// ------------------------------------------------------------------ host side
+struct RingPlan { int E, G, chunk; bool single; size_t smem; };
+
+static bool ring_plan(int64_t n, size_t esize, RingPlan* p) {
+    for (int E = 1; E <= 8; E *= 2) {
+        const int64_t chunk = (int64_t)RING_THREADS * E;
+        const int64_t G = (n + chunk - 1) / chunk;
+        if (G <= 148) {   // one CTA per SM: co-resident whatever the register count
+            p->E = E; p->G = (int)G; p->chunk = (int)chunk; p->single = G == 1;
+            p->smem = p->single ? 2 * (size_t)chunk * esize : 0;
+            return true;
+        }
+    }
+    return false;
+}
+
+bool ring_supported(const net_desc* d) {
+    RingPlan p;
+    return d->topo.kind == NET_TOPO_RING && (d->model == NET_MODEL_KS || d->model == NET_MODEL_FHN) &&
+           ring_plan(d->n, d->dtype == NET_F32 ? 4 : 8, &p);
+}
+
+size_t ring_scratch_bytes(const net_desc* d) {
+    const size_t es = d->dtype == NET_F32 ? 4 : 8;
+    const size_t npad = (size_t)round_up(d->n, 64);
+    return 2 * (2 * npad * es) + 2 * (2 * RING_GMAX * sizeof(double)) + 256 + 1024;
+}
+
+template <class T, int MODEL, int E, bool SINGLE>
+static int32_t ring_launch_t(net* h, RingArgs& a, const RingPlan& p) {
+    auto kern = ring_persistent_kernel<T, MODEL, E, SINGLE>;
+    if (p.smem > 48 * 1024)
+        OSC_CUDA(h, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.smem));
+    if (!SINGLE) OSC_CUDA(h, cudaMemsetAsync(a.bar, 0, sizeof(unsigned), h->stream));
+    void* params[] = {&a, &h->mp};
+    if (SINGLE)
+        OSC_CUDA(h, cudaLaunchKernel((const void*)kern, dim3(1), dim3(RING_THREADS), params, p.smem, h->stream));
+    else
+        OSC_CUDA(h, cudaLaunchCooperativeKernel((const void*)kern, dim3(p.G), dim3(RING_THREADS), params, p.smem, h->stream));
+    h->launches += 1;
+    return NET_OK;
+}
+
+template <class T, int MODEL>
+static int32_t ring_launch_e(net* h, RingArgs& a, const RingPlan& p) {
+    if (p.single) {
+        switch (p.E) {
+            case 1: return ring_launch_t<T, MODEL, 1, true>(h, a, p);
+            case 2: return ring_launch_t<T, MODEL, 2, true>(h, a, p);
+            case 4: return ring_launch_t<T, MODEL, 4, true>(h, a, p);
+            default: return ring_launch_t<T, MODEL, 8, true>(h, a, p);
+        }
+    }
+    switch (p.E) {
+        case 1: return ring_launch_t<T, MODEL, 1, false>(h, a, p);
+        case 2: return ring_launch_t<T, MODEL, 2, false>(h, a, p);
+        case 4: return ring_launch_t<T, MODEL, 4, false>(h, a, p);
+        default: return ring_launch_t<T, MODEL, 8, false>(h, a, p);
+    }
+}
+
+// y_in -> y_out over n_steps RK4 steps (rhs_only: y_out = f(y_in))
+int32_t ring_run(net* h, const void* y_in, void* y_out, int64_t n_steps, double dt, int rhs_only) {
+    RingPlan p;
+    if (!ring_plan(h->n, h->esize, &p)) return set_err(h, NET_ERR_UNSUPPORTED, "ring too large for the persistent kernel");
+    RingArgs a;
+    memset(&a, 0, sizeof(a));
+    a.y_in = y_in; a.y_out = y_out; a.elem_param = h->b.elem_param;
+    a.n = h->n; a.ld = h->ld; a.npad = round_up(h->n, 64);
+    a.P = h->tv.P; a.include_self = h->tv.include_self; a.chunk = p.chunk; a.G = p.G;
+    a.n_steps = n_steps; a.dt = dt; a.rhs_only = rhs_only;
+    char* s = (char*)h->b.scratch;
+    const size_t sbytes = 2 * (size_t)a.npad * h->esize;
+    a.S[0] = s; a.S[1] = s + sbytes;
+    a.tot[0] = (double*)(s + 2 * sbytes);
+    a.tot[1] = a.tot[0] + 2 * RING_GMAX;
+    a.bar = (unsigned*)(a.tot[1] + 2 * RING_GMAX);
+    const bool f32 = h->desc.dtype == NET_F32;
+    if (h->desc.model == NET_MODEL_KS)
+        return f32 ? ring_launch_e<float, NET_MODEL_KS>(h, a, p) : ring_launch_e<double, NET_MODEL_KS>(h, a, p);
+    return f32 ? ring_launch_e<float, NET_MODEL_FHN>(h, a, p) : ring_launch_e<double, NET_MODEL_FHN>(h, a, p);
+}
+
+}  // namespace oscnet
