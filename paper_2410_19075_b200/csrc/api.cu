@@ -159,6 +159,20 @@ static int32_t copy_state(net* h, void* internal, void* external, bool to_intern
     cudaMemcpyKind kind = ext_is_device ? cudaMemcpyDeviceToDevice
                                         : (to_internal ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToHost);
     size_t row = (size_t)h->n * h->esize;
+    if (h->pairs) {
+        // interleaved internal layout: go through Y3 (dead between steps) as SoA staging
+        void* soa = h->b.Y3;
+        int32_t rc;
+        if (to_internal) {
+            OSC_CUDA(h, cudaMemcpy2DAsync(soa, (size_t)h->ld * h->esize, external, row, row, h->nvar, kind, h->stream));
+            if ((rc = pairs_pack(h, soa, internal))) return rc;
+        } else {
+            if ((rc = pairs_unpack(h, internal, soa))) return rc;
+            OSC_CUDA(h, cudaMemcpy2DAsync(external, row, soa, (size_t)h->ld * h->esize, row, h->nvar, kind, h->stream));
+        }
+        if (!ext_is_device) OSC_CUDA(h, cudaStreamSynchronize(h->stream));
+        return NET_OK;
+    }
     if (to_internal)
         OSC_CUDA(h, cudaMemcpy2DAsync(internal, (size_t)h->ld * h->esize, external, row, row, h->nvar, kind, h->stream));
     else
@@ -193,12 +207,14 @@ static StageArgs stage_args(net* h, int stage, double dt) {
     return a;
 }
 
+// exchange fields derived from y (HH: S(V); KS on the bulk-copy lattice kernels: (cos, sin) phi)
 static int32_t ensure_s(net* h) {
-    if (h->b.s_y && !h->s_valid) {
-        int32_t rc = hh_compute_s(h, h->b.y, h->b.s_y);
-        if (rc) return rc;
-        h->s_valid = 1;
-    }
+    if (h->s_valid) return NET_OK;
+    int32_t rc = NET_OK;
+    if (h->b.s_y) rc = hh_compute_s(h, h->b.y, h->b.s_y);
+    if (rc == NET_OK) rc = fast_refresh_exchange(h);
+    if (rc) return rc;
+    h->s_valid = 1;
     return NET_OK;
 }
 
@@ -297,6 +313,8 @@ int32_t net_create(const net_desc* desc, const void* params, size_t params_bytes
     h->ld = round_up(desc->n, 64);
     h->stream = (cudaStream_t)cuda_stream;
     h->b = L.b;
+    h->var_stride = h->ld;
+    h->elem_stride = 1;
     fill_params(h, params);
     const int fk = desc->method == NET_METHOD_DIRECT ? FAST_NONE : fast_select(desc);
     if (desc->method == NET_METHOD_FAST && fk == FAST_NONE) {

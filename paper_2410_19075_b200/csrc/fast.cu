@@ -7,6 +7,11 @@ int32_t csr_warp_stage(net* h, const StageArgs& a);
 bool lattice3d_supported(const net_desc* d);
 int32_t lattice3d_prepare(net* h);
 int32_t lattice3d_stage(net* h, const StageArgs& a);
+bool lattice_v2_supported(const net_desc* d);
+size_t lattice_v2_scratch_bytes(const net_desc* d);
+int32_t lattice_v2_prepare(net* h);
+int32_t lattice_v2_stage(net* h, const StageArgs& a);
+int32_t lattice_v2_refresh_exchange(net* h);
 bool ring_supported(const net_desc* d);
 size_t ring_scratch_bytes(const net_desc* d);
 int32_t ring_run(net* h, const void* y_in, void* y_out, int64_t n_steps, double dt, int rhs_only);
@@ -14,6 +19,7 @@ int32_t ring_run(net* h, const void* y_in, void* y_out, int64_t n_steps, double 
 int32_t fast_select(const net_desc* d) {
     const net_topology& t = d->topo;
     if (t.kind == NET_TOPO_CSR || t.kind == NET_TOPO_RANDOM_INDEGREE) return FAST_CSR_WARP;
+    if (lattice_v2_supported(d)) return FAST_LATTICE3D_V2;
     if (lattice3d_supported(d)) return FAST_LATTICE3D;
     if (ring_supported(d)) return d->model == NET_MODEL_KS ? FAST_RING_KS : FAST_RING_FHN;
     return FAST_NONE;
@@ -21,6 +27,7 @@ int32_t fast_select(const net_desc* d) {
 
 size_t fast_scratch_bytes(const net_desc* d, int32_t fast_kind) {
     if (fast_kind == FAST_RING_KS || fast_kind == FAST_RING_FHN) return ring_scratch_bytes(d);
+    if (fast_kind == FAST_LATTICE3D_V2) return lattice_v2_scratch_bytes(d);
     return 0;
 }
 
@@ -28,6 +35,13 @@ size_t fast_scratch_bytes(const net_desc* d, int32_t fast_kind) {
 // cannot take this shape (NET_ERR_UNSUPPORTED) falls back to DIRECT unless FAST was demanded.
 int32_t fast_prepare(net* h) {
     int32_t rc = NET_OK;
+    if (h->fast_kind == FAST_LATTICE3D_V2) {
+        rc = lattice_v2_prepare(h);
+        if (rc == NET_ERR_UNSUPPORTED) {     // shape the bulk-copy kernels cannot take: first generation
+            h->fast_kind = FAST_LATTICE3D;
+            rc = NET_OK;
+        }
+    }
     if (h->fast_kind == FAST_LATTICE3D) rc = lattice3d_prepare(h);
     if (rc == NET_ERR_UNSUPPORTED && h->desc.method != NET_METHOD_FAST) {
         h->fast_kind = FAST_NONE;
@@ -43,6 +57,7 @@ int32_t fast_stage(net* h, const StageArgs& a) {
     switch (h->fast_kind) {
         case FAST_CSR_WARP: return csr_warp_stage(h, a);
         case FAST_LATTICE3D: return lattice3d_stage(h, a);
+        case FAST_LATTICE3D_V2: return lattice_v2_stage(h, a);
         case FAST_RING_KS:
         case FAST_RING_FHN:
             // the ring family integrates whole runs (fast_integrate); as a stage it only serves
@@ -52,6 +67,11 @@ int32_t fast_stage(net* h, const StageArgs& a) {
         default: break;
     }
     return set_err(h, NET_ERR_UNSUPPORTED, "fast kernel family %d has no stage kernel", h->fast_kind);
+}
+
+int32_t fast_refresh_exchange(net* h) {
+    if (h->fast_kind == FAST_LATTICE3D_V2) return lattice_v2_refresh_exchange(h);
+    return NET_OK;
 }
 
 int32_t fast_integrate(net* h, int64_t n_steps, double dt, bool* handled) {

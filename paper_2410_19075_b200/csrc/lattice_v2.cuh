@@ -1,0 +1,408 @@
+// FAST method for 3D periodic lattices, second generation (configs 3 and 5).
+//
+// Same mathematics as lattice_fast.cu (x-run decomposition of the ball of PAPER.md:313, z-marching
+// CTA, register accumulators for the 2P+1 open output planes; exact in real arithmetic), rebuilt
+// around what bounds it on B200:
+//   * the two fields of the ball sum -- (u, v) for FHN, (cos phi, sin phi) for KS -- are stored
+//     INTERLEAVED as pairs, in global memory and in shared memory, so every add of the ball sum is
+//     one packed FADD2 (add.rn.f32x2) on an aligned register pair and every shared-memory access
+//     is a 16-byte LDS;
+//   * planes are staged by the bulk-copy engine: one cp.async.bulk (UBLKCP) per row piece,
+//     completing on an mbarrier, D planes ahead of the compute -- no register staging, no
+//     address arithmetic in the inner loop; the periodic wrap is resolved per row piece;
+//   * KS: the producing stage writes E = (cos phi, sin phi) of its output next to phi, so the
+//     sincos is paid exactly once per element per stage and halos are plain copies;
+//   * RK4 in the "Z form" (13 state records per step, at most two pointwise operands per stage):
+//       stage 0: Y2 = y + dt/2 f(y)        stage 1: Y3 = y + dt/2 f(Y2)
+//       stage 2: Y4 = y + dt f(Y3),  Z = (Y2 + 2 Y3 + Y4 - y)/3   (Z overwrites Y2)
+//       stage 3: y  = Z + dt/6 f(Y4)
+//     which is y + dt/6 (k1 + 2 k2 + 2 k3 + k4) with k_s recovered from the stage states.
+// Thread = X consecutive columns x TY rows; CTA = QX x SY threads; tile = (QX X) x (SY TY).
+#pragma once
+#include <type_traits>
+
+#include "models.cuh"
+
+namespace oscnet {
+
+// ------------------------------------------------------------------ pairs
+template <class T> struct PairOf;
+template <> struct PairOf<float> { typedef float2 type; };
+template <> struct PairOf<double> { typedef double2 type; };
+
+__device__ __forceinline__ float2 padd(float2 a, float2 b) {
+    unsigned long long r;
+    asm("add.rn.f32x2 %0, %1, %2;"
+        : "=l"(r)
+        : "l"(*reinterpret_cast<unsigned long long*>(&a)), "l"(*reinterpret_cast<unsigned long long*>(&b)));
+    return *reinterpret_cast<float2*>(&r);
+}
+__device__ __forceinline__ double2 padd(double2 a, double2 b) { return make_double2(a.x + b.x, a.y + b.y); }
+
+// half-width of the x-run at (|dz|, |dy|), -1 if the row does not meet the ball
+__host__ __device__ constexpr int l2_isqrt(int v) { int r = 0; while ((r + 1) * (r + 1) <= v) ++r; return r; }
+__host__ __device__ constexpr int l2_run_w(int P, int adz, int ady) {
+    int r = P * P - adz * adz - ady * ady;
+    return r < 0 ? -1 : l2_isqrt(r);
+}
+
+// ------------------------------------------------------------------ PTX helpers
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t* bar, unsigned count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, unsigned bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, unsigned parity) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "WAIT_%=:\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+        "@p bra DONE_%=;\n\t"
+        "bra WAIT_%=;\n\t"
+        "DONE_%=:\n\t}" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, unsigned bytes, uint64_t* bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+
+// N contiguous scalars from / to 16-byte (8-byte when N*sizeof == 8) aligned global memory
+template <int N>
+__device__ __forceinline__ void ldg_vec(const float* p, float (&v)[N]) {
+    if constexpr (N % 4 == 0) {
+#pragma unroll
+        for (int c = 0; c < N / 4; ++c) {
+            const float4 w = reinterpret_cast<const float4*>(p)[c];
+            v[4 * c] = w.x; v[4 * c + 1] = w.y; v[4 * c + 2] = w.z; v[4 * c + 3] = w.w;
+        }
+    } else if constexpr (N % 2 == 0) {
+#pragma unroll
+        for (int c = 0; c < N / 2; ++c) {
+            const float2 w = reinterpret_cast<const float2*>(p)[c];
+            v[2 * c] = w.x; v[2 * c + 1] = w.y;
+        }
+    } else {
+#pragma unroll
+        for (int c = 0; c < N; ++c) v[c] = p[c];
+    }
+}
+template <int N>
+__device__ __forceinline__ void ldg_vec(const double* p, double (&v)[N]) {
+    if constexpr (N % 2 == 0) {
+#pragma unroll
+        for (int c = 0; c < N / 2; ++c) {
+            const double2 w = reinterpret_cast<const double2*>(p)[c];
+            v[2 * c] = w.x; v[2 * c + 1] = w.y;
+        }
+    } else {
+#pragma unroll
+        for (int c = 0; c < N; ++c) v[c] = p[c];
+    }
+}
+template <int N>
+__device__ __forceinline__ void stg_vec(float* p, const float (&v)[N]) {
+    if constexpr (N % 4 == 0) {
+#pragma unroll
+        for (int c = 0; c < N / 4; ++c)
+            reinterpret_cast<float4*>(p)[c] = make_float4(v[4 * c], v[4 * c + 1], v[4 * c + 2], v[4 * c + 3]);
+    } else if constexpr (N % 2 == 0) {
+#pragma unroll
+        for (int c = 0; c < N / 2; ++c) reinterpret_cast<float2*>(p)[c] = make_float2(v[2 * c], v[2 * c + 1]);
+    } else {
+#pragma unroll
+        for (int c = 0; c < N; ++c) p[c] = v[c];
+    }
+}
+template <int N>
+__device__ __forceinline__ void stg_vec(double* p, const double (&v)[N]) {
+    if constexpr (N % 2 == 0) {
+#pragma unroll
+        for (int c = 0; c < N / 2; ++c) reinterpret_cast<double2*>(p)[c] = make_double2(v[2 * c], v[2 * c + 1]);
+    } else {
+#pragma unroll
+        for (int c = 0; c < N; ++c) p[c] = v[c];
+    }
+}
+
+template <class T> __host__ __device__ constexpr int l2_hx(int P) {
+    // x halo in pairs, rounded up so that every staged row piece is a multiple of 16 bytes
+    return sizeof(T) == 4 ? (P + 1) / 2 * 2 : P;
+}
+
+template <int J, int N, class F>
+__device__ __forceinline__ void l2_static_for(F&& f) {
+    if constexpr (J < N) {
+        f(std::integral_constant<int, J>{});
+        l2_static_for<J + 1, N>(f);
+    }
+}
+
+// ------------------------------------------------------------------ kernel
+// NOPS = number of pointwise operand arrays of this stage:
+//   FHN  stage 0: 0 (y is the centre of the staged plane) | 1: y | 2: y, Y2 | 3: Z | RHS: 0
+//   KS   stage 0, 1: y | 2: y, Y2, Y3 | 3: Z | RHS: 0
+template <class T, int MODEL, int P, int X, int TY, int NOPS, int MAXT, int MINB = 1>
+__global__ void __launch_bounds__(MAXT, MINB) lattice3d_v2_kernel(Lat2Args a, ModelParams mp, Lat2 g) {
+    typedef typename PairOf<T>::type Pr;
+    constexpr int HX = l2_hx<T>(P);
+    constexpr int NCOL = X + 2 * HX;          // pairs loaded per staged row by one thread
+    constexpr int OFF = HX - P;               // loaded index of column x - P
+    constexpr int NACC = 2 * P + 1;
+    constexpr int NVS = MODEL == NET_MODEL_KS ? 1 : 2;   // scalars per element of the state arrays
+    constexpr int EW = X * NVS;               // scalars per thread-row of a state array
+
+    extern __shared__ __align__(128) unsigned char l2_smem[];
+    const int PW = g.PW, PH = g.PH, NS = g.NS, D = g.D;
+    uint64_t* full = reinterpret_cast<uint64_t*>(l2_smem);                       // NS barriers
+    int* table = reinterpret_cast<int*>(l2_smem + 128);                          // PH x MAXPIECE x 3
+    const int table_bytes = (PH * LAT2_MAXPIECE * 3 * 4 + 127) / 128 * 128;
+    Pr* ring = reinterpret_cast<Pr*>(l2_smem + 128 + table_bytes);
+    const int plane_pairs = PW * PH;
+
+    const int nx = g.nx, ny = g.ny, nz = g.nz;
+    const int64_t nxy = (int64_t)nx * ny;
+    int bid = blockIdx.x;
+    const int tix = bid % g.tiles_x; bid /= g.tiles_x;
+    const int tiy = bid % g.tiles_y; bid /= g.tiles_y;
+    const int x0 = tix * g.TXt, y0 = tiy * g.TYt;
+    const int z0 = bid * g.Lz;
+    const int z1 = min(nz, z0 + g.Lz);
+    const int tid = threadIdx.x;
+    const int q = tid % g.QX, st = tid / g.QX;
+    const int x = x0 + q * X;
+    const bool owner = st < g.SY && x < nx && q * X < g.TXt;
+    const int yrow0 = y0 + st * TY;
+
+    const Pr* __restrict__ Ein = (const Pr*)a.Ein;
+    const T* op0 = (const T*)a.op0;     // op1 may alias out2 (Z overwrites Y2 element by element)
+    const T* op1 = (const T*)a.op1;
+    const T* op2 = (const T*)a.op2;
+    const int stage = a.stage;
+    const T dt = (T)a.dt;
+
+    // ---- prologue: row-piece table (z independent), barriers
+    for (int r = tid; r < PH; r += blockDim.x) {
+        int gy = (y0 - P + r) % ny; if (gy < 0) gy += ny;
+        int start = x0 - HX, remaining = PW, dst = r * PW;
+        for (int pc = 0; pc < LAT2_MAXPIECE; ++pc) {
+            int xs = start % nx; if (xs < 0) xs += nx;
+            int len = remaining < nx - xs ? remaining : nx - xs;
+            table[(r * LAT2_MAXPIECE + pc) * 3 + 0] = gy * nx + xs;      // source pair index in a plane
+            table[(r * LAT2_MAXPIECE + pc) * 3 + 1] = dst;               // destination pair index
+            table[(r * LAT2_MAXPIECE + pc) * 3 + 2] = len;               // pairs (0 = unused piece)
+            start += len; remaining -= len; dst += len;
+        }
+    }
+    if (tid == 0) {
+        for (int s = 0; s < NS; ++s) mbar_init(full + s, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+
+    const unsigned plane_bytes = (unsigned)(plane_pairs * sizeof(Pr));
+    auto issue_plane = [&](int idx) {          // called by all lanes of warp 0
+        const int p = z0 - P + idx;
+        int zz = p % nz; if (zz < 0) zz += nz;
+        const int slot = idx % NS;
+        const Pr* src = Ein + (int64_t)zz * nxy;
+        Pr* dstb = ring + (size_t)slot * plane_pairs;
+        const int lane = tid & 31;
+        if (lane == 0) mbar_expect_tx(full + slot, plane_bytes);
+        __syncwarp();
+        for (int r = lane; r < PH; r += 32) {
+#pragma unroll
+            for (int pc = 0; pc < LAT2_MAXPIECE; ++pc) {
+                const int len = table[(r * LAT2_MAXPIECE + pc) * 3 + 2];
+                if (len > 0)
+                    bulk_g2s(dstb + table[(r * LAT2_MAXPIECE + pc) * 3 + 1],
+                             src + table[(r * LAT2_MAXPIECE + pc) * 3 + 0], (unsigned)(len * sizeof(Pr)),
+                             full + slot);
+            }
+        }
+    };
+
+    const int nplanes = (z1 - z0) + 2 * P;
+    if (tid < 32)
+        for (int idx = 0; idx <= D && idx < nplanes; ++idx) issue_plane(idx);
+
+    Pr acc[NACC][TY][X];
+#pragma unroll
+    for (int k = 0; k < NACC; ++k)
+#pragma unroll
+        for (int r = 0; r < TY; ++r)
+#pragma unroll
+            for (int i = 0; i < X; ++i) acc[k][r][i] = Pr{T(0), T(0)};
+
+    const int deg = g.n_ball - (g.include_self ? 0 : 1);
+    const T inv_deg = deg > 0 ? T(1) / T(deg) : T(0);
+
+    // One plane.  J = idx mod NACC selects, at compile time, which accumulator is which open
+    // output plane: accumulator (J + P + dz) mod NACC collects output plane p + dz.
+    auto do_plane = [&](int idx, auto Jc) {
+        constexpr int J = decltype(Jc)::value;
+        const int p = z0 - P + idx;
+        const int zo = p - P;
+        const int slot = idx % NS;
+        const bool finishing = owner && zo >= z0;
+        // pointwise operands of the plane finished in this iteration: issued before the wait
+        T o0[TY][EW], o1[TY][EW], o2[TY][EW], om[TY][X];
+        if (finishing) {
+#pragma unroll
+            for (int r = 0; r < TY; ++r) {
+                const int yy = yrow0 + r;
+                if (yy < ny) {
+                    const int64_t i = (int64_t)zo * nxy + (int64_t)yy * nx + x;
+                    if (NOPS >= 1) ldg_vec<EW>(op0 + i * NVS, o0[r]);
+                    if (NOPS >= 2) ldg_vec<EW>(op1 + i * NVS, o1[r]);
+                    if (NOPS >= 3) ldg_vec<EW>(op2 + i * NVS, o2[r]);
+                    if (MODEL == NET_MODEL_KS) ldg_vec<X>((const T*)a.omega + i, om[r]);
+                }
+            }
+        }
+        mbar_wait(full + slot, (unsigned)((idx / NS) & 1));
+        if (owner) {
+            const Pr* b = ring + (size_t)slot * plane_pairs + (st * TY) * PW + q * X;
+            Pr A[P > 1 ? P - 1 : 1][TY][X];      // in-plane sums of |dz| = 1 .. P-1
+            bool Aset[P > 1 ? P - 1 : 1][TY];
+#pragma unroll
+            for (int k = 0; k < (P > 1 ? P - 1 : 1); ++k)
+#pragma unroll
+                for (int r = 0; r < TY; ++r) Aset[k][r] = false;
+#pragma unroll
+            for (int rr = 0; rr < TY + 2 * P; ++rr) {           // staged row rr <-> y = yrow0 - P + rr
+                const int dist = rr < P ? P - rr : (rr >= TY + P ? rr - (TY + P - 1) : 0);
+                const int wmax = l2_run_w(P, 0, dist);
+                Pr v[NCOL];
+                const Pr* row = b + rr * PW;
+                if constexpr (sizeof(T) == 4) {
+#pragma unroll
+                    for (int c = 0; c < NCOL / 2; ++c) {
+                        float4 w4 = *reinterpret_cast<const float4*>(row + 2 * c);
+                        v[2 * c] = make_float2(w4.x, w4.y);
+                        v[2 * c + 1] = make_float2(w4.z, w4.w);
+                    }
+                } else {
+#pragma unroll
+                    for (int c = 0; c < NCOL; ++c) v[c] = row[c];
+                }
+                Pr R[P + 1][X];
+#pragma unroll
+                for (int i = 0; i < X; ++i) {
+                    R[0][i] = v[OFF + P + i];
+#pragma unroll
+                    for (int w = 1; w <= P; ++w)
+                        if (w <= wmax) R[w][i] = padd(R[w - 1][i], padd(v[OFF + P + i - w], v[OFF + P + i + w]));
+                }
+#pragma unroll
+                for (int r = 0; r < TY; ++r) {
+                    const int ady = rr - P - r < 0 ? -(rr - P - r) : rr - P - r;
+                    if (ady > P) continue;
+                    // |dz| = 0: straight into the accumulator of output plane p
+                    {
+                        const int w = l2_run_w(P, 0, ady);
+#pragma unroll
+                        for (int i = 0; i < X; ++i) acc[(J + P) % NACC][r][i] = padd(acc[(J + P) % NACC][r][i], R[w][i]);
+                    }
+                    // 0 < |dz| < P: in-plane partial sums
+#pragma unroll
+                    for (int k = 1; k < P; ++k) {
+                        const int w = l2_run_w(P, k, ady);
+                        if (w >= 0) {
+#pragma unroll
+                            for (int i = 0; i < X; ++i)
+                                A[k - 1][r][i] = Aset[k - 1][r] ? padd(A[k - 1][r][i], R[w][i]) : R[w][i];
+                            Aset[k - 1][r] = true;
+                        }
+                    }
+                    // |dz| = P: the centre point alone.  Output plane p + P sees its first
+                    // contribution (assignment), output plane p - P its last.
+                    if (ady == 0) {
+#pragma unroll
+                        for (int i = 0; i < X; ++i) {
+                            acc[(J + 2 * P) % NACC][r][i] = R[0][i];
+                            acc[J % NACC][r][i] = padd(acc[J % NACC][r][i], R[0][i]);
+                        }
+                    }
+                }
+            }
+#pragma unroll
+            for (int k = 1; k < P; ++k)
+#pragma unroll
+                for (int r = 0; r < TY; ++r)
+#pragma unroll
+                    for (int i = 0; i < X; ++i) {
+                        acc[(J + P - k) % NACC][r][i] = padd(acc[(J + P - k) % NACC][r][i], A[k - 1][r][i]);
+                        acc[(J + P + k) % NACC][r][i] = padd(acc[(J + P + k) % NACC][r][i], A[k - 1][r][i]);
+                    }
+        }
+        // ---- finish output plane zo (accumulator J)
+        if (finishing) {
+            int cslot = (idx - P) % NS;
+            const Pr* cb = ring + (size_t)cslot * plane_pairs + (st * TY + P) * PW + q * X + HX;
+#pragma unroll
+            for (int r = 0; r < TY; ++r) {
+                const int yy = yrow0 + r;
+                if (yy < ny) {
+                    const int64_t i = (int64_t)zo * nxy + (int64_t)yy * nx + x;
+                    T ov[EW], zv[EW], ev[2 * X];
+#pragma unroll
+                    for (int e = 0; e < X; ++e) {
+                        const Pr c = cb[r * PW + e];
+                        const Pr W = acc[J % NACC][r][e];
+                        T k[NVS], yv[NVS], y2[NVS], y3[NVS];
+                        if (MODEL == NET_MODEL_KS) {
+                            T C = W.x, S = W.y;
+                            if (!g.include_self) { C -= c.x; S -= c.y; }
+                            k[0] = ks_rhs_factorised<T>(mp, om[r][e], C, S, c.x, c.y, inv_deg);
+                            yv[0] = NOPS >= 1 ? o0[r][e] : T(0);
+                            y2[0] = NOPS >= 2 ? o1[r][e] : T(0);
+                            y3[0] = NOPS >= 3 ? o2[r][e] : T(0);
+                        } else {
+                            const T nb = T(g.n_ball);
+                            const T Cu = W.x - nb * c.x, Cv = W.y - nb * c.y;
+                            fhn_rhs<T>(mp, c.x, c.y, Cu, Cv, inv_deg, &k[0], &k[NVS - 1]);
+                            // stage 0: y is the stage input itself; stage 2: Y3 is
+                            yv[0] = NOPS >= 1 ? o0[r][2 * e] : c.x;
+                            yv[NVS - 1] = NOPS >= 1 ? o0[r][2 * e + 1] : c.y;
+                            y2[0] = NOPS >= 2 ? o1[r][2 * e] : T(0);
+                            y2[NVS - 1] = NOPS >= 2 ? o1[r][2 * e + 1] : T(0);
+                            y3[0] = c.x; y3[NVS - 1] = c.y;
+                        }
+#pragma unroll
+                        for (int vv = 0; vv < NVS; ++vv) {
+                            T o;
+                            if (stage <= 1) o = yv[vv] + (T(0.5) * dt) * k[vv];
+                            else if (stage == 2) {
+                                o = yv[vv] + dt * k[vv];
+                                zv[e * NVS + vv] = (y2[vv] + T(2) * y3[vv] + o - yv[vv]) * T(1.0 / 3.0);
+                            } else if (stage == 3) o = yv[vv] + (dt * T(1.0 / 6.0)) * k[vv];   // yv = Z
+                            else o = k[vv];
+                            ov[e * NVS + vv] = o;
+                        }
+                        if (MODEL == NET_MODEL_KS && stage != STAGE_RHS_ONLY) {
+                            T s_, c_;
+                            Math<T>::sincos(ov[e], &s_, &c_);
+                            ev[2 * e] = c_; ev[2 * e + 1] = s_;
+                        }
+                    }
+                    stg_vec<EW>((T*)a.out + i * NVS, ov);
+                    if (stage == 2) stg_vec<EW>((T*)a.out2 + i * NVS, zv);
+                    if (MODEL == NET_MODEL_KS && stage != STAGE_RHS_ONLY) stg_vec<2 * X>((T*)a.Eout + 2 * i, ev);
+                }
+            }
+        }
+        __syncthreads();
+        // the slot of plane p - P is free: refill it with plane p + D + 1
+        if (tid < 32 && idx + D + 1 < nplanes) issue_plane(idx + D + 1);
+    };
+
+    // planes in groups of NACC so that the accumulator roles are compile-time constants
+    for (int base = 0; base < nplanes; base += NACC)
+        l2_static_for<0, NACC>([&](auto Jc) {
+            if (base + decltype(Jc)::value < nplanes) do_plane(base + decltype(Jc)::value, Jc);
+        });
+}
+
+}  // namespace oscnet

@@ -102,6 +102,33 @@ struct Lat3 {
     int32_t include_self;
 };
 
+// launch geometry and arguments of the second-generation 3D lattice kernels (lattice_v2.cuh)
+constexpr int LAT2_MAXPIECE = 4;
+
+struct Lat2 {
+    int32_t nx, ny, nz;
+    int32_t QX, SY;            // threads per tile row / strips of TY rows
+    int32_t TXt, TYt;          // tile = TXt x TYt outputs
+    int32_t tiles_x, tiles_y;
+    int32_t Lz, nchunks;
+    int32_t PW, PH;            // staged plane: (TXt + 2 HX) x (TYt + 2 P) pairs
+    int32_t NS, D;             // ring slots = P + 1 + D, prefetch distance D
+    int32_t n_ball, include_self;
+};
+
+struct Lat2Args {
+    const void* Ein;           // stencil source: pairs [n]
+    const void* op0;           // pointwise operands (FHN: pairs; KS: scalars); see kernel
+    const void* op1;
+    const void* op2;
+    const void* omega;         // KS
+    void* out;                 // FHN pairs / KS scalar
+    void* out2;                // stage 2: Z
+    void* Eout;                // KS: pairs of the output state
+    double dt;
+    int32_t stage;
+};
+
 }  // namespace oscnet
 
 struct net {
@@ -134,6 +161,15 @@ struct net {
     unsigned lat_grid;
     int lat_threads;
     size_t lat_smem;
+    oscnet::Lat2 lat2;     // FAST_LATTICE3D_V2 launch geometry
+    unsigned lat2_grid;
+    int lat2_threads;
+    size_t lat2_smem;
+    void *E_a, *E_b;       // KS on FAST_LATTICE3D_V2: (cos, sin) pairs of the stage states
+    // state layout: variable v of element i at v*var_stride + i*elem_stride
+    // (SoA [nvar][ld]: ld, 1; interleaved pairs of FAST_LATTICE3D_V2 FHN: 1, 2)
+    int64_t var_stride, elem_stride;
+    int32_t pairs;         // 1 = interleaved layout
     char err[512];
 };
 
@@ -160,12 +196,16 @@ int32_t hh_compute_s(net* h, const void* V, void* s);     // s = S(V)
 int32_t hh_steady_gates(net* h);
 
 // csr_fast.cu / lattice_fast.cu / ring_fast.cu ------------------------------
-enum { FAST_NONE = 0, FAST_CSR_WARP = 1, FAST_LATTICE3D = 2, FAST_RING_FHN = 3, FAST_RING_KS = 4 };
+enum { FAST_NONE = 0, FAST_CSR_WARP = 1, FAST_LATTICE3D = 2, FAST_RING_FHN = 3, FAST_RING_KS = 4,
+       FAST_LATTICE3D_V2 = 5 };
 int32_t fast_select(const net_desc* d);                   // FAST_* available for this desc
 size_t fast_scratch_bytes(const net_desc* d, int32_t fast_kind);
 int32_t fast_prepare(net* h);                             // once, at the end of net_create
 int32_t fast_stage(net* h, const StageArgs& a);
 int32_t fast_integrate(net* h, int64_t n_steps, double dt, bool* handled);  // persistent kernels
+int32_t fast_refresh_exchange(net* h);                    // exchange fields of y (after set_state)
+int32_t pairs_pack(net* h, const void* soa, void* pairs);    // [2][ld] -> interleaved
+int32_t pairs_unpack(net* h, const void* pairs, void* soa);
 
 // observables.cu ------------------------------------------------------------
 int32_t obs_phase(net* h, const void* state, double* d_theta);
