@@ -69,7 +69,7 @@ static int32_t validate(net* h, const net_desc* d) {
 
 // Workspace layout.  Every region is 256-byte aligned.  `base` may be null (size query).
 struct Layout {
-    size_t total;
+    size_t total, state_bytes;
     Buffers b;
 };
 
@@ -87,10 +87,12 @@ static Layout make_layout(const net_desc* d, char* base) {
     const int64_t ld = round_up(d->n, 64);
     size_t cur = 0;
     auto P = [&](size_t bytes) -> void* { size_t at = take(cur, bytes); return base ? (void*)(base + at) : (void*)(uintptr_t)(at + 256); };
-    const size_t state = (size_t)nv * ld * es;
+    const int fk = d->method == NET_METHOD_DIRECT ? FAST_NONE : fast_select(d);
+    size_t state = (size_t)nv * ld * es;
+    if (fast_state_bytes(d, fk) > state) state = fast_state_bytes(d, fk);
+    L.state_bytes = state;
     L.b.y = P(state); L.b.Y2 = P(state); L.b.Y3 = P(state); L.b.Y4 = P(state);
     L.b.elem_param = P((size_t)ld * es);
-    const int fk = d->method == NET_METHOD_DIRECT ? FAST_NONE : fast_select(d);
     if (d->model == NET_MODEL_HH && fk == FAST_CSR_WARP) {
         L.b.s_y = P((size_t)ld * es); L.b.s_Y2 = P((size_t)ld * es);
         L.b.s_Y3 = P((size_t)ld * es); L.b.s_Y4 = P((size_t)ld * es);
@@ -313,8 +315,7 @@ int32_t net_create(const net_desc* desc, const void* params, size_t params_bytes
     h->ld = round_up(desc->n, 64);
     h->stream = (cudaStream_t)cuda_stream;
     h->b = L.b;
-    h->var_stride = h->ld;
-    h->elem_stride = 1;
+    h->state_bytes = L.state_bytes;
     fill_params(h, params);
     const int fk = desc->method == NET_METHOD_DIRECT ? FAST_NONE : fast_select(desc);
     if (desc->method == NET_METHOD_FAST && fk == FAST_NONE) {
@@ -333,7 +334,7 @@ int32_t net_create(const net_desc* desc, const void* params, size_t params_bytes
     if (rc == NET_OK) rc = fast_prepare(h);
     cudaError_t e = cudaSuccess;
     if (rc == NET_OK) {
-        size_t state = (size_t)h->nvar * h->ld * h->esize;
+        size_t state = h->state_bytes;
         e = cudaMemsetAsync(h->b.y, 0, state, h->stream);
         if (e == cudaSuccess) e = cudaMemsetAsync(h->b.Y2, 0, state, h->stream);
         if (e == cudaSuccess) e = cudaMemsetAsync(h->b.Y3, 0, state, h->stream);

@@ -9,6 +9,7 @@ int32_t lattice3d_prepare(net* h);
 int32_t lattice3d_stage(net* h, const StageArgs& a);
 bool lattice_v2_supported(const net_desc* d);
 size_t lattice_v2_scratch_bytes(const net_desc* d);
+size_t lattice_v2_state_bytes(const net_desc* d);
 int32_t lattice_v2_prepare(net* h);
 int32_t lattice_v2_stage(net* h, const StageArgs& a);
 int32_t lattice_v2_refresh_exchange(net* h);
@@ -29,6 +30,10 @@ size_t fast_scratch_bytes(const net_desc* d, int32_t fast_kind) {
     if (fast_kind == FAST_RING_KS || fast_kind == FAST_RING_FHN) return ring_scratch_bytes(d);
     if (fast_kind == FAST_LATTICE3D_V2) return lattice_v2_scratch_bytes(d);
     return 0;
+}
+
+size_t fast_state_bytes(const net_desc* d, int32_t fast_kind) {
+    return fast_kind == FAST_LATTICE3D_V2 ? lattice_v2_state_bytes(d) : 0;
 }
 
 // Launch geometry, shared-memory opt-in and occupancy of the selected family.  A family that

@@ -7,9 +7,11 @@
 //     INTERLEAVED as pairs, in global memory and in shared memory, so every add of the ball sum is
 //     one packed FADD2 (add.rn.f32x2) on an aligned register pair and every shared-memory access
 //     is a 16-byte LDS;
-//   * planes are staged by the bulk-copy engine: one cp.async.bulk (UBLKCP) per row piece,
-//     completing on an mbarrier, D planes ahead of the compute -- no register staging, no
-//     address arithmetic in the inner loop; the periodic wrap is resolved per row piece;
+//   * the pair fields live in GHOST-PADDED arrays (x padded by GX = halo rounded to 16 bytes, y by
+//     GY = P on both sides; the producer of a field also writes the periodic images), so every
+//     staged plane -- tile plus halo -- is ONE TMA tensor load (cp.async.bulk.tensor.3d,
+//     UTMALDG) completing on an mbarrier, issued D planes ahead of the compute by one thread:
+//     no register staging and no address arithmetic in the inner loop;
 //   * KS: the producing stage writes E = (cos phi, sin phi) of its output next to phi, so the
 //     sincos is paid exactly once per element per stage and halos are plain copies;
 //   * RK4 in the "Z form" (13 state records per step, at most two pointwise operands per stage):
@@ -19,6 +21,8 @@
 //     which is y + dt/6 (k1 + 2 k2 + 2 k3 + k4) with k_s recovered from the stage states.
 // Thread = X consecutive columns x TY rows; CTA = QX x SY threads; tile = (QX X) x (SY TY).
 #pragma once
+#include <cuda.h>
+
 #include <type_traits>
 
 #include "models.cuh"
@@ -63,9 +67,10 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, unsigned parity) {
         "bra WAIT_%=;\n\t"
         "DONE_%=:\n\t}" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
 }
-__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, unsigned bytes, uint64_t* bar) {
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-                 ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+__device__ __forceinline__ void tma_load_3d(void* dst, const CUtensorMap* tmap, int c0, int c1, int c2, uint64_t* bar) {
+    asm volatile(
+        "cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];"
+        ::"r"(smem_u32(dst)), "l"(tmap), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2) : "memory");
 }
 
 // N contiguous scalars from / to 16-byte (8-byte when N*sizeof == 8) aligned global memory
@@ -144,25 +149,28 @@ __device__ __forceinline__ void l2_static_for(F&& f) {
 //   FHN  stage 0: 0 (y is the centre of the staged plane) | 1: y | 2: y, Y2 | 3: Z | RHS: 0
 //   KS   stage 0, 1: y | 2: y, Y2, Y3 | 3: Z | RHS: 0
 template <class T, int MODEL, int P, int X, int TY, int NOPS, int MAXT, int MINB = 1>
-__global__ void __launch_bounds__(MAXT, MINB) lattice3d_v2_kernel(Lat2Args a, ModelParams mp, Lat2 g) {
+__global__ void __launch_bounds__(MAXT, MINB) lattice3d_v2_kernel(const __grid_constant__ CUtensorMap tmap,
+                                                                   Lat2Args a, ModelParams mp, Lat2 g) {
     typedef typename PairOf<T>::type Pr;
-    constexpr int HX = l2_hx<T>(P);
+    constexpr int HX = l2_hx<T>(P);           // = GX, the x ghost width of the padded arrays
     constexpr int NCOL = X + 2 * HX;          // pairs loaded per staged row by one thread
     constexpr int OFF = HX - P;               // loaded index of column x - P
     constexpr int NACC = 2 * P + 1;
     constexpr int NVS = MODEL == NET_MODEL_KS ? 1 : 2;   // scalars per element of the state arrays
     constexpr int EW = X * NVS;               // scalars per thread-row of a state array
+    constexpr int U8 = (int)sizeof(Pr) / 8;   // 8-byte TMA elements per pair
 
     extern __shared__ __align__(128) unsigned char l2_smem[];
     const int PW = g.PW, PH = g.PH, NS = g.NS, D = g.D;
     uint64_t* full = reinterpret_cast<uint64_t*>(l2_smem);                       // NS barriers
-    int* table = reinterpret_cast<int*>(l2_smem + 128);                          // PH x MAXPIECE x 3
-    const int table_bytes = (PH * LAT2_MAXPIECE * 3 * 4 + 127) / 128 * 128;
-    Pr* ring = reinterpret_cast<Pr*>(l2_smem + 128 + table_bytes);
-    const int plane_pairs = PW * PH;
+    const unsigned box_bytes = (unsigned)(PW * PH * sizeof(Pr));
+    const unsigned plane_bytes = (box_bytes + 127u) / 128u * 128u;
+    unsigned char* ring = l2_smem + 128;
 
     const int nx = g.nx, ny = g.ny, nz = g.nz;
-    const int64_t nxy = (int64_t)nx * ny;
+    const int nxp = nx + 2 * HX, nyp = ny + 2 * P;
+    const int64_t nxy = (int64_t)nx * ny;           // unpadded plane (KS scalar arrays)
+    const int64_t pxy = (int64_t)nxp * nyp;         // padded plane (pair arrays)
     int bid = blockIdx.x;
     const int tix = bid % g.tiles_x; bid /= g.tiles_x;
     const int tiy = bid % g.tiles_y; bid /= g.tiles_y;
@@ -174,58 +182,33 @@ __global__ void __launch_bounds__(MAXT, MINB) lattice3d_v2_kernel(Lat2Args a, Mo
     const int x = x0 + q * X;
     const bool owner = st < g.SY && x < nx && q * X < g.TXt;
     const int yrow0 = y0 + st * TY;
+    // periodic images this thread also writes: column shift (pairs) and row shift (rows), 0 = none
+    const int gxs = x < HX ? nx : (x >= nx - HX ? -nx : 0);
 
-    const Pr* __restrict__ Ein = (const Pr*)a.Ein;
     const T* op0 = (const T*)a.op0;     // op1 may alias out2 (Z overwrites Y2 element by element)
     const T* op1 = (const T*)a.op1;
     const T* op2 = (const T*)a.op2;
     const int stage = a.stage;
     const T dt = (T)a.dt;
 
-    // ---- prologue: row-piece table (z independent), barriers
-    for (int r = tid; r < PH; r += blockDim.x) {
-        int gy = (y0 - P + r) % ny; if (gy < 0) gy += ny;
-        int start = x0 - HX, remaining = PW, dst = r * PW;
-        for (int pc = 0; pc < LAT2_MAXPIECE; ++pc) {
-            int xs = start % nx; if (xs < 0) xs += nx;
-            int len = remaining < nx - xs ? remaining : nx - xs;
-            table[(r * LAT2_MAXPIECE + pc) * 3 + 0] = gy * nx + xs;      // source pair index in a plane
-            table[(r * LAT2_MAXPIECE + pc) * 3 + 1] = dst;               // destination pair index
-            table[(r * LAT2_MAXPIECE + pc) * 3 + 2] = len;               // pairs (0 = unused piece)
-            start += len; remaining -= len; dst += len;
-        }
-    }
     if (tid == 0) {
         for (int s = 0; s < NS; ++s) mbar_init(full + s, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        asm volatile("prefetch.tensormap [%0];" ::"l"(&tmap) : "memory");
     }
     __syncthreads();
 
-    const unsigned plane_bytes = (unsigned)(plane_pairs * sizeof(Pr));
-    auto issue_plane = [&](int idx) {          // called by all lanes of warp 0
-        const int p = z0 - P + idx;
-        int zz = p % nz; if (zz < 0) zz += nz;
-        const int slot = idx % NS;
-        const Pr* src = Ein + (int64_t)zz * nxy;
-        Pr* dstb = ring + (size_t)slot * plane_pairs;
-        const int lane = tid & 31;
-        if (lane == 0) mbar_expect_tx(full + slot, plane_bytes);
-        __syncwarp();
-        for (int r = lane; r < PH; r += 32) {
-#pragma unroll
-            for (int pc = 0; pc < LAT2_MAXPIECE; ++pc) {
-                const int len = table[(r * LAT2_MAXPIECE + pc) * 3 + 2];
-                if (len > 0)
-                    bulk_g2s(dstb + table[(r * LAT2_MAXPIECE + pc) * 3 + 1],
-                             src + table[(r * LAT2_MAXPIECE + pc) * 3 + 0], (unsigned)(len * sizeof(Pr)),
-                             full + slot);
-            }
-        }
+    // plane idx of this chunk (lattice plane z0 - P + idx, periodic) -> ring slot idx mod NS.
+    // The box starts at padded coordinates (x0, y0) = lattice (x0 - GX, y0 - P).
+    auto issue_plane = [&](int idx, int slot) {          // one thread
+        int zz = (z0 - P + idx) % nz; if (zz < 0) zz += nz;
+        mbar_expect_tx(full + slot, box_bytes);
+        tma_load_3d(ring + (size_t)slot * plane_bytes, &tmap, x0 * U8, y0, zz, full + slot);
     };
 
     const int nplanes = (z1 - z0) + 2 * P;
-    if (tid < 32)
-        for (int idx = 0; idx <= D && idx < nplanes; ++idx) issue_plane(idx);
+    if (tid == 0)
+        for (int idx = 0; idx <= D && idx < nplanes; ++idx) issue_plane(idx, idx);
 
     Pr acc[NACC][TY][X];
 #pragma unroll
@@ -240,11 +223,11 @@ __global__ void __launch_bounds__(MAXT, MINB) lattice3d_v2_kernel(Lat2Args a, Mo
 
     // One plane.  J = idx mod NACC selects, at compile time, which accumulator is which open
     // output plane: accumulator (J + P + dz) mod NACC collects output plane p + dz.
+    int slot = 0, cslot = NS - P, islot = (D + 1) % NS;   // ring slots of planes idx, idx - P, idx + D + 1
+    unsigned phase = 0;
     auto do_plane = [&](int idx, auto Jc) {
         constexpr int J = decltype(Jc)::value;
-        const int p = z0 - P + idx;
-        const int zo = p - P;
-        const int slot = idx % NS;
+        const int zo = z0 - 2 * P + idx;          // output plane completed by this iteration
         const bool finishing = owner && zo >= z0;
         // pointwise operands of the plane finished in this iteration: issued before the wait
         T o0[TY][EW], o1[TY][EW], o2[TY][EW], om[TY][X];
@@ -253,17 +236,20 @@ __global__ void __launch_bounds__(MAXT, MINB) lattice3d_v2_kernel(Lat2Args a, Mo
             for (int r = 0; r < TY; ++r) {
                 const int yy = yrow0 + r;
                 if (yy < ny) {
-                    const int64_t i = (int64_t)zo * nxy + (int64_t)yy * nx + x;
-                    if (NOPS >= 1) ldg_vec<EW>(op0 + i * NVS, o0[r]);
-                    if (NOPS >= 2) ldg_vec<EW>(op1 + i * NVS, o1[r]);
-                    if (NOPS >= 3) ldg_vec<EW>(op2 + i * NVS, o2[r]);
+                    // state arrays: FHN padded pairs, KS plain scalars
+                    const int64_t i = MODEL == NET_MODEL_KS
+                        ? (int64_t)zo * nxy + (int64_t)yy * nx + x
+                        : ((int64_t)zo * pxy + (int64_t)(yy + P) * nxp + (x + HX)) * 2;
+                    if (NOPS >= 1) ldg_vec<EW>(op0 + i, o0[r]);
+                    if (NOPS >= 2) ldg_vec<EW>(op1 + i, o1[r]);
+                    if (NOPS >= 3) ldg_vec<EW>(op2 + i, o2[r]);
                     if (MODEL == NET_MODEL_KS) ldg_vec<X>((const T*)a.omega + i, om[r]);
                 }
             }
         }
-        mbar_wait(full + slot, (unsigned)((idx / NS) & 1));
+        mbar_wait(full + slot, phase);
         if (owner) {
-            const Pr* b = ring + (size_t)slot * plane_pairs + (st * TY) * PW + q * X;
+            const Pr* b = reinterpret_cast<const Pr*>(ring + (size_t)slot * plane_bytes) + (st * TY) * PW + q * X;
             Pr A[P > 1 ? P - 1 : 1][TY][X];      // in-plane sums of |dz| = 1 .. P-1
             bool Aset[P > 1 ? P - 1 : 1][TY];
 #pragma unroll
@@ -339,13 +325,22 @@ __global__ void __launch_bounds__(MAXT, MINB) lattice3d_v2_kernel(Lat2Args a, Mo
         }
         // ---- finish output plane zo (accumulator J)
         if (finishing) {
-            int cslot = (idx - P) % NS;
-            const Pr* cb = ring + (size_t)cslot * plane_pairs + (st * TY + P) * PW + q * X + HX;
+            const Pr* cb = reinterpret_cast<const Pr*>(ring + (size_t)cslot * plane_bytes) + (st * TY + P) * PW + q * X + HX;
 #pragma unroll
             for (int r = 0; r < TY; ++r) {
                 const int yy = yrow0 + r;
                 if (yy < ny) {
-                    const int64_t i = (int64_t)zo * nxy + (int64_t)yy * nx + x;
+                    const int64_t il = (int64_t)zo * nxy + (int64_t)yy * nx + x;                    // plain scalar arrays
+                    const int64_t ip = (int64_t)zo * pxy + (int64_t)(yy + P) * nxp + (x + HX);     // padded pair arrays
+                    const int gys = yy < P ? ny : (yy >= ny - P ? -ny : 0);
+                    auto store_pairs = [&](T* base, const T (&vals)[2 * X]) {    // with the periodic images
+                        stg_vec<2 * X>(base + 2 * ip, vals);
+                        if (gxs != 0) stg_vec<2 * X>(base + 2 * (ip + gxs), vals);
+                        if (gys != 0) {
+                            stg_vec<2 * X>(base + 2 * (ip + (int64_t)gys * nxp), vals);
+                            if (gxs != 0) stg_vec<2 * X>(base + 2 * (ip + (int64_t)gys * nxp + gxs), vals);
+                        }
+                    };
                     T ov[EW], zv[EW], ev[2 * X];
 #pragma unroll
                     for (int e = 0; e < X; ++e) {
@@ -387,15 +382,24 @@ __global__ void __launch_bounds__(MAXT, MINB) lattice3d_v2_kernel(Lat2Args a, Mo
                             ev[2 * e] = c_; ev[2 * e + 1] = s_;
                         }
                     }
-                    stg_vec<EW>((T*)a.out + i * NVS, ov);
-                    if (stage == 2) stg_vec<EW>((T*)a.out2 + i * NVS, zv);
-                    if (MODEL == NET_MODEL_KS && stage != STAGE_RHS_ONLY) stg_vec<2 * X>((T*)a.Eout + 2 * i, ev);
+                    if constexpr (MODEL == NET_MODEL_KS) {
+                        stg_vec<EW>((T*)a.out + il, ov);
+                        if (stage == 2) stg_vec<EW>((T*)a.out2 + il, zv);
+                        if (stage != STAGE_RHS_ONLY) store_pairs((T*)a.Eout, ev);
+                    } else {
+                        store_pairs((T*)a.out, ov);
+                        if (stage == 2) stg_vec<EW>((T*)a.out2 + 2 * ip, zv);    // Z is never a stencil source
+                    }
                 }
             }
         }
         __syncthreads();
-        // the slot of plane p - P is free: refill it with plane p + D + 1
-        if (tid < 32 && idx + D + 1 < nplanes) issue_plane(idx + D + 1);
+        // the slot of plane idx - P is free: refill it with plane idx + D + 1
+        if (tid == 0 && idx + D + 1 < nplanes) issue_plane(idx + D + 1, islot);
+        slot = slot + 1 == NS ? 0 : slot + 1;
+        cslot = cslot + 1 == NS ? 0 : cslot + 1;
+        islot = islot + 1 == NS ? 0 : islot + 1;
+        if (slot == 0) phase ^= 1u;
     };
 
     // planes in groups of NACC so that the accumulator roles are compile-time constants

@@ -1,8 +1,8 @@
-// fp32 instantiations of the second-generation 3D lattice kernels (lattice_v2.cuh).
+// f32 instantiations of the second-generation 3D lattice kernels (lattice_v2.cuh).
 #include "lattice_v2_host.cuh"
 
 namespace oscnet {
-int32_t lattice_v2_entry_f32(net* h, const Lat2Args* a, int nops, Lat2* g, int* threads, size_t* smem, unsigned* grid) {
-    return l2_entry<float>(h, a, nops, g, threads, smem, grid);
+int32_t lattice_v2_entry_f32(net* h, const Lat2Args* a, int nops, int which_map) {
+    return l2_entry<float>(h, a, nops, which_map);
 }
 }  // namespace oscnet

@@ -11,15 +11,14 @@ constexpr int RED_BLOCKS = 592;  // 4 per SM
 constexpr int RED_THREADS = 256;
 
 template <class T>
-__global__ void phase_kernel(const T* __restrict__ y, int64_t n, int64_t vs, int64_t es, int model,
+__global__ void phase_kernel(const T* __restrict__ y, int64_t n, int64_t ld, int model,
                              ModelParams mp, double* __restrict__ theta) {
-    // variable v of element i at v*vs + i*es (SoA or interleaved pairs)
     for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n;
          i += (int64_t)gridDim.x * blockDim.x) {
         double th;
-        if (model == NET_MODEL_KS) th = (double)y[i * es];
-        else if (model == NET_MODEL_FHN) th = atan2((double)y[vs + i * es], (double)y[i * es]);
-        else th = atan2((double)y[3 * vs + i * es] - mp.n_c, ((double)y[i * es] - mp.V_c) * mp.inv_V_s);
+        if (model == NET_MODEL_KS) th = (double)y[i];
+        else if (model == NET_MODEL_FHN) th = atan2((double)y[ld + i], (double)y[i]);
+        else th = atan2((double)y[3 * ld + i] - mp.n_c, ((double)y[i] - mp.V_c) * mp.inv_V_s);
         theta[i] = th;
     }
 }
@@ -110,10 +109,15 @@ static unsigned grid_for(int64_t items) {
 }
 
 int32_t obs_phase(net* h, const void* state, double* d_theta) {
+    if (h->pairs) {   // padded pair layout: through Y3 (dead between steps) as SoA
+        int32_t rc = pairs_unpack(h, state, h->b.Y3);
+        if (rc) return rc;
+        state = h->b.Y3;
+    }
     if (h->desc.dtype == NET_F32)
-        phase_kernel<float><<<grid_for(h->n), 256, 0, h->stream>>>((const float*)state, h->n, h->var_stride, h->elem_stride, h->desc.model, h->mp, d_theta);
+        phase_kernel<float><<<grid_for(h->n), 256, 0, h->stream>>>((const float*)state, h->n, h->ld, h->desc.model, h->mp, d_theta);
     else
-        phase_kernel<double><<<grid_for(h->n), 256, 0, h->stream>>>((const double*)state, h->n, h->var_stride, h->elem_stride, h->desc.model, h->mp, d_theta);
+        phase_kernel<double><<<grid_for(h->n), 256, 0, h->stream>>>((const double*)state, h->n, h->ld, h->desc.model, h->mp, d_theta);
     h->launches += 1;
     OSC_CUDA(h, cudaGetLastError());
     return NET_OK;

@@ -1,6 +1,7 @@
 // Internal declarations shared by the translation units of liboscnet.so.
 // Nothing here is part of the C ABI (include/oscnet.h is).
 #pragma once
+#include <cuda.h>
 #include <cuda_runtime.h>
 #include <stdint.h>
 #include <stdio.h>
@@ -161,15 +162,14 @@ struct net {
     unsigned lat_grid;
     int lat_threads;
     size_t lat_smem;
+    CUtensorMap tmap[4];   // FAST_LATTICE3D_V2: TMA maps of the stencil sources (FHN y,Y2,Y3,Y4; KS E_a,E_b)
+    size_t state_bytes;    // bytes of each of y, Y2, Y3, Y4
     oscnet::Lat2 lat2;     // FAST_LATTICE3D_V2 launch geometry
     unsigned lat2_grid;
     int lat2_threads;
     size_t lat2_smem;
     void *E_a, *E_b;       // KS on FAST_LATTICE3D_V2: (cos, sin) pairs of the stage states
-    // state layout: variable v of element i at v*var_stride + i*elem_stride
-    // (SoA [nvar][ld]: ld, 1; interleaved pairs of FAST_LATTICE3D_V2 FHN: 1, 2)
-    int64_t var_stride, elem_stride;
-    int32_t pairs;         // 1 = interleaved layout
+    int32_t pairs;         // 1 = state arrays are ghost-padded interleaved pairs (FHN on FAST_LATTICE3D_V2)
     char err[512];
 };
 
@@ -200,11 +200,12 @@ enum { FAST_NONE = 0, FAST_CSR_WARP = 1, FAST_LATTICE3D = 2, FAST_RING_FHN = 3, 
        FAST_LATTICE3D_V2 = 5 };
 int32_t fast_select(const net_desc* d);                   // FAST_* available for this desc
 size_t fast_scratch_bytes(const net_desc* d, int32_t fast_kind);
+size_t fast_state_bytes(const net_desc* d, int32_t fast_kind);   // 0 = the default nvar*ld elements
 int32_t fast_prepare(net* h);                             // once, at the end of net_create
 int32_t fast_stage(net* h, const StageArgs& a);
 int32_t fast_integrate(net* h, int64_t n_steps, double dt, bool* handled);  // persistent kernels
 int32_t fast_refresh_exchange(net* h);                    // exchange fields of y (after set_state)
-int32_t pairs_pack(net* h, const void* soa, void* pairs);    // [2][ld] -> interleaved
+int32_t pairs_pack(net* h, const void* soa, void* pairs);    // SoA [2][ld] -> padded pairs (+ ghosts)
 int32_t pairs_unpack(net* h, const void* pairs, void* soa);
 
 // observables.cu ------------------------------------------------------------
