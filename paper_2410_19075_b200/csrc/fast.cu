@@ -13,6 +13,9 @@ size_t lattice_v2_state_bytes(const net_desc* d);
 int32_t lattice_v2_prepare(net* h);
 int32_t lattice_v2_stage(net* h, const StageArgs& a);
 int32_t lattice_v2_refresh_exchange(net* h);
+bool lattice_v3_supported(const net_desc* d);
+int32_t lattice_v3_prepare(net* h);
+int32_t lattice_v3_stage(net* h, const StageArgs& a);
 bool ring_supported(const net_desc* d);
 size_t ring_scratch_bytes(const net_desc* d);
 int32_t ring_run(net* h, const void* y_in, void* y_out, int64_t n_steps, double dt, int rhs_only);
@@ -20,6 +23,7 @@ int32_t ring_run(net* h, const void* y_in, void* y_out, int64_t n_steps, double 
 int32_t fast_select(const net_desc* d) {
     const net_topology& t = d->topo;
     if (t.kind == NET_TOPO_CSR || t.kind == NET_TOPO_RANDOM_INDEGREE) return FAST_CSR_WARP;
+    if (lattice_v3_supported(d)) return FAST_LATTICE3D_V3;
     if (lattice_v2_supported(d)) return FAST_LATTICE3D_V2;
     if (lattice3d_supported(d)) return FAST_LATTICE3D;
     if (ring_supported(d)) return d->model == NET_MODEL_KS ? FAST_RING_KS : FAST_RING_FHN;
@@ -28,18 +32,25 @@ int32_t fast_select(const net_desc* d) {
 
 size_t fast_scratch_bytes(const net_desc* d, int32_t fast_kind) {
     if (fast_kind == FAST_RING_KS || fast_kind == FAST_RING_FHN) return ring_scratch_bytes(d);
-    if (fast_kind == FAST_LATTICE3D_V2) return lattice_v2_scratch_bytes(d);
+    if (fast_kind == FAST_LATTICE3D_V2 || fast_kind == FAST_LATTICE3D_V3) return lattice_v2_scratch_bytes(d);
     return 0;
 }
 
 size_t fast_state_bytes(const net_desc* d, int32_t fast_kind) {
-    return fast_kind == FAST_LATTICE3D_V2 ? lattice_v2_state_bytes(d) : 0;
+    return fast_kind == FAST_LATTICE3D_V2 || fast_kind == FAST_LATTICE3D_V3 ? lattice_v2_state_bytes(d) : 0;
 }
 
 // Launch geometry, shared-memory opt-in and occupancy of the selected family.  A family that
 // cannot take this shape (NET_ERR_UNSUPPORTED) falls back to DIRECT unless FAST was demanded.
 int32_t fast_prepare(net* h) {
     int32_t rc = NET_OK;
+    if (h->fast_kind == FAST_LATTICE3D_V3) {
+        rc = lattice_v3_prepare(h);
+        if (rc == NET_ERR_UNSUPPORTED) {     // same layout, second-generation kernels
+            h->fast_kind = FAST_LATTICE3D_V2;
+            rc = NET_OK;
+        }
+    }
     if (h->fast_kind == FAST_LATTICE3D_V2) {
         rc = lattice_v2_prepare(h);
         if (rc == NET_ERR_UNSUPPORTED) {     // shape the bulk-copy kernels cannot take: first generation
@@ -63,6 +74,7 @@ int32_t fast_stage(net* h, const StageArgs& a) {
         case FAST_CSR_WARP: return csr_warp_stage(h, a);
         case FAST_LATTICE3D: return lattice3d_stage(h, a);
         case FAST_LATTICE3D_V2: return lattice_v2_stage(h, a);
+        case FAST_LATTICE3D_V3: return lattice_v3_stage(h, a);
         case FAST_RING_KS:
         case FAST_RING_FHN:
             // the ring family integrates whole runs (fast_integrate); as a stage it only serves
@@ -75,7 +87,7 @@ int32_t fast_stage(net* h, const StageArgs& a) {
 }
 
 int32_t fast_refresh_exchange(net* h) {
-    if (h->fast_kind == FAST_LATTICE3D_V2) return lattice_v2_refresh_exchange(h);
+    if (h->fast_kind == FAST_LATTICE3D_V2 || h->fast_kind == FAST_LATTICE3D_V3) return lattice_v2_refresh_exchange(h);
     return NET_OK;
 }
 

@@ -1,0 +1,8 @@
+// f32 fhn instantiations of the third-generation 3D lattice kernels (lat3_kernel.cuh).
+#include "lat3_host.cuh"
+
+namespace oscnet {
+int32_t lattice_v3_entry_f32_fhn(net* h, int stage, double dt, void* rhs_out) {
+    return l3_entry<float, NET_MODEL_FHN>(h, stage, dt, rhs_out);
+}
+}  // namespace oscnet

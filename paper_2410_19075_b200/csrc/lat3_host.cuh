@@ -1,0 +1,268 @@
+// Host side of the third-generation 3D lattice kernels (lat3_kernel.cuh): tile / pipeline /
+// chunk selection, TMA tensor maps of the stencil sources and of the operand tiles, launch.
+// Included by one translation unit per (dtype, model) so that the build stays parallel.
+#pragma once
+#include <stdlib.h>
+
+#include "lat3_kernel.cuh"
+
+namespace oscnet {
+
+// thread shape per (dtype, P): X columns x TY rows of outputs per thread
+template <class T, int P> struct L3Shape;
+template <> struct L3Shape<float, 2> { static constexpr int X = 2, TY = 4; };
+template <> struct L3Shape<float, 4> { static constexpr int X = 2, TY = 2; };
+template <> struct L3Shape<double, 2> { static constexpr int X = 2, TY = 2; };
+template <> struct L3Shape<double, 4> { static constexpr int X = 2, TY = 1; };
+constexpr int L3_MAXT = 288;     // up to 8 consumer warps + the producer warp
+constexpr int L3_MINB = 1;
+
+typedef CUresult (*l3_encode_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                 const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                 CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+inline int32_t l3_encoder(net* h, l3_encode_fn* out) {
+    static l3_encode_fn encode = nullptr;
+    if (!encode) {
+        void* fn = nullptr;
+        cudaDriverEntryPointQueryResult qres;
+        cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres);
+        if (e != cudaSuccess || qres != cudaDriverEntryPointSuccess || !fn)
+            return set_err(h, NET_ERR_CUDA, "cuTensorMapEncodeTiled is not available from the driver");
+        encode = (l3_encode_fn)fn;
+    }
+    *out = encode;
+    return NET_OK;
+}
+
+// 3D map over an array of `esz`-byte elements (4 or 8) with extents (ex, ey, ez) and box (bx, by, 1)
+inline int32_t l3_encode(net* h, CUtensorMap* tm, void* base, int esz, uint64_t ex, uint64_t ey, uint64_t ez,
+                         uint32_t bx, uint32_t by) {
+    l3_encode_fn encode;
+    int32_t rc = l3_encoder(h, &encode);
+    if (rc) return rc;
+    cuuint64_t dims[3] = {ex, ey, ez};
+    cuuint64_t strides[2] = {ex * (uint64_t)esz, ex * ey * (uint64_t)esz};
+    cuuint32_t box[3] = {bx, by, 1};
+    cuuint32_t estr[3] = {1, 1, 1};
+    CUresult r = encode(tm, esz == 4 ? CU_TENSOR_MAP_DATA_TYPE_UINT32 : CU_TENSOR_MAP_DATA_TYPE_UINT64, 3, base,
+                        dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                        CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return set_err(h, NET_ERR_CUDA, "cuTensorMapEncodeTiled failed (%d)", (int)r);
+    return NET_OK;
+}
+
+template <class T, int MODEL, int P, int STAGE>
+static auto l3_kernel_ptr() {
+    typedef L3Shape<T, P> S;
+    return lat3_kernel<T, MODEL, P, STAGE, S::X, S::TY, L3_MAXT, L3_MINB>;
+}
+
+inline size_t l3_smem_bytes(const L3Geom& g, int P, int nt) {
+    return 256 + (size_t)(P + 1 + g.D) * g.st_stride + (size_t)(g.D + 1) * nt * g.op_stride;
+}
+
+// Geometry of one stage.  Tiles: the (TXt, SY) with the best lane / cover efficiency among
+// those whose staged boxes TMA can take; pipeline depth D: the deepest that still leaves
+// `want_ctas` CTAs per SM; z chunks: fewest waves.  OSCNET_LAT3 = "TXt,SY,Lz,D,CTAS" overrides.
+template <class T, int MODEL, int P, int STAGE>
+static int32_t l3_configure_stage(net* h) {
+    typedef L3Shape<T, P> S;
+    constexpr int X = S::X, TY = S::TY;
+    constexpr int HX = l2_hx<T>(P);
+    constexpr int U8 = 2 * (int)sizeof(T) / 8;
+    constexpr bool KS = MODEL == NET_MODEL_KS;
+    constexpr int NT = L3Ops<MODEL, STAGE>::N;
+    const TopoView& tv = h->tv;
+    L3Geom g;
+    memset(&g, 0, sizeof(g));
+    g.nx = tv.nx; g.ny = tv.ny; g.nz = tv.nz;
+    int want_tx = 0, want_sy = 0, want_lz = 0, want_d = 0, want_ctas = 0;
+    if (const char* e = getenv("OSCNET_LAT3")) sscanf(e, "%d,%d,%d,%d,%d", &want_tx, &want_sy, &want_lz, &want_d, &want_ctas);
+    if (want_ctas <= 0) want_ctas = 2;
+    // operand / stencil rows must be whole 16-byte vectors: scalar f32 tiles need TXt % 4 == 0
+    const int xq = (KS && sizeof(T) == 4) ? 4 : X;
+    if (g.nx % xq != 0) return NET_ERR_UNSUPPORTED;
+    double best = -1.0;
+    for (int tiles_x = 1; tiles_x <= g.nx / xq; ++tiles_x) {
+        int TXt = ((g.nx + tiles_x - 1) / tiles_x + xq - 1) / xq * xq;
+        if (want_tx > 0) TXt = (want_tx + xq - 1) / xq * xq;
+        if (TXt > g.nx) TXt = g.nx;
+        const int tx = (g.nx + TXt - 1) / TXt;
+        const int QX = TXt / X;
+        if ((TXt + 2 * HX) * U8 > 256) { if (want_tx > 0) return NET_ERR_UNSUPPORTED; continue; }
+        for (int SY = 1; SY * QX <= L3_MAXT - 32 && SY * TY <= 256 - 2 * P; ++SY) {
+            if (want_sy > 0 && SY != want_sy) continue;
+            const int TYt = SY * TY, ty = (g.ny + TYt - 1) / TYt;
+            const int threads = QX * SY, warps = (threads + 31) / 32;
+            const double lane_eff = (double)threads / (32.0 * warps);
+            const double cover = (double)g.nx * g.ny / ((double)tx * TXt * ty * TYt);
+            const double halo = (double)(TXt + 2 * HX) * (TYt + 2 * P) / ((double)TXt * TYt);
+            // small CTAs (about four consumer warps) desynchronise better; mild preference
+            const double size_pen = warps <= 4 ? 1.0 : 1.0 - 0.02 * (warps - 4);
+            const double score = lane_eff * cover * size_pen / (1.0 + 0.25 * (halo - 1.0));
+            if (score > best) { best = score; g.TXt = TXt; g.TYt = TYt; g.QX = QX; g.SY = SY; g.tiles_x = tx; g.tiles_y = ty; }
+        }
+        if (want_tx > 0) break;
+    }
+    if (best < 0) return NET_ERR_UNSUPPORTED;
+    g.PW = g.TXt + 2 * HX;
+    g.PH = g.TYt + 2 * P;
+    g.ncw = (g.QX * g.SY + 31) / 32;
+    g.st_bytes = (unsigned)((size_t)g.PW * g.PH * 2 * sizeof(T));
+    g.st_stride = (g.st_bytes + 127u) / 128u * 128u;
+    g.op_bytes = (unsigned)((size_t)g.TXt * g.TYt * (KS ? 1 : 2) * sizeof(T));
+    g.op_stride = (g.op_bytes + 127u) / 128u * 128u;
+    const int threads = 32 * (g.ncw + 1);
+    auto kern = l3_kernel_ptr<T, MODEL, P, STAGE>();
+    int dev = 0, sms = 148;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    const size_t smem_cap = 227 * 1024;
+    g.D = 0;
+    for (int D = 4; D >= 1; --D) {
+        g.D = D;
+        if (want_d > 0) g.D = want_d;
+        if (l3_smem_bytes(g, P, NT) * want_ctas + 1024 * want_ctas <= smem_cap || want_d > 0) break;
+        g.D = 0;
+    }
+    if (g.D == 0) {      // not even D = 1 at the wanted occupancy: one CTA per SM, deepest pipeline that fits
+        for (int D = 4; D >= 1 && g.D == 0; --D) { g.D = D; if (l3_smem_bytes(g, P, NT) + 1024 > smem_cap) g.D = 0; }
+        if (g.D == 0) return NET_ERR_UNSUPPORTED;
+    }
+    const size_t smem = l3_smem_bytes(g, P, NT);
+    if (smem + 1024 > smem_cap) return NET_ERR_UNSUPPORTED;
+    OSC_CUDA(h, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    int occ = 0;
+    OSC_CUDA(h, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, threads, smem));
+    if (occ < 1) return NET_ERR_UNSUPPORTED;
+    const int64_t slots = (int64_t)occ * sms, tiles = (int64_t)g.tiles_x * g.tiles_y;
+    int64_t best_cost = -1;
+    for (int nch = 1; nch <= g.nz; ++nch) {
+        const int Lz = (g.nz + nch - 1) / nch;
+        const int chunks = (g.nz + Lz - 1) / Lz;
+        const int64_t waves = (tiles * chunks + slots - 1) / slots;
+        const int64_t cost = waves * (Lz + 2 * P + 4);
+        if (best_cost < 0 || cost < best_cost) { best_cost = cost; g.Lz = Lz; g.nchunks = chunks; }
+    }
+    if (want_lz > 0) { g.Lz = want_lz; g.nchunks = (g.nz + g.Lz - 1) / g.Lz; }
+    h->lat3[STAGE] = g;
+    h->lat3_threads[STAGE] = threads;
+    h->lat3_smem[STAGE] = smem;
+    h->lat3_grid[STAGE] = (unsigned)(tiles * g.nchunks);
+    if (getenv("OSCNET_VERBOSE"))
+        fprintf(stderr, "lat3 stage %d: tile %dx%d (QX %d SY %d, %d consumer warps) tiles %dx%d Lz %d chunks %d D %d smem %zu occ %d grid %u\n",
+                STAGE, g.TXt, g.TYt, g.QX, g.SY, g.ncw, g.tiles_x, g.tiles_y, g.Lz, g.nchunks, g.D, smem, occ, h->lat3_grid[STAGE]);
+    return NET_OK;
+}
+
+template <class T, int MODEL, int P>
+static int32_t l3_configure(net* h) {
+    constexpr int HX = l2_hx<T>(P);
+    constexpr int U8 = 2 * (int)sizeof(T) / 8;
+    constexpr bool KS = MODEL == NET_MODEL_KS;
+    int32_t rc;
+    if ((rc = l3_configure_stage<T, MODEL, P, L3_S0>(h))) return rc;
+    if ((rc = l3_configure_stage<T, MODEL, P, L3_S1>(h))) return rc;
+    if ((rc = l3_configure_stage<T, MODEL, P, L3_S2>(h))) return rc;
+    if ((rc = l3_configure_stage<T, MODEL, P, L3_S3>(h))) return rc;
+    if ((rc = l3_configure_stage<T, MODEL, P, L3_RHS>(h))) return rc;
+    // the tile is the same for every stage (only D differs), so one set of maps serves all
+    const L3Geom& g = h->lat3[0];
+    const uint64_t nxp = (uint64_t)g.nx + 2 * HX, nyp = (uint64_t)g.ny + 2 * P;
+    void* st_src[4] = {h->b.y, h->b.Y2, h->b.Y3, h->b.Y4};
+    if (KS) { st_src[0] = h->E_a; st_src[1] = h->E_b; }
+    for (int k = 0; k < (KS ? 2 : 4); ++k)
+        if ((rc = l3_encode(h, &h->tm3_st[k], st_src[k], 8, nxp * U8, nyp, (uint64_t)g.nz, (uint32_t)(g.PW * U8), (uint32_t)g.PH))) return rc;
+    if (KS) {
+        void* op_src[4] = {h->b.y, h->b.Y2, h->b.Y3, h->b.elem_param};
+        for (int k = 0; k < 4; ++k)
+            if ((rc = l3_encode(h, &h->tm3_op[k], op_src[k], (int)sizeof(T), (uint64_t)g.nx, (uint64_t)g.ny, (uint64_t)g.nz, (uint32_t)g.TXt, (uint32_t)g.TYt))) return rc;
+    } else {
+        void* op_src[2] = {h->b.y, h->b.Y2};
+        for (int k = 0; k < 2; ++k)
+            if ((rc = l3_encode(h, &h->tm3_op[k], op_src[k], 8, nxp * U8, nyp, (uint64_t)g.nz, (uint32_t)(g.TXt * U8), (uint32_t)g.TYt))) return rc;
+        h->tm3_op[2] = h->tm3_op[0];
+        h->tm3_op[3] = h->tm3_op[0];
+    }
+    return NET_OK;
+}
+
+template <class T, int MODEL, int P>
+static L3Params<T> l3_params(const net* h, int stage, double dt) {
+    L3Params<T> p;
+    memset(&p, 0, sizeof(p));
+    const ModelParams& mp = h->mp;
+    const int n_ball = h->tv.noff + (h->tv.include_self ? 0 : 1);
+    const int deg = h->tv.noff;
+    const double inv_deg = deg > 0 ? 1.0 / deg : 0.0;
+    const double hh = stage == 0 || stage == 1 ? 0.5 * dt : stage == 2 ? dt : stage == 3 ? dt / 6.0 : 0.0;
+    p.h = (T)hh;
+    p.nb = (T)n_ball;
+    const double s = mp.sigma * inv_deg;
+    p.cuu = (T)(s * mp.buu * mp.inv_eps); p.cuv = (T)(s * mp.buv * mp.inv_eps);
+    p.cvu = (T)(s * mp.bvu); p.cvv = (T)(s * mp.bvv);
+    p.ie = (T)mp.inv_eps; p.ie3 = (T)(-mp.inv_eps / 3.0); p.a = (T)mp.a;
+    p.kd = (T)(mp.K * inv_deg); p.ca = (T)mp.cos_a; p.sa = (T)mp.sin_a;
+    p.include_self = h->tv.include_self;
+    return p;
+}
+
+template <class T, int MODEL, int P, int STAGE>
+static int32_t l3_launch_stage(net* h, const L3Ptrs& a, double dt, const CUtensorMap& st, const CUtensorMap* op) {
+    auto kern = l3_kernel_ptr<T, MODEL, P, STAGE>();
+    const L3Params<T> p = l3_params<T, MODEL, P>(h, STAGE, dt);
+    kern<<<h->lat3_grid[STAGE], h->lat3_threads[STAGE], h->lat3_smem[STAGE], h->stream>>>(
+        st, op[0], op[1], op[2], op[3], a, p, h->lat3[STAGE]);
+    h->launches += 1;
+    OSC_CUDA(h, cudaGetLastError());
+    return NET_OK;
+}
+
+// Buffer roles per stage (Z form): in = y, Y2, Y3, Y4; out = Y2, Y3, Y4 (+ Z into Y2), y.
+template <class T, int MODEL, int P>
+static int32_t l3_stage(net* h, int stage, double dt, void* rhs_out) {
+    constexpr bool KS = MODEL == NET_MODEL_KS;
+    const Buffers& b = h->b;
+    L3Ptrs a;
+    memset(&a, 0, sizeof(a));
+    CUtensorMap op[4] = {h->tm3_op[0], h->tm3_op[0], h->tm3_op[0], h->tm3_op[0]};
+    const CUtensorMap* tm = h->tm3_st;
+    const CUtensorMap* to = h->tm3_op;     // FHN: y, Y2 | KS: y, Y2, Y3, omega
+    switch (stage) {
+        case 0:
+            a.out = b.Y2; a.Eout = h->E_b;
+            if (KS) { op[0] = to[0]; op[1] = to[3]; }
+            return l3_launch_stage<T, MODEL, P, L3_S0>(h, a, dt, tm[0], op);
+        case 1:
+            a.out = b.Y3; a.Eout = h->E_a;
+            op[0] = to[0];
+            if (KS) op[1] = to[3];
+            return l3_launch_stage<T, MODEL, P, L3_S1>(h, a, dt, tm[1], op);
+        case 2:
+            a.out = b.Y4; a.out2 = b.Y2; a.Eout = h->E_b;
+            op[0] = to[0]; op[1] = to[1];
+            if (KS) { op[2] = to[2]; op[3] = to[3]; }
+            return l3_launch_stage<T, MODEL, P, L3_S2>(h, a, dt, tm[KS ? 0 : 2], op);
+        case 3:
+            a.out = b.y; a.Eout = h->E_a;
+            op[0] = to[1];                     // Z lives in Y2
+            if (KS) op[1] = to[3];
+            return l3_launch_stage<T, MODEL, P, L3_S3>(h, a, dt, tm[KS ? 1 : 3], op);
+        default:
+            a.out = rhs_out;
+            if (KS) op[0] = to[3];
+            return l3_launch_stage<T, MODEL, P, L3_RHS>(h, a, dt, tm[0], op);
+    }
+}
+
+// entry point of one (dtype, model): configure (stage < 0) or launch
+template <class T, int MODEL>
+static int32_t l3_entry(net* h, int stage, double dt, void* rhs_out) {
+    const int P = h->tv.P;
+    if (P == 2) return stage < 0 ? l3_configure<T, MODEL, 2>(h) : l3_stage<T, MODEL, 2>(h, stage, dt, rhs_out);
+    if (P == 4) return stage < 0 ? l3_configure<T, MODEL, 4>(h) : l3_stage<T, MODEL, 4>(h, stage, dt, rhs_out);
+    return NET_ERR_UNSUPPORTED;
+}
+
+}  // namespace oscnet

@@ -158,3 +158,50 @@ int32_t lattice_v2_refresh_exchange(net* h) {
 }
 
 }  // namespace oscnet
+
+// ------------------------------------------------------------------ third generation (lat3_kernel.cuh)
+// Same data layout as the second generation (ghost-padded pair arrays, KS exchange fields E_a / E_b);
+// only the stage kernels differ.
+namespace oscnet {
+
+int32_t lattice_v3_entry_f32_fhn(net* h, int stage, double dt, void* rhs_out);
+int32_t lattice_v3_entry_f32_ks(net* h, int stage, double dt, void* rhs_out);
+int32_t lattice_v3_entry_f64_fhn(net* h, int stage, double dt, void* rhs_out);
+int32_t lattice_v3_entry_f64_ks(net* h, int stage, double dt, void* rhs_out);
+
+static int32_t l3_dispatch(net* h, int stage, double dt, void* rhs_out) {
+    const bool ks = h->desc.model == NET_MODEL_KS;
+    if (h->desc.dtype == NET_F32)
+        return ks ? lattice_v3_entry_f32_ks(h, stage, dt, rhs_out) : lattice_v3_entry_f32_fhn(h, stage, dt, rhs_out);
+    return ks ? lattice_v3_entry_f64_ks(h, stage, dt, rhs_out) : lattice_v3_entry_f64_fhn(h, stage, dt, rhs_out);
+}
+
+bool lattice_v3_supported(const net_desc* d) {
+    if (!lattice_v2_supported(d)) return false;
+    if (getenv("OSCNET_NO_LAT3")) return false;
+    // KS operand tiles are rows of scalars: whole 16-byte vectors
+    if (d->model == NET_MODEL_KS && d->dtype == NET_F32 && d->topo.extent[0] % 4 != 0) return false;
+    return true;
+}
+
+int32_t lattice_v3_prepare(net* h) {
+    if (h->desc.model == NET_MODEL_KS) {
+        char* s = (char*)h->b.scratch;
+        h->E_a = s;
+        h->E_b = s + (padded_pairs(&h->desc) * 2 * h->esize + 255) / 256 * 256;
+    }
+    int32_t rc = l3_dispatch(h, -1, 0.0, nullptr);
+    if (rc) return rc;
+    if (h->desc.model == NET_MODEL_FHN) h->pairs = 1;
+    else {
+        OSC_CUDA(h, cudaMemsetAsync(h->E_a, 0, padded_pairs(&h->desc) * 2 * h->esize, h->stream));
+        OSC_CUDA(h, cudaMemsetAsync(h->E_b, 0, padded_pairs(&h->desc) * 2 * h->esize, h->stream));
+    }
+    return NET_OK;
+}
+
+int32_t lattice_v3_stage(net* h, const StageArgs& sa) {
+    return l3_dispatch(h, sa.stage == STAGE_RHS_ONLY ? 4 : sa.stage, sa.dt, sa.out);
+}
+
+}  // namespace oscnet

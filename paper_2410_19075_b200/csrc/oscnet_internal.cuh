@@ -130,6 +130,25 @@ struct Lat2Args {
     int32_t stage;
 };
 
+// launch geometry and output pointers of the third-generation 3D lattice kernels (lat3_kernel.cuh)
+struct L3Geom {
+    int nx, ny, nz;
+    int QX, SY;                // consumer threads per tile row / strips of TY rows
+    int TXt, TYt;              // tile = TXt x TYt outputs
+    int tiles_x, tiles_y, Lz, nchunks;
+    int PW, PH;                // staged stencil box: (TXt + 2 HX) x (TYt + 2 P) pairs
+    int D;                     // prefetch distance in planes
+    int ncw;                   // consumer warps (the producer is warp ncw)
+    unsigned st_bytes, st_stride;   // stencil box bytes / ring stride (128-byte multiple)
+    unsigned op_bytes, op_stride;   // one operand tile bytes / stride
+};
+
+struct L3Ptrs {
+    void* out;                 // FHN: padded pairs; KS: plain scalars
+    void* out2;                // stage 2: Z
+    void* Eout;                // KS: padded (cos, sin) pairs of the output state
+};
+
 }  // namespace oscnet
 
 struct net {
@@ -169,6 +188,12 @@ struct net {
     int lat2_threads;
     size_t lat2_smem;
     void *E_a, *E_b;       // KS on FAST_LATTICE3D_V2: (cos, sin) pairs of the stage states
+    CUtensorMap tm3_st[4]; // FAST_LATTICE3D_V3: stencil maps (FHN y,Y2,Y3,Y4; KS E_a,E_b)
+    CUtensorMap tm3_op[4]; // operand maps (FHN y,Y2 centre boxes; KS y,Y2,Y3,omega scalars)
+    oscnet::L3Geom lat3[5]; // per stage (0-3, RHS)
+    unsigned lat3_grid[5];
+    int lat3_threads[5];
+    size_t lat3_smem[5];
     int32_t pairs;         // 1 = state arrays are ghost-padded interleaved pairs (FHN on FAST_LATTICE3D_V2)
     char err[512];
 };
@@ -197,7 +222,7 @@ int32_t hh_steady_gates(net* h);
 
 // csr_fast.cu / lattice_fast.cu / ring_fast.cu ------------------------------
 enum { FAST_NONE = 0, FAST_CSR_WARP = 1, FAST_LATTICE3D = 2, FAST_RING_FHN = 3, FAST_RING_KS = 4,
-       FAST_LATTICE3D_V2 = 5 };
+       FAST_LATTICE3D_V2 = 5, FAST_LATTICE3D_V3 = 6 };
 int32_t fast_select(const net_desc* d);                   // FAST_* available for this desc
 size_t fast_scratch_bytes(const net_desc* d, int32_t fast_kind);
 size_t fast_state_bytes(const net_desc* d, int32_t fast_kind);   // 0 = the default nvar*ld elements
