@@ -27,7 +27,7 @@ ABI_SYMBOLS = [
     "net_workspace_bytes", "net_create", "net_destroy", "net_set_state", "net_get_state",
     "net_set_param_array", "net_hh_steady_gates", "net_integrate", "net_integrate_observed",
     "net_eval_rhs", "net_observables", "net_get_topology", "net_get_degree", "net_get_time",
-    "net_set_time", "net_get_counters", "net_synchronize", "net_last_error", "net_version",
+    "net_set_time", "net_get_counters", "net_get_kernel_family", "net_synchronize", "net_last_error", "net_version",
 ]
 
 
@@ -191,6 +191,12 @@ def net_get_counters(h):
     k, m = C.c_int64(), C.c_int32()
     _check(lib().net_get_counters(h, C.byref(k), C.byref(m)), h)
     return k.value, m.value
+
+
+def net_get_kernel_family(h):
+    f = C.c_int32()
+    _check(lib().net_get_kernel_family(h, C.byref(f)), h)
+    return f.value
 
 
 def net_synchronize(h):
@@ -372,6 +378,9 @@ class Net:
 
     def counters(self):
         return net_get_counters(self.h)
+
+    def kernel_family(self):
+        return net_get_kernel_family(self.h)
 
     def synchronize(self):
         net_synchronize(self.h)

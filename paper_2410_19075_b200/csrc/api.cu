@@ -93,7 +93,7 @@ static Layout make_layout(const net_desc* d, char* base) {
     L.state_bytes = state;
     L.b.y = P(state); L.b.Y2 = P(state); L.b.Y3 = P(state); L.b.Y4 = P(state);
     L.b.elem_param = P((size_t)ld * es);
-    if (d->model == NET_MODEL_HH && fk == FAST_CSR_WARP) {
+    if (d->model == NET_MODEL_HH && (fk == FAST_CSR_WARP || fk == FAST_CSR_BLOCKED)) {
         L.b.s_y = P((size_t)ld * es); L.b.s_Y2 = P((size_t)ld * es);
         L.b.s_Y3 = P((size_t)ld * es); L.b.s_Y4 = P((size_t)ld * es);
     }
@@ -541,6 +541,12 @@ int32_t net_get_counters(net_t* h, int64_t* kernel_launches, int32_t* method_in_
     if (!h) return NET_ERR_INVALID;
     if (kernel_launches) *kernel_launches = h->launches;
     if (method_in_use) *method_in_use = h->method;
+    return NET_OK;
+}
+
+int32_t net_get_kernel_family(net_t* h, int32_t* family) {
+    if (!h) return NET_ERR_INVALID;
+    if (family) *family = h->method == NET_METHOD_FAST ? h->fast_kind : FAST_NONE;
     return NET_OK;
 }
 

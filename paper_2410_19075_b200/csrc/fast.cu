@@ -4,6 +4,10 @@
 namespace oscnet {
 
 int32_t csr_warp_stage(net* h, const StageArgs& a);
+bool csr_blocked_supported(const net_desc* d);
+size_t csr_blocked_scratch_bytes(const net_desc* d);
+int32_t csr_blocked_prepare(net* h);
+int32_t csr_blocked_stage(net* h, const StageArgs& a);
 bool lattice3d_supported(const net_desc* d);
 int32_t lattice3d_prepare(net* h);
 int32_t lattice3d_stage(net* h, const StageArgs& a);
@@ -22,7 +26,8 @@ int32_t ring_run(net* h, const void* y_in, void* y_out, int64_t n_steps, double 
 
 int32_t fast_select(const net_desc* d) {
     const net_topology& t = d->topo;
-    if (t.kind == NET_TOPO_CSR || t.kind == NET_TOPO_RANDOM_INDEGREE) return FAST_CSR_WARP;
+    if (t.kind == NET_TOPO_CSR || t.kind == NET_TOPO_RANDOM_INDEGREE)
+        return csr_blocked_supported(d) ? FAST_CSR_BLOCKED : FAST_CSR_WARP;
     if (lattice_v3_supported(d)) return FAST_LATTICE3D_V3;
     if (lattice_v2_supported(d)) return FAST_LATTICE3D_V2;
     if (lattice3d_supported(d)) return FAST_LATTICE3D;
@@ -33,6 +38,7 @@ int32_t fast_select(const net_desc* d) {
 size_t fast_scratch_bytes(const net_desc* d, int32_t fast_kind) {
     if (fast_kind == FAST_RING_KS || fast_kind == FAST_RING_FHN) return ring_scratch_bytes(d);
     if (fast_kind == FAST_LATTICE3D_V2 || fast_kind == FAST_LATTICE3D_V3) return lattice_v2_scratch_bytes(d);
+    if (fast_kind == FAST_CSR_BLOCKED) return csr_blocked_scratch_bytes(d);
     return 0;
 }
 
@@ -44,6 +50,13 @@ size_t fast_state_bytes(const net_desc* d, int32_t fast_kind) {
 // cannot take this shape (NET_ERR_UNSUPPORTED) falls back to DIRECT unless FAST was demanded.
 int32_t fast_prepare(net* h) {
     int32_t rc = NET_OK;
+    if (h->fast_kind == FAST_CSR_BLOCKED) {
+        rc = csr_blocked_prepare(h);
+        if (rc == NET_ERR_UNSUPPORTED) {     // a segment the 16-bit offsets cannot take: warp-per-row gathers
+            h->fast_kind = FAST_CSR_WARP;
+            rc = NET_OK;
+        }
+    }
     if (h->fast_kind == FAST_LATTICE3D_V3) {
         rc = lattice_v3_prepare(h);
         if (rc == NET_ERR_UNSUPPORTED) {     // same layout, second-generation kernels
@@ -72,6 +85,7 @@ int32_t fast_prepare(net* h) {
 int32_t fast_stage(net* h, const StageArgs& a) {
     switch (h->fast_kind) {
         case FAST_CSR_WARP: return csr_warp_stage(h, a);
+        case FAST_CSR_BLOCKED: return csr_blocked_stage(h, a);
         case FAST_LATTICE3D: return lattice3d_stage(h, a);
         case FAST_LATTICE3D_V2: return lattice_v2_stage(h, a);
         case FAST_LATTICE3D_V3: return lattice_v3_stage(h, a);

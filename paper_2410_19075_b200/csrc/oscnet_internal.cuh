@@ -194,6 +194,10 @@ struct net {
     unsigned lat3_grid[5];
     int lat3_threads[5];
     size_t lat3_smem[5];
+    char cb_geom[96];      // FAST_CSR_BLOCKED: CbGeom (csr_blocked.cu)
+    unsigned cb_grid;
+    int32_t cb_es;         // entries staged in shared memory
+    size_t cb_smem;
     int32_t pairs;         // 1 = state arrays are ghost-padded interleaved pairs (FHN on FAST_LATTICE3D_V2)
     char err[512];
 };
@@ -222,7 +226,7 @@ int32_t hh_steady_gates(net* h);
 
 // csr_fast.cu / lattice_fast.cu / ring_fast.cu ------------------------------
 enum { FAST_NONE = 0, FAST_CSR_WARP = 1, FAST_LATTICE3D = 2, FAST_RING_FHN = 3, FAST_RING_KS = 4,
-       FAST_LATTICE3D_V2 = 5, FAST_LATTICE3D_V3 = 6 };
+       FAST_LATTICE3D_V2 = 5, FAST_LATTICE3D_V3 = 6, FAST_CSR_BLOCKED = 7 };
 int32_t fast_select(const net_desc* d);                   // FAST_* available for this desc
 size_t fast_scratch_bytes(const net_desc* d, int32_t fast_kind);
 size_t fast_state_bytes(const net_desc* d, int32_t fast_kind);   // 0 = the default nvar*ld elements
