@@ -206,6 +206,11 @@ int32_t net_set_time(net_t* net, double t, int64_t step);
  * the method actually in use (NET_METHOD_DIRECT or NET_METHOD_FAST). */
 int32_t net_get_counters(net_t* net, int64_t* kernel_launches, int32_t* method_in_use);
 
+/* Which kernel family serves the fused RHS + RK4 stages of this net (diagnostic; DESIGN.md
+ * section 5): NET_FAMILY_DIRECT 0 (Alg. 1 form), CSR_WARP 1, LATTICE3D 2,
+ * RING (persistent, FHN 3 / KS 4), LATTICE3D_V2 5, LATTICE3D_V3 6, CSR_BLOCKED 7. */
+int32_t net_get_kernel_family(net_t* net, int32_t* family);
+
 /* Blocks until the stream is idle; returns NET_ERR_CUDA if anything failed asynchronously. */
 int32_t net_synchronize(net_t* net);
 

@@ -49,6 +49,22 @@ __device__ __forceinline__ void cb_prefetch_l2(const void* src, unsigned bytes) 
     asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(src), "r"(bytes) : "memory");
 }
 
+__device__ __forceinline__ unsigned cb_lds_u32(unsigned addr) {
+    unsigned v;
+    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(addr));
+    return v;
+}
+__device__ __forceinline__ double cb_lds(unsigned addr, double) {
+    double v;
+    asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(addr));
+    return v;
+}
+__device__ __forceinline__ float cb_lds(unsigned addr, float) {
+    float v;
+    asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(addr));
+    return v;
+}
+
 // ------------------------------------------------------------------ build kernels (once per net)
 // counts: roff[seg(c, b)][l + 1] = index pairs (words) of row (c, l) in block b; roff[seg][0] = 0
 __global__ void cb_count_kernel(CbGeom g, const int64_t* __restrict__ row_ptr, const int32_t* __restrict__ col_idx,
@@ -194,7 +210,11 @@ csr_blocked_stage_kernel(StageArgs a, ModelParams mp, TopoView tv, CbGeom g) {
     __shared__ uint64_t bar;
     T* sblk = reinterpret_cast<T*>(cb_smem);                 // W values of s + the zero slot
     const size_t ent_at = ((size_t)g.W + 16) * sizeof(T);
-    const unsigned* sent = reinterpret_cast<const unsigned*>(cb_smem + ent_at);
+    constexpr unsigned SH = sizeof(T) == 8 ? 3u : 2u;          // index -> byte offset
+    constexpr unsigned MASK = 0xffffu << SH;
+    const unsigned sblk_a = smem_u32(cb_smem);
+    const unsigned zw_a = sblk_a + ((unsigned)g.W + 8u) * (unsigned)sizeof(T);   // word (W, W)
+    const unsigned sent_a = sblk_a + (unsigned)ent_at;
     const T* __restrict__ gsrc = (const T*)a.s_in;
     const int t = threadIdx.x;
     const int CR1 = g.CR + 1;
@@ -202,6 +222,7 @@ csr_blocked_stage_kernel(StageArgs a, ModelParams mp, TopoView tv, CbGeom g) {
         mbar_init(&bar, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         sblk[g.W] = T(0);
+        *reinterpret_cast<unsigned*>(cb_smem + ((size_t)g.W + 8) * sizeof(T)) = (unsigned)g.W | (unsigned)g.W << 16;
     }
     __syncthreads();
     unsigned phase = 0;
@@ -259,22 +280,31 @@ csr_blocked_stage_kernel(StageArgs a, ModelParams mp, TopoView tv, CbGeom g) {
             if (b + 1 < g.B) load_offs(b + 1, nxt);
             mbar_wait(&bar, phase);
             phase ^= 1u;
-            // warp-uniform trip counts (the longest run among the 32 lanes), predicated bodies
+            // warp-uniform trip counts (the longest run among the 32 lanes); lanes whose run is
+            // over read the word that points twice at the zero slot, so the body has no branch
 #pragma unroll
             for (int m = 0; m < M; ++m) {
                 const unsigned o0 = offs[m] & 0xffffu, np = (offs[m] >> 16) - o0;
                 const unsigned kmax = __reduce_max_sync(0xffffffffu, np);
-                const unsigned* __restrict__ src = ES ? sent + o0 : ent + o0;
                 T a0 = T(0), a1 = T(0);
-                if constexpr (!ES) {
-                    if (np > 0) { a0 = sblk[first[m] & 0xffffu]; a1 = sblk[first[m] >> 16]; }
-                }
+                if constexpr (ES) {
+                    const unsigned p0 = sent_a + o0 * 4u;
 #pragma unroll 2
-                for (unsigned k = ES ? 0u : 1u; k < kmax; ++k) {
-                    if (k < np) {
-                        const unsigned w = ES ? src[k] : __ldg(src + k);
-                        a0 += sblk[w & 0xffffu];
-                        a1 += sblk[w >> 16];
+                    for (unsigned k = 0; k < kmax; ++k) {
+                        const unsigned w = cb_lds_u32(k < np ? p0 + k * 4u : zw_a);
+                        a0 += cb_lds(sblk_a + ((w << SH) & MASK), T(0));
+                        a1 += cb_lds(sblk_a + ((w >> (16 - SH)) & MASK), T(0));
+                    }
+                } else {
+                    const unsigned* __restrict__ src = ent + o0;
+                    if (np > 0) { a0 = sblk[first[m] & 0xffffu]; a1 = sblk[first[m] >> 16]; }
+#pragma unroll 1
+                    for (unsigned k = 1; k < kmax; ++k) {
+                        if (k < np) {
+                            const unsigned w = __ldg(src + k);
+                            a0 += sblk[w & 0xffffu];
+                            a1 += sblk[w >> 16];
+                        }
                     }
                 }
                 acc[m] += a0 + a1;

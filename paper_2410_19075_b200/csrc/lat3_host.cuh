@@ -55,7 +55,7 @@ inline int32_t l3_encode(net* h, CUtensorMap* tm, void* base, int esz, uint64_t 
 template <class T, int MODEL, int P, int STAGE>
 static auto l3_kernel_ptr() {
     typedef L3Shape<T, P> S;
-    return lat3_kernel<T, MODEL, P, STAGE, S::X, S::TY, L3_MAXT, L3_MINB>;
+    return lat3_kernel<T, MODEL, P, STAGE, S::X, S::TY, L3_MAXT, L3_MINB, (P > 2 && sizeof(T) == 4)>;
 }
 
 inline size_t l3_smem_bytes(const L3Geom& g, int P, int nt) {

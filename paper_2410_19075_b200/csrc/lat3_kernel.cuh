@@ -54,7 +54,11 @@ __device__ __forceinline__ double2 pfma(double2 a, double2 b, double2 c) {
     return make_double2(fma(a.x, b.x, c.x), fma(a.y, b.y, c.y));
 }
 
-template <class T, int MODEL, int P, int STAGE, int X, int TY, int MAXT, int MINB>
+// ROT: the accumulators of the open output planes are shifted down one slot after every plane
+// (register moves) instead of being addressed by a compile-time phase J, which needs 2P + 1
+// copies of the plane body: for P = 4 those copies (130 KB of SASS) overflow the instruction
+// cache once the decoupled warps drift apart (profiles/r01_lat3_ncu.md, cfg 3a: no_instruction).
+template <class T, int MODEL, int P, int STAGE, int X, int TY, int MAXT, int MINB, bool ROT>
 __global__ void __launch_bounds__(MAXT, MINB)
 lat3_kernel(const __grid_constant__ CUtensorMap tm_st, const __grid_constant__ CUtensorMap tm_op0,
             const __grid_constant__ CUtensorMap tm_op1, const __grid_constant__ CUtensorMap tm_op2,
@@ -308,10 +312,23 @@ lat3_kernel(const __grid_constant__ CUtensorMap tm_st, const __grid_constant__ C
         if (++b == NB) { b = 0; phase ^= 1u; }
     };
 
-    for (int base = 0; base < nplanes; base += NACC)
-        l2_static_for<0, NACC>([&](auto Jc) {
-            if (base + decltype(Jc)::value < nplanes) do_plane(base + decltype(Jc)::value, Jc);
-        });
+    if constexpr (ROT) {
+#pragma unroll 1
+        for (int i = 0; i < nplanes; ++i) {
+            do_plane(i, std::integral_constant<int, 0>{});
+#pragma unroll
+            for (int k = 0; k + 1 < NACC; ++k)
+#pragma unroll
+                for (int r = 0; r < TY; ++r)
+#pragma unroll
+                    for (int e = 0; e < X; ++e) acc[k][r][e] = acc[k + 1][r][e];
+        }
+    } else {
+        for (int base = 0; base < nplanes; base += NACC)
+            l2_static_for<0, NACC>([&](auto Jc) {
+                if (base + decltype(Jc)::value < nplanes) do_plane(base + decltype(Jc)::value, Jc);
+            });
+    }
 }
 
 }  // namespace oscnet
