@@ -52,6 +52,23 @@ inline int32_t l3_encode(net* h, CUtensorMap* tm, void* base, int esz, uint64_t 
     return NET_OK;
 }
 
+// 4D map over two planes of 8-byte elements: extents (ex, ey, ez, 2), box (bx, by, 1, 2)
+inline int32_t l3_encode_planes(net* h, CUtensorMap* tm, void* base, uint64_t ex, uint64_t ey, uint64_t ez,
+                                uint32_t bx, uint32_t by) {
+    l3_encode_fn encode;
+    int32_t rc = l3_encoder(h, &encode);
+    if (rc) return rc;
+    cuuint64_t dims[4] = {ex, ey, ez, 2};
+    cuuint64_t strides[3] = {ex * 8, ex * ey * 8, ex * ey * ez * 8};
+    cuuint32_t box[4] = {bx, by, 1, 2};
+    cuuint32_t estr[4] = {1, 1, 1, 1};
+    CUresult r = encode(tm, CU_TENSOR_MAP_DATA_TYPE_UINT64, 4, base, dims, strides, box, estr,
+                        CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                        CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return set_err(h, NET_ERR_CUDA, "cuTensorMapEncodeTiled (planes) failed (%d)", (int)r);
+    return NET_OK;
+}
+
 template <class T, int MODEL, int P, int STAGE>
 static auto l3_kernel_ptr() {
     typedef L3Shape<T, P> S;
@@ -172,8 +189,14 @@ static int32_t l3_configure(net* h) {
     const uint64_t nxp = (uint64_t)g.nx + 2 * HX, nyp = (uint64_t)g.ny + 2 * P;
     void* st_src[4] = {h->b.y, h->b.Y2, h->b.Y3, h->b.Y4};
     if (KS) { st_src[0] = h->E_a; st_src[1] = h->E_b; }
-    for (int k = 0; k < (KS ? 2 : 4); ++k)
-        if ((rc = l3_encode(h, &h->tm3_st[k], st_src[k], 8, nxp * U8, nyp, (uint64_t)g.nz, (uint32_t)(g.PW * U8), (uint32_t)g.PH))) return rc;
+    constexpr bool PLANAR = KS && sizeof(T) == 8;     // (cos | sin) planes instead of pairs (lat3_kernel.cuh)
+    for (int st = 0; st < 5; ++st) h->lat3[st].plane = (long long)(nxp * nyp * (uint64_t)g.nz);
+    for (int k = 0; k < (KS ? 2 : 4); ++k) {
+        if (PLANAR) rc = l3_encode_planes(h, &h->tm3_st[k], st_src[k], nxp, nyp, (uint64_t)g.nz, (uint32_t)g.PW, (uint32_t)g.PH);
+        else rc = l3_encode(h, &h->tm3_st[k], st_src[k], 8, nxp * U8, nyp, (uint64_t)g.nz, (uint32_t)(g.PW * U8), (uint32_t)g.PH);
+        if (rc) return rc;
+    }
+    h->ks_planar = PLANAR ? 1 : 0;
     if (KS) {
         void* op_src[4] = {h->b.y, h->b.Y2, h->b.Y3, h->b.elem_param};
         for (int k = 0; k < 4; ++k)

@@ -65,6 +65,11 @@ lat3_kernel(const __grid_constant__ CUtensorMap tm_st, const __grid_constant__ C
             const __grid_constant__ CUtensorMap tm_op3, L3Ptrs a, L3Params<T> mp, L3Geom g) {
     typedef typename PairOf<T>::type Pr;
     constexpr bool KS = MODEL == NET_MODEL_KS;
+    // fp64 KS keeps (cos phi) and (sin phi) as two PLANES (global and staged): a thread's row of
+    // 16-byte pairs at a 32-byte lane stride costs two shared-memory wavefronts per vector load
+    // (profiles/r01_lat3_ncu.md, cfg 3b: half of the wavefronts were bank conflicts); rows of
+    // doubles at a 16-byte lane stride cost one.
+    constexpr bool PLANAR = KS && sizeof(T) == 8;
     constexpr int HX = l2_hx<T>(P);           // x ghost width of the padded pair arrays
     constexpr int NCOL = X + 2 * HX;          // pairs a thread reads per staged row
     constexpr int OFF = HX - P;
@@ -110,7 +115,8 @@ lat3_kernel(const __grid_constant__ CUtensorMap tm_st, const __grid_constant__ C
                 const bool ops = NT > 0 && j >= 2 * P;
                 mbar_expect_tx(full + b, g.st_bytes + (ops ? NT * g.op_bytes : 0u));
                 int zz = (z0 - P + j) % nz; if (zz < 0) zz += nz;
-                tma_load_3d(st_ring + (size_t)ss * g.st_stride, &tm_st, x0 * U8, y0, zz, full + b);
+                if constexpr (PLANAR) tma_load_4d(st_ring + (size_t)ss * g.st_stride, &tm_st, x0, y0, zz, 0, full + b);
+                else tma_load_3d(st_ring + (size_t)ss * g.st_stride, &tm_st, x0 * U8, y0, zz, full + b);
                 if (ops) {
                     const int zo = z0 - 2 * P + j;
                     unsigned char* ob = op_ring + (size_t)b * NT * g.op_stride;
@@ -156,6 +162,8 @@ lat3_kernel(const __grid_constant__ CUtensorMap tm_st, const __grid_constant__ C
         mbar_wait(full + b, phase);
         if (owner) {
             const Pr* sb = reinterpret_cast<const Pr*>(st_ring + (size_t)slot * g.st_stride) + (st * TY) * PW + q * X;
+            const T* sbc = reinterpret_cast<const T*>(st_ring + (size_t)slot * g.st_stride) + (st * TY) * PW + q * X;   // PLANAR: cos box
+            const int splane = PW * g.PH;                                                                                 // ... sin box behind it
             Pr A[P > 1 ? P - 1 : 1][TY][X];
             bool Aset[P > 1 ? P - 1 : 1][TY];
 #pragma unroll
@@ -174,6 +182,15 @@ lat3_kernel(const __grid_constant__ CUtensorMap tm_st, const __grid_constant__ C
                         float4 w4 = *reinterpret_cast<const float4*>(row + 2 * c);
                         v[2 * c] = make_float2(w4.x, w4.y);
                         v[2 * c + 1] = make_float2(w4.z, w4.w);
+                    }
+                } else if constexpr (PLANAR) {
+                    const T* rc = sbc + rr * PW;
+#pragma unroll
+                    for (int c = 0; c < NCOL / 2; ++c) {
+                        const double2 wc = *reinterpret_cast<const double2*>(rc + 2 * c);
+                        const double2 ws = *reinterpret_cast<const double2*>(rc + splane + 2 * c);
+                        v[2 * c] = make_double2(wc.x, ws.x);
+                        v[2 * c + 1] = make_double2(wc.y, ws.y);
                     }
                 } else {
 #pragma unroll
@@ -255,7 +272,11 @@ lat3_kernel(const __grid_constant__ CUtensorMap tm_st, const __grid_constant__ C
                 T ov[EW], zv[EW], ev[2 * X];
 #pragma unroll
                 for (int e = 0; e < X; ++e) {
-                    const Pr c = cb[r * PW + e];
+                    Pr c;
+                    if constexpr (PLANAR) {
+                        const T* cc = reinterpret_cast<const T*>(st_ring + (size_t)cslot * g.st_stride) + (st * TY + P + r) * PW + q * X + HX + e;
+                        c.x = cc[0]; c.y = cc[PW * g.PH];
+                    } else c = cb[r * PW + e];
                     const Pr W = acc[J % NACC][r][e];
                     if constexpr (KS) {
                         T C = W.x, S = W.y;
@@ -271,7 +292,7 @@ lat3_kernel(const __grid_constant__ CUtensorMap tm_st, const __grid_constant__ C
                         ov[e] = o;
                         if constexpr (STAGE != L3_RHS) {
                             T s_, c_;
-                            Math<T>::sincos(o, &s_, &c_);
+                            sincos_stage<T>(o, &s_, &c_);
                             ev[2 * e] = c_; ev[2 * e + 1] = s_;
                         }
                     } else {
@@ -297,7 +318,22 @@ lat3_kernel(const __grid_constant__ CUtensorMap tm_st, const __grid_constant__ C
                 if constexpr (KS) {
                     stg_vec<EW>((T*)a.out + il, ov);
                     if constexpr (STAGE == L3_S2) stg_vec<EW>((T*)a.out2 + il, zv);
-                    if constexpr (STAGE != L3_RHS) store_pairs((T*)a.Eout, ev);
+                    if constexpr (STAGE != L3_RHS) {
+                        if constexpr (PLANAR) {
+                            T cv[X], sv[X];
+#pragma unroll
+                            for (int e = 0; e < X; ++e) { cv[e] = ev[2 * e]; sv[e] = ev[2 * e + 1]; }
+                            T* Ec = (T*)a.Eout;
+                            T* Es = Ec + g.plane;
+                            auto store_planes = [&](int64_t at) { stg_vec<X>(Ec + at, cv); stg_vec<X>(Es + at, sv); };
+                            store_planes(ip);
+                            if (gxs != 0) store_planes(ip + gxs);
+                            if (gys != 0) {
+                                store_planes(ip + (int64_t)gys * nxp);
+                                if (gxs != 0) store_planes(ip + (int64_t)gys * nxp + gxs);
+                            }
+                        } else store_pairs((T*)a.Eout, ev);
+                    }
                 } else {
                     store_pairs((T*)a.out, ov);
                     if constexpr (STAGE == L3_S2) stg_vec<EW>((T*)a.out2 + 2 * ip, zv);   // Z is never a stencil source

@@ -53,6 +53,12 @@ __device__ __forceinline__ void tma_load_3d(void* dst, const CUtensorMap* tmap, 
         ::"r"(smem_u32(dst)), "l"(tmap), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2) : "memory");
 }
 
+__device__ __forceinline__ void tma_load_4d(void* dst, const CUtensorMap* tmap, int c0, int c1, int c2, int c3, uint64_t* bar) {
+    asm volatile(
+        "cp.async.bulk.tensor.4d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5, %6}], [%2];"
+        ::"r"(smem_u32(dst)), "l"(tmap), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2), "r"(c3) : "memory");
+}
+
 // N contiguous scalars from / to 16-byte (8-byte when N*sizeof == 8) aligned global memory
 template <int N>
 __device__ __forceinline__ void ldg_vec(const float* p, float (&v)[N]) {

@@ -40,6 +40,7 @@ size_t lattice_v2_scratch_bytes(const net_desc* d) {
 }
 
 int32_t lattice_v2_prepare(net* h) {
+    h->ks_planar = 0;
     if (h->desc.model == NET_MODEL_KS) {
         char* s = (char*)h->b.scratch;
         h->E_a = s;
@@ -82,8 +83,9 @@ int32_t lattice_v2_stage(net* h, const StageArgs& sa) {
 }
 
 // ------------------------------------------------------------------ layout helpers
-// MODE 0: pairs <- (soa[i], soa[ld+i]);  MODE 1: pairs <- (cos, sin) soa[i].  Every padded
-// position, ghosts included, takes the value of its periodic image.
+// MODE 0: pairs <- (soa[i], soa[ld+i]);  MODE 1: pairs <- (cos, sin) soa[i];  MODE 2: two planes
+// (cos soa[i] | sin soa[i]).  Every padded position, ghosts included, takes the value of its
+// periodic image.
 template <class T, int MODE>
 __global__ void pad_fill_kernel(const T* __restrict__ soa, T* __restrict__ pr, int nx, int ny, int nz,
                                 int GX, int GY, int64_t ld) {
@@ -100,7 +102,8 @@ __global__ void pad_fill_kernel(const T* __restrict__ soa, T* __restrict__ pr, i
         else {
             T s, c;
             Math<T>::sincos(soa[i], &s, &c);
-            pr[2 * e] = c; pr[2 * e + 1] = s;
+            if (MODE == 1) { pr[2 * e] = c; pr[2 * e + 1] = s; }
+            else { pr[e] = c; pr[total + e] = s; }
         }
     }
 }
@@ -154,7 +157,7 @@ int32_t pairs_unpack(net* h, const void* pairs, void* soa) {
 
 int32_t lattice_v2_refresh_exchange(net* h) {
     if (h->desc.model != NET_MODEL_KS) return NET_OK;
-    return pad_fill<1>(h, h->b.y, h->E_a);
+    return h->ks_planar ? pad_fill<2>(h, h->b.y, h->E_a) : pad_fill<1>(h, h->b.y, h->E_a);
 }
 
 }  // namespace oscnet

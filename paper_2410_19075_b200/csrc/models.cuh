@@ -21,6 +21,22 @@ template <> struct Math<float> {
     static __device__ __forceinline__ float abs(float x) { return ::fabsf(x); }
 };
 
+// (sin, cos) of an unwrapped fp32 phase on the SFU: two-term Cody-Waite reduction to [-pi, pi]
+// (k = rint(x / 2 pi), r = x - k * 2 pi with 2 pi split hi + lo), then MUFU.SIN / MUFU.COS.
+// Absolute error about 5e-7 for |x| up to a few 1e4 (sin.approx is 2^-20.9 on [-pi, pi]); the
+// north star lets the sin/cos pair go to the SFU "with the error of that choice measured":
+// tests/test_gpu_parity.py::test_fast_rewrite_error_against_direct_on_gpu does.  The fp64 path
+// keeps the library sincos.
+__device__ __forceinline__ void sincos_sfu(float x, float* s, float* c) {
+    const float k = rintf(x * 0.15915494309189535f);
+    float r = fmaf(k, -6.2831854820251465f, x);          // 2 pi rounded to fp32
+    r = fmaf(k, 1.7484555e-7f, r);                       // minus (2 pi - fl(2 pi))
+    *s = __sinf(r);
+    *c = __cosf(r);
+}
+template <class T> __device__ __forceinline__ void sincos_stage(T x, T* s, T* c) { Math<T>::sincos(x, s, c); }
+template <> __device__ __forceinline__ void sincos_stage<float>(float x, float* s, float* c) { sincos_sfu(x, s, c); }
+
 // ----------------------------------------------------------------- Kuramoto
 // Direct form: f = omega + (K/Omega) * sum_j sin(phi_j - phi_i - alpha); `sum` is that sum.
 template <class T>

@@ -141,6 +141,7 @@ struct L3Geom {
     int ncw;                   // consumer warps (the producer is warp ncw)
     unsigned st_bytes, st_stride;   // stencil box bytes / ring stride (128-byte multiple)
     unsigned op_bytes, op_stride;   // one operand tile bytes / stride
+    long long plane;                // fp64 KS: elements between the cos and the sin plane of E
 };
 
 struct L3Ptrs {
@@ -198,6 +199,7 @@ struct net {
     unsigned cb_grid;
     int32_t cb_es;         // entries staged in shared memory
     size_t cb_smem;
+    int32_t ks_planar;     // 1 = KS exchange fields E_a / E_b are two planes (cos | sin), not pairs (fp64 on FAST_LATTICE3D_V3)
     int32_t pairs;         // 1 = state arrays are ghost-padded interleaved pairs (FHN on FAST_LATTICE3D_V2)
     char err[512];
 };
