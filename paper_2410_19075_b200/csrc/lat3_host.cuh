@@ -117,7 +117,10 @@ static int32_t l3_configure_stage(net* h) {
             const double halo = (double)(TXt + 2 * HX) * (TYt + 2 * P) / ((double)TXt * TYt);
             // small CTAs (about four consumer warps) desynchronise better; mild preference
             const double size_pen = warps <= 4 ? 1.0 : 1.0 - 0.02 * (warps - 4);
-            const double score = lane_eff * cover * size_pen / (1.0 + 0.25 * (halo - 1.0));
+            // fp64 planes: rows of fewer than 16 threads put the 8 lanes of a vector-load phase on
+            // several staged rows, whose pitch collides in the banks (measured on cfg 3b)
+            const double bank_pen = (KS && sizeof(T) == 8 && QX < 16) ? 0.85 : 1.0;
+            const double score = lane_eff * cover * size_pen * bank_pen / (1.0 + 0.25 * (halo - 1.0));
             if (score > best) { best = score; g.TXt = TXt; g.TYt = TYt; g.QX = QX; g.SY = SY; g.tiles_x = tx; g.tiles_y = ty; }
         }
         if (want_tx > 0) break;
