@@ -22,6 +22,7 @@
 // The cancellation of the prefix differences is bounded by (chunk length) x ulp x max|field| on
 // Sloc plus G x ulp(double) on BT; the RHS divides it by Omega (measured: tests).
 #include <cooperative_groups.h>
+#include <stdlib.h>
 
 #include "models.cuh"
 
@@ -38,7 +39,7 @@ struct RingArgs {
     double* tot[2];          // 2 x [2][RING_GMAX] chunk totals
     unsigned int* bar;       // grid barrier counter (zeroed before the launch)
     int64_t n, ld, npad;
-    int32_t P, include_self, chunk, G;
+    int32_t P, include_self, chunk, G, chunk_shift;
     int64_t n_steps;
     double dt;
     int32_t rhs_only;
@@ -177,31 +178,62 @@ __global__ void __launch_bounds__(RING_THREADS) ring_persistent_kernel(RingArgs 
             if (threadIdx.x == 0) { BT[0][G] = u0; BT[1][G] = u1; }
             __syncthreads();
         }
-        // window sums, local field, RK4 update
+        // window sums, local field, RK4 update.  W(i) = Pref(i+P) - Pref(i-P-1) with the ring wrap
+        // taken as one extra full-ring term (the total = BT[G], no load).  All 4 E prefix loads
+        // of a thread are issued together, branch-free: one L2 round trip per stage, not one per
+        // term (the serial form cost 1.4 us per element and stage on config 2).
         T k[E][NV];
+        T W0v[E], W1v[E];
+        {
+            int64_t jh[E], jl[E];
+            int nwrap[E];
+            bool has_lo[E];
+#pragma unroll
+            for (int e = 0; e < E; ++e) {
+                const int64_t i = ok[e] ? i0 + e : 0;
+                int64_t hi = i + P, lo = i - P - 1;
+                int w = 0;
+                if (hi >= n) { hi -= n; ++w; }
+                if (lo < -1) { lo += n; ++w; }
+                has_lo[e] = lo >= 0;
+                jh[e] = hi; jl[e] = has_lo[e] ? lo : 0;
+                nwrap[e] = w;
+            }
+            T h0[E], h1[E], l0[E], l1[E];
+#pragma unroll
+            for (int e = 0; e < E; ++e) {
+                h0[e] = SINGLE ? Sg[jh[e]] : ld_l2(Sg + jh[e]);
+                h1[e] = SINGLE ? Sg[sstride + jh[e]] : ld_l2(Sg + sstride + jh[e]);
+                l0[e] = SINGLE ? Sg[jl[e]] : ld_l2(Sg + jl[e]);
+                l1[e] = SINGLE ? Sg[sstride + jl[e]] : ld_l2(Sg + sstride + jl[e]);
+            }
+#pragma unroll
+            for (int e = 0; e < E; ++e) {
+                double bt0 = 0.0, bt1 = 0.0;
+                T sl0 = h0[e], sl1 = h1[e];
+                if (!SINGLE) {
+                    const int bh = (int)(jh[e] >> a.chunk_shift);   // chunk = 256 E is a power of two
+                    bt0 = BT[0][bh]; bt1 = BT[1][bh];
+                }
+                if (has_lo[e]) {
+                    sl0 -= l0[e]; sl1 -= l1[e];
+                    if (!SINGLE) {
+                        const int bl = (int)(jl[e] >> a.chunk_shift);
+                        bt0 -= BT[0][bl]; bt1 -= BT[1][bl];
+                    }
+                }
+                // full-ring terms: Pref(n-1) = total of the ring
+                T tot0, tot1;
+                if (SINGLE) { tot0 = Sg[n - 1]; tot1 = Sg[sstride + n - 1]; }
+                else { tot0 = T(0); tot1 = T(0); bt0 += (double)nwrap[e] * BT[0][G]; bt1 += (double)nwrap[e] * BT[1][G]; }
+                if (SINGLE) { sl0 += T(nwrap[e]) * tot0; sl1 += T(nwrap[e]) * tot1; }
+                W0v[e] = ok[e] ? (T)bt0 + sl0 : T(0);
+                W1v[e] = ok[e] ? (T)bt1 + sl1 : T(0);
+            }
+        }
 #pragma unroll
         for (int e = 0; e < E; ++e) {
-            T W0 = T(0), W1 = T(0);
-            if (ok[e]) {
-                const int64_t i = i0 + e;
-                double bt0 = 0.0, bt1 = 0.0;
-                T sl0 = T(0), sl1 = T(0);
-                auto term = [&](int64_t j, int sign) {     // +- Pref(j)
-                    const int bj = SINGLE ? 0 : (int)(j / chunk);
-                    const int64_t at = SINGLE ? j : j;
-                    const T v0 = SINGLE ? Sg[at] : ld_l2(Sg + at);
-                    const T v1 = SINGLE ? Sg[sstride + at] : ld_l2(Sg + sstride + at);
-                    if (sign > 0) { sl0 += v0; sl1 += v1; if (!SINGLE) { bt0 += BT[0][bj]; bt1 += BT[1][bj]; } }
-                    else { sl0 -= v0; sl1 -= v1; if (!SINGLE) { bt0 -= BT[0][bj]; bt1 -= BT[1][bj]; } }
-                };
-                int64_t hi = i + P, lo = i - P - 1;
-                if (hi >= n) { term(n - 1, +1); hi -= n; }
-                term(hi, +1);
-                if (lo < -1) { term(n - 1, +1); lo += n; }
-                if (lo >= 0) term(lo, -1);
-                W0 = (T)bt0 + sl0;
-                W1 = (T)bt1 + sl1;
-            }
+            const T W0 = W0v[e], W1 = W1v[e];
             if (MODEL == NET_MODEL_KS) {
                 T C = W0, S = W1;
                 if (!a.include_self) { C -= f0[e]; S -= f1[e]; }
@@ -244,11 +276,15 @@ __global__ void __launch_bounds__(RING_THREADS) ring_persistent_kernel(RingArgs 
 // ------------------------------------------------------------------ host side
 struct RingPlan { int E, G, chunk; bool single; size_t smem; };
 
-static bool ring_plan(int64_t n, size_t esize, RingPlan* p) {
-    for (int E = 1; E <= 8; E *= 2) {
+// gmax: CTAs that can be co-resident (one per SM always can; two per SM when the occupancy
+// query at launch agrees -- fewer elements per thread shorten the dependent chain of a stage)
+static bool ring_plan(int64_t n, size_t esize, RingPlan* p, int gmax = 148) {
+    int emin = 1;
+    if (const char* e = getenv("OSCNET_RING_E")) emin = atoi(e) > 0 ? atoi(e) : 1;   // tuning aid
+    for (int E = emin; E <= 8; E *= 2) {
         const int64_t chunk = (int64_t)RING_THREADS * E;
         const int64_t G = (n + chunk - 1) / chunk;
-        if (G <= 148) {   // one CTA per SM: co-resident whatever the register count
+        if (G <= gmax && G <= RING_GMAX) {
             p->E = E; p->G = (int)G; p->chunk = (int)chunk; p->single = G == 1;
             p->smem = p->single ? 2 * (size_t)chunk * esize : 0;
             return true;
@@ -274,6 +310,13 @@ static int32_t ring_launch_t(net* h, RingArgs& a, const RingPlan& p) {
     auto kern = ring_persistent_kernel<T, MODEL, E, SINGLE>;
     if (p.smem > 48 * 1024)
         OSC_CUDA(h, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.smem));
+    if (!SINGLE && p.G > 148) {      // more than one CTA per SM: must all be resident
+        int dev = 0, sms = 148, occ = 0;
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+        OSC_CUDA(h, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, RING_THREADS, p.smem));
+        if ((int64_t)occ * sms < p.G) return NET_ERR_UNSUPPORTED;
+    }
     if (!SINGLE) OSC_CUDA(h, cudaMemsetAsync(a.bar, 0, sizeof(unsigned), h->stream));
     void* params[] = {&a, &h->mp};
     if (SINGLE)
@@ -303,14 +346,14 @@ static int32_t ring_launch_e(net* h, RingArgs& a, const RingPlan& p) {
 }
 
 // y_in -> y_out over n_steps RK4 steps (rhs_only: y_out = f(y_in))
-int32_t ring_run(net* h, const void* y_in, void* y_out, int64_t n_steps, double dt, int rhs_only) {
-    RingPlan p;
-    if (!ring_plan(h->n, h->esize, &p)) return set_err(h, NET_ERR_UNSUPPORTED, "ring too large for the persistent kernel");
+static int32_t ring_run_plan(net* h, const RingPlan& p, const void* y_in, void* y_out, int64_t n_steps, double dt, int rhs_only) {
     RingArgs a;
     memset(&a, 0, sizeof(a));
     a.y_in = y_in; a.y_out = y_out; a.elem_param = h->b.elem_param;
     a.n = h->n; a.ld = h->ld; a.npad = round_up(h->n, 64);
     a.P = h->tv.P; a.include_self = h->tv.include_self; a.chunk = p.chunk; a.G = p.G;
+    a.chunk_shift = 0;
+    while ((1 << a.chunk_shift) < p.chunk) ++a.chunk_shift;
     a.n_steps = n_steps; a.dt = dt; a.rhs_only = rhs_only;
     char* s = (char*)h->b.scratch;
     const size_t sbytes = 2 * (size_t)a.npad * h->esize;
@@ -322,6 +365,14 @@ int32_t ring_run(net* h, const void* y_in, void* y_out, int64_t n_steps, double 
     if (h->desc.model == NET_MODEL_KS)
         return f32 ? ring_launch_e<float, NET_MODEL_KS>(h, a, p) : ring_launch_e<double, NET_MODEL_KS>(h, a, p);
     return f32 ? ring_launch_e<float, NET_MODEL_FHN>(h, a, p) : ring_launch_e<double, NET_MODEL_FHN>(h, a, p);
+}
+
+int32_t ring_run(net* h, const void* y_in, void* y_out, int64_t n_steps, double dt, int rhs_only) {
+    RingPlan p;
+    // (two CTAs per SM -- gmax = 296, half the elements per thread -- measured slower on config 2:
+    // 4.8e9 against 5.0e9 osc-steps/s; the 256-way barrier costs more than the shorter chain saves)
+    if (!ring_plan(h->n, h->esize, &p)) return set_err(h, NET_ERR_UNSUPPORTED, "ring too large for the persistent kernel");
+    return ring_run_plan(h, p, y_in, y_out, n_steps, dt, rhs_only);
 }
 
 }  // namespace oscnet
