@@ -178,6 +178,17 @@ def measure(w, device, steps, warmup, e2e=True, seed=1):
     return out
 
 
+def ncu_traffic(cfg):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the stage kernel, from the
+    committed `ncu --set full` capture of this build (profiles/ncu_traffic.json: mean over the
+    captured launches; None when there is no capture for this workload)."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "ncu_traffic.json")) as f:
+            return json.load(f).get(cfg, {}).get("bytes_per_launch")
+    except Exception:
+        return None
+
+
 def roofline_object(w, m, steps):
     """roofline of the dominant kernel (the fused RHS+RK4 stage kernel; every launch in the timed
     region is one of its four stage instances)."""
@@ -196,7 +207,9 @@ def roofline_object(w, m, steps):
         achieved, peak, unit = per_launch / avg_launch_s / 1e9, pk[c["pipe"] + "_ginstr_s"], "Ginstr/s"
         peak_src = "148 SM x %d lanes x sm_max_mhz (%s pipe)" % (R.LANES[c["pipe"]], c["pipe"])
     return {"bound": c["bound"], "achieved": achieved, "peak": peak, "unit": unit,
-            "frac": achieved / peak, "traffic": None, "kernel": "fused RHS+RK4 stage kernel",
+            "frac": achieved / peak, "traffic": ncu_traffic(w.cfg),
+            "kernel": "fused RHS+RK4 stage kernel",
+            "frac_of_nominal_8tbs": (achieved / 8000.0 if c["bound"] == "hbm" else None),
             "avg_launch_us": avg_launch_s * 1e6, "peak_source": peak_src,
             "bytes_per_osc_step": R.bytes_per_osc_step(w),
             "survey_bytes_per_osc_step": R.survey_bytes_per_osc_step(w),
@@ -205,8 +218,8 @@ def roofline_object(w, m, steps):
 
 
 # ------------------------------------------------------------------ CPU oracle arm
-SAMPLE = {"1": dict(), "2": dict(n=8192), "3a": dict(n1=64), "3b": dict(n1=64),
-          "4": dict(n=200_000), "5": dict(n1=96)}
+SAMPLE = {"1": dict(), "2": dict(n=16384), "3a": dict(n1=64), "3b": dict(n1=64),
+          "4": dict(n=200_000), "5": dict(n1=160)}
 
 
 def oracle_sample(cfg, seed=1):

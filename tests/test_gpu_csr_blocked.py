@@ -18,11 +18,11 @@ FAMILY_CSR_WARP, FAMILY_CSR_BLOCKED = 1, 7
 # (n, in-degree, "W,CR" or None for the library's own choice, dtype)
 CASES = [
     (20000, 100, "512,96", "f64"),      # 40 blocks, 209 chunks > 148 CTAs, M = 1
-    (20000, 100, "4096,1024", "f64"),   # 5 blocks, 20 chunks, ragged last block and chunk
+    (20000, 20, "4096,1024", "f64"),    # 5 blocks, 20 chunks, ragged last block and chunk, 20 % overflow
     (20011, 37, "1000,2500", "f64"),    # odd sizes, M = 3
     (9000, 64, "16,8192", "f64"),       # blocks of 16 columns (563 of them), M = 8... one chunk pair
     (50000, 20, None, "f64"),           # library geometry (n >= 32768): 2 blocks
-    (20000, 100, "4096,1024", "f32"),
+    (20000, 20, "4096,1024", "f32"),
 ]
 IDS = ["n%d-k%d-%s-%s" % (n, k, g or "auto", dt) for n, k, g, dt in CASES]
 
