@@ -180,13 +180,17 @@ def measure(w, device, steps, warmup, e2e=True, seed=1):
 
 def ncu_traffic(cfg):
     """dram__bytes_read.sum + dram__bytes_write.sum per launch of the stage kernel, from the
-    committed `ncu --set full` capture of this build (profiles/ncu_traffic.json: mean over the
-    captured launches; None when there is no capture for this workload)."""
+    committed `ncu --set full` capture of this build (profiles/ncu_traffic.csv: cfg, mean bytes
+    per captured launch, launches captured; None when there is no line for this workload)."""
     try:
-        with open(os.path.join(ROOT, "profiles", "ncu_traffic.json")) as f:
-            return json.load(f).get(cfg, {}).get("bytes_per_launch")
+        with open(os.path.join(ROOT, "profiles", "ncu_traffic.csv")) as f:
+            for line in f:
+                parts = [p.strip() for p in line.split(",")]
+                if len(parts) >= 2 and parts[0] == cfg:
+                    return float(parts[1])
     except Exception:
-        return None
+        pass
+    return None
 
 
 def roofline_object(w, m, steps):
@@ -250,7 +254,7 @@ def oracle_sample(cfg, seed=1):
     return w, net, y0, ora.omp_threads()
 
 
-def time_oracle(cfg, budget_s=12.0, rk4_steps=None):
+def time_oracle(cfg, budget_s=20.0, rk4_steps=None):
     """oscillator-steps/s of the oracle on its sample; about budget_s of CPU work."""
     w, net, y0, cores = oracle_sample(cfg)
     t0 = time.perf_counter()
