@@ -79,6 +79,50 @@ inline size_t l3_smem_bytes(const L3Geom& g, int P, int nt) {
     return 256 + (size_t)(P + 1 + g.D) * g.st_stride + (size_t)(g.D + 1) * nt * g.op_stride;
 }
 
+// Calls f(TXt, SY, score) for every tile the staged boxes and the thread budget allow.  Score:
+// lane / cover efficiency over the halo overhead, with the measured preferences below.
+template <class T, int MODEL, int P, class F>
+static int32_t l3_enumerate(int nx, int ny, int want_tx, int want_sy, F&& f) {
+    typedef L3Shape<T, P> S;
+    constexpr int X = S::X, TY = S::TY;
+    constexpr int HX = l2_hx<T>(P);
+    constexpr int U8 = 2 * (int)sizeof(T) / 8;
+    constexpr bool KS = MODEL == NET_MODEL_KS;
+    const int xq = (KS && sizeof(T) == 4) ? 4 : X;
+    for (int tiles_x = 1; tiles_x <= nx / xq; ++tiles_x) {
+        int TXt = ((nx + tiles_x - 1) / tiles_x + xq - 1) / xq * xq;
+        if (want_tx > 0) TXt = (want_tx + xq - 1) / xq * xq;
+        if (TXt > nx) TXt = nx;
+        const int tx = (nx + TXt - 1) / TXt;
+        const int QX = TXt / X;
+        if ((TXt + 2 * HX) * U8 > 256) { if (want_tx > 0) return NET_ERR_UNSUPPORTED; continue; }
+        for (int SY = 1; SY * QX <= L3_MAXT - 32 && SY * TY <= 256 - 2 * P; ++SY) {
+            if (want_sy > 0 && SY != want_sy) continue;
+            const int TYt = SY * TY, ty = (ny + TYt - 1) / TYt;
+            const int threads = QX * SY, warps = (threads + 31) / 32;
+            const double lane_eff = (double)threads / (32.0 * warps);
+            const double cover = (double)nx * ny / ((double)tx * TXt * ty * TYt);
+            const double halo = (double)(TXt + 2 * HX) * (TYt + 2 * P) / ((double)TXt * TYt);
+            // small CTAs (about four consumer warps) desynchronise better; mild preference
+            const double size_pen = warps <= 4 ? 1.0 : 1.0 - 0.02 * (warps - 4);
+            // shared-memory banks: the lanes of one vector-load phase (8 lanes of LDS.128) that fall
+            // on the next strip of rows are TY staged rows further on; if that distance is a
+            // multiple of 128 bytes they hit the banks of the lanes before them (measured: 39 % of
+            // the wavefronts of cfg 5 were such conflicts).  Phases never straddle strips when QX
+            // is a multiple of 8.  fp64 planes: the rule that held on cfg 3b is simply >= 16
+            // threads per staged row.
+            constexpr bool PLANAR = KS && sizeof(T) == 8;
+            const int row_bytes = (TXt + 2 * HX) * (PLANAR ? 8 : 2 * (int)sizeof(T));
+            const bool straddle = QX % 8 != 0 && SY > 1;
+            const double bank_pen = PLANAR ? (QX < 16 ? 0.85 : 1.0)
+                                           : ((straddle && (TY * row_bytes) % 128 == 0) ? 0.85 : 1.0);
+            f(TXt, SY, lane_eff * cover * size_pen * bank_pen / (1.0 + 0.25 * (halo - 1.0)));
+        }
+        if (want_tx > 0) break;
+    }
+    return NET_OK;
+}
+
 // Geometry of one stage.  Tiles: the (TXt, SY) with the best lane / cover efficiency among
 // those whose staged boxes TMA can take; pipeline depth D: the deepest that still leaves
 // `want_ctas` CTAs per SM; z chunks: fewest waves.  OSCNET_LAT3 = "TXt,SY,Lz,D,CTAS" overrides.
@@ -100,31 +144,15 @@ static int32_t l3_configure_stage(net* h) {
     // operand / stencil rows must be whole 16-byte vectors: scalar f32 tiles need TXt % 4 == 0
     const int xq = (KS && sizeof(T) == 4) ? 4 : X;
     if (g.nx % xq != 0) return NET_ERR_UNSUPPORTED;
+    if (want_tx <= 0 && h->l3_force_tx > 0) { want_tx = h->l3_force_tx; want_sy = h->l3_force_sy; }   // autotuned
     double best = -1.0;
-    for (int tiles_x = 1; tiles_x <= g.nx / xq; ++tiles_x) {
-        int TXt = ((g.nx + tiles_x - 1) / tiles_x + xq - 1) / xq * xq;
-        if (want_tx > 0) TXt = (want_tx + xq - 1) / xq * xq;
-        if (TXt > g.nx) TXt = g.nx;
-        const int tx = (g.nx + TXt - 1) / TXt;
-        const int QX = TXt / X;
-        if ((TXt + 2 * HX) * U8 > 256) { if (want_tx > 0) return NET_ERR_UNSUPPORTED; continue; }
-        for (int SY = 1; SY * QX <= L3_MAXT - 32 && SY * TY <= 256 - 2 * P; ++SY) {
-            if (want_sy > 0 && SY != want_sy) continue;
-            const int TYt = SY * TY, ty = (g.ny + TYt - 1) / TYt;
-            const int threads = QX * SY, warps = (threads + 31) / 32;
-            const double lane_eff = (double)threads / (32.0 * warps);
-            const double cover = (double)g.nx * g.ny / ((double)tx * TXt * ty * TYt);
-            const double halo = (double)(TXt + 2 * HX) * (TYt + 2 * P) / ((double)TXt * TYt);
-            // small CTAs (about four consumer warps) desynchronise better; mild preference
-            const double size_pen = warps <= 4 ? 1.0 : 1.0 - 0.02 * (warps - 4);
-            // fp64 planes: rows of fewer than 16 threads put the 8 lanes of a vector-load phase on
-            // several staged rows, whose pitch collides in the banks (measured on cfg 3b)
-            const double bank_pen = (KS && sizeof(T) == 8 && QX < 16) ? 0.85 : 1.0;
-            const double score = lane_eff * cover * size_pen * bank_pen / (1.0 + 0.25 * (halo - 1.0));
-            if (score > best) { best = score; g.TXt = TXt; g.TYt = TYt; g.QX = QX; g.SY = SY; g.tiles_x = tx; g.tiles_y = ty; }
+    int rc_enum = l3_enumerate<T, MODEL, P>(g.nx, g.ny, want_tx, want_sy, [&](int TXt, int SY, double score) {
+        if (score > best) {
+            best = score; g.TXt = TXt; g.TYt = SY * TY; g.QX = TXt / X; g.SY = SY;
+            g.tiles_x = (g.nx + TXt - 1) / TXt; g.tiles_y = (g.ny + g.TYt - 1) / g.TYt;
         }
-        if (want_tx > 0) break;
-    }
+    });
+    if (rc_enum) return rc_enum;
     if (best < 0) return NET_ERR_UNSUPPORTED;
     g.PW = g.TXt + 2 * HX;
     g.PH = g.TYt + 2 * P;
@@ -176,8 +204,9 @@ static int32_t l3_configure_stage(net* h) {
     return NET_OK;
 }
 
+// all stages + tensor maps for the tile l3_configure_stage picks (by score, or h->l3_force_*)
 template <class T, int MODEL, int P>
-static int32_t l3_configure(net* h) {
+static int32_t l3_configure_tile(net* h) {
     constexpr int HX = l2_hx<T>(P);
     constexpr int U8 = 2 * (int)sizeof(T) / 8;
     constexpr bool KS = MODEL == NET_MODEL_KS;
@@ -280,6 +309,76 @@ static int32_t l3_stage(net* h, int stage, double dt, void* rhs_out) {
             if (KS) op[0] = to[3];
             return l3_launch_stage<T, MODEL, P, L3_RHS>(h, a, dt, tm[0], op);
     }
+}
+
+// Tile autotuner ("measure, don't guess"): the score of l3_enumerate ranks tiles by geometry, but
+// bank conflicts, wave quantisation and the depth of the pipeline decide among the leaders (cfg 5:
+// 4.8e10 with the best-scoring tile, 5.3e10 with the best-measured one).  For nets large enough to
+// matter the best-scoring tile of each of the leading tile widths is timed on stages 1 and 2
+// (zeroed buffers; net_create re-zeroes the state afterwards) and the fastest is kept.  The
+// arithmetic of every output is the same for every tile, so results do not depend on the pick.
+// OSCNET_LAT3 (explicit geometry) or OSCNET_NO_AUTOTUNE switch it off.
+template <class T, int MODEL, int P>
+static int32_t l3_configure(net* h) {
+    typedef L3Shape<T, P> S;
+    h->l3_force_tx = h->l3_force_sy = 0;
+    int32_t rc = l3_configure_tile<T, MODEL, P>(h);
+    if (rc) return rc;
+    if (getenv("OSCNET_LAT3") || getenv("OSCNET_NO_AUTOTUNE") || h->n < (1 << 21)) return NET_OK;
+    struct Cand { int tx, sy; double score; };
+    constexpr int KMAX = 10;
+    Cand cand[KMAX];
+    int nc = 0;
+    l3_enumerate<T, MODEL, P>(h->tv.nx, h->tv.ny, 0, 0, [&](int TXt, int SY, double score) {
+        for (int q = 0; q < nc; ++q)
+            if (cand[q].tx == TXt) {           // one entry per tile width: its best SY
+                if (score > cand[q].score) { cand[q].sy = SY; cand[q].score = score; }
+                return;
+            }
+        if (nc < KMAX) { cand[nc++] = Cand{TXt, SY, score}; return; }
+        int worst = 0;
+        for (int q = 1; q < nc; ++q) if (cand[q].score < cand[worst].score) worst = q;
+        if (score > cand[worst].score) cand[worst] = Cand{TXt, SY, score};
+    });
+    const size_t sb = h->state_bytes;
+    OSC_CUDA(h, cudaMemsetAsync(h->b.y, 0, sb, h->stream));
+    OSC_CUDA(h, cudaMemsetAsync(h->b.Y2, 0, sb, h->stream));
+    OSC_CUDA(h, cudaMemsetAsync(h->b.Y3, 0, sb, h->stream));
+    OSC_CUDA(h, cudaMemsetAsync(h->b.Y4, 0, sb, h->stream));
+    OSC_CUDA(h, cudaMemsetAsync(h->b.elem_param, 0, (size_t)h->ld * h->esize, h->stream));
+    if (MODEL == NET_MODEL_KS) {
+        const size_t eb = (size_t)h->lat3[0].plane * 2 * sizeof(T);
+        OSC_CUDA(h, cudaMemsetAsync(h->E_a, 0, eb, h->stream));
+        OSC_CUDA(h, cudaMemsetAsync(h->E_b, 0, eb, h->stream));
+    }
+    cudaEvent_t e0, e1;
+    OSC_CUDA(h, cudaEventCreate(&e0));
+    OSC_CUDA(h, cudaEventCreate(&e1));
+    float best_ms = -1.f;
+    int best = -1;
+    const int64_t launches_before = h->launches;
+    for (int q = 0; q < nc; ++q) {
+        h->l3_force_tx = cand[q].tx; h->l3_force_sy = cand[q].sy;
+        if (l3_configure_tile<T, MODEL, P>(h) != NET_OK) continue;
+        float ms = 0.f;
+        bool ok = true;
+        for (int rep = 0; rep < 3 && ok; ++rep) {           // rep 0 warms up
+            if (rep == 1) ok = cudaEventRecord(e0, h->stream) == cudaSuccess;
+            ok = ok && l3_stage<T, MODEL, P>(h, 1, 1e-3, nullptr) == NET_OK && l3_stage<T, MODEL, P>(h, 2, 1e-3, nullptr) == NET_OK;
+        }
+        ok = ok && cudaEventRecord(e1, h->stream) == cudaSuccess && cudaEventSynchronize(e1) == cudaSuccess &&
+             cudaEventElapsedTime(&ms, e0, e1) == cudaSuccess;
+        if (getenv("OSCNET_VERBOSE"))
+            fprintf(stderr, "lat3 autotune: tile %dx%d score %.3f -> %.3f ms%s\n", cand[q].tx, cand[q].sy * S::TY, cand[q].score, ms, ok ? "" : " (failed)");
+        if (ok && (best < 0 || ms < best_ms)) { best = q; best_ms = ms; }
+    }
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    h->launches = launches_before;
+    if (cudaGetLastError() != cudaSuccess) best = -1;
+    if (best >= 0) { h->l3_force_tx = cand[best].tx; h->l3_force_sy = cand[best].sy; }
+    else h->l3_force_tx = h->l3_force_sy = 0;
+    return l3_configure_tile<T, MODEL, P>(h);
 }
 
 // entry point of one (dtype, model): configure (stage < 0) or launch
