@@ -140,7 +140,7 @@ static int32_t l3_configure_stage(net* h) {
     g.nx = tv.nx; g.ny = tv.ny; g.nz = tv.nz;
     int want_tx = 0, want_sy = 0, want_lz = 0, want_d = 0, want_ctas = 0;
     if (const char* e = getenv("OSCNET_LAT3")) sscanf(e, "%d,%d,%d,%d,%d", &want_tx, &want_sy, &want_lz, &want_d, &want_ctas);
-    if (want_ctas <= 0) want_ctas = 2;
+    if (want_ctas <= 0) want_ctas = h->l3_force_ctas > 0 ? h->l3_force_ctas : 2;
     // operand / stencil rows must be whole 16-byte vectors: scalar f32 tiles need TXt % 4 == 0
     const int xq = (KS && sizeof(T) == 4) ? 4 : X;
     if (g.nx % xq != 0) return NET_ERR_UNSUPPORTED;
@@ -321,11 +321,11 @@ static int32_t l3_stage(net* h, int stage, double dt, void* rhs_out) {
 template <class T, int MODEL, int P>
 static int32_t l3_configure(net* h) {
     typedef L3Shape<T, P> S;
-    h->l3_force_tx = h->l3_force_sy = 0;
+    h->l3_force_tx = h->l3_force_sy = h->l3_force_ctas = 0;
     int32_t rc = l3_configure_tile<T, MODEL, P>(h);
     if (rc) return rc;
     if (getenv("OSCNET_LAT3") || getenv("OSCNET_NO_AUTOTUNE") || h->n < (1 << 21)) return NET_OK;
-    struct Cand { int tx, sy; double score; };
+    struct Cand { int tx, sy; double score; int ctas; };
     constexpr int KMAX = 10;
     Cand cand[KMAX];
     int nc = 0;
@@ -335,10 +335,10 @@ static int32_t l3_configure(net* h) {
                 if (score > cand[q].score) { cand[q].sy = SY; cand[q].score = score; }
                 return;
             }
-        if (nc < KMAX) { cand[nc++] = Cand{TXt, SY, score}; return; }
+        if (nc < KMAX) { cand[nc++] = Cand{TXt, SY, score, 2}; return; }
         int worst = 0;
         for (int q = 1; q < nc; ++q) if (cand[q].score < cand[worst].score) worst = q;
-        if (score > cand[worst].score) cand[worst] = Cand{TXt, SY, score};
+        if (score > cand[worst].score) cand[worst] = Cand{TXt, SY, score, 2};
     });
     const size_t sb = h->state_bytes;
     OSC_CUDA(h, cudaMemsetAsync(h->b.y, 0, sb, h->stream));
@@ -357,9 +357,9 @@ static int32_t l3_configure(net* h) {
     float best_ms = -1.f;
     int best = -1;
     const int64_t launches_before = h->launches;
-    for (int q = 0; q < nc; ++q) {
-        h->l3_force_tx = cand[q].tx; h->l3_force_sy = cand[q].sy;
-        if (l3_configure_tile<T, MODEL, P>(h) != NET_OK) continue;
+    auto time_cand = [&](const Cand& c, float* ms_out) -> bool {
+        h->l3_force_tx = c.tx; h->l3_force_sy = c.sy; h->l3_force_ctas = c.ctas;
+        if (l3_configure_tile<T, MODEL, P>(h) != NET_OK) return false;
         float ms = 0.f;
         bool ok = true;
         for (int rep = 0; rep < 3 && ok; ++rep) {           // rep 0 warms up
@@ -369,15 +369,28 @@ static int32_t l3_configure(net* h) {
         ok = ok && cudaEventRecord(e1, h->stream) == cudaSuccess && cudaEventSynchronize(e1) == cudaSuccess &&
              cudaEventElapsedTime(&ms, e0, e1) == cudaSuccess;
         if (getenv("OSCNET_VERBOSE"))
-            fprintf(stderr, "lat3 autotune: tile %dx%d score %.3f -> %.3f ms%s\n", cand[q].tx, cand[q].sy * S::TY, cand[q].score, ms, ok ? "" : " (failed)");
-        if (ok && (best < 0 || ms < best_ms)) { best = q; best_ms = ms; }
+            fprintf(stderr, "lat3 autotune: tile %dx%d ctas %d score %.3f -> %.3f ms%s\n", c.tx, c.sy * S::TY, c.ctas, c.score, ms, ok ? "" : " (failed)");
+        *ms_out = ms;
+        return ok;
+    };
+    Cand best_c = Cand{0, 0, 0.0, 0};
+    for (int q = 0; q < nc; ++q) {
+        float ms;
+        if (time_cand(cand[q], &ms) && (best < 0 || ms < best_ms)) { best = q; best_ms = ms; best_c = cand[q]; }
     }
+    if (best >= 0)                                           // shallower pipelines of the winner
+        for (int ctas = 3; ctas <= 4; ++ctas) {
+            Cand c = cand[best];
+            c.ctas = ctas;
+            float ms;
+            if (time_cand(c, &ms) && ms < best_ms) { best_ms = ms; best_c = c; }
+        }
     cudaEventDestroy(e0);
     cudaEventDestroy(e1);
     h->launches = launches_before;
     if (cudaGetLastError() != cudaSuccess) best = -1;
-    if (best >= 0) { h->l3_force_tx = cand[best].tx; h->l3_force_sy = cand[best].sy; }
-    else h->l3_force_tx = h->l3_force_sy = 0;
+    if (best >= 0) { h->l3_force_tx = best_c.tx; h->l3_force_sy = best_c.sy; h->l3_force_ctas = best_c.ctas; }
+    else h->l3_force_tx = h->l3_force_sy = h->l3_force_ctas = 0;
     return l3_configure_tile<T, MODEL, P>(h);
 }
 
