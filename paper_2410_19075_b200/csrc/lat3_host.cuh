@@ -5,6 +5,7 @@
 #include <stdlib.h>
 
 #include "lat3_kernel.cuh"
+#include "lat3s_kernel.cuh"
 
 namespace oscnet {
 
@@ -16,6 +17,13 @@ template <> struct L3Shape<double, 2> { static constexpr int X = 2, TY = 2; };
 template <> struct L3Shape<double, 4> { static constexpr int X = 2, TY = 1; };
 constexpr int L3_MAXT = 288;     // up to 8 consumer warps + the producer warp
 constexpr int L3_MINB = 1;
+// fp64 KS runs the field-split kernel (lat3s_kernel.cuh): two lanes per 2 x 2 block of outputs
+template <class T, int MODEL, int P> struct L3Sh {
+    static constexpr bool SPLIT = MODEL == NET_MODEL_KS && sizeof(T) == 8;
+    static constexpr int X = SPLIT ? 2 : L3Shape<T, P>::X;
+    static constexpr int TY = SPLIT ? 2 : L3Shape<T, P>::TY;
+    static constexpr int UPW = SPLIT ? 16 : 32;      // blocks of X x TY outputs per consumer warp
+};
 
 typedef CUresult (*l3_encode_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
@@ -71,8 +79,13 @@ inline int32_t l3_encode_planes(net* h, CUtensorMap* tm, void* base, uint64_t ex
 
 template <class T, int MODEL, int P, int STAGE>
 static auto l3_kernel_ptr() {
-    typedef L3Shape<T, P> S;
-    return lat3_kernel<T, MODEL, P, STAGE, S::X, S::TY, L3_MAXT, L3_MINB, (P > 2 && sizeof(T) == 4)>;
+    typedef L3Sh<T, MODEL, P> S;
+    if constexpr (S::SPLIT) {
+        static const bool rot = getenv("OSCNET_L3S_ROT") ? atoi(getenv("OSCNET_L3S_ROT")) != 0 : (P > 2);
+        return rot ? lat3s_kernel<T, P, STAGE, L3_MAXT, L3_MINB, true> : lat3s_kernel<T, P, STAGE, L3_MAXT, L3_MINB, false>;
+    } else {
+        return lat3_kernel<T, MODEL, P, STAGE, S::X, S::TY, L3_MAXT, L3_MINB, (P > 2 && sizeof(T) == 4)>;
+    }
 }
 
 inline size_t l3_smem_bytes(const L3Geom& g, int P, int nt) {
@@ -83,7 +96,7 @@ inline size_t l3_smem_bytes(const L3Geom& g, int P, int nt) {
 // lane / cover efficiency over the halo overhead, with the measured preferences below.
 template <class T, int MODEL, int P, class F>
 static int32_t l3_enumerate(int nx, int ny, int want_tx, int want_sy, F&& f) {
-    typedef L3Shape<T, P> S;
+    typedef L3Sh<T, MODEL, P> S;
     constexpr int X = S::X, TY = S::TY;
     constexpr int HX = l2_hx<T>(P);
     constexpr int U8 = 2 * (int)sizeof(T) / 8;
@@ -96,11 +109,11 @@ static int32_t l3_enumerate(int nx, int ny, int want_tx, int want_sy, F&& f) {
         const int tx = (nx + TXt - 1) / TXt;
         const int QX = TXt / X;
         if ((TXt + 2 * HX) * U8 > 256) { if (want_tx > 0) return NET_ERR_UNSUPPORTED; continue; }
-        for (int SY = 1; SY * QX <= L3_MAXT - 32 && SY * TY <= 256 - 2 * P; ++SY) {
+        for (int SY = 1; (SY * QX + S::UPW - 1) / S::UPW * 32 <= L3_MAXT - 32 && SY * TY <= 256 - 2 * P; ++SY) {
             if (want_sy > 0 && SY != want_sy) continue;
             const int TYt = SY * TY, ty = (ny + TYt - 1) / TYt;
-            const int threads = QX * SY, warps = (threads + 31) / 32;
-            const double lane_eff = (double)threads / (32.0 * warps);
+            const int units = QX * SY, warps = (units + S::UPW - 1) / S::UPW;
+            const double lane_eff = (double)units / ((double)S::UPW * warps);
             const double cover = (double)nx * ny / ((double)tx * TXt * ty * TYt);
             const double halo = (double)(TXt + 2 * HX) * (TYt + 2 * P) / ((double)TXt * TYt);
             // small CTAs (about four consumer warps) desynchronise better; mild preference
@@ -114,7 +127,7 @@ static int32_t l3_enumerate(int nx, int ny, int want_tx, int want_sy, F&& f) {
             constexpr bool PLANAR = KS && sizeof(T) == 8;
             const int row_bytes = (TXt + 2 * HX) * (PLANAR ? 8 : 2 * (int)sizeof(T));
             const bool straddle = QX % 8 != 0 && SY > 1;
-            const double bank_pen = PLANAR ? (QX < 16 ? 0.85 : 1.0)
+            const double bank_pen = PLANAR ? (QX % 8 != 0 ? 0.85 : 1.0)
                                            : ((straddle && (TY * row_bytes) % 128 == 0) ? 0.85 : 1.0);
             f(TXt, SY, lane_eff * cover * size_pen * bank_pen / (1.0 + 0.25 * (halo - 1.0)));
         }
@@ -128,7 +141,7 @@ static int32_t l3_enumerate(int nx, int ny, int want_tx, int want_sy, F&& f) {
 // `want_ctas` CTAs per SM; z chunks: fewest waves.  OSCNET_LAT3 = "TXt,SY,Lz,D,CTAS" overrides.
 template <class T, int MODEL, int P, int STAGE>
 static int32_t l3_configure_stage(net* h) {
-    typedef L3Shape<T, P> S;
+    typedef L3Sh<T, MODEL, P> S;
     constexpr int X = S::X, TY = S::TY;
     constexpr int HX = l2_hx<T>(P);
     constexpr int U8 = 2 * (int)sizeof(T) / 8;
@@ -156,7 +169,7 @@ static int32_t l3_configure_stage(net* h) {
     if (best < 0) return NET_ERR_UNSUPPORTED;
     g.PW = g.TXt + 2 * HX;
     g.PH = g.TYt + 2 * P;
-    g.ncw = (g.QX * g.SY + 31) / 32;
+    g.ncw = (g.QX * g.SY + S::UPW - 1) / S::UPW;
     g.st_bytes = (unsigned)((size_t)g.PW * g.PH * 2 * sizeof(T));
     g.st_stride = (g.st_bytes + 127u) / 128u * 128u;
     g.op_bytes = (unsigned)((size_t)g.TXt * g.TYt * (KS ? 1 : 2) * sizeof(T));
@@ -320,7 +333,7 @@ static int32_t l3_stage(net* h, int stage, double dt, void* rhs_out) {
 // OSCNET_LAT3 (explicit geometry) or OSCNET_NO_AUTOTUNE switch it off.
 template <class T, int MODEL, int P>
 static int32_t l3_configure(net* h) {
-    typedef L3Shape<T, P> S;
+    typedef L3Sh<T, MODEL, P> S;
     h->l3_force_tx = h->l3_force_sy = h->l3_force_ctas = 0;
     int32_t rc = l3_configure_tile<T, MODEL, P>(h);
     if (rc) return rc;

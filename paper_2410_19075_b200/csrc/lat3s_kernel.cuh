@@ -1,0 +1,270 @@
+// Field-split variant of the third-generation 3D lattice kernel for fp64 Kuramoto-Sakaguchi
+// lattices (config 3b).
+//
+// Same mathematics and the same producer / mbarrier pipeline as lat3_kernel.cuh (x-run
+// decomposition of the ball of PAPER.md:313, z-marching register accumulators, factorised sine
+// of Alg. 1).  What the ncu capture of lat3_kernel on cfg 3b showed
+// (profiles/r01_final_ncu.md): with both fields of the ball sum, (cos phi, sin phi), carried as a
+// pair by every thread, the fp64 accumulators of the 2P + 1 open planes leave room for only
+// X x TY = 2 x 1 outputs per thread, so every thread loads and run-sums 2P + 1 staged rows for
+// ONE output row -- 45 LDS.128 and 164 DADD per output, two thirds of the kernel time in
+// shared-memory wavefronts.
+// Here the two lanes  l  and  l ^ 16  of a warp share one 2 x 2 block of outputs and each carries
+// ONE field (lanes 0-15 the cos plane, lanes 16-31 the sin plane): the same 72 accumulator
+// registers now cover 2 x 2 outputs of one field, the staged rows are shared by two output rows
+// (25 LDS.128 and 114 DADD per output), and the two partial results meet once per finished plane
+// through a warp shuffle; lane f then finishes output row f of the block.
+#pragma once
+#include "lat3_kernel.cuh"
+
+namespace oscnet {
+
+template <class T, int P, int STAGE, int MAXT, int MINB, bool ROT>
+__global__ void __launch_bounds__(MAXT, MINB)
+lat3s_kernel(const __grid_constant__ CUtensorMap tm_st, const __grid_constant__ CUtensorMap tm_op0,
+             const __grid_constant__ CUtensorMap tm_op1, const __grid_constant__ CUtensorMap tm_op2,
+             const __grid_constant__ CUtensorMap tm_op3, L3Ptrs a, L3Params<T> mp, L3Geom g) {
+    static_assert(sizeof(T) == 8, "field-split kernel: fp64 planes");
+    constexpr int MODEL = NET_MODEL_KS;
+    constexpr int X = 2, TY = 2;
+    constexpr int HX = l2_hx<T>(P);           // x ghost width of the padded planes
+    constexpr int OFF = HX - P;
+    constexpr int NCOL = X + 2 * P;           // scalars a thread reads per staged row
+    constexpr int NACC = 2 * P + 1;
+    constexpr int NT = L3Ops<MODEL, STAGE>::N;
+    static_assert(OFF % 2 == 0 && NCOL % 2 == 0, "16-byte row pieces");
+
+    extern __shared__ __align__(128) unsigned char l3_smem[];
+    const int D = g.D, NB = D + 1, NS = P + 1 + D;
+    uint64_t* full = reinterpret_cast<uint64_t*>(l3_smem);      // NB barriers
+    uint64_t* done = full + NB;                                  // NB barriers
+    unsigned char* st_ring = l3_smem + 256;
+    unsigned char* op_ring = st_ring + (size_t)NS * g.st_stride;
+
+    const int nx = g.nx, ny = g.ny, nz = g.nz;
+    int bid = blockIdx.x;
+    const int tix = bid % g.tiles_x; bid /= g.tiles_x;
+    const int tiy = bid % g.tiles_y; bid /= g.tiles_y;
+    const int x0 = tix * g.TXt, y0 = tiy * g.TYt;
+    const int z0 = bid * g.Lz;
+    const int z1 = min(nz, z0 + g.Lz);
+    const int nplanes = (z1 - z0) + 2 * P;
+    const int tid = threadIdx.x;
+
+    if (tid == 0) {
+        for (int s = 0; s < NB; ++s) { mbar_init(full + s, 1); mbar_init(done + s, (unsigned)g.ncw); }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+
+    // ------------------------------------------------------------------ producer warp
+    if ((tid >> 5) == g.ncw) {
+        if ((tid & 31) == 0) {
+            asm volatile("prefetch.tensormap [%0];" ::"l"(&tm_st) : "memory");
+            if (NT >= 1) asm volatile("prefetch.tensormap [%0];" ::"l"(&tm_op0) : "memory");
+            if (NT >= 2) asm volatile("prefetch.tensormap [%0];" ::"l"(&tm_op1) : "memory");
+            int b = 0, ss = 0;
+            unsigned round = 0;
+            for (int j = 0; j < nplanes; ++j) {
+                if (round > 0) mbar_wait(done + b, (round & 1u) ^ 1u);
+                const bool ops = NT > 0 && j >= 2 * P;
+                mbar_expect_tx(full + b, g.st_bytes + (ops ? NT * g.op_bytes : 0u));
+                int zz = (z0 - P + j) % nz; if (zz < 0) zz += nz;
+                tma_load_4d(st_ring + (size_t)ss * g.st_stride, &tm_st, x0, y0, zz, 0, full + b);
+                if (ops) {
+                    const int zo = z0 - 2 * P + j;
+                    unsigned char* ob = op_ring + (size_t)b * NT * g.op_stride;
+                    if (NT >= 1) tma_load_3d(ob, &tm_op0, x0, y0, zo, full + b);
+                    if (NT >= 2) tma_load_3d(ob + g.op_stride, &tm_op1, x0, y0, zo, full + b);
+                    if (NT >= 3) tma_load_3d(ob + 2 * (size_t)g.op_stride, &tm_op2, x0, y0, zo, full + b);
+                    if (NT >= 4) tma_load_3d(ob + 3 * (size_t)g.op_stride, &tm_op3, x0, y0, zo, full + b);
+                }
+                ss = ss + 1 == NS ? 0 : ss + 1;
+                if (++b == NB) { b = 0; ++round; }
+            }
+        }
+        return;
+    }
+
+    // ------------------------------------------------------------------ consumer warps
+    // lanes l and l ^ 16 own the same 2 x 2 block of outputs ("unit"), one field each
+    const int PW = g.PW;
+    const int lane = tid & 31;
+    const int f = lane >> 4;                              // 0: cos plane, 1: sin plane
+    const int unit = (tid >> 5) * 16 + (lane & 15);
+    const int q = unit % g.QX, st = unit / g.QX;
+    const int x = x0 + q * X;
+    const bool owner = st < g.SY && x < nx;
+    const int yrow0 = y0 + st * TY;
+    const int nxp = nx + 2 * HX, nyp = ny + 2 * P;
+    const int64_t nxy = (int64_t)nx * ny;
+    const int64_t pxy = (int64_t)nxp * nyp;
+    const int gxs = x < HX ? nx : (x >= nx - HX ? -nx : 0);   // periodic image this thread also writes
+    const int splane = PW * g.PH;                             // scalars between the staged cos and sin boxes
+
+    T acc[NACC][TY][X];
+#pragma unroll
+    for (int k = 0; k < NACC; ++k)
+#pragma unroll
+        for (int r = 0; r < TY; ++r)
+#pragma unroll
+            for (int i = 0; i < X; ++i) acc[k][r][i] = T(0);
+
+    int slot = 0, cslot = NS - P, b = 0;      // ring slots of planes i and i - P; barrier index
+    unsigned phase = 0;
+
+    auto do_plane = [&](int i, auto Jc) {
+        constexpr int J = decltype(Jc)::value;
+        const int zo = z0 - 2 * P + i;            // output plane completed by this iteration
+        mbar_wait(full + b, phase);
+        if (owner) {
+            const T* sb = reinterpret_cast<const T*>(st_ring + (size_t)slot * g.st_stride) + f * splane + (st * TY) * PW + q * X + OFF;
+            T A[P > 1 ? P - 1 : 1][TY][X];
+            bool Aset[P > 1 ? P - 1 : 1][TY];
+#pragma unroll
+            for (int k = 0; k < (P > 1 ? P - 1 : 1); ++k)
+#pragma unroll
+                for (int r = 0; r < TY; ++r) Aset[k][r] = false;
+#pragma unroll
+            for (int rr = 0; rr < TY + 2 * P; ++rr) {           // staged row rr <-> y = yrow0 - P + rr
+                const int dist = rr < P ? P - rr : (rr >= TY + P ? rr - (TY + P - 1) : 0);
+                const int wmax = l2_run_w(P, 0, dist);
+                T v[NCOL];
+                const T* row = sb + rr * PW;
+#pragma unroll
+                for (int c = 0; c < NCOL / 2; ++c) {
+                    if (2 * c + 1 < P - wmax || 2 * c > P + X - 1 + wmax) continue;     // columns no run of this row reaches
+                    const double2 w2 = *reinterpret_cast<const double2*>(row + 2 * c);
+                    v[2 * c] = w2.x; v[2 * c + 1] = w2.y;
+                }
+                T R[P + 1][X];
+#pragma unroll
+                for (int e = 0; e < X; ++e) {
+                    R[0][e] = v[P + e];
+#pragma unroll
+                    for (int w = 1; w <= P; ++w)
+                        if (w <= wmax) R[w][e] = R[w - 1][e] + (v[P + e - w] + v[P + e + w]);
+                }
+#pragma unroll
+                for (int r = 0; r < TY; ++r) {
+                    const int ady = rr - P - r < 0 ? -(rr - P - r) : rr - P - r;
+                    if (ady > P) continue;
+                    {   // |dz| = 0: straight into the accumulator of output plane i
+                        const int w = l2_run_w(P, 0, ady);
+#pragma unroll
+                        for (int e = 0; e < X; ++e) acc[(J + P) % NACC][r][e] += R[w][e];
+                    }
+#pragma unroll
+                    for (int k = 1; k < P; ++k) {    // 0 < |dz| < P: in-plane partial sums
+                        const int w = l2_run_w(P, k, ady);
+                        if (w >= 0) {
+#pragma unroll
+                            for (int e = 0; e < X; ++e)
+                                A[k - 1][r][e] = Aset[k - 1][r] ? A[k - 1][r][e] + R[w][e] : R[w][e];
+                            Aset[k - 1][r] = true;
+                        }
+                    }
+                    if (ady == 0) {                  // |dz| = P: the centre alone (first / last contribution)
+#pragma unroll
+                        for (int e = 0; e < X; ++e) {
+                            acc[(J + 2 * P) % NACC][r][e] = R[0][e];
+                            acc[J % NACC][r][e] += R[0][e];
+                        }
+                    }
+                }
+            }
+#pragma unroll
+            for (int k = 1; k < P; ++k)
+#pragma unroll
+                for (int r = 0; r < TY; ++r)
+#pragma unroll
+                    for (int e = 0; e < X; ++e) {
+                        acc[(J + P - k) % NACC][r][e] += A[k - 1][r][e];
+                        acc[(J + P + k) % NACC][r][e] += A[k - 1][r][e];
+                    }
+        }
+        // ---- finish output plane zo (accumulator J): lane f takes output row f of the block
+        if (zo >= z0) {                                   // uniform over the CTA
+            T other[X];
+#pragma unroll
+            for (int e = 0; e < X; ++e) {
+                const T send = f ? acc[J % NACC][0][e] : acc[J % NACC][1][e];    // the row the partner finishes
+                other[e] = __shfl_xor_sync(0xffffffffu, send, 16);
+            }
+            const int r = f;
+            const int yy = yrow0 + r;
+            if (owner && yy < ny) {
+                const T* cc = reinterpret_cast<const T*>(st_ring + (size_t)cslot * g.st_stride) + (st * TY + P + r) * PW + q * X + HX;
+                const T* ob = reinterpret_cast<const T*>(op_ring + (size_t)b * NT * g.op_stride) + (st * TY + r) * g.TXt + q * X;
+                const int ostride = g.op_stride / (int)sizeof(T);    // scalars between operand tiles
+                const int64_t il = (int64_t)zo * nxy + (int64_t)yy * nx + x;                    // plain scalar arrays
+                const int64_t ip = (int64_t)zo * pxy + (int64_t)(yy + P) * nxp + (x + HX);     // padded planes
+                const int gys = yy < P ? ny : (yy >= ny - P ? -ny : 0);
+                T o0[X], o1[X], o2[X], o3[X];
+                if (NT >= 1) ldg_vec<X>(ob, o0);
+                if (NT >= 2) ldg_vec<X>(ob + ostride, o1);
+                if (NT >= 3) ldg_vec<X>(ob + 2 * ostride, o2);
+                if (NT >= 4) ldg_vec<X>(ob + 3 * ostride, o3);
+                T cx[X], cy[X];
+                ldg_vec<X>(cc, cx);
+                ldg_vec<X>(cc + splane, cy);
+                T ov[X], zv[X], cv[X], sv[X];
+#pragma unroll
+                for (int e = 0; e < X; ++e) {
+                    const T own = f ? acc[J % NACC][1][e] : acc[J % NACC][0][e];
+                    T C = f ? other[e] : own, S = f ? own : other[e];
+                    if (!mp.include_self) { C -= cx[e]; S -= cy[e]; }
+                    const T cia = cx[e] * mp.ca - cy[e] * mp.sa;      // cos(phi_i + alpha)
+                    const T sia = cy[e] * mp.ca + cx[e] * mp.sa;      // sin(phi_i + alpha)
+                    const T om = NT == 4 ? o3[e] : NT == 2 ? o1[e] : o0[e];
+                    const T k = om + mp.kd * (S * cia - C * sia);
+                    T o;
+                    if constexpr (STAGE == L3_RHS) o = k;
+                    else o = o0[e] + mp.h * k;                   // y (stages 0-2) or Z (stage 3)
+                    if constexpr (STAGE == L3_S2) zv[e] = (o1[e] + T(2) * o2[e] + o - o0[e]) * T(1.0 / 3.0);
+                    ov[e] = o;
+                    if constexpr (STAGE != L3_RHS) sincos_stage<T>(o, &sv[e], &cv[e]);
+                }
+                stg_vec<X>((T*)a.out + il, ov);
+                if constexpr (STAGE == L3_S2) stg_vec<X>((T*)a.out2 + il, zv);
+                if constexpr (STAGE != L3_RHS) {
+                    T* Ec = (T*)a.Eout;
+                    T* Es = Ec + g.plane;
+                    auto store_planes = [&](int64_t at) { stg_vec<X>(Ec + at, cv); stg_vec<X>(Es + at, sv); };
+                    store_planes(ip);
+                    if (gxs != 0) store_planes(ip + gxs);
+                    if (gys != 0) {
+                        store_planes(ip + (int64_t)gys * nxp);
+                        if (gxs != 0) store_planes(ip + (int64_t)gys * nxp + gxs);
+                    }
+                }
+            }
+        }
+        // this warp is done with barrier b: stencil plane i - P and operand slot b may be refilled
+        __syncwarp();
+        if (lane == 0) mbar_arrive(done + b);
+        slot = slot + 1 == NS ? 0 : slot + 1;
+        cslot = cslot + 1 == NS ? 0 : cslot + 1;
+        if (++b == NB) { b = 0; phase ^= 1u; }
+    };
+
+    if constexpr (ROT) {
+#pragma unroll 1
+        for (int i = 0; i < nplanes; ++i) {
+            do_plane(i, std::integral_constant<int, 0>{});
+#pragma unroll
+            for (int k = 0; k + 1 < NACC; ++k)
+#pragma unroll
+                for (int r = 0; r < TY; ++r)
+#pragma unroll
+                    for (int e = 0; e < X; ++e) acc[k][r][e] = acc[k + 1][r][e];
+        }
+    } else {
+        for (int base = 0; base < nplanes; base += NACC)
+            l2_static_for<0, NACC>([&](auto Jc) {
+                if (base + decltype(Jc)::value < nplanes) do_plane(base + decltype(Jc)::value, Jc);
+            });
+    }
+}
+
+}  // namespace oscnet
