@@ -17,13 +17,26 @@ template <> struct L3Shape<double, 2> { static constexpr int X = 2, TY = 2; };
 template <> struct L3Shape<double, 4> { static constexpr int X = 2, TY = 1; };
 constexpr int L3_MAXT = 288;     // up to 8 consumer warps + the producer warp
 constexpr int L3_MINB = 1;
-// fp64 KS runs the field-split kernel (lat3s_kernel.cuh): two lanes per 2 x 2 block of outputs
+// KS runs the field-split kernel (lat3s_kernel.cuh): two lanes per 2 x 2 block of outputs, the
+// exchange field E as two planes (cos | sin)
 template <class T, int MODEL, int P> struct L3Sh {
-    static constexpr bool SPLIT = MODEL == NET_MODEL_KS && sizeof(T) == 8;
+    static constexpr bool SPLIT = MODEL == NET_MODEL_KS;
     static constexpr int X = SPLIT ? 2 : L3Shape<T, P>::X;
     static constexpr int TY = SPLIT ? 2 : L3Shape<T, P>::TY;
     static constexpr int UPW = SPLIT ? 16 : 32;      // blocks of X x TY outputs per consumer warp
 };
+
+// Field-split kernel: extra columns of the staged box that make the shared-memory row pitch
+// continue the bank sequence where a thread-row ends, so that a half-warp (fp32, LDS.64) or
+// quarter-warp (fp64, LDS.128) of consecutive blocks that straddles two thread-rows still covers
+// 128 consecutive bytes modulo 128 (the ncu capture of the unpadded kernel: 40 % of the
+// shared-memory wavefronts of cfg 3a were such conflicts).  -1: no pitch does it for this width.
+template <class T> inline int l3s_pad(int TXt, int HX, int TY) {
+    const int q = 16 / (int)sizeof(T);                     // scalars per 16 bytes (TMA inner-box granule)
+    for (int pad = 0; pad * (int)sizeof(T) < 128; pad += q)
+        if (((TY * (TXt + 2 * HX + pad) - TXt) * (int)sizeof(T)) % 128 == 0) return pad;
+    return -1;
+}
 
 typedef CUresult (*l3_encode_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
@@ -60,17 +73,18 @@ inline int32_t l3_encode(net* h, CUtensorMap* tm, void* base, int esz, uint64_t 
     return NET_OK;
 }
 
-// 4D map over two planes of 8-byte elements: extents (ex, ey, ez, 2), box (bx, by, 1, 2)
-inline int32_t l3_encode_planes(net* h, CUtensorMap* tm, void* base, uint64_t ex, uint64_t ey, uint64_t ez,
+// 4D map over two planes of `esz`-byte elements: extents (ex, ey, ez, 2), box (bx, by, 1, 2)
+inline int32_t l3_encode_planes(net* h, CUtensorMap* tm, void* base, int esz, uint64_t ex, uint64_t ey, uint64_t ez,
                                 uint32_t bx, uint32_t by) {
     l3_encode_fn encode;
     int32_t rc = l3_encoder(h, &encode);
     if (rc) return rc;
     cuuint64_t dims[4] = {ex, ey, ez, 2};
-    cuuint64_t strides[3] = {ex * 8, ex * ey * 8, ex * ey * ez * 8};
+    const uint64_t e8 = (uint64_t)esz;
+    cuuint64_t strides[3] = {ex * e8, ex * ey * e8, ex * ey * ez * e8};
     cuuint32_t box[4] = {bx, by, 1, 2};
     cuuint32_t estr[4] = {1, 1, 1, 1};
-    CUresult r = encode(tm, CU_TENSOR_MAP_DATA_TYPE_UINT64, 4, base, dims, strides, box, estr,
+    CUresult r = encode(tm, esz == 4 ? CU_TENSOR_MAP_DATA_TYPE_UINT32 : CU_TENSOR_MAP_DATA_TYPE_UINT64, 4, base, dims, strides, box, estr,
                         CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
                         CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) return set_err(h, NET_ERR_CUDA, "cuTensorMapEncodeTiled (planes) failed (%d)", (int)r);
@@ -81,8 +95,9 @@ template <class T, int MODEL, int P, int STAGE>
 static auto l3_kernel_ptr() {
     typedef L3Sh<T, MODEL, P> S;
     if constexpr (S::SPLIT) {
-        static const bool rot = getenv("OSCNET_L3S_ROT") ? atoi(getenv("OSCNET_L3S_ROT")) != 0 : (P > 2);
-        return rot ? lat3s_kernel<T, P, STAGE, L3_MAXT, L3_MINB, true> : lat3s_kernel<T, P, STAGE, L3_MAXT, L3_MINB, false>;
+        // fp64, P = 4: rotating accumulators (small code, no spills); fp32: compile-time phases
+        // measured faster (cfg 3a 2.26e10 vs 1.97e10)
+        return lat3s_kernel<T, P, STAGE, L3_MAXT, L3_MINB, (P > 2 && sizeof(T) == 8)>;
     } else {
         return lat3_kernel<T, MODEL, P, STAGE, S::X, S::TY, L3_MAXT, L3_MINB, (P > 2 && sizeof(T) == 4)>;
     }
@@ -124,10 +139,10 @@ static int32_t l3_enumerate(int nx, int ny, int want_tx, int want_sy, F&& f) {
             // the wavefronts of cfg 5 were such conflicts).  Phases never straddle strips when QX
             // is a multiple of 8.  fp64 planes: the rule that held on cfg 3b is simply >= 16
             // threads per staged row.
-            constexpr bool PLANAR = KS && sizeof(T) == 8;
-            const int row_bytes = (TXt + 2 * HX) * (PLANAR ? 8 : 2 * (int)sizeof(T));
+            constexpr bool PLANAR = S::SPLIT;
+            const int row_bytes = (TXt + 2 * HX) * (PLANAR ? (int)sizeof(T) : 2 * (int)sizeof(T));
             const bool straddle = QX % 8 != 0 && SY > 1;
-            const double bank_pen = PLANAR ? (QX % 8 != 0 ? 0.85 : 1.0)
+            const double bank_pen = PLANAR ? (QX % (sizeof(T) == 8 ? 8 : 16) != 0 && l3s_pad<T>(TXt, HX, TY) < 0 ? 0.85 : 1.0)
                                            : ((straddle && (TY * row_bytes) % 128 == 0) ? 0.85 : 1.0);
             f(TXt, SY, lane_eff * cover * size_pen * bank_pen / (1.0 + 0.25 * (halo - 1.0)));
         }
@@ -168,6 +183,10 @@ static int32_t l3_configure_stage(net* h) {
     if (rc_enum) return rc_enum;
     if (best < 0) return NET_ERR_UNSUPPORTED;
     g.PW = g.TXt + 2 * HX;
+    if (S::SPLIT && g.QX % (sizeof(T) == 8 ? 8 : 16) != 0 && !getenv("OSCNET_L3S_NOPAD")) {
+        const int pad = l3s_pad<T>(g.TXt, HX, TY);
+        if (pad > 0 && (g.PW + pad) * U8 <= 256) g.PW += pad;
+    }
     g.PH = g.TYt + 2 * P;
     g.ncw = (g.QX * g.SY + S::UPW - 1) / S::UPW;
     g.st_bytes = (unsigned)((size_t)g.PW * g.PH * 2 * sizeof(T));
@@ -234,10 +253,10 @@ static int32_t l3_configure_tile(net* h) {
     const uint64_t nxp = (uint64_t)g.nx + 2 * HX, nyp = (uint64_t)g.ny + 2 * P;
     void* st_src[4] = {h->b.y, h->b.Y2, h->b.Y3, h->b.Y4};
     if (KS) { st_src[0] = h->E_a; st_src[1] = h->E_b; }
-    constexpr bool PLANAR = KS && sizeof(T) == 8;     // (cos | sin) planes instead of pairs (lat3_kernel.cuh)
+    constexpr bool PLANAR = L3Sh<T, MODEL, P>::SPLIT;   // (cos | sin) planes instead of pairs (lat3s_kernel.cuh)
     for (int st = 0; st < 5; ++st) h->lat3[st].plane = (long long)(nxp * nyp * (uint64_t)g.nz);
     for (int k = 0; k < (KS ? 2 : 4); ++k) {
-        if (PLANAR) rc = l3_encode_planes(h, &h->tm3_st[k], st_src[k], nxp, nyp, (uint64_t)g.nz, (uint32_t)g.PW, (uint32_t)g.PH);
+        if (PLANAR) rc = l3_encode_planes(h, &h->tm3_st[k], st_src[k], (int)sizeof(T), nxp, nyp, (uint64_t)g.nz, (uint32_t)g.PW, (uint32_t)g.PH);
         else rc = l3_encode(h, &h->tm3_st[k], st_src[k], 8, nxp * U8, nyp, (uint64_t)g.nz, (uint32_t)(g.PW * U8), (uint32_t)g.PH);
         if (rc) return rc;
     }

@@ -1,5 +1,5 @@
-// Field-split variant of the third-generation 3D lattice kernel for fp64 Kuramoto-Sakaguchi
-// lattices (config 3b).
+// Field-split variant of the third-generation 3D lattice kernel for Kuramoto-Sakaguchi lattices
+// (configs 3a and 3b).
 //
 // Same mathematics and the same producer / mbarrier pipeline as lat3_kernel.cuh (x-run
 // decomposition of the ball of PAPER.md:313, z-marching register accumulators, factorised sine
@@ -14,6 +14,11 @@
 // registers now cover 2 x 2 outputs of one field, the staged rows are shared by two output rows
 // (25 LDS.128 and 114 DADD per output), and the two partial results meet once per finished plane
 // through a warp shuffle; lane f then finishes output row f of the block.
+// fp32 (cfg 3a): the same split halves the registers a thread needs for its accumulators (the two
+// x-adjacent columns of one field form the packed f32x2 operand instead of the (cos, sin) pair), so
+// twice as many warps are resident -- that kernel was bound by dependent-issue latency at 12 warps
+// per SM, not by a pipe (add.f32x2 moves as many lanes per clock as add.f32: measured 64 vs 128
+// thread-instructions per clock and SM).
 #pragma once
 #include "lat3_kernel.cuh"
 
@@ -24,7 +29,8 @@ __global__ void __launch_bounds__(MAXT, MINB)
 lat3s_kernel(const __grid_constant__ CUtensorMap tm_st, const __grid_constant__ CUtensorMap tm_op0,
              const __grid_constant__ CUtensorMap tm_op1, const __grid_constant__ CUtensorMap tm_op2,
              const __grid_constant__ CUtensorMap tm_op3, L3Ptrs a, L3Params<T> mp, L3Geom g) {
-    static_assert(sizeof(T) == 8, "field-split kernel: fp64 planes");
+    typedef typename PairOf<T>::type Pr;      // the two x-adjacent columns of a thread, one field
+    static_assert(P % 2 == 0, "column pairs of even shifts are aligned register pairs");
     constexpr int MODEL = NET_MODEL_KS;
     constexpr int X = 2, TY = 2;
     constexpr int HX = l2_hx<T>(P);           // x ghost width of the padded planes
@@ -32,7 +38,7 @@ lat3s_kernel(const __grid_constant__ CUtensorMap tm_st, const __grid_constant__ 
     constexpr int NCOL = X + 2 * P;           // scalars a thread reads per staged row
     constexpr int NACC = 2 * P + 1;
     constexpr int NT = L3Ops<MODEL, STAGE>::N;
-    static_assert(OFF % 2 == 0 && NCOL % 2 == 0, "16-byte row pieces");
+    static_assert(OFF % 2 == 0 && NCOL % 2 == 0, "aligned column pairs");
 
     extern __shared__ __align__(128) unsigned char l3_smem[];
     const int D = g.D, NB = D + 1, NS = P + 1 + D;
@@ -102,13 +108,11 @@ lat3s_kernel(const __grid_constant__ CUtensorMap tm_st, const __grid_constant__ 
     const int gxs = x < HX ? nx : (x >= nx - HX ? -nx : 0);   // periodic image this thread also writes
     const int splane = PW * g.PH;                             // scalars between the staged cos and sin boxes
 
-    T acc[NACC][TY][X];
+    Pr acc[NACC][TY];
 #pragma unroll
     for (int k = 0; k < NACC; ++k)
 #pragma unroll
-        for (int r = 0; r < TY; ++r)
-#pragma unroll
-            for (int i = 0; i < X; ++i) acc[k][r][i] = T(0);
+        for (int r = 0; r < TY; ++r) acc[k][r] = Pr{T(0), T(0)};
 
     int slot = 0, cslot = NS - P, b = 0;      // ring slots of planes i and i - P; barrier index
     unsigned phase = 0;
@@ -119,7 +123,7 @@ lat3s_kernel(const __grid_constant__ CUtensorMap tm_st, const __grid_constant__ 
         mbar_wait(full + b, phase);
         if (owner) {
             const T* sb = reinterpret_cast<const T*>(st_ring + (size_t)slot * g.st_stride) + f * splane + (st * TY) * PW + q * X + OFF;
-            T A[P > 1 ? P - 1 : 1][TY][X];
+            Pr A[P > 1 ? P - 1 : 1][TY];
             bool Aset[P > 1 ? P - 1 : 1][TY];
 #pragma unroll
             for (int k = 0; k < (P > 1 ? P - 1 : 1); ++k)
@@ -129,68 +133,60 @@ lat3s_kernel(const __grid_constant__ CUtensorMap tm_st, const __grid_constant__ 
             for (int rr = 0; rr < TY + 2 * P; ++rr) {           // staged row rr <-> y = yrow0 - P + rr
                 const int dist = rr < P ? P - rr : (rr >= TY + P ? rr - (TY + P - 1) : 0);
                 const int wmax = l2_run_w(P, 0, dist);
-                T v[NCOL];
-                const T* row = sb + rr * PW;
+                Pr v[NCOL / 2];                                  // v[c] = columns (2c, 2c + 1) of the row piece
+                const Pr* row = reinterpret_cast<const Pr*>(sb + rr * PW);
 #pragma unroll
                 for (int c = 0; c < NCOL / 2; ++c) {
                     if (2 * c + 1 < P - wmax || 2 * c > P + X - 1 + wmax) continue;     // columns no run of this row reaches
-                    const double2 w2 = *reinterpret_cast<const double2*>(row + 2 * c);
-                    v[2 * c] = w2.x; v[2 * c + 1] = w2.y;
+                    v[c] = row[c];
                 }
-                T R[P + 1][X];
+                auto col = [&](int j) -> T { return (j & 1) ? v[j / 2].y : v[j / 2].x; };
+                Pr R[P + 1];
+                R[0] = v[P / 2];
 #pragma unroll
-                for (int e = 0; e < X; ++e) {
-                    R[0][e] = v[P + e];
-#pragma unroll
-                    for (int w = 1; w <= P; ++w)
-                        if (w <= wmax) R[w][e] = R[w - 1][e] + (v[P + e - w] + v[P + e + w]);
-                }
+                for (int w = 1; w <= P; ++w)
+                    if (w <= wmax) {
+                        Pr side;
+                        if (w % 2 == 0) side = padd(v[(P - w) / 2], v[(P + w) / 2]);
+                        else side = Pr{col(P - w) + col(P + w), col(P + 1 - w) + col(P + 1 + w)};
+                        R[w] = padd(R[w - 1], side);
+                    }
 #pragma unroll
                 for (int r = 0; r < TY; ++r) {
                     const int ady = rr - P - r < 0 ? -(rr - P - r) : rr - P - r;
                     if (ady > P) continue;
                     {   // |dz| = 0: straight into the accumulator of output plane i
                         const int w = l2_run_w(P, 0, ady);
-#pragma unroll
-                        for (int e = 0; e < X; ++e) acc[(J + P) % NACC][r][e] += R[w][e];
+                        acc[(J + P) % NACC][r] = padd(acc[(J + P) % NACC][r], R[w]);
                     }
 #pragma unroll
                     for (int k = 1; k < P; ++k) {    // 0 < |dz| < P: in-plane partial sums
                         const int w = l2_run_w(P, k, ady);
                         if (w >= 0) {
-#pragma unroll
-                            for (int e = 0; e < X; ++e)
-                                A[k - 1][r][e] = Aset[k - 1][r] ? A[k - 1][r][e] + R[w][e] : R[w][e];
+                            A[k - 1][r] = Aset[k - 1][r] ? padd(A[k - 1][r], R[w]) : R[w];
                             Aset[k - 1][r] = true;
                         }
                     }
                     if (ady == 0) {                  // |dz| = P: the centre alone (first / last contribution)
-#pragma unroll
-                        for (int e = 0; e < X; ++e) {
-                            acc[(J + 2 * P) % NACC][r][e] = R[0][e];
-                            acc[J % NACC][r][e] += R[0][e];
-                        }
+                        acc[(J + 2 * P) % NACC][r] = R[0];
+                        acc[J % NACC][r] = padd(acc[J % NACC][r], R[0]);
                     }
                 }
             }
 #pragma unroll
             for (int k = 1; k < P; ++k)
 #pragma unroll
-                for (int r = 0; r < TY; ++r)
-#pragma unroll
-                    for (int e = 0; e < X; ++e) {
-                        acc[(J + P - k) % NACC][r][e] += A[k - 1][r][e];
-                        acc[(J + P + k) % NACC][r][e] += A[k - 1][r][e];
-                    }
+                for (int r = 0; r < TY; ++r) {
+                    acc[(J + P - k) % NACC][r] = padd(acc[(J + P - k) % NACC][r], A[k - 1][r]);
+                    acc[(J + P + k) % NACC][r] = padd(acc[(J + P + k) % NACC][r], A[k - 1][r]);
+                }
         }
         // ---- finish output plane zo (accumulator J): lane f takes output row f of the block
         if (zo >= z0) {                                   // uniform over the CTA
-            T other[X];
-#pragma unroll
-            for (int e = 0; e < X; ++e) {
-                const T send = f ? acc[J % NACC][0][e] : acc[J % NACC][1][e];    // the row the partner finishes
-                other[e] = __shfl_xor_sync(0xffffffffu, send, 16);
-            }
+            const Pr send = f ? acc[J % NACC][0] : acc[J % NACC][1];    // the row the partner finishes
+            const T other[X] = {__shfl_xor_sync(0xffffffffu, send.x, 16), __shfl_xor_sync(0xffffffffu, send.y, 16)};
+            const Pr ownp = f ? acc[J % NACC][1] : acc[J % NACC][0];
+            const T ownv[X] = {ownp.x, ownp.y};
             const int r = f;
             const int yy = yrow0 + r;
             if (owner && yy < ny) {
@@ -211,7 +207,7 @@ lat3s_kernel(const __grid_constant__ CUtensorMap tm_st, const __grid_constant__ 
                 T ov[X], zv[X], cv[X], sv[X];
 #pragma unroll
                 for (int e = 0; e < X; ++e) {
-                    const T own = f ? acc[J % NACC][1][e] : acc[J % NACC][0][e];
+                    const T own = ownv[e];
                     T C = f ? other[e] : own, S = f ? own : other[e];
                     if (!mp.include_self) { C -= cx[e]; S -= cy[e]; }
                     const T cia = cx[e] * mp.ca - cy[e] * mp.sa;      // cos(phi_i + alpha)
@@ -255,9 +251,7 @@ lat3s_kernel(const __grid_constant__ CUtensorMap tm_st, const __grid_constant__ 
 #pragma unroll
             for (int k = 0; k + 1 < NACC; ++k)
 #pragma unroll
-                for (int r = 0; r < TY; ++r)
-#pragma unroll
-                    for (int e = 0; e < X; ++e) acc[k][r][e] = acc[k + 1][r][e];
+                for (int r = 0; r < TY; ++r) acc[k][r] = acc[k + 1][r];
         }
     } else {
         for (int base = 0; base < nplanes; base += NACC)
