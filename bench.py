@@ -28,9 +28,14 @@ if ROOT not in sys.path:
 
 METRIC = "oscillator-steps/s"
 HEADLINE = "5"
-PER_CONFIG = ("1", "2", "3a", "3b", "4", "5")
+PER_CONFIG = ("1", "1b", "2", "3a", "3b", "4", "5")   # 1b: config 1 as a batch of nets (extra, SURVEY.md 8(d) iii)
 # RK4 steps per bench step (= per net_integrate call)
-BENCH_RK4 = {"1": 1000, "2": 200, "3a": 10, "3b": 10, "4": 100, "5": 10}
+BENCH_RK4 = {"1": 1000, "1b": 1000, "2": 200, "3a": 10, "3b": 10, "4": 100, "5": 10}
+
+
+def ntot(w):
+    """Elements of all replicas of the workload (batch > 1: independent nets integrated together)."""
+    return w.n * getattr(w, "batch", 1)
 
 
 # ------------------------------------------------------------------ inputs
@@ -42,16 +47,16 @@ def make_inputs(w, seed=1):
     dt = np.float32 if w.dtype == "f32" else np.float64
     elem = None
     if w.model == configs.KS:
-        y0 = inputs.ks_phases(w.n, seed).reshape(1, -1)
+        y0 = inputs.ks_phases(ntot(w), seed).reshape(1, -1)
         if w.extra.get("omega") == "lorentzian":
-            elem = inputs.lorentzian_omega(w.n, seed, w.extra["gamma"], w.extra["omega_max"])
+            elem = inputs.lorentzian_omega(ntot(w), seed, w.extra["gamma"], w.extra["omega_max"])
     elif w.model == configs.FHN:
-        y0 = inputs.fhn_circle(w.n, seed)
+        y0 = inputs.fhn_circle(ntot(w), seed)
     else:
-        V = inputs.hh_voltage(w.n, seed)
-        y0 = np.zeros((4, w.n))
+        V = inputs.hh_voltage(ntot(w), seed)
+        y0 = np.zeros((4, ntot(w)))
         y0[0] = V
-        elem = inputs.hh_current(w.n, seed)
+        elem = inputs.hh_current(ntot(w), seed)
     return np.ascontiguousarray(y0.astype(dt)), None if elem is None else elem.astype(dt)
 
 
@@ -203,11 +208,11 @@ def roofline_object(w, m, steps):
     sec = m["ms"] * 1e-3
     avg_launch_s = sec / max(1, m["launches"])
     if c["bound"] == "hbm":
-        per_launch = R.bytes_per_osc_step(w) * w.n * rk4 / max(1, m["launches"])
+        per_launch = R.bytes_per_osc_step(w) * ntot(w) * rk4 / max(1, m["launches"])
         achieved, peak, unit = per_launch / avg_launch_s / 1e9, pk["hbm_gbs"], "GB/s"
         peak_src = "MEASURED_PEAKS.json hbm_gbs" if pk["hbm_source"] == "measured" else "guide fallback"
     else:
-        per_launch = c["ops"] * w.n * rk4 / max(1, m["launches"])
+        per_launch = c["ops"] * ntot(w) * rk4 / max(1, m["launches"])
         achieved, peak, unit = per_launch / avg_launch_s / 1e9, pk[c["pipe"] + "_ginstr_s"], "Ginstr/s"
         peak_src = "148 SM x %d lanes x sm_max_mhz (%s pipe)" % (R.LANES[c["pipe"]], c["pipe"])
     return {"bound": c["bound"], "achieved": achieved, "peak": peak, "unit": unit,
@@ -218,7 +223,7 @@ def roofline_object(w, m, steps):
             "bytes_per_osc_step": R.bytes_per_osc_step(w),
             "survey_bytes_per_osc_step": R.survey_bytes_per_osc_step(w),
             "ceiling_osc_steps_per_s": c["osc_steps_per_s"],
-            "frac_of_ceiling": (w.n * rk4 / sec) / c["osc_steps_per_s"]}
+            "frac_of_ceiling": (ntot(w) * rk4 / sec) / c["osc_steps_per_s"]}
 
 
 # ------------------------------------------------------------------ CPU oracle arm
@@ -309,13 +314,13 @@ def line_for(w, m, steps, n_gpus, units_total=None, ms_max=None):
     """The JSON fields of one measured workload (headline or per_config entry)."""
     rk4 = steps * m["rk4_per_step"]
     ms = m["ms"] if ms_max is None else ms_max
-    units = w.n * rk4 * n_gpus if units_total is None else units_total
+    units = ntot(w) * rk4 * n_gpus if units_total is None else units_total
     out = {"workload": w.name, "cfg": w.cfg, "value": units / (ms * 1e-3), "unit": METRIC,
            "ms_per_step": ms / steps, "rk4_steps_per_step": m["rk4_per_step"],
            "dtype": w.dtype, "method": "FAST" if m["method"] == 2 else "DIRECT",
            "gpu_launches": m["launches"], "roofline": roofline_object(w, m, steps)}
     if "e2e_ms" in m:
-        out["e2e"] = {"value": w.n * rk4 * n_gpus / (m["e2e_ms"] * 1e-3), "unit": METRIC,
+        out["e2e"] = {"value": ntot(w) * rk4 * n_gpus / (m["e2e_ms"] * 1e-3), "unit": METRIC,
                       "h2d_bytes_per_step": m["h2d"], "d2h_bytes_per_step": m["d2h"]}
     return out
 
@@ -334,8 +339,8 @@ def run_ours(args):
     w = configs.get(args.config)
     m = measure(w, device, args.steps, args.warmup, e2e=True)
     rk4 = args.steps * m["rk4_per_step"]
-    units, ms_max, value = replicas.aggregate(w.n * rk4, m["ms"], device)
-    _, e2e_ms_max, e2e_value = replicas.aggregate(w.n * rk4, m["e2e_ms"], device)
+    units, ms_max, value = replicas.aggregate(ntot(w) * rk4, m["ms"], device)
+    _, e2e_ms_max, e2e_value = replicas.aggregate(ntot(w) * rk4, m["e2e_ms"], device)
     head = line_for(w, m, args.steps, ws, units, ms_max)
     line = {"metric": METRIC, "value": value, "unit": METRIC, "n_gpus": ws, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms_max / args.steps, "higher_is_better": True,

@@ -55,7 +55,7 @@ enum {
     NET_ERR_SIZE = -2,        /* workspace too small or misaligned (needs 256-byte alignment) */
     NET_ERR_TOPOLOGY = -3,    /* CSR not monotone / index out of range / self-loop where forbidden */
     NET_ERR_CUDA = -4,        /* a CUDA call failed; message holds cudaGetErrorString */
-    NET_ERR_UNSUPPORTED = -5  /* valid request this build does not implement (e.g. batch > 1) */
+    NET_ERR_UNSUPPORTED = -5  /* valid request this build does not implement (e.g. batch > 1 on a lattice) */
 };
 
 enum { NET_MODEL_KS = 0, NET_MODEL_FHN = 1, NET_MODEL_HH = 2 };
@@ -135,8 +135,15 @@ typedef struct {
 typedef struct {
     int32_t model;  /* NET_MODEL_*  */
     int32_t dtype;  /* NET_F32 | NET_F64: storage and arithmetic type of the state */
-    int64_t n;      /* number of elements (64-bit) */
-    int32_t batch;  /* independent replicas of the net; this build supports 1 */
+    int64_t n;      /* number of elements of ONE net (64-bit) */
+    int32_t batch;  /* >= 1: independent replicas of the net integrated together ("a large number of
+                     * network instances simultaneously"), each with its own state and
+                     * per-element parameters.  Every array that is [..][n] for batch = 1 becomes
+                     * [..][batch][n] (replica-major, n contiguous); element ids in net_get_topology
+                     * and the observables run over 0 .. batch*n - 1 (the coupling matrix of the batch
+                     * is block diagonal; global observables are ensemble values).  batch > 1 is
+                     * built for NET_TOPO_RING; other topologies return NET_ERR_UNSUPPORTED.
+                     * n * batch <= 2^31 - 1. */
     int32_t method; /* NET_METHOD_* */
     net_topology topo;
 } net_desc;

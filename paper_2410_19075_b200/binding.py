@@ -222,18 +222,19 @@ class Net:
     """Owns a workspace tensor and a handle; methods mirror the C ABI."""
 
     def __init__(self, model, dtype, n, topo, params, method=METHOD_AUTO, device="cuda:0",
-                 stream=None):
+                 stream=None, batch=1):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("oscnet needs a CUDA device (no CPU fallback)")
         self.torch = torch
         self.device = torch.device(device)
-        self.model, self.dtype, self.n = model, dtype, int(n)
+        # self.n: elements of all replicas together (arrays are [nvar][batch][n] = [nvar][self.n])
+        self.model, self.dtype, self.n, self.batch = model, dtype, int(n) * int(batch), int(batch)
         self.nvar = NVAR[model]
         self.np_dtype = _np_dtype(dtype)
         self.torch_dtype = torch.float32 if dtype == F32 else torch.float64
         d = Desc()
-        d.model, d.dtype, d.n, d.batch, d.method = model, dtype, self.n, 1, method
+        d.model, d.dtype, d.n, d.batch, d.method = model, dtype, int(n), int(batch), method
         t = d.topo
         t.kind = topo["kind"]
         ext = list(topo.get("extent", ())) + [1, 1, 1]
@@ -281,7 +282,7 @@ class Net:
         else:
             topo = dict(kind=TOPO_RANDOM_INDEGREE, in_degree=w.in_degree, seed=w.topo_seed)
         return cls(w.model, dtype, w.n, topo, w.params, method=method, device=device,
-                   stream=stream)
+                   stream=stream, batch=getattr(w, "batch", 1))
 
     def close(self):
         if getattr(self, "h", None):

@@ -28,6 +28,7 @@ class Workload:
     radius: int = 0                 # ring: P neighbours each side; lattice: Euclidean radius
     in_degree: int = 0              # RANDOM_INDEGREE
     topo_seed: int = 1
+    batch: int = 1                  # independent replicas integrated together (rings)
     extra: dict = field(default_factory=dict)
 
     @property
@@ -41,8 +42,14 @@ _HH = dict(gNa=120.0, gK=36.0, gL=0.3, ENa=50.0, EK=-77.0, EL=-54.4, C=1.0,
            g_syn=0.1, E_syn=0.0, theta_syn=0.0, k_syn=2.0)
 
 
-def get(cfg, n=None, n1=None):
+def get(cfg, n=None, n1=None, batch=None):
     cfg = str(cfg)
+    if cfg == "1b":
+        # extra, not a BASELINE.json config (SURVEY.md 8(d) iii): config 1 as a batch of independent
+        # rings, one per CTA, 8 per SM -- where the FP64 pipe, not the latency of one tiny net, binds
+        batch = batch or 148 * 8
+        w = get("1", n=n)
+        return replace(w, cfg="1b", name="KS ring N=%d P=64 f64 x %d independent nets" % (w.n, batch), batch=batch)
     if cfg == "1":
         n = n or 256
         return Workload("1", "KS ring N=%d P=64 f64" % n, KS, RING, n, "f64", 0.025, 1000, 1,

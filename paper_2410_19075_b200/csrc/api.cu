@@ -33,7 +33,10 @@ static int32_t validate(net* h, const net_desc* d) {
     if (model_nvar(d->model) < 0) return set_err(h, NET_ERR_INVALID, "unknown model %d", d->model);
     if (d->dtype != NET_F32 && d->dtype != NET_F64) return set_err(h, NET_ERR_INVALID, "unknown dtype %d", d->dtype);
     if (d->n < 1 || d->n > 2147483647LL) return set_err(h, NET_ERR_INVALID, "n = %lld outside [1, 2^31-1] (col_idx is int32)", (long long)d->n);
-    if (d->batch != 1) return set_err(h, d->batch < 1 ? NET_ERR_INVALID : NET_ERR_UNSUPPORTED, "batch = %d: this build supports batch = 1", d->batch);
+    if (d->batch < 1) return set_err(h, NET_ERR_INVALID, "batch = %d < 1", d->batch);
+    if (d->batch > 1 && d->topo.kind != NET_TOPO_RING)
+        return set_err(h, NET_ERR_UNSUPPORTED, "batch = %d: this build batches ring nets only", d->batch);
+    if (d->n * (int64_t)d->batch > 2147483647LL) return set_err(h, NET_ERR_INVALID, "n * batch exceeds 2^31-1");
     if (d->method < NET_METHOD_AUTO || d->method > NET_METHOD_FAST) return set_err(h, NET_ERR_INVALID, "unknown method %d", d->method);
     const net_topology& t = d->topo;
     switch (t.kind) {
@@ -64,6 +67,18 @@ static int32_t validate(net* h, const net_desc* d) {
             break;
         default: return set_err(h, NET_ERR_INVALID, "unknown topology kind %d", t.kind);
     }
+    return NET_OK;
+}
+
+// Inside the library a batch of B independent rings of N elements ("a large number
+// of network instances simultaneously") is ONE net of B*N elements whose coupling
+// matrix is block diagonal: desc.n becomes the total, the ring period is desc.n / desc.batch, and
+// the state layout SoA [nvar][batch][N] is the SoA [nvar][B*N] every kernel already uses.
+static int32_t normalise(const net_desc* in, net_desc* out) {
+    int32_t rc = validate(nullptr, in);
+    if (rc) return rc;
+    *out = *in;
+    out->n = in->n * (int64_t)in->batch;
     return NET_OK;
 }
 
@@ -282,18 +297,21 @@ const char* net_last_error(const net_t* h) { return h ? h->err : g_err; }
 
 int32_t net_workspace_bytes(const net_desc* desc, size_t* bytes) {
     if (!bytes) return set_err(nullptr, NET_ERR_INVALID, "bytes is NULL");
-    int32_t rc = validate(nullptr, desc);
+    net_desc nd;
+    int32_t rc = normalise(desc, &nd);
     if (rc) return rc;
-    *bytes = make_layout(desc, nullptr).total;
+    *bytes = make_layout(&nd, nullptr).total;
     return NET_OK;
 }
 
-int32_t net_create(const net_desc* desc, const void* params, size_t params_bytes, void* d_workspace,
+int32_t net_create(const net_desc* user_desc, const void* params, size_t params_bytes, void* d_workspace,
                    size_t workspace_bytes, void* cuda_stream, net_t** out) {
     if (!out) return set_err(nullptr, NET_ERR_INVALID, "out is NULL");
     *out = nullptr;
-    int32_t rc = validate(nullptr, desc);
+    net_desc nd;
+    int32_t rc = normalise(user_desc, &nd);
     if (rc) return rc;
+    const net_desc* desc = &nd;                 // n = total elements of the batch from here on
     size_t want = desc->model == NET_MODEL_KS ? sizeof(net_ks_params)
                 : desc->model == NET_MODEL_FHN ? sizeof(net_fhn_params) : sizeof(net_hh_params);
     if (!params || params_bytes != want)

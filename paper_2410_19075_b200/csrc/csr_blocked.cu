@@ -67,10 +67,64 @@ __device__ __forceinline__ float cb_lds(unsigned addr, float) {
 // One thread per (padded) row walks its sorted entries once: the first CB_SLOTS sources of every
 // column block go to the slot word of (chunk, block, row), the rest are counted (FILL = false)
 // or written to the row's overflow list (FILL = true).  flag[4] != 0: rows not sorted by column.
+// Slot order (FILL = false).  The stage kernel reads slot k of NBK consecutive rows with one
+// shared-memory wavefront if their addresses fall into different banks (NBK = 128 bytes / element:
+// the 16 lanes of a half-warp for fp64, the 32 lanes of a warp for fp32); random sources made
+// 52 % of the wavefronts of config 4 bank conflicts (profiles/r01_final_ncu.md).  Which of the
+// four slots of a word holds which source is free, and so is the bank of the zero an unused slot
+// points at (NBK zeros follow the s block), so the rows of a group are placed one after the
+// other, each taking the permutation of its sources that collides least with the rows before it.
+__device__ const unsigned char CB_PERM[24][4] = {
+    {0, 1, 2, 3}, {0, 1, 3, 2}, {0, 2, 1, 3}, {0, 2, 3, 1}, {0, 3, 1, 2}, {0, 3, 2, 1}, {1, 0, 2, 3}, {1, 0, 3, 2},
+    {1, 2, 0, 3}, {1, 2, 3, 0}, {1, 3, 0, 2}, {1, 3, 2, 0}, {2, 0, 1, 3}, {2, 0, 3, 1}, {2, 1, 0, 3}, {2, 1, 3, 0},
+    {2, 3, 0, 1}, {2, 3, 1, 0}, {3, 0, 1, 2}, {3, 0, 2, 1}, {3, 1, 0, 2}, {3, 1, 2, 0}, {3, 2, 0, 1}, {3, 2, 1, 0}};
+
+__device__ __forceinline__ void cb_place_slots(unsigned (&s)[CB_SLOTS], int n, unsigned W, int nbk, bool arrange) {
+    if (!arrange) return;
+    const int lane = threadIdx.x & 31, gbase = lane / nbk * nbk;
+    const unsigned all = nbk == 32 ? 0xffffffffu : (1u << nbk) - 1u;
+    unsigned mask[CB_SLOTS] = {0u, 0u, 0u, 0u};      // banks taken at slot position k by the rows placed so far
+    int zb[CB_SLOTS] = {-1, -1, -1, -1};             // bank of the zero the unused slots at position k read
+    unsigned out[CB_SLOTS] = {s[0], s[1], s[2], s[3]};
+    for (int j = 0; j < nbk; ++j) {
+        if (lane - gbase == j) {
+            int best = 0, bestc = 1 << 30;
+            for (int p = 0; p < 24; ++p) {
+                int cst = 0;
+                for (int e = 0; e < n; ++e) cst += (int)((mask[CB_PERM[p][e]] >> (s[e] % (unsigned)nbk)) & 1u);
+                if (cst < bestc) { bestc = cst; best = p; }
+            }
+            bool used[CB_SLOTS] = {false, false, false, false};
+            for (int e = 0; e < n; ++e) {
+                const int pos = CB_PERM[best][e];
+                out[pos] = s[e]; used[pos] = true;
+                mask[pos] |= 1u << (s[e] % (unsigned)nbk);
+            }
+            for (int pos = 0; pos < CB_SLOTS; ++pos)
+                if (!used[pos]) {
+                    if (zb[pos] < 0) {
+                        const unsigned fr = ~mask[pos] & all;
+                        zb[pos] = fr ? __ffs((int)fr) - 1 : 0;
+                        mask[pos] |= 1u << zb[pos];
+                    }
+                    out[pos] = W + (unsigned)zb[pos];
+                }
+        }
+#pragma unroll
+        for (int k = 0; k < CB_SLOTS; ++k) {
+            mask[k] = __shfl_sync(0xffffffffu, mask[k], gbase + j);
+            zb[k] = __shfl_sync(0xffffffffu, zb[k], gbase + j);
+        }
+    }
+#pragma unroll
+    for (int k = 0; k < CB_SLOTS; ++k) s[k] = out[k];
+}
+
 template <bool FILL>
 __global__ void cb_build_kernel(CbGeom g, const int64_t* __restrict__ row_ptr, const int32_t* __restrict__ col_idx,
                                 int32_t ku, uint2* slots, int32_t* ovf_cnt, const int32_t* __restrict__ ovf_ptr,
-                                int32_t* ovf_idx, int64_t ovf_cap, int32_t* flag) {
+                                int32_t* ovf_idx, int64_t ovf_cap, int32_t* flag, int nbk) {
+    // whole warps walk the loops together: rows are padded to multiples of 32 per chunk
     for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < (int64_t)g.nchunks * g.CR;
          i += (int64_t)gridDim.x * blockDim.x) {
         const int c = (int)(i / g.CR), l = (int)(i % g.CR);      // chunks are contiguous ranges of CR rows
@@ -99,7 +153,11 @@ __global__ void cb_build_kernel(CbGeom g, const int64_t* __restrict__ row_ptr, c
                 }
                 ++cnt;
             }
-            if (!FILL) slots[((int64_t)c * g.B + b) * g.CR + l] = make_uint2(s[0] | s[1] << 16, s[2] | s[3] << 16);
+            if (!FILL) {
+                __syncwarp();
+                cb_place_slots(s, cnt < CB_SLOTS ? cnt : CB_SLOTS, (unsigned)g.W, nbk, nbk > 0);
+                slots[((int64_t)c * g.B + b) * g.CR + l] = make_uint2(s[0] | s[1] << 16, s[2] | s[3] << 16);
+            }
         }
         if (q != e0) atomicExch(flag + 4, 2);
         if (!FILL) ovf_cnt[i] = (int32_t)(nov > 0x7fffffff ? 0x7fffffff : nov);
@@ -178,8 +236,8 @@ csr_blocked_stage_kernel(StageArgs a, ModelParams mp, TopoView tv, CbGeom g) {
     if (t == 0) {
         mbar_init(&bar, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-        sblk[g.W] = T(0);
     }
+    if (t < 128 / (int)sizeof(T)) sblk[g.W + t] = T(0);          // one zero per bank for the unused slots
     __syncthreads();
     unsigned phase = 0;
     for (int c = blockIdx.x; c < g.nchunks; c += gridDim.x) {
@@ -261,15 +319,15 @@ static bool cb_geometry(const net_desc* d, CbGeom* g) {
     if (want_cr > 0) CR = round_up(want_cr, 32);
     if (CR > CB_MMAX * CB_THREADS) CR = CB_MMAX * CB_THREADS;
     const int64_t nchunks = (n + CR - 1) / CR;
-    int W = (int)(CB_SMEM_BUDGET / es) - 16;
-    if (W > 65520) W = 65520;                             // W itself is the index of the zero slot
+    int W = (int)(CB_SMEM_BUDGET / es) - 32;
+    if (W > 65488) W = 65488;                             // W .. W + 31 are the indices of the zero slots
     int B = (int)((n + W - 1) / W);
     const double mean_deg = (double)cb_nnz(d) / (double)n;
     const int B_fill = (int)(mean_deg / 2.2 + 0.999);     // blocks that bring the mean per slot word to 2.2
     if (B_fill > B) B = B_fill;
     if (B > n / 16) B = (int)(n / 16 > 0 ? n / 16 : 1);
     W = (int)round_up((n + B - 1) / B, 16);               // equal blocks, 16-element granules
-    if (want_w > 0) W = (int)round_up(want_w < 16 ? 16 : (want_w > 65520 ? 65520 : want_w), 16);
+    if (want_w > 0) W = (int)round_up(want_w < 16 ? 16 : (want_w > 65488 ? 65488 : want_w), 16);
     B = (int)((n + W - 1) / W);
     if (nchunks * B > (int64_t)1 << 24) return false;
     memset(g, 0, sizeof(*g));
@@ -338,16 +396,17 @@ int32_t csr_blocked_prepare(net* h) {
     const unsigned grid = (unsigned)((rows + 255) / 256 > 148 * 16 ? 148 * 16 : (rows + 255) / 256);
     const int32_t ku = h->tv.k_uniform;
     OSC_CUDA(h, cudaMemsetAsync(h->b.flag + 4, 0, 2 * sizeof(int32_t), st));   // flag[4]: verdict, flag[5]: overflow entries
-    cb_build_kernel<false><<<grid, 256, 0, st>>>(g, h->tv.row_ptr, h->tv.col_idx, ku, slots, ovf_cnt, nullptr, nullptr, 0, h->b.flag);
+    const int nbk = getenv("OSCNET_CSRB_NOARRANGE") ? 0 : 128 / (int)h->esize;
+    cb_build_kernel<false><<<grid, 256, 0, st>>>(g, h->tv.row_ptr, h->tv.col_idx, ku, slots, ovf_cnt, nullptr, nullptr, 0, h->b.flag, nbk);
     cb_scan_kernel<<<1, 1024, 0, st>>>(rows, ovf_cnt, ovf_ptr, L.ovf_cap, h->b.flag);
-    cb_build_kernel<true><<<grid, 256, 0, st>>>(g, h->tv.row_ptr, h->tv.col_idx, ku, nullptr, nullptr, ovf_ptr, ovf_idx, L.ovf_cap, h->b.flag);
+    cb_build_kernel<true><<<grid, 256, 0, st>>>(g, h->tv.row_ptr, h->tv.col_idx, ku, nullptr, nullptr, ovf_ptr, ovf_idx, L.ovf_cap, h->b.flag, 0);
     h->launches += 3;
     OSC_CUDA(h, cudaGetLastError());
     int32_t flag[2] = {0, 0};
     OSC_CUDA(h, cudaMemcpyAsync(flag, h->b.flag + 4, sizeof(flag), cudaMemcpyDeviceToHost, st));
     OSC_CUDA(h, cudaStreamSynchronize(st));
     if (flag[0] != 0) return NET_ERR_UNSUPPORTED;
-    const size_t smem = ((size_t)g.W + 16) * h->esize;        // + the zero slot, 128-byte granule
+    const size_t smem = ((size_t)g.W + 32) * h->esize;        // + the zero slots
     if (smem > CB_SMEM_BUDGET + 1024) return NET_ERR_UNSUPPORTED;
     const void* kern = h->desc.dtype == NET_F32 ? cb_kernel_for<float>(g.M) : cb_kernel_for<double>(g.M);
     OSC_CUDA(h, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));

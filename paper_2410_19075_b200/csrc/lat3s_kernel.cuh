@@ -24,7 +24,7 @@
 
 namespace oscnet {
 
-template <class T, int P, int STAGE, int MAXT, int MINB, bool ROT>
+template <class T, int P, int STAGE, int TY, int MAXT, int MINB, bool ROT>
 __global__ void __launch_bounds__(MAXT, MINB)
 lat3s_kernel(const __grid_constant__ CUtensorMap tm_st, const __grid_constant__ CUtensorMap tm_op0,
              const __grid_constant__ CUtensorMap tm_op1, const __grid_constant__ CUtensorMap tm_op2,
@@ -32,7 +32,8 @@ lat3s_kernel(const __grid_constant__ CUtensorMap tm_st, const __grid_constant__ 
     typedef typename PairOf<T>::type Pr;      // the two x-adjacent columns of a thread, one field
     static_assert(P % 2 == 0, "column pairs of even shifts are aligned register pairs");
     constexpr int MODEL = NET_MODEL_KS;
-    constexpr int X = 2, TY = 2;
+    constexpr int X = 2;
+    static_assert(TY % 2 == 0, "the two lanes of a block split its rows");
     constexpr int HX = l2_hx<T>(P);           // x ghost width of the padded planes
     constexpr int OFF = HX - P;
     constexpr int NCOL = X + 2 * P;           // scalars a thread reads per staged row
@@ -181,13 +182,15 @@ lat3s_kernel(const __grid_constant__ CUtensorMap tm_st, const __grid_constant__ 
                     acc[(J + P + k) % NACC][r] = padd(acc[(J + P + k) % NACC][r], A[k - 1][r]);
                 }
         }
-        // ---- finish output plane zo (accumulator J): lane f takes output row f of the block
+        // ---- finish output plane zo (accumulator J): lane f takes the output rows 2m + f of the block
         if (zo >= z0) {                                   // uniform over the CTA
-            const Pr send = f ? acc[J % NACC][0] : acc[J % NACC][1];    // the row the partner finishes
+#pragma unroll
+          for (int m = 0; m < TY / 2; ++m) {              // rows 2m, 2m + 1: lane f finishes row 2m + f
+            const Pr send = f ? acc[J % NACC][2 * m] : acc[J % NACC][2 * m + 1];    // the row the partner finishes
             const T other[X] = {__shfl_xor_sync(0xffffffffu, send.x, 16), __shfl_xor_sync(0xffffffffu, send.y, 16)};
-            const Pr ownp = f ? acc[J % NACC][1] : acc[J % NACC][0];
+            const Pr ownp = f ? acc[J % NACC][2 * m + 1] : acc[J % NACC][2 * m];
             const T ownv[X] = {ownp.x, ownp.y};
-            const int r = f;
+            const int r = 2 * m + f;
             const int yy = yrow0 + r;
             if (owner && yy < ny) {
                 const T* cc = reinterpret_cast<const T*>(st_ring + (size_t)cslot * g.st_stride) + (st * TY + P + r) * PW + q * X + HX;
@@ -235,6 +238,7 @@ lat3s_kernel(const __grid_constant__ CUtensorMap tm_st, const __grid_constant__ 
                     }
                 }
             }
+          }
         }
         // this warp is done with barrier b: stencil plane i - P and operand slot b may be refilled
         __syncwarp();

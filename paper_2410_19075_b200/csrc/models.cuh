@@ -111,12 +111,13 @@ template <int TOPO, class F>
 __device__ __forceinline__ int for_each_neighbor(const TopoView& tv, int64_t n, int64_t i, F&& f) {
     if (TOPO == NET_TOPO_RING) {
         int P = tv.P;
+        const int64_t rn = tv.ring_n, base = i / rn * rn;    // a batch is block diagonal: rings of rn elements
         for (int d = -P; d <= P; ++d) {
             if (d == 0 && !tv.include_self) continue;
-            int64_t j = i + d;
-            if (j < 0) j += n;
-            if (j >= n) j -= n;
-            f(j);
+            int64_t j = i - base + d;
+            if (j < 0) j += rn;
+            if (j >= rn) j -= rn;
+            f(base + j);
         }
         return 2 * P + (tv.include_self ? 1 : 0);
     } else if (TOPO == NET_TOPO_LATTICE) {

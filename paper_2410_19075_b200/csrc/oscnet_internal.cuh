@@ -32,6 +32,7 @@ struct TopoView {
     int32_t include_self;
     int32_t noff;          // lattice: number of offsets (= Omega)
     int32_t k_uniform;     // RANDOM_INDEGREE: in-degree; else 0
+    int64_t ring_n;        // ring: period (elements per ring; n / batch)
     const int32_t* off;    // lattice: noff x (dx,dy,dz), sorted by (dz,dy,dx)
     const int64_t* row_ptr;
     const int32_t* col_idx;

@@ -38,7 +38,7 @@ struct RingArgs {
     void* S[2];              // 2 x [2][npad] prefix buffers (T)
     double* tot[2];          // 2 x [2][RING_GMAX] chunk totals
     unsigned int* bar;       // grid barrier counter (zeroed before the launch)
-    int64_t n, ld, npad;
+    int64_t n, ld, npad;     // n: elements per ring (a batch holds several rings back to back)
     int32_t P, include_self, chunk, G, chunk_shift;
     int64_t n_steps;
     double dt;
@@ -101,11 +101,13 @@ __global__ void __launch_bounds__(RING_THREADS) ring_persistent_kernel(RingArgs 
 
     const int64_t n = a.n, ld = a.ld;
     const int chunk = a.chunk, G = a.G, P = a.P;
-    const int b = blockIdx.x;
+    // single-CTA rings: CTA = one ring of the batch; otherwise CTA = one chunk of the one ring
+    const int b = SINGLE ? 0 : blockIdx.x;
+    const int64_t goff = SINGLE ? (int64_t)blockIdx.x * n : 0;   // first element of this CTA's ring
     const int64_t cbeg = (int64_t)b * chunk;
-    const int64_t i0 = cbeg + (int64_t)threadIdx.x * E;      // first element of this thread
-    const T* __restrict__ yin = (const T*)a.y_in;
-    const T* __restrict__ ep = (const T*)a.elem_param;
+    const int64_t i0 = cbeg + (int64_t)threadIdx.x * E;      // first element of this thread (inside its ring)
+    const T* __restrict__ yin = (const T*)a.y_in + goff;
+    const T* __restrict__ ep = (const T*)a.elem_param + goff;
     const T dt = (T)a.dt;
     const int deg = 2 * P + (a.include_self ? 1 : 0);
     const T inv_deg = deg > 0 ? T(1) / T(deg) : T(0);
@@ -244,7 +246,7 @@ __global__ void __launch_bounds__(RING_THREADS) ring_persistent_kernel(RingArgs 
             }
         }
         if (a.rhs_only) {
-            T* out = (T*)a.y_out;
+            T* out = (T*)a.y_out + goff;
 #pragma unroll
             for (int e = 0; e < E; ++e)
                 if (ok[e])
@@ -265,7 +267,7 @@ __global__ void __launch_bounds__(RING_THREADS) ring_persistent_kernel(RingArgs 
             }
         if (SINGLE) __syncthreads();   // the shared prefix buffer is rewritten by the next stage
     }
-    T* out = (T*)a.y_out;
+    T* out = (T*)a.y_out + goff;
 #pragma unroll
     for (int e = 0; e < E; ++e)
         if (ok[e])
@@ -293,10 +295,12 @@ static bool ring_plan(int64_t n, size_t esize, RingPlan* p, int gmax = 148) {
     return false;
 }
 
+// d->n is the total over the batch (api.cu: normalise); batches need rings that fit one CTA
 bool ring_supported(const net_desc* d) {
     RingPlan p;
+    const int batch = d->batch > 0 ? d->batch : 1;
     return d->topo.kind == NET_TOPO_RING && (d->model == NET_MODEL_KS || d->model == NET_MODEL_FHN) &&
-           ring_plan(d->n, d->dtype == NET_F32 ? 4 : 8, &p);
+           ring_plan(d->n / batch, d->dtype == NET_F32 ? 4 : 8, &p, batch > 1 ? 1 : 148);
 }
 
 size_t ring_scratch_bytes(const net_desc* d) {
@@ -319,8 +323,8 @@ static int32_t ring_launch_t(net* h, RingArgs& a, const RingPlan& p) {
     }
     if (!SINGLE) OSC_CUDA(h, cudaMemsetAsync(a.bar, 0, sizeof(unsigned), h->stream));
     void* params[] = {&a, &h->mp};
-    if (SINGLE)
-        OSC_CUDA(h, cudaLaunchKernel((const void*)kern, dim3(1), dim3(RING_THREADS), params, p.smem, h->stream));
+    if (SINGLE)      // one CTA per ring of the batch
+        OSC_CUDA(h, cudaLaunchKernel((const void*)kern, dim3((unsigned)h->desc.batch), dim3(RING_THREADS), params, p.smem, h->stream));
     else
         OSC_CUDA(h, cudaLaunchCooperativeKernel((const void*)kern, dim3(p.G), dim3(RING_THREADS), params, p.smem, h->stream));
     h->launches += 1;
@@ -350,7 +354,7 @@ static int32_t ring_run_plan(net* h, const RingPlan& p, const void* y_in, void* 
     RingArgs a;
     memset(&a, 0, sizeof(a));
     a.y_in = y_in; a.y_out = y_out; a.elem_param = h->b.elem_param;
-    a.n = h->n; a.ld = h->ld; a.npad = round_up(h->n, 64);
+    a.n = h->tv.ring_n; a.ld = h->ld; a.npad = round_up(h->n, 64);
     a.P = h->tv.P; a.include_self = h->tv.include_self; a.chunk = p.chunk; a.G = p.G;
     a.chunk_shift = 0;
     while ((1 << a.chunk_shift) < p.chunk) ++a.chunk_shift;
@@ -371,7 +375,7 @@ int32_t ring_run(net* h, const void* y_in, void* y_out, int64_t n_steps, double 
     RingPlan p;
     // (two CTAs per SM -- gmax = 296, half the elements per thread -- measured slower on config 2:
     // 4.8e9 against 5.0e9 osc-steps/s; the 256-way barrier costs more than the shorter chain saves)
-    if (!ring_plan(h->n, h->esize, &p)) return set_err(h, NET_ERR_UNSUPPORTED, "ring too large for the persistent kernel");
+    if (!ring_plan(h->tv.ring_n, h->esize, &p, h->desc.batch > 1 ? 1 : 148)) return set_err(h, NET_ERR_UNSUPPORTED, "ring too large for the persistent kernel");
     return ring_run_plan(h, p, y_in, y_out, n_steps, dt, rhs_only);
 }
 

@@ -136,12 +136,13 @@ __global__ void expand_rows_kernel(TopoView tv, int64_t n, int64_t row_begin, in
             ++have;
         };
         if (tv.kind == NET_TOPO_RING) {
+            const int64_t rn = tv.ring_n, base = i / rn * rn;
             for (int d = -tv.P; d <= tv.P; ++d) {
                 if (d == 0 && !tv.include_self) continue;
-                int64_t j = i + d;
-                if (j < 0) j += n;
-                if (j >= n) j -= n;
-                put(j);
+                int64_t j = i - base + d;
+                if (j < 0) j += rn;
+                if (j >= rn) j -= rn;
+                put(base + j);
             }
         } else {
             int x = (int)(i % tv.nx);
@@ -168,7 +169,7 @@ __global__ void expand_ring_kernel(int64_t n, int32_t P, int32_t include_self, i
          e += (int64_t)gridDim.x * blockDim.x) {
         const int64_t r = e / deg;
         const int32_t q = (int32_t)(e - r * deg);
-        const int64_t i = row_begin + r;
+        const int64_t gi = row_begin + r, base = gi / n * n, i = gi - base;   // n = ring period; i local to its ring
         int64_t d = (int64_t)q - P;
         if (!include_self && d >= 0) d += 1;
         int64_t j = i + d;
@@ -182,7 +183,7 @@ __global__ void expand_ring_kernel(int64_t n, int32_t P, int32_t include_self, i
         } else pos = q;
         if (j < 0) j += n;
         if (j >= n) j -= n;
-        col_idx[r * (int64_t)deg + pos] = (int32_t)j;
+        col_idx[r * (int64_t)deg + pos] = (int32_t)(base + j);
     }
 }
 
@@ -212,6 +213,7 @@ int32_t topo_build(net* h) {
     tv.nx = tv.ny = tv.nz = 1;
     tv.P = t.radius;
     tv.include_self = t.include_self ? 1 : 0;
+    tv.ring_n = h->n / (h->desc.batch > 0 ? h->desc.batch : 1);
     cudaStream_t st = h->stream;
     OSC_CUDA(h, cudaMemsetAsync(h->b.flag, 0, 4 * sizeof(int32_t), st));
     if (t.kind == NET_TOPO_RING) {
@@ -271,7 +273,7 @@ int32_t topo_expand(net* h, int64_t row_begin, int64_t row_count, int64_t* d_row
         int32_t deg = h->degree_uniform;
         uniform_row_ptr_kernel<<<grid_for(row_count + 1), 256, 0, st>>>(d_row_ptr, row_count, deg);
         if (row_count > 0 && deg > 0 && h->tv.kind == NET_TOPO_RING)
-            expand_ring_kernel<<<grid_for(row_count * (int64_t)deg), 256, 0, st>>>(h->n, h->tv.P, h->tv.include_self, row_begin, row_count, deg, d_col_idx);
+            expand_ring_kernel<<<grid_for(row_count * (int64_t)deg), 256, 0, st>>>(h->tv.ring_n, h->tv.P, h->tv.include_self, row_begin, row_count, deg, d_col_idx);
         else if (row_count > 0)
             expand_rows_kernel<<<grid_for(row_count), 256, 0, st>>>(h->tv, h->n, row_begin, row_count, deg, d_col_idx);
         h->launches += 2;

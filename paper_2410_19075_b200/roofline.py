@@ -78,6 +78,10 @@ def ops_per_osc_step(w):
         return ("fp64", 4 * (7 * 35 + 80 + w.in_degree))
     if w.cfg == "2":
         return ("fp64", 4 * 60)
+    if w.cfg == "1b":
+        # shipped (prefix-sum) formulation per stage: fp64 sincos ~110, block scan of two fields ~30,
+        # window differences + local field + RK4 update ~20
+        return ("fp64", 4 * 160)
     return ("fp64", 4 * (110 + 2 * 2 * w.radius))
 
 

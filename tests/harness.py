@@ -9,28 +9,44 @@ TOL_TRAJ = {"f64": 1e-9, "f32": 1e-4}      # absolute after 100 steps (phases mo
 TOL_STATS = 1e-3
 
 
+def ntot(w):
+    """Elements of all replicas of the workload together."""
+    return w.n * getattr(w, "batch", 1)
+
+
 def make_inputs(w, seed=1):
-    """Seeded inputs in float64, already rounded to the dtype of the net (reading R13)."""
+    """Seeded inputs in float64, already rounded to the dtype of the net (reading R13).
+    A batch gets independent draws for every replica: arrays are [nvar][batch * n]."""
     dt = np.float32 if w.dtype == "f32" else np.float64
+    n_all = ntot(w)
     rnd = lambda a: np.ascontiguousarray(a.astype(dt).astype(np.float64))
     elem = None
     if w.model == configs.KS:
-        y0 = inputs.ks_phases(w.n, seed).reshape(1, -1)
+        y0 = inputs.ks_phases(n_all, seed).reshape(1, -1)
         if w.extra.get("omega") == "lorentzian":
-            elem = inputs.lorentzian_omega(w.n, seed, w.extra["gamma"], w.extra["omega_max"])
+            elem = inputs.lorentzian_omega(n_all, seed, w.extra["gamma"], w.extra["omega_max"])
         else:
-            elem = np.full(w.n, w.params["omega0"])
+            elem = np.full(n_all, w.params["omega0"])
     elif w.model == configs.FHN:
-        y0 = inputs.fhn_circle(w.n, seed)
+        y0 = inputs.fhn_circle(n_all, seed)
     else:
-        V = rnd(inputs.hh_voltage(w.n, seed))
+        V = rnd(inputs.hh_voltage(n_all, seed))
         m, h, g = ora.hh_steady_gates(V)           # tests may call the oracle
         y0 = np.stack([V, m, h, g])
-        elem = inputs.hh_current(w.n, seed)
+        elem = inputs.hh_current(n_all, seed)
     return dict(y0=rnd(y0), elem=None if elem is None else rnd(elem))
 
 
 def oracle_topology(w, row_begin=0, row_count=None):
+    if w.topo == configs.RING and getattr(w, "batch", 1) > 1:
+        # the batch as one block-diagonal net: ring r owns elements r*n .. (r+1)*n - 1
+        rp1, ci1 = ora.topology_ring(w.n, w.radius, False, 0, None)
+        B = w.batch
+        ci = np.concatenate([ci1.astype(np.int64) + r * w.n for r in range(B)]).astype(np.int32)
+        rp = np.concatenate([[0], np.cumsum(np.tile(np.diff(rp1), B))]).astype(np.int64)
+        row_count = ntot(w) - row_begin if row_count is None else row_count
+        lo, hi = rp[row_begin], rp[row_begin + row_count]
+        return rp[row_begin:row_begin + row_count + 1] - lo, ci[lo:hi]
     if w.topo == configs.RING:
         return ora.topology_ring(w.n, w.radius, False, row_begin, row_count)
     if w.topo == configs.LATTICE:
@@ -44,7 +60,7 @@ def make_oracle(w, inp, rows=None):
     if rows is None:
         rp, ci = oracle_topology(w)
     else:
-        lens = np.zeros(w.n + 1, dtype=np.int64)
+        lens = np.zeros(ntot(w) + 1, dtype=np.int64)
         parts = []
         for r in rows:
             _, c = oracle_topology(w, int(r), 1)
@@ -54,10 +70,10 @@ def make_oracle(w, inp, rows=None):
         ci = np.concatenate(parts) if parts else np.zeros(0, dtype=np.int32)
     p = w.params
     if w.model == configs.KS:
-        return ora.OracleNet.ks(w.n, rp, ci, p["K"], p["alpha"], inp["elem"])
+        return ora.OracleNet.ks(ntot(w), rp, ci, p["K"], p["alpha"], inp["elem"])
     if w.model == configs.FHN:
-        return ora.OracleNet.fhn(w.n, rp, ci, p["eps"], p["a"], p["sigma"], p["phi"])
-    return ora.OracleNet.hh(w.n, rp, ci, inp["elem"], **p)
+        return ora.OracleNet.fhn(ntot(w), rp, ci, p["eps"], p["a"], p["sigma"], p["phi"])
+    return ora.OracleNet.hh(ntot(w), rp, ci, inp["elem"], **p)
 
 
 def make_gpu(w, inp, method=0):

@@ -51,6 +51,22 @@ def test_version_and_pure_host_calls(built_lib):
     d.batch, d.model = 1, 7
     with pytest.raises(B.OscnetError):
         B.net_workspace_bytes(d)
+    # batches of rings: the workspace grows with the number of replicas; batch < 1 is invalid
+    r = B.Desc()
+    r.model, r.dtype, r.n, r.batch, r.method = B.MODEL_KS, B.F64, 256, 1, B.METHOD_AUTO
+    r.topo.kind, r.topo.ndim, r.topo.radius = B.TOPO_RING, 1, 64
+    one = B.net_workspace_bytes(r)
+    r.batch = 1184
+    many = B.net_workspace_bytes(r)
+    assert many >= one + 4 * 8 * 256 * 1183
+    r.batch = 0
+    with pytest.raises(B.OscnetError) as e:
+        B.net_workspace_bytes(r)
+    assert e.value.code == -1
+    r.batch, r.n = 1 << 20, 1 << 12           # n * batch > 2^31 - 1
+    with pytest.raises(B.OscnetError) as e:
+        B.net_workspace_bytes(r)
+    assert e.value.code == -1
 
 
 def test_product_path_does_not_import_oracle():

@@ -1,0 +1,74 @@
+"""Batches of independent rings (net_desc.batch > 1, "a large number
+of network instances simultaneously"): the batch is one block-diagonal net, so the oracle of the
+batch is the plain definition on the block-diagonal CSR; replica r must also equal the same ring
+integrated alone (no leakage between replicas)."""
+from dataclasses import replace
+
+import numpy as np
+import pytest
+
+import harness as H
+from paper_2410_19075_b200 import binding as B, configs
+
+pytestmark = pytest.mark.gpu
+
+CASES = [
+    ("1", dict(n=256), 5),       # config 1 itself, five replicas
+    ("1", dict(n=300), 3),       # ragged: 300 elements on 512 lanes (E = 2)
+    ("2", dict(n=1024), 4),      # FHN ring, R = 358
+    ("2", dict(n=2000), 2),      # E = 8, ragged tail
+]
+
+
+def _w(cfg, kw, batch):
+    w = configs.get(cfg, **kw)
+    return replace(w, batch=batch, name=w.name + " x %d" % batch)
+
+
+@pytest.mark.parametrize("cfg,kw,batch", CASES)
+@pytest.mark.parametrize("method", [B.METHOD_FAST, B.METHOD_DIRECT])
+def test_batch_matches_block_diagonal_oracle(cfg, kw, batch, method):
+    w = _w(cfg, kw, batch)
+    inp = H.make_inputs(w, seed=3)
+    onet = H.make_oracle(w, inp)
+    net = H.make_gpu(w, inp, method=method)
+    assert net.counters()[1] == method
+    # topology: bit-exact block-diagonal CSR, element ids 0 .. batch*n - 1
+    rp, ci = net.get_topology()
+    rp0, ci0 = H.oracle_topology(w)
+    assert np.array_equal(rp, rp0) and np.array_equal(ci, ci0)
+    e_rhs = H.rel_maxnorm(net.eval_rhs(), onet.rhs(inp["y0"]), H.rhs_floor(w))
+    assert e_rhs <= H.TOL_RHS[w.dtype], e_rhs
+    net.integrate(100, w.dt)
+    e_tr = H.traj_err(w, net.get_state(), onet.rk4(inp["y0"], 100, w.dt))
+    assert e_tr <= H.TOL_TRAJ[w.dtype], e_tr
+    net.close()
+
+
+def test_replica_equals_the_ring_integrated_alone():
+    w = _w("1", dict(n=256), 4)
+    inp = H.make_inputs(w, seed=5)
+    net = H.make_gpu(w, inp, method=B.METHOD_FAST)
+    net.integrate(50, w.dt)
+    got = net.get_state().reshape(w.nvar, w.batch, w.n)
+    net.close()
+    w1 = configs.get("1", n=256)
+    for r in (0, 3):
+        sl = slice(r * w.n, (r + 1) * w.n)
+        inp1 = dict(y0=inp["y0"][:, sl].copy(), elem=inp["elem"][sl].copy())
+        n1 = H.make_gpu(w1, inp1, method=B.METHOD_FAST)
+        n1.integrate(50, w.dt)
+        alone = n1.get_state()
+        n1.close()
+        assert np.array_equal(got[:, r, :], alone)      # same kernel, same arithmetic: bit-identical
+
+
+def test_batch_on_other_topologies_is_refused():
+    w = replace(configs.get("5", n1=16), batch=2)
+    with pytest.raises(B.OscnetError) as ei:
+        B.Net.from_workload(w)
+    assert ei.value.code == -5
+    w = replace(configs.get("1"), batch=0)
+    with pytest.raises(B.OscnetError) as ei:
+        B.Net.from_workload(w)
+    assert ei.value.code == -1
