@@ -177,6 +177,19 @@ def measure(w, device, steps, warmup, e2e=True, seed=1):
         replicas.barrier()
         out.update(e2e_ms=ev0.elapsed_time(ev1), h2d=host_in.numel() * host_in.element_size(),
                    d2h=host_out.numel() * host_out.element_size())
+    # the same step with the workload's observables switched on (global / local order parameter and
+    # mean phase velocity sampled every obs_every RK4 steps; reported separately)
+    if e2e:
+        net.integrate_observed(S, w.dt, w.obs_every)
+        replicas.barrier()
+        torch.cuda.synchronize()
+        ev0.record(stream)
+        for _ in range(steps):
+            net.integrate_observed(S, w.dt, w.obs_every)     # includes the D2H of the 8 statistics
+        ev1.record(stream)
+        torch.cuda.synchronize()
+        replicas.barrier()
+        out.update(obs_ms=ev0.elapsed_time(ev1))
     net.close()
     del net
     torch.cuda.empty_cache()
@@ -322,6 +335,11 @@ def line_for(w, m, steps, n_gpus, units_total=None, ms_max=None):
     if "e2e_ms" in m:
         out["e2e"] = {"value": ntot(w) * rk4 * n_gpus / (m["e2e_ms"] * 1e-3), "unit": METRIC,
                       "h2d_bytes_per_step": m["h2d"], "d2h_bytes_per_step": m["d2h"]}
+    if "obs_ms" in m:
+        out["with_observables"] = {"value": ntot(w) * rk4 * n_gpus / (m["obs_ms"] * 1e-3), "unit": METRIC,
+                                   "obs_every": w.obs_every,
+                                   "what": "net_integrate_observed: global and local order parameter, mean phase "
+                                           "velocity sampled every obs_every RK4 steps, statistics read back"}
     return out
 
 
@@ -355,6 +373,10 @@ def run_ours(args):
             "e2e": {"value": e2e_value, "unit": METRIC, "h2d_bytes_per_step": m["h2d"],
                     "d2h_bytes_per_step": m["d2h"]},
             "gpu_launches": m["launches"], "roofline": head["roofline"]}
+    if "with_observables" in head and ws == 1:
+        line["with_observables"] = head["with_observables"]
+    if getattr(w, "batch", 1) > 1:
+        line["config"]["batch"] = w.batch
     if rank == 0 and ws == 1 and not args.no_per_config:
         per = []
         for cfg in PER_CONFIG:

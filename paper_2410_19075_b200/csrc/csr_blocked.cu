@@ -14,8 +14,9 @@
 //   * once per net the CSR arrays are re-ordered into a blocked ELL form: for every (chunk c,
 //     block b, row l) FOUR 16-bit slots (one 8-byte word, coalesced across the rows of a warp)
 //     holding the first four sources of row l that lie in block b, as indices local to the block;
-//     unused slots hold W, the index of a slot that holds 0, so the gather loop has no branch and
-//     no trip count.  The few entries beyond four per (row, block) -- 5 % on config 4 -- go to a
+//     unused slots point at one of the zeros that follow the block (one per bank), so the gather
+//     loop has no branch and no trip count; the order of the slots of a word is chosen against
+//     shared-memory bank conflicts (cb_place_slots).  The few entries beyond four per (row, block) -- 5 % on config 4 -- go to a
 //     per-row overflow list and are gathered from global memory after the last block;
 //   * per stage a CTA walks b = 0..B-1: bulk-copy s[b*W .. (b+1)*W) into shared memory
 //     (cp.async.bulk on an mbarrier; all CTAs read the same block at about the same time, L2
@@ -43,6 +44,8 @@ struct CbGeom {
     const uint2* slots;          // [nchunks][B][CR] words of four 16-bit local indices
     const int32_t* ovf_ptr;      // [nchunks * CR + 1] overflow list of every row
     const int32_t* ovf_idx;      // global source indices
+    void* partial;               // pair kernel: [nchunks * CR] sums of the partner's half of the blocks
+    unsigned* pair_flag;         // pair kernel: [nchunks] launches completed by every CTA
 };
 
 __device__ __forceinline__ void cb_bulk_load(void* dst, const void* src, unsigned bytes, uint64_t* bar) {
@@ -292,6 +295,119 @@ csr_blocked_stage_kernel(StageArgs a, ModelParams mp, TopoView tv, CbGeom g) {
     }
 }
 
+// Pair form (2D partition).  What bounds the kernel above on config 4 is the L2 -> SM traffic of
+// the s blocks: each of the 148 CTAs streams ALL of s every stage (1.18 GB).  Here CTAs 2p and
+// 2p + 1 both take the rows of chunks 2p AND 2p + 1 but only one half of the column blocks each,
+// so every CTA streams half of s (the slot-word and gather work per CTA is unchanged); the two
+// halves of every row sum meet through global memory: each CTA publishes its sums for the
+// partner's chunk, raises its launch counter (release), waits for the partner's (acquire) and
+// finishes its own chunk as  (blocks of the lower half) + (blocks of the upper half).  The launch
+// is cooperative, so the two CTAs of a pair are co-resident.
+__device__ __forceinline__ unsigned cb_ld_acquire(const unsigned* p) {
+    unsigned v;
+    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ void cb_st_release(unsigned* p, unsigned v) {
+    asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+
+template <class T, int M>
+__global__ void __launch_bounds__(CB_THREADS, 1)
+csr_blocked_pair_kernel(StageArgs a, ModelParams mp, TopoView tv, CbGeom g) {
+    extern __shared__ __align__(128) unsigned char cb_smem[];
+    __shared__ uint64_t bar;
+    __shared__ unsigned epoch_s;
+    constexpr unsigned SH = sizeof(T) == 8 ? 3u : 2u;
+    constexpr unsigned MASK = 0xffffu << SH;
+    T* sblk = reinterpret_cast<T*>(cb_smem);
+    const unsigned sblk_a = smem_u32(cb_smem);
+    const T* __restrict__ gsrc = (const T*)a.s_in;
+    const int t = threadIdx.x;
+    const int pair = blockIdx.x >> 1, half = blockIdx.x & 1;
+    if (t == 0) {
+        mbar_init(&bar, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        epoch_s = g.pair_flag[blockIdx.x] + 1u;        // launches are stream-ordered: the partner's counter is at the same value
+    }
+    if (t < 128 / (int)sizeof(T)) sblk[g.W + t] = T(0);
+    __syncthreads();
+    const int bh = (g.B + 1) / 2;
+    const int b_lo = half ? bh : 0, b_hi = half ? g.B : bh;
+    unsigned phase = 0;
+    T acc0[M], acc1[M];                                // rows of chunk 2p, of chunk 2p + 1
+#pragma unroll
+    for (int m = 0; m < M; ++m) { acc0[m] = T(0); acc1[m] = T(0); }
+    for (int b = b_lo; b < b_hi; ++b) {
+        const int64_t col0 = (int64_t)b * g.W;
+        const uint2* __restrict__ sl0 = g.slots + ((int64_t)(2 * pair) * g.B + b) * g.CR;
+        const uint2* __restrict__ sl1 = g.slots + ((int64_t)(2 * pair + 1) * g.B + b) * g.CR;
+        __syncthreads();                           // every thread is done with the previous block
+        if (t == 0) {
+            const int64_t cnt = g.n - col0 < g.W ? g.n - col0 : g.W;
+            constexpr int V = 16 / (int)sizeof(T);
+            const unsigned bytes = (unsigned)((cnt + V - 1) / V * V * sizeof(T));
+            mbar_expect_tx(&bar, bytes);
+            for (unsigned o = 0; o < bytes; o += CB_COPY)
+                cb_bulk_load(cb_smem + o, (const unsigned char*)(gsrc + col0) + o, bytes - o < CB_COPY ? bytes - o : CB_COPY, &bar);
+        } else if (b + 1 < b_hi && (t == 32 || t == 64)) {   // next block's slot words towards L2
+            cb_prefetch_l2((t == 32 ? sl0 : sl1) + g.CR, (unsigned)((size_t)g.CR * sizeof(uint2)));
+        }
+        uint2 w[M], u[M];                          // both chunks' slot words are in flight while the block arrives
+#pragma unroll
+        for (int m = 0; m < M; ++m) {
+            const int l = m * CB_THREADS + t;
+            w[m] = l < g.CR ? __ldg(sl0 + l) : make_uint2((unsigned)g.W * 0x10001u, (unsigned)g.W * 0x10001u);
+            u[m] = l < g.CR ? __ldg(sl1 + l) : make_uint2((unsigned)g.W * 0x10001u, (unsigned)g.W * 0x10001u);
+        }
+        mbar_wait(&bar, phase);
+        phase ^= 1u;
+#pragma unroll
+        for (int m = 0; m < M; ++m) {
+            const T v0 = cb_lds(sblk_a + ((w[m].x << SH) & MASK), T(0));
+            const T v1 = cb_lds(sblk_a + ((w[m].x >> (16 - SH)) & MASK), T(0));
+            const T v2 = cb_lds(sblk_a + ((w[m].y << SH) & MASK), T(0));
+            const T v3 = cb_lds(sblk_a + ((w[m].y >> (16 - SH)) & MASK), T(0));
+            acc0[m] += (v0 + v1) + (v2 + v3);
+            const T x0 = cb_lds(sblk_a + ((u[m].x << SH) & MASK), T(0));
+            const T x1 = cb_lds(sblk_a + ((u[m].x >> (16 - SH)) & MASK), T(0));
+            const T x2 = cb_lds(sblk_a + ((u[m].y << SH) & MASK), T(0));
+            const T x3 = cb_lds(sblk_a + ((u[m].y >> (16 - SH)) & MASK), T(0));
+            acc1[m] += (x0 + x1) + (x2 + x3);
+        }
+    }
+    // ---- publish the sums of the partner's chunk, wait for the partner's sums of mine
+    const int c_own = 2 * pair + half, c_other = 2 * pair + (1 - half);
+    T* part = (T*)g.partial;
+#pragma unroll
+    for (int m = 0; m < M; ++m) {
+        const int l = m * CB_THREADS + t;
+        if (l < g.CR) __stcg(part + (int64_t)c_other * g.CR + l, half ? acc0[m] : acc1[m]);
+    }
+    __threadfence();
+    __syncthreads();
+    if (t == 0) {
+        const unsigned epoch = epoch_s;
+        cb_st_release(g.pair_flag + blockIdx.x, epoch);
+        while (cb_ld_acquire(g.pair_flag + (blockIdx.x ^ 1)) < epoch) {}
+    }
+    __syncthreads();
+    const int64_t row0 = (int64_t)c_own * g.CR;
+#pragma unroll
+    for (int m = 0; m < M; ++m) {
+        const int l = m * CB_THREADS + t;
+        const int64_t i = row0 + l;
+        if (l >= g.CR || i >= g.n) continue;
+        const T mine = half ? acc1[m] : acc0[m];
+        const T theirs = __ldcg(part + row0 + l);
+        T sum = half ? theirs + mine : mine + theirs;      // lower half of the blocks + upper half
+        const int q1 = g.ovf_ptr[i + 1];
+        for (int q = g.ovf_ptr[i]; q < q1; ++q) sum += gsrc[g.ovf_idx[q]];
+        const int deg = tv.k_uniform > 0 ? tv.k_uniform : (int)(tv.row_ptr[i + 1] - tv.row_ptr[i]);
+        cb_finish_hh<T>(a, mp, i, sum, deg);
+    }
+}
+
 // ------------------------------------------------------------------ host side
 constexpr size_t CB_SMEM_BUDGET = 224 * 1024;   // of the 227 KB a CTA may own
 
@@ -343,7 +459,7 @@ bool csr_blocked_supported(const net_desc* d) {
 
 // scratch: slots | ovf_ptr | ovf_cnt | ovf_idx.  The overflow list may take a quarter of nnz;
 // a graph that needs more (far from uniform rows) goes back to the warp-per-row kernel.
-struct CbLayout { size_t slots, ovf_ptr, ovf_cnt, ovf_idx, total; int64_t ovf_cap; };
+struct CbLayout { size_t slots, ovf_ptr, ovf_cnt, ovf_idx, partial, pair_flag, total; int64_t ovf_cap; };
 static CbLayout cb_layout(const net_desc* d, const CbGeom& g) {
     CbLayout L;
     size_t cur = 0;
@@ -354,6 +470,8 @@ static CbLayout cb_layout(const net_desc* d, const CbGeom& g) {
     L.ovf_ptr = take((rows + 1) * sizeof(int32_t));
     L.ovf_cnt = take((rows + 1) * sizeof(int32_t));
     L.ovf_idx = take((size_t)L.ovf_cap * sizeof(int32_t));
+    L.partial = take(rows * (d->dtype == NET_F32 ? 4 : 8));
+    L.pair_flag = take((size_t)g.nchunks * sizeof(unsigned) + 64);
     L.total = cur;
     return L;
 }
@@ -378,6 +496,20 @@ static const void* cb_kernel_for(int M) {
     }
 }
 
+template <class T>
+static const void* cb_pair_kernel_for(int M) {
+    switch (M) {
+        case 1: return (const void*)csr_blocked_pair_kernel<T, 1>;
+        case 2: return (const void*)csr_blocked_pair_kernel<T, 2>;
+        case 3: return (const void*)csr_blocked_pair_kernel<T, 3>;
+        case 4: return (const void*)csr_blocked_pair_kernel<T, 4>;
+        case 5: return (const void*)csr_blocked_pair_kernel<T, 5>;
+        case 6: return (const void*)csr_blocked_pair_kernel<T, 6>;
+        case 7: return (const void*)csr_blocked_pair_kernel<T, 7>;
+        default: return (const void*)csr_blocked_pair_kernel<T, 8>;
+    }
+}
+
 // Builds the blocked ELL arrays in the scratch region.  NET_ERR_UNSUPPORTED (rows not sorted,
 // overflow list too long) sends the net back to the warp-per-row kernel.
 int32_t csr_blocked_prepare(net* h) {
@@ -391,7 +523,9 @@ int32_t csr_blocked_prepare(net* h) {
     int32_t* ovf_cnt = (int32_t*)(s + L.ovf_cnt);
     int32_t* ovf_idx = (int32_t*)(s + L.ovf_idx);
     g.slots = slots; g.ovf_ptr = ovf_ptr; g.ovf_idx = ovf_idx;
+    g.partial = s + L.partial; g.pair_flag = (unsigned*)(s + L.pair_flag);
     cudaStream_t st = h->stream;
+    OSC_CUDA(h, cudaMemsetAsync(g.pair_flag, 0, (size_t)g.nchunks * sizeof(unsigned), st));
     const int64_t rows = (int64_t)g.nchunks * g.CR;
     const unsigned grid = (unsigned)((rows + 255) / 256 > 148 * 16 ? 148 * 16 : (rows + 255) / 256);
     const int32_t ku = h->tv.k_uniform;
@@ -417,9 +551,22 @@ int32_t csr_blocked_prepare(net* h) {
     memcpy(h->cb_geom, &g, sizeof(g));
     h->cb_grid = (unsigned)(g.nchunks < sms ? g.nchunks : sms);
     h->cb_smem = smem;
+    // pair form: one chunk per CTA, an even number of them, all co-resident (cooperative launch)
+    h->cb_pair = 0;
+    int coop = 0;
+    cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev);
+    const char* pe = getenv("OSCNET_CSRB_PAIR");
+    if (coop && g.nchunks % 2 == 0 && g.nchunks <= sms && g.B >= 2 && !(pe && atoi(pe) == 0)) {
+        const void* pk = h->desc.dtype == NET_F32 ? cb_pair_kernel_for<float>(g.M) : cb_pair_kernel_for<double>(g.M);
+        int occ = 0;
+        if (cudaFuncSetAttribute(pk, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) == cudaSuccess &&
+            cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, pk, CB_THREADS, smem) == cudaSuccess && occ * sms >= g.nchunks)
+            h->cb_pair = 1;
+        else cudaGetLastError();
+    }
     if (getenv("OSCNET_VERBOSE"))
-        fprintf(stderr, "csr_blocked: W %d B %d CR %d chunks %d M %d overflow %d of %lld entries smem %zu grid %u scratch %zu\n",
-                g.W, g.B, g.CR, g.nchunks, g.M, flag[1], (long long)h->nnz, smem, h->cb_grid, L.total);
+        fprintf(stderr, "csr_blocked: W %d B %d CR %d chunks %d M %d overflow %d of %lld entries smem %zu grid %u scratch %zu pair %d\n",
+                g.W, g.B, g.CR, g.nchunks, g.M, flag[1], (long long)h->nnz, smem, h->cb_grid, L.total, h->cb_pair);
     return NET_OK;
 }
 
@@ -429,7 +576,23 @@ int32_t csr_blocked_stage(net* h, const StageArgs& a) {
     const void* kern = h->desc.dtype == NET_F32 ? cb_kernel_for<float>(g.M) : cb_kernel_for<double>(g.M);
     StageArgs aa = a;
     void* params[] = {&aa, &h->mp, &h->tv, &g};
-    OSC_CUDA(h, cudaLaunchKernel(kern, dim3(h->cb_grid), dim3(CB_THREADS), params, h->cb_smem, h->stream));
+    if (h->cb_pair) {
+        const void* pk = h->desc.dtype == NET_F32 ? cb_pair_kernel_for<float>(g.M) : cb_pair_kernel_for<double>(g.M);
+        cudaLaunchConfig_t cfg;
+        memset(&cfg, 0, sizeof(cfg));
+        cfg.gridDim = dim3((unsigned)g.nchunks);
+        cfg.blockDim = dim3(CB_THREADS);
+        cfg.dynamicSmemBytes = h->cb_smem;
+        cfg.stream = h->stream;
+        cudaLaunchAttribute attr[1];
+        attr[0].id = cudaLaunchAttributeCooperative;
+        attr[0].val.cooperative = 1;
+        cfg.attrs = attr;
+        cfg.numAttrs = 1;
+        OSC_CUDA(h, cudaLaunchKernelExC(&cfg, pk, params));
+    } else {
+        OSC_CUDA(h, cudaLaunchKernel(kern, dim3(h->cb_grid), dim3(CB_THREADS), params, h->cb_smem, h->stream));
+    }
     h->launches += 1;
     return NET_OK;
 }

@@ -198,6 +198,7 @@ struct net {
     size_t lat3_smem[5];
     char cb_geom[96];      // FAST_CSR_BLOCKED: CbGeom (csr_blocked.cu)
     unsigned cb_grid;
+    int32_t cb_pair;       // 1 = pair form of the blocked CSR kernel (each CTA streams half of the s blocks)
     int32_t cb_es;         // entries staged in shared memory
     size_t cb_smem;
     int32_t l3_force_tx, l3_force_sy, l3_force_ctas;   // FAST_LATTICE3D_V3: tile chosen by the autotuner (0 = by score)
