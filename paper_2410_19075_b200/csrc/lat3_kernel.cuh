@@ -2,7 +2,10 @@
 // z-marching ball sums fed entirely by TMA.
 //
 // Mathematics as before (x-run decomposition of the ball of PAPER.md:313, register accumulators
-// for the 2P+1 open output planes, factorised sine for KS; exact in real arithmetic).  What
+// for the 2P+1 open output planes; exact in real arithmetic).  This file holds the pair form --
+// both fields of the ball sum as one packed pair per thread -- that FitzHugh-Nagumo lattices run;
+// Kuramoto-Sakaguchi lattices run the field-split form (lat3s_kernel.cuh), which shares the
+// operand-tile table, the parameter block and the producer protocol defined here.  What
 // changed is what the second generation was bound by on B200 (profiles/r01_baseline_ncu.md:
 // 17 % occupancy, one CTA-wide barrier per plane, operand loads exposed once per plane, 93
 // instructions per element):
@@ -64,19 +67,14 @@ lat3_kernel(const __grid_constant__ CUtensorMap tm_st, const __grid_constant__ C
             const __grid_constant__ CUtensorMap tm_op1, const __grid_constant__ CUtensorMap tm_op2,
             const __grid_constant__ CUtensorMap tm_op3, L3Ptrs a, L3Params<T> mp, L3Geom g) {
     typedef typename PairOf<T>::type Pr;
-    constexpr bool KS = MODEL == NET_MODEL_KS;
-    // fp64 KS keeps (cos phi) and (sin phi) as two PLANES (global and staged): a thread's row of
-    // 16-byte pairs at a 32-byte lane stride costs two shared-memory wavefronts per vector load
-    // (profiles/r01_lat3_ncu.md, cfg 3b: half of the wavefronts were bank conflicts); rows of
-    // doubles at a 16-byte lane stride cost one.
-    constexpr bool PLANAR = KS && sizeof(T) == 8;
+    static_assert(MODEL == NET_MODEL_FHN, "pair form: FHN; KS lattices run lat3s_kernel");
     constexpr int HX = l2_hx<T>(P);           // x ghost width of the padded pair arrays
     constexpr int NCOL = X + 2 * HX;          // pairs a thread reads per staged row
     constexpr int OFF = HX - P;
     constexpr int NACC = 2 * P + 1;
     constexpr int NT = L3Ops<MODEL, STAGE>::N;
     constexpr int U8 = (int)sizeof(Pr) / 8;   // 8-byte TMA elements per pair
-    constexpr int EW = KS ? X : 2 * X;        // scalars per thread-row of an operand / output tile
+    constexpr int EW = 2 * X;                 // scalars per thread-row of an operand / output tile
 
     extern __shared__ __align__(128) unsigned char l3_smem[];
     const int D = g.D, NB = D + 1, NS = P + 1 + D;
@@ -115,13 +113,12 @@ lat3_kernel(const __grid_constant__ CUtensorMap tm_st, const __grid_constant__ C
                 const bool ops = NT > 0 && j >= 2 * P;
                 mbar_expect_tx(full + b, g.st_bytes + (ops ? NT * g.op_bytes : 0u));
                 int zz = (z0 - P + j) % nz; if (zz < 0) zz += nz;
-                if constexpr (PLANAR) tma_load_4d(st_ring + (size_t)ss * g.st_stride, &tm_st, x0, y0, zz, 0, full + b);
-                else tma_load_3d(st_ring + (size_t)ss * g.st_stride, &tm_st, x0 * U8, y0, zz, full + b);
+                tma_load_3d(st_ring + (size_t)ss * g.st_stride, &tm_st, x0 * U8, y0, zz, full + b);
                 if (ops) {
                     const int zo = z0 - 2 * P + j;
                     unsigned char* ob = op_ring + (size_t)b * NT * g.op_stride;
-                    // FHN operands: centre boxes of padded pair arrays; KS: plain scalar arrays
-                    const int cx = KS ? x0 : (x0 + HX) * U8, cy = KS ? y0 : y0 + P;
+                    // operands: centre boxes of the padded pair arrays
+                    const int cx = (x0 + HX) * U8, cy = y0 + P;
                     if (NT >= 1) tma_load_3d(ob, &tm_op0, cx, cy, zo, full + b);
                     if (NT >= 2) tma_load_3d(ob + g.op_stride, &tm_op1, cx, cy, zo, full + b);
                     if (NT >= 3) tma_load_3d(ob + 2 * (size_t)g.op_stride, &tm_op2, cx, cy, zo, full + b);
@@ -141,7 +138,6 @@ lat3_kernel(const __grid_constant__ CUtensorMap tm_st, const __grid_constant__ C
     const bool owner = st < g.SY && x < nx;
     const int yrow0 = y0 + st * TY;
     const int nxp = nx + 2 * HX, nyp = ny + 2 * P;
-    const int64_t nxy = (int64_t)nx * ny;
     const int64_t pxy = (int64_t)nxp * nyp;
     const int gxs = x < HX ? nx : (x >= nx - HX ? -nx : 0);   // periodic image this thread also writes
 
@@ -162,8 +158,6 @@ lat3_kernel(const __grid_constant__ CUtensorMap tm_st, const __grid_constant__ C
         mbar_wait(full + b, phase);
         if (owner) {
             const Pr* sb = reinterpret_cast<const Pr*>(st_ring + (size_t)slot * g.st_stride) + (st * TY) * PW + q * X;
-            const T* sbc = reinterpret_cast<const T*>(st_ring + (size_t)slot * g.st_stride) + (st * TY) * PW + q * X;   // PLANAR: cos box
-            const int splane = PW * g.PH;                                                                                 // ... sin box behind it
             Pr A[P > 1 ? P - 1 : 1][TY][X];
             bool Aset[P > 1 ? P - 1 : 1][TY];
 #pragma unroll
@@ -182,15 +176,6 @@ lat3_kernel(const __grid_constant__ CUtensorMap tm_st, const __grid_constant__ C
                         float4 w4 = *reinterpret_cast<const float4*>(row + 2 * c);
                         v[2 * c] = make_float2(w4.x, w4.y);
                         v[2 * c + 1] = make_float2(w4.z, w4.w);
-                    }
-                } else if constexpr (PLANAR) {
-                    const T* rc = sbc + rr * PW;
-#pragma unroll
-                    for (int c = 0; c < NCOL / 2; ++c) {
-                        const double2 wc = *reinterpret_cast<const double2*>(rc + 2 * c);
-                        const double2 ws = *reinterpret_cast<const double2*>(rc + splane + 2 * c);
-                        v[2 * c] = make_double2(wc.x, ws.x);
-                        v[2 * c + 1] = make_double2(wc.y, ws.y);
                     }
                 } else {
 #pragma unroll
@@ -245,14 +230,13 @@ lat3_kernel(const __grid_constant__ CUtensorMap tm_st, const __grid_constant__ C
         // ---- finish output plane zo (accumulator J)
         if (owner && zo >= z0) {
             const Pr* cb = reinterpret_cast<const Pr*>(st_ring + (size_t)cslot * g.st_stride) + (st * TY + P) * PW + q * X + HX;
-            const T* ob = reinterpret_cast<const T*>(op_ring + (size_t)b * NT * g.op_stride) + (st * TY) * (g.TXt * (KS ? 1 : 2)) + q * EW;
+            const T* ob = reinterpret_cast<const T*>(op_ring + (size_t)b * NT * g.op_stride) + (st * TY) * (g.TXt * 2) + q * EW;
             const int ostride = g.op_stride / (int)sizeof(T);    // scalars between operand tiles
-            const int orow = g.TXt * (KS ? 1 : 2);               // scalars per tile row
+            const int orow = g.TXt * 2;                          // scalars per tile row
 #pragma unroll
             for (int r = 0; r < TY; ++r) {
                 const int yy = yrow0 + r;
                 if (yy >= ny) continue;
-                const int64_t il = (int64_t)zo * nxy + (int64_t)yy * nx + x;                    // plain scalar arrays
                 const int64_t ip = (int64_t)zo * pxy + (int64_t)(yy + P) * nxp + (x + HX);     // padded pair arrays
                 const int gys = yy < P ? ny : (yy >= ny - P ? -ny : 0);
                 auto store_pairs = [&](T* base, const T (&vals)[2 * X]) {    // with the periodic images
@@ -264,80 +248,35 @@ lat3_kernel(const __grid_constant__ CUtensorMap tm_st, const __grid_constant__ C
                     }
                 };
                 // operand tiles of this thread-row: shared memory, 16-byte vectors where X allows
-                T o0[EW], o1[EW], o2[EW], o3[EW];
+                T o0[EW], o1[EW];
                 if (NT >= 1) ldg_vec<EW>(ob + r * orow, o0);
                 if (NT >= 2) ldg_vec<EW>(ob + ostride + r * orow, o1);
-                if (NT >= 3) ldg_vec<EW>(ob + 2 * ostride + r * orow, o2);
-                if (NT >= 4) ldg_vec<EW>(ob + 3 * ostride + r * orow, o3);
-                T ov[EW], zv[EW], ev[2 * X];
+                T ov[EW];
+                [[maybe_unused]] T zv[EW];
 #pragma unroll
                 for (int e = 0; e < X; ++e) {
-                    Pr c;
-                    if constexpr (PLANAR) {
-                        const T* cc = reinterpret_cast<const T*>(st_ring + (size_t)cslot * g.st_stride) + (st * TY + P + r) * PW + q * X + HX + e;
-                        c.x = cc[0]; c.y = cc[PW * g.PH];
-                    } else c = cb[r * PW + e];
+                    const Pr c = cb[r * PW + e];
                     const Pr W = acc[J % NACC][r][e];
-                    if constexpr (KS) {
-                        T C = W.x, S = W.y;
-                        if (!mp.include_self) { C -= c.x; S -= c.y; }
-                        const T cia = c.x * mp.ca - c.y * mp.sa;      // cos(phi_i + alpha)
-                        const T sia = c.y * mp.ca + c.x * mp.sa;      // sin(phi_i + alpha)
-                        const T om = NT == 4 ? o3[e] : NT == 2 ? o1[e] : o0[e];
-                        const T k = om + mp.kd * (S * cia - C * sia);
-                        T o;
-                        if constexpr (STAGE == L3_RHS) o = k;
-                        else o = o0[e] + mp.h * k;                   // y (stages 0-2) or Z (stage 3)
-                        if constexpr (STAGE == L3_S2) zv[e] = (o1[e] + T(2) * o2[e] + o - o0[e]) * T(1.0 / 3.0);
-                        ov[e] = o;
-                        if constexpr (STAGE != L3_RHS) {
-                            T s_, c_;
-                            sincos_stage<T>(o, &s_, &c_);
-                            ev[2 * e] = c_; ev[2 * e + 1] = s_;
-                        }
-                    } else {
-                        // sum_j (u_j - u_i) over the ball = W - n_ball c whether or not the centre counts
-                        const Pr Cc = pfma(c, Pr{-mp.nb, -mp.nb}, W);
-                        const T u = c.x, v = c.y;
-                        const T rr_ = fma(u * u, mp.ie3, mp.ie);      // (1 - u^2/3)/eps
-                        T gu = fma(mp.cuu, Cc.x, mp.cuv * Cc.y);
-                        gu = fma(-mp.ie, v, gu);
-                        const T ku = fma(u, rr_, gu);
-                        const T kv = fma(mp.cvu, Cc.x, fma(mp.cvv, Cc.y, u + mp.a));
-                        T ou, ovv;
-                        if constexpr (STAGE == L3_RHS) { ou = ku; ovv = kv; }
-                        else if constexpr (STAGE == L3_S0) { ou = fma(mp.h, ku, u); ovv = fma(mp.h, kv, v); }
-                        else { ou = fma(mp.h, ku, o0[2 * e]); ovv = fma(mp.h, kv, o0[2 * e + 1]); }
-                        if constexpr (STAGE == L3_S2) {
-                            zv[2 * e] = (o1[2 * e] + T(2) * u + ou - o0[2 * e]) * T(1.0 / 3.0);
-                            zv[2 * e + 1] = (o1[2 * e + 1] + T(2) * v + ovv - o0[2 * e + 1]) * T(1.0 / 3.0);
-                        }
-                        ov[2 * e] = ou; ov[2 * e + 1] = ovv;
+                    // sum_j (u_j - u_i) over the ball = W - n_ball c whether or not the centre counts
+                    const Pr Cc = pfma(c, Pr{-mp.nb, -mp.nb}, W);
+                    const T u = c.x, v = c.y;
+                    const T rr_ = fma(u * u, mp.ie3, mp.ie);      // (1 - u^2/3)/eps
+                    T gu = fma(mp.cuu, Cc.x, mp.cuv * Cc.y);
+                    gu = fma(-mp.ie, v, gu);
+                    const T ku = fma(u, rr_, gu);
+                    const T kv = fma(mp.cvu, Cc.x, fma(mp.cvv, Cc.y, u + mp.a));
+                    T ou, ovv;
+                    if constexpr (STAGE == L3_RHS) { ou = ku; ovv = kv; }
+                    else if constexpr (STAGE == L3_S0) { ou = fma(mp.h, ku, u); ovv = fma(mp.h, kv, v); }
+                    else { ou = fma(mp.h, ku, o0[2 * e]); ovv = fma(mp.h, kv, o0[2 * e + 1]); }
+                    if constexpr (STAGE == L3_S2) {
+                        zv[2 * e] = (o1[2 * e] + T(2) * u + ou - o0[2 * e]) * T(1.0 / 3.0);
+                        zv[2 * e + 1] = (o1[2 * e + 1] + T(2) * v + ovv - o0[2 * e + 1]) * T(1.0 / 3.0);
                     }
+                    ov[2 * e] = ou; ov[2 * e + 1] = ovv;
                 }
-                if constexpr (KS) {
-                    stg_vec<EW>((T*)a.out + il, ov);
-                    if constexpr (STAGE == L3_S2) stg_vec<EW>((T*)a.out2 + il, zv);
-                    if constexpr (STAGE != L3_RHS) {
-                        if constexpr (PLANAR) {
-                            T cv[X], sv[X];
-#pragma unroll
-                            for (int e = 0; e < X; ++e) { cv[e] = ev[2 * e]; sv[e] = ev[2 * e + 1]; }
-                            T* Ec = (T*)a.Eout;
-                            T* Es = Ec + g.plane;
-                            auto store_planes = [&](int64_t at) { stg_vec<X>(Ec + at, cv); stg_vec<X>(Es + at, sv); };
-                            store_planes(ip);
-                            if (gxs != 0) store_planes(ip + gxs);
-                            if (gys != 0) {
-                                store_planes(ip + (int64_t)gys * nxp);
-                                if (gxs != 0) store_planes(ip + (int64_t)gys * nxp + gxs);
-                            }
-                        } else store_pairs((T*)a.Eout, ev);
-                    }
-                } else {
-                    store_pairs((T*)a.out, ov);
-                    if constexpr (STAGE == L3_S2) stg_vec<EW>((T*)a.out2 + 2 * ip, zv);   // Z is never a stencil source
-                }
+                store_pairs((T*)a.out, ov);
+                if constexpr (STAGE == L3_S2) stg_vec<EW>((T*)a.out2 + 2 * ip, zv);   // Z is never a stencil source
             }
         }
         // this warp is done with barrier b: stencil plane i - P and operand slot b may be refilled
