@@ -119,10 +119,12 @@ class ClockSampler:
 
 
 # ------------------------------------------------------------------ our arm
-def build_net(w, device, seed=1):
+def build_net(w, device, seed=1, method=None, y0_map=None):
     from paper_2410_19075_b200 import binding as B, configs
     y0, elem = make_inputs(w, seed)
-    net = B.Net.from_workload(w, device=device)
+    if y0_map is not None:
+        y0 = y0_map(y0)
+    net = B.Net.from_workload(w, device=device, method=B.METHOD_AUTO if method is None else method)
     net.set_state(y0)
     if elem is not None:
         net.set_param_array(B.PARAM_OMEGA if w.model == configs.KS else B.PARAM_IEXT, elem)
@@ -193,6 +195,36 @@ def measure(w, device, steps, warmup, e2e=True, seed=1):
     net.close()
     del net
     torch.cuda.empty_cache()
+    return out
+
+
+def rewrite_error(w, device):
+    """Error of the exact-in-mathematics rewrites of the coupling sum (run sums, prefix sums,
+    factorised sine, blocked gathers), measured on the GPU itself at the full size of the workload
+    (BASELINE.json item 3): max_v ||f_FAST - f_DIRECT||_inf / ||f_DIRECT||_inf of one
+    right-hand side, in the seeded incoherent state and in a nearly coherent one.  DIRECT is the
+    plain per-link form of Alg. 1 in the arithmetic type of the net."""
+    import numpy as np
+    from paper_2410_19075_b200 import binding as B, configs
+    out = {}
+    states = [("incoherent", None)]
+    if w.model != configs.HH:                  # HH gates are set to their steady state of V by the library
+        states.append(("coherent", lambda y: (y * 1e-2 + 0.3).astype(y.dtype)))
+    for name, ymap in states:
+        f = {}
+        for method in (B.METHOD_FAST, B.METHOD_DIRECT):
+            net, _ = build_net(w, device, method=method, y0_map=ymap)
+            f[method] = net.eval_rhs().astype(np.float64)
+            net.close()
+            del net
+        err = 0.0
+        for v in range(f[B.METHOD_FAST].shape[0]):
+            ref = np.abs(f[B.METHOD_DIRECT][v]).max()
+            if w.model == configs.HH:
+                ref = max(ref, 1.0)            # reading R11: gates start at steady state, f = 0 there
+            err = max(err, float(np.abs(f[B.METHOD_FAST][v] - f[B.METHOD_DIRECT][v]).max() / ref))
+        out[name] = err
+    out["norm"] = "max over variables of ||f_FAST - f_DIRECT||_inf / ||f_DIRECT||_inf, one RHS at full size, on the GPU"
     return out
 
 
@@ -377,6 +409,8 @@ def run_ours(args):
         line["with_observables"] = head["with_observables"]
     if getattr(w, "batch", 1) > 1:
         line["config"]["batch"] = w.batch
+    if rank == 0 and ws == 1 and not args.no_rewrite_error:
+        line["rewrite_error"] = rewrite_error(w, device)
     if rank == 0 and ws == 1 and not args.no_per_config:
         per = []
         for cfg in PER_CONFIG:
@@ -387,6 +421,8 @@ def run_ours(args):
             mc = measure(wc, device, k, max(3, args.warmup), e2e=True)
             e = line_for(wc, mc, k, 1)
             e["clocks"] = mc["clocks"]
+            if not args.no_rewrite_error:
+                e["rewrite_error"] = rewrite_error(wc, device)
             per.append(e)
         line["per_config"] = per
     if rank == 0 and ws == 1 and not args.no_cpu_baseline:
@@ -410,6 +446,7 @@ def main():
     ap.add_argument("--config", default=HEADLINE, choices=list(PER_CONFIG))
     ap.add_argument("--no-per-config", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-rewrite-error", action="store_true")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     return run_reference(args) if args.impl == "reference" else run_ours(args)
