@@ -169,10 +169,34 @@ __global__ void __launch_bounds__(RING_THREADS) ring_persistent_kernel(RingArgs 
         // ---- B: every chunk's prefix is visible
         if (SINGLE) __syncthreads();
         else grid_barrier(a.bar, (unsigned)((q + 1) * G));
+        // the chunk totals and the 4 E prefix values of this thread are requested together: both
+        // are in flight during the same L2 round trip
+        double c0 = 0.0, c1 = 0.0;
+        if (!SINGLE && threadIdx.x < G) { c0 = ld_l2(a.tot[buf] + threadIdx.x); c1 = ld_l2(a.tot[buf] + RING_GMAX + threadIdx.x); }
+        int64_t jh[E], jl[E];
+        int nwrap[E];
+        bool has_lo[E];
+#pragma unroll
+        for (int e = 0; e < E; ++e) {
+            const int64_t i = ok[e] ? i0 + e : 0;
+            int64_t hi = i + P, lo = i - P - 1;
+            int w = 0;
+            if (hi >= n) { hi -= n; ++w; }
+            if (lo < -1) { lo += n; ++w; }
+            has_lo[e] = lo >= 0;
+            jh[e] = hi; jl[e] = has_lo[e] ? lo : 0;
+            nwrap[e] = w;
+        }
+        T h0[E], h1[E], l0[E], l1[E];
+#pragma unroll
+        for (int e = 0; e < E; ++e) {
+            h0[e] = SINGLE ? Sg[jh[e]] : ld_l2(Sg + jh[e]);
+            h1[e] = SINGLE ? Sg[sstride + jh[e]] : ld_l2(Sg + sstride + jh[e]);
+            l0[e] = SINGLE ? Sg[jl[e]] : ld_l2(Sg + jl[e]);
+            l1[e] = SINGLE ? Sg[sstride + jl[e]] : ld_l2(Sg + sstride + jl[e]);
+        }
         // ---- C: block offsets
         if (!SINGLE) {
-            double c0 = threadIdx.x < G ? ld_l2(a.tot[buf] + threadIdx.x) : 0.0;
-            double c1 = threadIdx.x < G ? ld_l2(a.tot[buf] + RING_GMAX + threadIdx.x) : 0.0;
             const double v0 = c0, v1 = c1;
             double u0, u1;
             block_scan2<double>(c0, c1, u0, u1, wsumD);
@@ -187,28 +211,6 @@ __global__ void __launch_bounds__(RING_THREADS) ring_persistent_kernel(RingArgs 
         T k[E][NV];
         T W0v[E], W1v[E];
         {
-            int64_t jh[E], jl[E];
-            int nwrap[E];
-            bool has_lo[E];
-#pragma unroll
-            for (int e = 0; e < E; ++e) {
-                const int64_t i = ok[e] ? i0 + e : 0;
-                int64_t hi = i + P, lo = i - P - 1;
-                int w = 0;
-                if (hi >= n) { hi -= n; ++w; }
-                if (lo < -1) { lo += n; ++w; }
-                has_lo[e] = lo >= 0;
-                jh[e] = hi; jl[e] = has_lo[e] ? lo : 0;
-                nwrap[e] = w;
-            }
-            T h0[E], h1[E], l0[E], l1[E];
-#pragma unroll
-            for (int e = 0; e < E; ++e) {
-                h0[e] = SINGLE ? Sg[jh[e]] : ld_l2(Sg + jh[e]);
-                h1[e] = SINGLE ? Sg[sstride + jh[e]] : ld_l2(Sg + sstride + jh[e]);
-                l0[e] = SINGLE ? Sg[jl[e]] : ld_l2(Sg + jl[e]);
-                l1[e] = SINGLE ? Sg[sstride + jl[e]] : ld_l2(Sg + sstride + jl[e]);
-            }
 #pragma unroll
             for (int e = 0; e < E; ++e) {
                 double bt0 = 0.0, bt1 = 0.0;
