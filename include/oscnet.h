@@ -76,7 +76,9 @@ enum {
     NET_OBS_GLOBAL_ORDER = 1,        /* double[2] = {R, Psi}: R e^{i Psi} = (1/N) sum_j e^{i theta_j} */
     NET_OBS_LOCAL_ORDER = 2,         /* double[n]: R_i over the coupling neighbourhood plus i */
     NET_OBS_MEAN_PHASE_VELOCITY = 3, /* double[n] over the window of net_integrate_observed */
-    NET_OBS_STATS = 4                /* double[8], see net_integrate_observed */
+    NET_OBS_STATS = 4,               /* double[8], see net_integrate_observed */
+    NET_OBS_REPLICA_ORDER = 5        /* double[2*batch] = {R_r, Psi_r} of every replica r of a batch (batch = 1:
+                                      * the same as NET_OBS_GLOBAL_ORDER) */
 };
 
 /* Kuramoto-Sakaguchi, eq. (3) with m=0, eps=1, mu=K/Omega_i:

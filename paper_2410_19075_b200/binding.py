@@ -20,7 +20,7 @@ TOPO_RING, TOPO_LATTICE, TOPO_CSR, TOPO_RANDOM_INDEGREE = 0, 1, 2, 3
 F32, F64 = 0, 1
 METHOD_AUTO, METHOD_DIRECT, METHOD_FAST = 0, 1, 2
 PARAM_OMEGA, PARAM_IEXT = 0, 1
-OBS_PHASE, OBS_GLOBAL_ORDER, OBS_LOCAL_ORDER, OBS_MEAN_PHASE_VELOCITY, OBS_STATS = 0, 1, 2, 3, 4
+OBS_PHASE, OBS_GLOBAL_ORDER, OBS_LOCAL_ORDER, OBS_MEAN_PHASE_VELOCITY, OBS_STATS, OBS_REPLICA_ORDER = 0, 1, 2, 3, 4, 5
 NVAR = {MODEL_KS: 1, MODEL_FHN: 2, MODEL_HH: 4}
 
 ABI_SYMBOLS = [
@@ -353,7 +353,8 @@ class Net:
         return out
 
     def observable(self, what):
-        size = 2 if what == OBS_GLOBAL_ORDER else 8 if what == OBS_STATS else self.n
+        size = (2 if what == OBS_GLOBAL_ORDER else 8 if what == OBS_STATS else
+                2 * self.batch if what == OBS_REPLICA_ORDER else self.n)
         out = np.empty(size)
         net_observables(self.h, what, out.ctypes.data, False)
         return out

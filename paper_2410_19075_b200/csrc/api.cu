@@ -471,6 +471,13 @@ int32_t net_observables(net_t* h, int32_t what, void* dst, int32_t dst_is_device
             if ((rc = obs_global_order(h, theta, h->b.obs_acc + 8))) return rc;
             src = h->b.obs_acc + 8; bytes = 2 * sizeof(double);
             break;
+        case NET_OBS_REPLICA_ORDER:
+            // obs_loc (n doubles) receives the 2 * batch results; n >= 2 * batch since every ring has n >= 2
+            if (2 * (int64_t)h->desc.batch > h->n) return set_err(h, NET_ERR_UNSUPPORTED, "replica order parameter: rings of one element");
+            if ((rc = obs_phase(h, h->b.y, theta))) return rc;
+            if ((rc = obs_replica_order(h, theta, h->b.obs_loc))) return rc;
+            src = h->b.obs_loc; bytes = 2 * sizeof(double) * (size_t)h->desc.batch;
+            break;
         case NET_OBS_LOCAL_ORDER: {
             // obs_theta_prev doubles as theta scratch here (obs_tmp holds cos/sin); an observed
             // run re-initialises it at its first window sample

@@ -74,6 +74,26 @@ __global__ void reduce_finish_kernel(const double* __restrict__ partial, int nb,
     }
 }
 
+// Order parameter of every replica of a batch: CTA r reduces elements [r*rn, (r+1)*rn) in a fixed
+// order; out[2r] = R_r, out[2r+1] = Psi_r.
+__global__ void replica_order_kernel(const double* __restrict__ theta, int64_t rn, double* __restrict__ out) {
+    __shared__ double sh[8];
+    const double* th = theta + (int64_t)blockIdx.x * rn;
+    double a = 0, b = 0;
+    for (int64_t i = threadIdx.x; i < rn; i += blockDim.x) {
+        double s, c;
+        sincos(th[i], &s, &c);
+        a += c; b += s;
+    }
+    const double ra = block_sum(a, sh);
+    const double rb = block_sum(b, sh);
+    if (threadIdx.x == 0) {
+        const double c = ra / (double)rn, s = rb / (double)rn;
+        out[2 * blockIdx.x] = sqrt(c * c + s * s);
+        out[2 * blockIdx.x + 1] = atan2(s, c);
+    }
+}
+
 __global__ void cossin_kernel(const double* __restrict__ theta, int64_t n, double* __restrict__ cs) {
     for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n;
          i += (int64_t)gridDim.x * blockDim.x) {
@@ -133,6 +153,14 @@ static int32_t reduce(net* h, const double* x, int mode, const double* mean, dou
 
 int32_t obs_global_order(net* h, const double* d_theta, double* d_out2) {
     return reduce(h, d_theta, 0, nullptr, d_out2, nullptr);
+}
+
+int32_t obs_replica_order(net* h, const double* d_theta, double* d_out) {
+    const int batch = h->desc.batch > 0 ? h->desc.batch : 1;
+    replica_order_kernel<<<batch, RED_THREADS, 0, h->stream>>>(d_theta, h->n / batch, d_out);
+    h->launches += 1;
+    OSC_CUDA(h, cudaGetLastError());
+    return NET_OK;
 }
 
 int32_t obs_local_order(net* h, const double* d_theta, double* d_out) {

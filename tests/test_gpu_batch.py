@@ -72,3 +72,29 @@ def test_batch_on_other_topologies_is_refused():
     with pytest.raises(B.OscnetError) as ei:
         B.Net.from_workload(w)
     assert ei.value.code == -1
+
+
+def test_replica_order_parameter_matches_oracle_per_ring():
+    """NET_OBS_REPLICA_ORDER: {R_r, Psi_r} of every replica = the oracle's global order parameter of
+    that ring's phases alone; the ensemble value (NET_OBS_GLOBAL_ORDER) = the oracle's over all."""
+    from oracle import oracle as ora
+    for cfg, kw, batch in (("1", dict(n=256), 6), ("2", dict(n=1024), 3)):
+        w = _w(cfg, kw, batch)
+        inp = H.make_inputs(w, seed=9)
+        onet = H.make_oracle(w, inp)
+        net = H.make_gpu(w, inp)
+        net.integrate(20, w.dt)
+        y = net.get_state().astype(np.float64)
+        theta = net.observable(B.OBS_PHASE)
+        got = net.observable(B.OBS_REPLICA_ORDER).reshape(batch, 2)
+        ens = net.observable(B.OBS_GLOBAL_ORDER)
+        net.close()
+        th_ref = y[0] if w.model == configs.KS else np.arctan2(y[1], y[0])
+        np.testing.assert_allclose(theta, th_ref, atol=1e-13)
+        ring = ora.OracleNet.ks(w.n, *ora.topology_ring(w.n, w.radius), 1.0, 0.0, np.zeros(w.n))
+        for r in range(batch):
+            R, Psi = ring.global_order(th_ref[r * w.n:(r + 1) * w.n])
+            assert abs(got[r, 0] - R) < 1e-13
+            assert abs(np.angle(np.exp(1j * (got[r, 1] - Psi)))) < 1e-11
+        R, Psi = onet.global_order(th_ref)
+        assert abs(ens[0] - R) < 1e-13
