@@ -24,6 +24,9 @@ template <class T, int MODEL, int P> struct L3Sh {
     static constexpr int X = SPLIT ? 2 : L3Shape<T, P>::X;
     static constexpr int TY = SPLIT ? 2 : L3Shape<T, P>::TY;   // fp32 with TY = 4 measured slower (2.03e10 vs 2.30e10 on cfg 3a)
     static constexpr int UPW = SPLIT ? 16 : 32;      // blocks of X x TY outputs per consumer warp
+    // fp32 field-split: 7 consumer warps + producer, two CTAs per SM => 128 registers per thread
+    static constexpr int MAXT = (SPLIT && sizeof(T) == 4) ? 256 : L3_MAXT;
+    static constexpr int MINB = (SPLIT && sizeof(T) == 4) ? 2 : L3_MINB;
 };
 
 // Field-split kernel: extra columns of the staged box that make the shared-memory row pitch
@@ -97,7 +100,7 @@ static auto l3_kernel_ptr() {
     if constexpr (S::SPLIT) {
         // fp64, P = 4: rotating accumulators (small code, no spills); fp32: compile-time phases
         // measured faster (cfg 3a 2.26e10 vs 1.97e10)
-        return lat3s_kernel<T, P, STAGE, S::TY, L3_MAXT, L3_MINB, (P > 2 && sizeof(T) == 8)>;
+        return lat3s_kernel<T, P, STAGE, S::TY, S::MAXT, S::MINB, (P > 2 && sizeof(T) == 8)>;
     } else {
         return lat3_kernel<T, MODEL, P, STAGE, S::X, S::TY, L3_MAXT, L3_MINB, (P > 2 && sizeof(T) == 4)>;
     }
@@ -124,7 +127,7 @@ static int32_t l3_enumerate(int nx, int ny, int want_tx, int want_sy, F&& f) {
         const int tx = (nx + TXt - 1) / TXt;
         const int QX = TXt / X;
         if ((TXt + 2 * HX) * U8 > 256) { if (want_tx > 0) return NET_ERR_UNSUPPORTED; continue; }
-        for (int SY = 1; (SY * QX + S::UPW - 1) / S::UPW * 32 <= L3_MAXT - 32 && SY * TY <= 256 - 2 * P; ++SY) {
+        for (int SY = 1; (SY * QX + S::UPW - 1) / S::UPW * 32 <= S::MAXT - 32 && SY * TY <= 256 - 2 * P; ++SY) {
             if (want_sy > 0 && SY != want_sy) continue;
             const int TYt = SY * TY, ty = (ny + TYt - 1) / TYt;
             const int units = QX * SY, warps = (units + S::UPW - 1) / S::UPW;
@@ -346,7 +349,7 @@ static int32_t l3_stage(net* h, int stage, double dt, void* rhs_out) {
 // Tile autotuner ("measure, don't guess"): the score of l3_enumerate ranks tiles by geometry, but
 // bank conflicts, wave quantisation and the depth of the pipeline decide among the leaders (cfg 5:
 // 4.8e10 with the best-scoring tile, 5.3e10 with the best-measured one).  For nets large enough to
-// matter the best-scoring tile of each of the leading tile widths is timed on stages 1 and 2
+// matter the best-scoring tile of each of the leading tile widths is timed on one whole RK4 step
 // (zeroed buffers; net_create re-zeroes the state afterwards) and the fastest is kept.  The
 // arithmetic of every output is the same for every tile, so results do not depend on the pick.
 // OSCNET_LAT3 (explicit geometry) or OSCNET_NO_AUTOTUNE switch it off.
@@ -394,11 +397,11 @@ static int32_t l3_configure(net* h) {
         if (l3_configure_tile<T, MODEL, P>(h) != NET_OK) return false;
         float ms = 0.f;
         bool ok = true;
-        // one warm-up pass, then the fastest of four timed passes (a single pass is noisy enough to
+        // one warm-up pass, then the fastest of three timed passes (a single pass is noisy enough to
         // flip the ranking of tiles a few per cent apart)
-        for (int rep = 0; rep < 5 && ok; ++rep) {
+        for (int rep = 0; rep < 4 && ok; ++rep) {
             ok = cudaEventRecord(e0, h->stream) == cudaSuccess;
-            ok = ok && l3_stage<T, MODEL, P>(h, 1, 1e-3, nullptr) == NET_OK && l3_stage<T, MODEL, P>(h, 2, 1e-3, nullptr) == NET_OK;
+            for (int st = 0; st < 4 && ok; ++st) ok = l3_stage<T, MODEL, P>(h, st, 1e-3, nullptr) == NET_OK;   // one whole RK4 step
             float one = 0.f;
             ok = ok && cudaEventRecord(e1, h->stream) == cudaSuccess && cudaEventSynchronize(e1) == cudaSuccess &&
                  cudaEventElapsedTime(&one, e0, e1) == cudaSuccess;
@@ -409,17 +412,15 @@ static int32_t l3_configure(net* h) {
         *ms_out = ms;
         return ok;
     };
+    // every tile at three pipeline depths (the deepest that leaves 2, 3, 4 CTAs' worth of shared
+    // memory): deeper is not better -- cfg 3a, tile 40x8: D = 2 2.3e10, D = 4 2.0e10 osc-steps/s
     Cand best_c = Cand{0, 0, 0.0, 0};
-    for (int q = 0; q < nc; ++q) {
-        float ms;
-        if (time_cand(cand[q], &ms) && (best < 0 || ms < best_ms)) { best = q; best_ms = ms; best_c = cand[q]; }
-    }
-    if (best >= 0)                                           // shallower pipelines of the winner
-        for (int ctas = 3; ctas <= 4; ++ctas) {
-            Cand c = cand[best];
+    for (int q = 0; q < nc; ++q)
+        for (int ctas = 2; ctas <= 4; ++ctas) {
+            Cand c = cand[q];
             c.ctas = ctas;
             float ms;
-            if (time_cand(c, &ms) && ms < best_ms) { best_ms = ms; best_c = c; }
+            if (time_cand(c, &ms) && (best < 0 || ms < best_ms)) { best = q; best_ms = ms; best_c = c; }
         }
     cudaEventDestroy(e0);
     cudaEventDestroy(e1);
