@@ -25,6 +25,7 @@ template <class T, int MODEL, int P> struct L3Sh {
     static constexpr int TY = SPLIT ? 2 : L3Shape<T, P>::TY;   // fp32 with TY = 4 measured slower (2.03e10 vs 2.30e10 on cfg 3a)
     static constexpr int UPW = SPLIT ? 16 : 32;      // blocks of X x TY outputs per consumer warp
     // fp32 field-split: 7 consumer warps + producer, two CTAs per SM => 128 registers per thread
+    // (fp64 at 160 threads x 3 CTAs, 128 registers: 1.10e10 against 1.08e10 on cfg 3b -- not kept)
     static constexpr int MAXT = (SPLIT && sizeof(T) == 4) ? 256 : L3_MAXT;
     static constexpr int MINB = (SPLIT && sizeof(T) == 4) ? 2 : L3_MINB;
 };
