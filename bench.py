@@ -179,6 +179,13 @@ def measure(w, device, steps, warmup, e2e=True, seed=1):
         replicas.barrier()
         out.update(e2e_ms=ev0.elapsed_time(ev1), h2d=host_in.numel() * host_in.element_size(),
                    d2h=host_out.numel() * host_out.element_size())
+    # ring nets are bound by the dependent chain of a stage: probe its primitives (SURVEY.md 8(d) ii)
+    from paper_2410_19075_b200 import configs as _cfgs
+    if w.topo == _cfgs.RING and getattr(w, "batch", 1) == 1 and method == 2:
+        try:
+            out["latency"] = net.probe_latency()
+        except Exception as exc:               # diagnostic only
+            out["latency"] = {"error": str(exc)}
     # the same step with the workload's observables switched on (global / local order parameter and
     # mean phase velocity sampled every obs_every RK4 steps; reported separately)
     if e2e:
@@ -367,6 +374,19 @@ def line_for(w, m, steps, n_gpus, units_total=None, ms_max=None):
     if "e2e_ms" in m:
         out["e2e"] = {"value": ntot(w) * rk4 * n_gpus / (m["e2e_ms"] * 1e-3), "unit": METRIC,
                       "h2d_bytes_per_step": m["h2d"], "d2h_bytes_per_step": m["d2h"]}
+    if "latency" in m and "error" not in m["latency"]:
+        from paper_2410_19075_b200 import configs as _cfgs
+        L = m["latency"]
+        stage_us = ms * 1e3 / (rk4 * 4)
+        # dependent chain of one stage of the persistent ring kernel: scan of the fields, grid barrier,
+        # one L2 round trip (totals + prefix values), scan of the totals (multi-CTA nets only), and for
+        # KS one fp64 sincos of the new phase
+        floor = L["block_scan_us"] + (L["fp64_sincos_us"] if w.model == _cfgs.KS else 0.0)
+        if L["grid_barrier_us"] > 0:
+            floor += L["grid_barrier_us"] + L["l2_round_trip_us"] + L["block_scan_us"]
+        out["latency_model"] = dict(L, stage_floor_us=floor, stage_us=stage_us, frac=floor / stage_us,
+                                    what="measured latencies of the primitives one stage chains (net_probe_latency); "
+                                         "frac = their sum / measured time per RK4 stage")
     if "obs_ms" in m:
         out["with_observables"] = {"value": ntot(w) * rk4 * n_gpus / (m["obs_ms"] * 1e-3), "unit": METRIC,
                                    "obs_every": w.obs_every,
@@ -407,6 +427,8 @@ def run_ours(args):
             "gpu_launches": m["launches"], "roofline": head["roofline"]}
     if "with_observables" in head and ws == 1:
         line["with_observables"] = head["with_observables"]
+    if "latency_model" in head and ws == 1:
+        line["latency_model"] = head["latency_model"]
     if getattr(w, "batch", 1) > 1:
         line["config"]["batch"] = w.batch
     if rank == 0 and ws == 1 and not args.no_rewrite_error:

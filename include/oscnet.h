@@ -228,6 +228,13 @@ int32_t net_synchronize(net_t* net);
 const char* net_last_error(const net_t* net);
 
 /* "oscnet <major>.<minor> sm_100a" */
+/* Diagnostic: latencies of the primitives one stage of a latency-bound (ring) net chains, measured on
+ * the net's stream with the net's scratch memory ("fraction of a measured latency
+ * model").  out4 (host, microseconds each) = {grid barrier over the CTAs this net's persistent kernel
+ * uses (0 for single-CTA nets), one dependent load served by L2, one 256-thread block scan of two
+ * doubles, one dependent fp64 sincos}.  Synchronises the stream; the state is not touched. */
+int32_t net_probe_latency(net_t* net, double* out4);
+
 const char* net_version(void);
 
 #ifdef __cplusplus

@@ -28,6 +28,7 @@ ABI_SYMBOLS = [
     "net_set_param_array", "net_hh_steady_gates", "net_integrate", "net_integrate_observed",
     "net_eval_rhs", "net_observables", "net_get_topology", "net_get_degree", "net_get_time",
     "net_set_time", "net_get_counters", "net_get_kernel_family", "net_synchronize", "net_last_error", "net_version",
+    "net_probe_latency",
 ]
 
 
@@ -99,6 +100,7 @@ def lib():
         L.net_set_time.argtypes = [C.c_void_p, C.c_double, C.c_int64]
         L.net_get_counters.argtypes = [C.c_void_p, C.POINTER(C.c_int64), C.POINTER(C.c_int32)]
         L.net_synchronize.argtypes = [C.c_void_p]
+        L.net_probe_latency.argtypes = [C.c_void_p, C.POINTER(C.c_double)]
         for name in ABI_SYMBOLS:
             if name not in ("net_last_error", "net_version"):
                 getattr(L, name).restype = C.c_int32
@@ -197,6 +199,12 @@ def net_get_kernel_family(h):
     f = C.c_int32()
     _check(lib().net_get_kernel_family(h, C.byref(f)), h)
     return f.value
+
+
+def net_probe_latency(h):
+    out = (C.c_double * 4)()
+    _check(lib().net_probe_latency(h, out), h)
+    return dict(grid_barrier_us=out[0], l2_round_trip_us=out[1], block_scan_us=out[2], fp64_sincos_us=out[3])
 
 
 def net_synchronize(h):
@@ -383,6 +391,9 @@ class Net:
 
     def kernel_family(self):
         return net_get_kernel_family(self.h)
+
+    def probe_latency(self):
+        return net_probe_latency(self.h)
 
     def synchronize(self):
         net_synchronize(self.h)

@@ -293,6 +293,11 @@ extern "C" {
 
 const char* net_version(void) { return "oscnet 0.1 sm_100a"; }
 
+int32_t net_probe_latency(net_t* h, double* out4) {
+    if (!h || !out4) return set_err(h, NET_ERR_INVALID, "net or out4 is NULL");
+    return ring_probe_latency(h, out4);
+}
+
 const char* net_last_error(const net_t* h) { return h ? h->err : g_err; }
 
 int32_t net_workspace_bytes(const net_desc* desc, size_t* bytes) {

@@ -373,6 +373,99 @@ static int32_t ring_run_plan(net* h, const RingPlan& p, const void* y_in, void* 
     return f32 ? ring_launch_e<float, NET_MODEL_FHN>(h, a, p) : ring_launch_e<double, NET_MODEL_FHN>(h, a, p);
 }
 
+// ------------------------------------------------------------------ latency probes
+// The ring configs are bound by the dependent chain of one stage, not by bytes or flops
+// (SURVEY.md 8(d)): block scan -> grid barrier -> one L2 round trip -> scan of the totals ->
+// local field (KS: one fp64 sincos).  These kernels time exactly those primitives, as the ring
+// kernel uses them, so that bench.py can quote the stage time against a measured floor.
+__global__ void __launch_bounds__(RING_THREADS) probe_barrier_kernel(unsigned* bar, int iters, int G) {
+    for (int it = 0; it < iters; ++it) grid_barrier(bar, (unsigned)(it + 1) * (unsigned)G);
+}
+__global__ void probe_ring_init_kernel(unsigned* ring, unsigned n, unsigned stride) {
+    for (unsigned i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) ring[i] = (i + stride) % n;
+}
+__global__ void probe_l2_kernel(const unsigned* ring, int iters, unsigned* sink) {
+    unsigned j = 0;
+    for (int it = 0; it < iters; ++it) j = __ldcg(ring + j);      // dependent loads served by L2
+    *sink = j;
+}
+__global__ void __launch_bounds__(RING_THREADS) probe_scan_kernel(int iters, double* sink) {
+    __shared__ double wsum[2][RING_THREADS / 32];
+    double a = 1.0 + threadIdx.x, b = 2.0, ta = 0, tb = 0;
+    for (int it = 0; it < iters; ++it) {
+        block_scan2<double>(a, b, ta, tb, wsum);
+        a = a * 1e-9 + ta * 1e-9; b = b * 1e-9 + tb * 1e-9;         // the next scan depends on this one
+    }
+    if (threadIdx.x == 0) *sink = a + b;
+}
+__global__ void probe_sincos_kernel(int iters, double x, double* sink) {
+    for (int it = 0; it < iters; ++it) {
+        double s, c;
+        sincos(x, &s, &c);
+        x += 1e-3 * s + 1e-3 * c;                                   // dependent chain
+    }
+    *sink = x;
+}
+
+// out[0] grid barrier over the CTAs of this net's ring plan (1 CTA: 0), out[1] dependent L2 load,
+// out[2] block scan of two doubles (256 threads), out[3] dependent fp64 sincos; microseconds each.
+int32_t ring_probe_latency(net* h, double* out) {
+    RingPlan p;
+    // only nets served by the persistent ring kernel: their scratch is rewritten by every launch
+    // (the scratch of a lattice net holds its exchange fields)
+    if (!(h->fast_kind == FAST_RING_KS || h->fast_kind == FAST_RING_FHN) ||
+        !ring_plan(h->tv.ring_n, h->esize, &p, h->desc.batch > 1 ? 1 : 148))
+        return set_err(h, NET_ERR_UNSUPPORTED, "latency probes: ring nets on the FAST path only");
+    const int G = p.G;
+    char* s = (char*)h->b.scratch;
+    const unsigned N = 1u << 20;                                     // 4 MB ring of indices, L2 resident
+    if (h->b.scratch_bytes < (size_t)N * 4 + 1024) return set_err(h, NET_ERR_SIZE, "scratch too small for the probes");
+    unsigned* ring = (unsigned*)s;
+    unsigned* bar = (unsigned*)(s + (size_t)N * 4);
+    double* sink = (double*)(s + (size_t)N * 4 + 256);
+    cudaStream_t st = h->stream;
+    cudaEvent_t e0, e1;
+    OSC_CUDA(h, cudaEventCreate(&e0));
+    OSC_CUDA(h, cudaEventCreate(&e1));
+    const int iters = 2000;
+    auto timed = [&](auto&& launch, double* us) -> int32_t {
+        float ms = 0.f;
+        for (int rep = 0; rep < 2; ++rep) {                          // rep 0 warms up
+            cudaEventRecord(e0, st);
+            int32_t rc = launch();
+            if (rc) return rc;
+            cudaEventRecord(e1, st);
+            OSC_CUDA(h, cudaEventSynchronize(e1));
+            OSC_CUDA(h, cudaEventElapsedTime(&ms, e0, e1));
+        }
+        *us = (double)ms * 1e3 / iters;
+        return NET_OK;
+    };
+    int32_t rc = NET_OK;
+    out[0] = 0.0;
+    if (G > 1) {
+        rc = timed([&]() -> int32_t {
+            OSC_CUDA(h, cudaMemsetAsync(bar, 0, sizeof(unsigned), st));
+            int it = iters, g = G;
+            void* params[] = {&bar, &it, &g};
+            OSC_CUDA(h, cudaLaunchCooperativeKernel((const void*)probe_barrier_kernel, dim3(G), dim3(RING_THREADS), params, 0, st));
+            return NET_OK;
+        }, &out[0]);
+    }
+    if (rc == NET_OK) {
+        probe_ring_init_kernel<<<296, 256, 0, st>>>(ring, N, 16411u);
+        rc = timed([&]() -> int32_t { probe_l2_kernel<<<1, 1, 0, st>>>(ring, iters, (unsigned*)sink); OSC_CUDA(h, cudaGetLastError()); return NET_OK; }, &out[1]);
+    }
+    if (rc == NET_OK)
+        rc = timed([&]() -> int32_t { probe_scan_kernel<<<1, RING_THREADS, 0, st>>>(iters, sink); OSC_CUDA(h, cudaGetLastError()); return NET_OK; }, &out[2]);
+    if (rc == NET_OK)
+        rc = timed([&]() -> int32_t { probe_sincos_kernel<<<1, 1, 0, st>>>(iters, 0.3, sink); OSC_CUDA(h, cudaGetLastError()); return NET_OK; }, &out[3]);
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    h->launches += 9;
+    return rc;
+}
+
 int32_t ring_run(net* h, const void* y_in, void* y_out, int64_t n_steps, double dt, int rhs_only) {
     RingPlan p;
     // (two CTAs per SM -- gmax = 296, half the elements per thread -- measured slower on config 2:

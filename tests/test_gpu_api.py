@@ -72,3 +72,31 @@ def test_errors_are_reported_not_thrown():
     assert e.value.code == -2
     launches, method = net.counters()
     assert launches >= 1 and method in (B.METHOD_DIRECT, B.METHOD_FAST)
+
+
+@pytest.mark.gpu
+def test_latency_probe_is_a_ring_diagnostic_and_leaves_the_state_alone():
+    """net_probe_latency: four positive latencies for a ring net on the FAST path (the grid barrier
+    is 0 for a single-CTA ring), state and results untouched; refused for other nets."""
+    import numpy as np
+    import harness as H
+    from paper_2410_19075_b200 import binding as B, configs
+    for cfg, kw, multi in (("1", {}, False), ("2", dict(n=8192), True)):
+        w = configs.get(cfg, **kw)
+        inp = H.make_inputs(w, seed=2)
+        net = H.make_gpu(w, inp)
+        before = net.get_state()
+        L = net.probe_latency()
+        assert (L["grid_barrier_us"] > 0) == multi
+        assert 0 < L["l2_round_trip_us"] < 5 and 0 < L["block_scan_us"] < 5 and 0 < L["fp64_sincos_us"] < 5
+        assert np.array_equal(net.get_state(), before)
+        net.integrate(10, w.dt)
+        ref = H.make_gpu(w, inp)
+        ref.integrate(10, w.dt)
+        assert np.array_equal(net.get_state(), ref.get_state())
+        net.close(); ref.close()
+    lat = H.make_gpu(configs.get("5", n1=16), H.make_inputs(configs.get("5", n1=16)))
+    with pytest.raises(B.OscnetError) as ei:
+        lat.probe_latency()
+    assert ei.value.code == -5
+    lat.close()
