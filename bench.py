@@ -266,7 +266,8 @@ def roofline_object(w, m, steps):
     else:
         per_launch = c["ops"] * ntot(w) * rk4 / max(1, m["launches"])
         achieved, peak, unit = per_launch / avg_launch_s / 1e9, pk[c["pipe"] + "_ginstr_s"], "Ginstr/s"
-        peak_src = "148 SM x %d lanes x sm_max_mhz (%s pipe)" % (R.LANES[c["pipe"]], c["pipe"])
+        peak_src = ("148 SM x %d lanes x sm_max_mhz (%s)" %
+                    (R.LANES[c["pipe"]], "issue slots, all pipes" if c["pipe"] == "issue" else c["pipe"] + " pipe"))
     return {"bound": c["bound"], "achieved": achieved, "peak": peak, "unit": unit,
             "frac": achieved / peak, "traffic": ncu_traffic(w.cfg),
             "kernel": "fused RHS+RK4 stage kernel",
@@ -274,6 +275,7 @@ def roofline_object(w, m, steps):
             "avg_launch_us": avg_launch_s * 1e6, "peak_source": peak_src,
             "bytes_per_osc_step": R.bytes_per_osc_step(w),
             "survey_bytes_per_osc_step": R.survey_bytes_per_osc_step(w),
+            "ops_per_osc_step": c["ops"], "ops_pipe": c["pipe"],
             "ceiling_osc_steps_per_s": c["osc_steps_per_s"],
             "frac_of_ceiling": (ntot(w) * rk4 / sec) / c["osc_steps_per_s"]}
 

@@ -11,7 +11,8 @@ FALLBACK_HBM_GBS = 6650.0
 SM_COUNT = 148
 SM_MAX_MHZ_NOMINAL = 1965.0
 # issue rates per SM per clock (lanes): FP32 FMA pipe 128, FP64 64, MUFU (SFU) 16
-LANES = {"fp32": 128, "fp64": 64, "mufu": 16}
+# "issue": warp instructions of all pipes, 4 schedulers x 32 lanes per SM and clock
+LANES = {"fp32": 128, "fp64": 64, "mufu": 16, "issue": 128}
 
 
 def peaks():
@@ -79,9 +80,10 @@ def ops_per_osc_step(w):
     if w.cfg == "2":
         return ("fp64", 4 * 60)
     if w.cfg == "1b":
-        # shipped (prefix-sum) formulation per stage: fp64 sincos ~110, block scan of two fields ~30,
-        # window differences + local field + RK4 update ~20
-        return ("fp64", 4 * 160)
+        # measured, not estimated (profiles/r01_split_ncu.md, cfg 1b): 275 instructions of all pipes
+        # per element and stage, 72 of them on the FP64 pipe (sincos, scan, window sums, RK4) -- the
+        # batch is bound by instruction issue (74 % of the slots), the FP64 pipe is 39 % busy
+        return ("issue", 4 * 275)
     return ("fp64", 4 * (110 + 2 * 2 * w.radius))
 
 
