@@ -12,8 +12,8 @@ import numpy as np
 
 from .build import build
 
-MODEL_KS, MODEL_FHN, MODEL_HH = 0, 1, 2
-NVAR = {MODEL_KS: 1, MODEL_FHN: 2, MODEL_HH: 4}
+MODEL_KS, MODEL_FHN, MODEL_HH, MODEL_KSI = 0, 1, 2, 3
+NVAR = {MODEL_KS: 1, MODEL_FHN: 2, MODEL_HH: 4, MODEL_KSI: 2}
 
 _lib = None
 
@@ -124,6 +124,12 @@ class OracleNet:
     @classmethod
     def ks(cls, n, row_ptr, col_idx, K, alpha, omega):
         return cls(MODEL_KS, n, row_ptr, col_idx, [K, alpha], omega)
+
+    @classmethod
+    def ksi(cls, n, row_ptr, col_idx, K, alpha, m, eps, omega=0.0):
+        """Kuramoto-Sakaguchi with inertia, eq. (3) PAPER.md:79 in full; state [phi | phi']
+        (oracle of the next row, SURVEY.md 8(f).1 -- not on the GPU path yet)."""
+        return cls(MODEL_KSI, n, row_ptr, col_idx, [K, alpha, m, eps], omega)
 
     @classmethod
     def fhn(cls, n, row_ptr, col_idx, eps, a, sigma, phi):

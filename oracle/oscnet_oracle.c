@@ -30,6 +30,8 @@
  *       on uniform states, zero-sum coupling, dense brute force.
  *   ora_rhs (HH)  : hand-computed rate values at V=-65 mV, rest state near the
  *       textbook -65 mV / m=0.0529 h=0.5961 n=0.3177, dense brute force.
+ *   ora_rhs (KSI) : (oracle of the NEXT row; not on the GPU path yet) dense
+ *       brute force, in-phase state, momentum balance for alpha=0, damped closed form for K=0.
  *   ora_rk4       : 4th-order convergence against a 16x finer step; exactness
  *       for constant RHS.
  *   ora_local_order, phase maps : R=1 for identical phases, splay state R=0.
@@ -44,6 +46,7 @@
 #define ORA_MODEL_KS 0
 #define ORA_MODEL_FHN 1
 #define ORA_MODEL_HH 2
+#define ORA_MODEL_KSI 3   /* Kuramoto-Sakaguchi with inertia, eq. (3) in full (next row) */
 
 /* ------------------------------------------------------------------ */
 /* Topology: canonical CSR, rows = in-neighbour lists (PAPER.md:147:    */
@@ -192,7 +195,8 @@ typedef struct {
 } ora_net;
 
 int32_t ora_nvar(int32_t model) {
-    return model == ORA_MODEL_KS ? 1 : model == ORA_MODEL_FHN ? 2 : model == ORA_MODEL_HH ? 4 : -1;
+    return model == ORA_MODEL_KS ? 1 : model == ORA_MODEL_FHN ? 2 : model == ORA_MODEL_HH ? 4 :
+           model == ORA_MODEL_KSI ? 2 : -1;
 }
 
 /* Kuramoto-Sakaguchi (eq. (3) with m=0, eps=1, mu=1/Omega, PAPER.md:79, :107;
@@ -215,6 +219,37 @@ static void rhs_ks(const ora_net* net, const double* y, double* f) {
         }
         if (links_amount > 0) der /= (double)links_amount;
         f[i] = net->elem_param[i] + K * der;
+    }
+}
+
+/* Kuramoto-Sakaguchi with inertia, eq. (3) PAPER.md:79 in full:
+ *   m phi_i'' + eps phi_i' = mu sum_j L_ij sin(phi_j - phi_i - alpha),
+ * the model of the paper's own performance tests (Fig. 6c: m = 1,
+ * eps = 0.05, mu = 0.01, 3D ball of radius 2 / 4 / 6).  As a first-order system in (phi, psi = phi'):
+ *   phi_i' = psi_i
+ *   psi_i' = ( -eps psi_i + omega_i + (K/Omega_i) sum_{j in row i} sin(phi_j - phi_i - alpha) ) / m
+ * with the coupling normalised as in rhs_ks (K/Omega_i = mu; reading R2) and an optional constant
+ * torque omega_i (0 in the paper).  State SoA [phi | psi].  p = {K, alpha, m, eps}.
+ * Pins (tests/test_oracle_dynamics.py): dense brute force, in-phase state, momentum balance
+ * sum_i psi_i' = -(eps/m) sum_i psi_i + sum_i omega_i / m for alpha = 0 on symmetric topologies, the
+ * damped closed form for K = 0 within the RK4 truncation error, reduction to rhs_ks as m -> 0 is
+ * NOT used (singular limit).  NOT YET on the GPU path: this is the oracle of the next row only. */
+static void rhs_ksi(const ora_net* net, const double* y, double* f) {
+    const int64_t n = net->n;
+    const double K = net->p[0], alpha = net->p[1], m = net->p[2], eps = net->p[3];
+    const double* phi = y;
+    const double* psi = y + n;
+#pragma omp parallel for schedule(static)
+    for (int64_t i = 0; i < n; ++i) {
+        double der = 0.0;
+        int64_t links_amount = 0;
+        for (int64_t e = net->row_ptr[i]; e < net->row_ptr[i + 1]; ++e, ++links_amount) {
+            int32_t j = net->col_idx[e];
+            der += sin(phi[j] - phi[i] - alpha);
+        }
+        if (links_amount > 0) der /= (double)links_amount;
+        f[i] = psi[i];
+        f[n + i] = (-eps * psi[i] + net->elem_param[i] + K * der) / m;
     }
 }
 
@@ -301,6 +336,7 @@ int ora_rhs(const ora_net* net, const double* y, double* f) {
         case ORA_MODEL_KS: rhs_ks(net, y, f); return 0;
         case ORA_MODEL_FHN: rhs_fhn(net, y, f); return 0;
         case ORA_MODEL_HH: rhs_hh(net, y, f); return 0;
+        case ORA_MODEL_KSI: rhs_ksi(net, y, f); return 0;
     }
     return -1;
 }
@@ -355,7 +391,7 @@ int ora_rk4(const ora_net* net, double* y, int64_t n_steps, double dt) {
  * (V - V_c)/V_s); pm = {V_c, n_c, V_s}. */
 void ora_phase(int32_t model, int64_t n, const double* y, const double* pm, double* theta) {
     for (int64_t i = 0; i < n; ++i) {
-        if (model == ORA_MODEL_KS)
+        if (model == ORA_MODEL_KS || model == ORA_MODEL_KSI)
             theta[i] = y[i];
         else if (model == ORA_MODEL_FHN)
             theta[i] = atan2(y[n + i], y[i]);

@@ -337,3 +337,93 @@ def test_mean_phase_velocity_uncoupled():
     k = int(round(2 * (tc[-1] - tc[0])))              # a whole number of periods, in steps
     st = net.run_statistics(y, 2 * k, 0.005, 4)
     assert abs(2 * np.pi / abs(st["vel"][0]) - period) < 2e-3 * period
+
+
+# ------------------------------------------------------------------ KS with inertia (next row)
+# eq. (3) PAPER.md:79 in full, m phi'' + eps phi' = mu sum_j L_ij sin(phi_j - phi_i - alpha): the
+# oracle of SURVEY.md 8(f).1, written and pinned before any kernel for it exists.
+
+@pytest.mark.parametrize("name,n,rp,ci", TOPOS, ids=[t[0] for t in TOPOS])
+def test_ksi_dense_brute_force(name, n, rp, ci):
+    K, alpha, m, eps = 0.8, 0.45, 1.3, 0.05
+    om = RNG.normal(size=n)
+    net = ora.OracleNet.ksi(n, rp, ci, K, alpha, m, eps, om)
+    y = RNG.normal(size=(2, n))
+    phi, psi = y
+    L = _dense(rp, ci, n)
+    S = (L * np.sin(phi[None, :] - phi[:, None] - alpha)).sum(axis=1)
+    deg = L.sum(axis=1)
+    ref_psi = (-eps * psi + om + K * S / np.maximum(deg, 1)) / m
+    f = net.rhs(y)
+    np.testing.assert_allclose(f[0], psi, atol=0, rtol=0)            # phi' = psi exactly
+    np.testing.assert_allclose(f[1], ref_psi, atol=1e-13)
+
+
+def test_ksi_in_phase_state():
+    """All phases equal: every link contributes sin(-alpha), so psi' = (-eps psi - K sin(alpha))/m for
+    every element (self link excluded), whatever the topology."""
+    K, alpha, m, eps = 1.1, 0.3, 2.0, 0.07
+    for name, n, rp, ci in TOPOS:
+        net = ora.OracleNet.ksi(n, rp, ci, K, alpha, m, eps)
+        y = np.stack([np.full(n, 0.9), np.full(n, -0.4)])
+        f = net.rhs(y)
+        np.testing.assert_allclose(f[1], (-eps * -0.4 - K * math.sin(alpha)) / m, atol=1e-15)
+        np.testing.assert_allclose(f[0], -0.4, atol=0)
+
+
+def test_ksi_momentum_balance_alpha0():
+    """alpha = 0 on a symmetric topology with uniform degree: the coupling terms cancel pairwise,
+    sum_i psi_i' = -(eps/m) sum_i psi_i + sum_i omega_i / m."""
+    K, m, eps = 0.9, 1.7, 0.05
+    for name, n, rp, ci in TOPOS[:3]:                      # ring and lattices are symmetric
+        om = RNG.normal(size=n)
+        net = ora.OracleNet.ksi(n, rp, ci, K, 0.0, m, eps, om)
+        y = RNG.normal(size=(2, n))
+        f = net.rhs(y)
+        assert abs(f[1].sum() - (-(eps / m) * y[1].sum() + om.sum() / m)) < 1e-12
+
+
+def test_ksi_uncoupled_damped_closed_form():
+    """K = 0: psi(t) = psi_inf + (psi0 - psi_inf) e^{-eps t / m}, psi_inf = omega / eps, and
+    phi(t) = phi0 + psi_inf t + (psi0 - psi_inf)(m/eps)(1 - e^{-eps t/m}).  RK4 reproduces it to its
+    truncation error, (eps dt / m)^5 / 120 per step relative to the transient -- 1e-11 here."""
+    n, m, eps, dt, steps = 8, 1.0, 0.5, 0.01, 400
+    rp, ci = ora.topology_ring(n, 2)
+    om = RNG.normal(size=n) * 0.2
+    net = ora.OracleNet.ksi(n, rp, ci, 0.0, 0.45, m, eps, om)
+    y0 = RNG.normal(size=(2, n))
+    y = net.rk4(y0, steps, dt)
+    t = steps * dt
+    pinf = om / eps
+    decay = math.exp(-eps * t / m)
+    psi = pinf + (y0[1] - pinf) * decay
+    phi = y0[0] + pinf * t + (y0[1] - pinf) * (m / eps) * (1 - decay)
+    np.testing.assert_allclose(y[1], psi, atol=1e-11)
+    np.testing.assert_allclose(y[0], phi, atol=1e-11)
+
+
+def test_ksi_rk4_fourth_order_and_energy_dissipation():
+    """Coupled case: halving dt divides the error against a 16x finer run by 16 +- 2; and for
+    alpha = 0, omega = 0 the energy  E = (m/2) sum psi^2 - (K/(2 Omega)) sum_ij L_ij cos(phi_j - phi_i)
+    decreases monotonically (dE/dt = -eps sum psi^2 <= 0) along the oracle trajectory."""
+    n, P = 11, 2
+    rp, ci = ora.topology_ring(n, P)
+    K, m, eps = 1.0, 1.0, 0.05
+    net = ora.OracleNet.ksi(n, rp, ci, K, 0.45, m, eps)
+    y0 = RNG.normal(size=(2, n))
+    T = 1.0
+    ref = net.rk4(y0, 1600, T / 1600)
+    errs = [np.abs(net.rk4(y0, k, T / k) - ref).max() for k in (25, 50, 100)]
+    assert 14.0 < errs[0] / errs[1] < 18.0 and 14.0 < errs[1] / errs[2] < 18.0
+    net0 = ora.OracleNet.ksi(n, rp, ci, K, 0.0, m, eps)
+    L = _dense(rp, ci, n)
+
+    def energy(y):
+        phi, psi = y
+        return 0.5 * m * (psi ** 2).sum() - K / (2.0 * 2 * P) * (L * np.cos(phi[None, :] - phi[:, None])).sum()
+
+    y, E = y0.copy(), []
+    for _ in range(40):
+        E.append(energy(y))
+        y = net0.rk4(y, 10, 0.01)
+    assert all(E[q + 1] < E[q] for q in range(len(E) - 1))
