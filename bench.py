@@ -28,9 +28,9 @@ if ROOT not in sys.path:
 
 METRIC = "oscillator-steps/s"
 HEADLINE = "5"
-PER_CONFIG = ("1", "1b", "2", "3a", "3b", "4", "5")   # 1b: config 1 as a batch of nets (extra, SURVEY.md 8(d) iii)
+PER_CONFIG = ("1", "1b", "2", "3a", "3b", "4", "5", "6")   # 1b: config 1 as a batch of nets (extra, SURVEY.md 8(d) iii)
 # RK4 steps per bench step (= per net_integrate call)
-BENCH_RK4 = {"1": 1000, "1b": 1000, "2": 200, "3a": 10, "3b": 10, "4": 100, "5": 10}
+BENCH_RK4 = {"6": 10, "1": 1000, "1b": 1000, "2": 200, "3a": 10, "3b": 10, "4": 100, "5": 10}
 
 
 def ntot(w):
@@ -50,6 +50,8 @@ def make_inputs(w, seed=1):
         y0 = inputs.ks_phases(ntot(w), seed).reshape(1, -1)
         if w.extra.get("omega") == "lorentzian":
             elem = inputs.lorentzian_omega(ntot(w), seed, w.extra["gamma"], w.extra["omega_max"])
+    elif w.model == configs.KSI:
+        y0 = np.stack([inputs.ks_phases(ntot(w), seed), 0.05 * inputs.fhn_circle(ntot(w), seed)[0]])
     elif w.model == configs.FHN:
         y0 = inputs.fhn_circle(ntot(w), seed)
     else:
@@ -127,7 +129,7 @@ def build_net(w, device, seed=1, method=None, y0_map=None):
     net = B.Net.from_workload(w, device=device, method=B.METHOD_AUTO if method is None else method)
     net.set_state(y0)
     if elem is not None:
-        net.set_param_array(B.PARAM_OMEGA if w.model == configs.KS else B.PARAM_IEXT, elem)
+        net.set_param_array(B.PARAM_OMEGA if w.model in (configs.KS, configs.KSI) else B.PARAM_IEXT, elem)
     if w.model == configs.HH:
         net.hh_steady_gates()
         y0 = net.get_state()                # full initial state (gates included) for the e2e leg
@@ -214,6 +216,8 @@ def rewrite_error(w, device):
     import numpy as np
     from paper_2410_19075_b200 import binding as B, configs
     out = {}
+    if w.model == configs.KSI:                 # DIRECT only in this build: no rewrite to measure
+        return {"note": "served by the DIRECT (per-link) form; no rewrite"}
     states = [("incoherent", None)]
     if w.model != configs.HH:                  # HH gates are set to their steady state of V by the library
         states.append(("coherent", lambda y: (y * 1e-2 + 0.3).astype(y.dtype)))

@@ -58,7 +58,8 @@ enum {
     NET_ERR_UNSUPPORTED = -5  /* valid request this build does not implement (e.g. batch > 1 on a lattice) */
 };
 
-enum { NET_MODEL_KS = 0, NET_MODEL_FHN = 1, NET_MODEL_HH = 2 };
+enum { NET_MODEL_KS = 0, NET_MODEL_FHN = 1, NET_MODEL_HH = 2,
+       NET_MODEL_KSI = 3 /* KS with inertia; NET_METHOD_DIRECT only in this build */ };
 enum { NET_TOPO_RING = 0, NET_TOPO_LATTICE = 1, NET_TOPO_CSR = 2, NET_TOPO_RANDOM_INDEGREE = 3 };
 enum { NET_F32 = 0, NET_F64 = 1 };
 
@@ -87,6 +88,17 @@ enum {
 typedef struct {
     double K, alpha, omega0;
 } net_ks_params;
+
+/* Kuramoto-Sakaguchi with inertia, eq. (3) in full (the model of the paper's performance
+ * tests), as a first-order system in (phi, psi = dphi/dt), nvar = 2:
+ *   dphi_i/dt = psi_i
+ *   dpsi_i/dt = ( -eps psi_i + omega_i + (K/Omega_i) sum_{j in row i} sin(phi_j - phi_i - alpha) ) / m
+ * (K/Omega_i = the paper's mu; omega_i = omega0 until net_set_param_array(NET_PARAM_OMEGA), 0 in the
+ * paper).  State [phi | psi].  Served by NET_METHOD_DIRECT (the per-link form of Alg. 1) on every
+ * topology; NET_METHOD_FAST returns NET_ERR_UNSUPPORTED in this build. */
+typedef struct {
+    double K, alpha, m, eps, omega0;
+} net_ksi_params;
 
 /* FitzHugh-Nagumo, eq. (2) with rotated 2x2 diffusive coupling:
  *   eps du_i/dt = u_i - u_i^3/3 - v_i + (sigma/Omega_i) sum_j [b_uu (u_j-u_i) + b_uv (v_j-v_i)]

@@ -15,13 +15,13 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(HERE, "liboscnet.so")
 
 NET_OK = 0
-MODEL_KS, MODEL_FHN, MODEL_HH = 0, 1, 2
+MODEL_KS, MODEL_FHN, MODEL_HH, MODEL_KSI = 0, 1, 2, 3
 TOPO_RING, TOPO_LATTICE, TOPO_CSR, TOPO_RANDOM_INDEGREE = 0, 1, 2, 3
 F32, F64 = 0, 1
 METHOD_AUTO, METHOD_DIRECT, METHOD_FAST = 0, 1, 2
 PARAM_OMEGA, PARAM_IEXT = 0, 1
 OBS_PHASE, OBS_GLOBAL_ORDER, OBS_LOCAL_ORDER, OBS_MEAN_PHASE_VELOCITY, OBS_STATS, OBS_REPLICA_ORDER = 0, 1, 2, 3, 4, 5
-NVAR = {MODEL_KS: 1, MODEL_FHN: 2, MODEL_HH: 4}
+NVAR = {MODEL_KS: 1, MODEL_FHN: 2, MODEL_HH: 4, MODEL_KSI: 2}
 
 ABI_SYMBOLS = [
     "net_workspace_bytes", "net_create", "net_destroy", "net_set_state", "net_get_state",
@@ -34,6 +34,11 @@ ABI_SYMBOLS = [
 
 class KSParams(C.Structure):
     _fields_ = [("K", C.c_double), ("alpha", C.c_double), ("omega0", C.c_double)]
+
+
+class KSIParams(C.Structure):
+    _fields_ = [("K", C.c_double), ("alpha", C.c_double), ("m", C.c_double), ("eps", C.c_double),
+                ("omega0", C.c_double)]
 
 
 class FHNParams(C.Structure):
@@ -215,6 +220,8 @@ def net_synchronize(h):
 def make_params(model, p):
     if model == MODEL_KS:
         return KSParams(p["K"], p["alpha"], p.get("omega0", 0.0))
+    if model == MODEL_KSI:
+        return KSIParams(p["K"], p["alpha"], p["m"], p["eps"], p.get("omega0", 0.0))
     if model == MODEL_FHN:
         return FHNParams(p["eps"], p["a"], p["sigma"], p["phi"])
     q = dict(HH_PHASE_MAP, I_ext0=0.0)

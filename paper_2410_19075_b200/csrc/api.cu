@@ -25,7 +25,7 @@ int32_t cuda_err(net* h, cudaError_t e, const char* what) {
 }
 
 static int model_nvar(int model) {
-    return model == NET_MODEL_KS ? 1 : model == NET_MODEL_FHN ? 2 : model == NET_MODEL_HH ? 4 : -1;
+    return model == NET_MODEL_KS ? 1 : model == NET_MODEL_FHN ? 2 : model == NET_MODEL_HH ? 4 : model == NET_MODEL_KSI ? 2 : -1;
 }
 
 static int32_t validate(net* h, const net_desc* d) {
@@ -143,6 +143,10 @@ static void fill_params(net* h, const void* params) {
     if (h->desc.model == NET_MODEL_KS) {
         const net_ks_params* p = (const net_ks_params*)params;
         mp.K = p->K; mp.alpha = p->alpha; mp.sin_a = sin(p->alpha); mp.cos_a = cos(p->alpha);
+    } else if (h->desc.model == NET_MODEL_KSI) {
+        const net_ksi_params* p = (const net_ksi_params*)params;
+        mp.K = p->K; mp.alpha = p->alpha; mp.sin_a = sin(p->alpha); mp.cos_a = cos(p->alpha);
+        mp.inv_m = 1.0 / p->m; mp.damp = p->eps;
     } else if (h->desc.model == NET_MODEL_FHN) {
         const net_fhn_params* p = (const net_fhn_params*)params;
         mp.inv_eps = 1.0 / p->eps; mp.a = p->a; mp.sigma = p->sigma;
@@ -318,7 +322,10 @@ int32_t net_create(const net_desc* user_desc, const void* params, size_t params_
     if (rc) return rc;
     const net_desc* desc = &nd;                 // n = total elements of the batch from here on
     size_t want = desc->model == NET_MODEL_KS ? sizeof(net_ks_params)
+                : desc->model == NET_MODEL_KSI ? sizeof(net_ksi_params)
                 : desc->model == NET_MODEL_FHN ? sizeof(net_fhn_params) : sizeof(net_hh_params);
+    if (desc->model == NET_MODEL_KSI && params && params_bytes == want && !(((const net_ksi_params*)params)->m > 0.0))
+        return set_err(nullptr, NET_ERR_INVALID, "KS with inertia: need m > 0");
     if (!params || params_bytes != want)
         return set_err(nullptr, NET_ERR_INVALID, "params is NULL or params_bytes %zu != %zu", params_bytes, want);
     if (!d_workspace) return set_err(nullptr, NET_ERR_INVALID, "d_workspace is NULL");
@@ -366,6 +373,7 @@ int32_t net_create(const net_desc* user_desc, const void* params, size_t params_
     }
     if (rc == NET_OK) {
         double v0 = desc->model == NET_MODEL_KS ? ((const net_ks_params*)params)->omega0
+                  : desc->model == NET_MODEL_KSI ? ((const net_ksi_params*)params)->omega0
                   : desc->model == NET_MODEL_HH ? ((const net_hh_params*)params)->I_ext0 : 0.0;
         rc = fill_elem_param(h, v0);
     }
@@ -405,7 +413,7 @@ int32_t net_get_state(net_t* h, void* dst, int32_t dst_is_device) {
 int32_t net_set_param_array(net_t* h, int32_t which, const void* src, int32_t src_is_device) {
     if (!h) return NET_ERR_INVALID;
     if (!src) return set_err(h, NET_ERR_INVALID, "src is NULL");
-    if (!((which == NET_PARAM_OMEGA && h->desc.model == NET_MODEL_KS) ||
+    if (!((which == NET_PARAM_OMEGA && (h->desc.model == NET_MODEL_KS || h->desc.model == NET_MODEL_KSI)) ||
           (which == NET_PARAM_IEXT && h->desc.model == NET_MODEL_HH)))
         return set_err(h, NET_ERR_INVALID, "parameter array %d does not belong to model %d", which, h->desc.model);
     OSC_CUDA(h, cudaMemcpyAsync(h->b.elem_param, src, (size_t)h->n * h->esize,

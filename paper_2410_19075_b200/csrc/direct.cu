@@ -18,7 +18,7 @@ __global__ void __launch_bounds__(256) direct_stage_kernel(StageArgs a, ModelPar
     const T dt = (T)a.dt;
     for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n;
          i += (int64_t)gridDim.x * blockDim.x) {
-        constexpr int NV = MODEL == NET_MODEL_KS ? 1 : MODEL == NET_MODEL_FHN ? 2 : 4;
+        constexpr int NV = MODEL == NET_MODEL_KS ? 1 : (MODEL == NET_MODEL_FHN || MODEL == NET_MODEL_KSI) ? 2 : 4;
         T k[NV], xin[NV];
 #pragma unroll
         for (int v = 0; v < NV; ++v) xin[v] = in[v * ld + i];
@@ -30,6 +30,16 @@ __global__ void __launch_bounds__(256) direct_stage_kernel(StageArgs a, ModelPar
             });
             T inv = deg > 0 ? T(1) / T(deg) : T(0);
             k[0] = ks_rhs_direct<T>(mp, ep[i], sum, inv);
+        } else if (MODEL == NET_MODEL_KSI) {
+            // eq. (3) in full: phi' = psi, psi' = (-eps psi + omega + (K/Omega) sum sin(...)) / m
+            T sum = 0;
+            const T pa = xin[0] + T(mp.alpha);
+            int deg = for_each_neighbor<TOPO>(tv, n, i, [&](int64_t j) {
+                sum += Math<T>::sin(in[j] - pa);
+            });
+            T inv = deg > 0 ? T(1) / T(deg) : T(0);
+            k[0] = xin[1];
+            k[1] = (ks_rhs_direct<T>(mp, ep[i], sum, inv) - T(mp.damp) * xin[1]) * T(mp.inv_m);
         } else if (MODEL == NET_MODEL_FHN) {
             T Cu = 0, Cv = 0;
             int deg = for_each_neighbor<TOPO>(tv, n, i, [&](int64_t j) {
@@ -86,6 +96,7 @@ static int32_t launch_model(net* h, const StageArgs& a) {
     switch (h->desc.model) {
         case NET_MODEL_KS: return launch_topo<T, NET_MODEL_KS>(h, a);
         case NET_MODEL_FHN: return launch_topo<T, NET_MODEL_FHN>(h, a);
+        case NET_MODEL_KSI: return launch_topo<T, NET_MODEL_KSI>(h, a);
         default: return launch_topo<T, NET_MODEL_HH>(h, a);
     }
 }

@@ -16,7 +16,7 @@ __global__ void phase_kernel(const T* __restrict__ y, int64_t n, int64_t ld, int
     for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n;
          i += (int64_t)gridDim.x * blockDim.x) {
         double th;
-        if (model == NET_MODEL_KS) th = (double)y[i];
+        if (model == NET_MODEL_KS || model == NET_MODEL_KSI) th = (double)y[i];
         else if (model == NET_MODEL_FHN) th = atan2((double)y[ld + i], (double)y[i]);
         else th = atan2((double)y[3 * ld + i] - mp.n_c, ((double)y[i] - mp.V_c) * mp.inv_V_s);
         theta[i] = th;
@@ -242,7 +242,7 @@ int32_t obs_window_finish(net* h, double t_a, double t_b, int64_t n_samples) {
     double T = t_b - t_a;
     double inv_T = T > 0 ? 1.0 / T : 0.0;
     unsigned g = grid_for(h->n);
-    int is_ks = h->desc.model == NET_MODEL_KS;
+    int is_ks = h->desc.model == NET_MODEL_KS || h->desc.model == NET_MODEL_KSI;
     if (h->desc.dtype == NET_F32)
         window_velocity_kernel<float><<<g, 256, 0, h->stream>>>((const float*)h->b.y, h->b.obs_ref, h->b.obs_wind, h->n, is_ks, inv_T, h->b.obs_vel);
     else

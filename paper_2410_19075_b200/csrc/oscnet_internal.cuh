@@ -14,8 +14,8 @@ namespace oscnet {
 // ---------------------------------------------------------------- parameters
 // Model parameters as passed to kernels (always double; kernels convert to T).
 struct ModelParams {
-    // KS
-    double K, alpha, sin_a, cos_a;
+    // KS (and KS with inertia: inv_m = 1/m, damp = eps)
+    double K, alpha, sin_a, cos_a, inv_m, damp;
     // FHN
     double inv_eps, a, sigma, buu, buv, bvu, bvv;
     // HH

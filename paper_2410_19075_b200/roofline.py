@@ -77,6 +77,9 @@ def ops_per_osc_step(w):
         return ("fp32", 4 * (2 * 5 + 2 * 13 + 30))
     if w.cfg == "4":
         return ("fp64", 4 * (7 * 35 + 80 + w.in_degree))
+    if w.cfg == "6":
+        # DIRECT (per-link) form of Alg. 1: one fp64 sine (~60 instructions) per link and stage
+        return ("fp64", 4 * (32 * 60 + 40))
     if w.cfg == "2":
         return ("fp64", 4 * 60)
     if w.cfg == "1b":

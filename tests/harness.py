@@ -27,6 +27,10 @@ def make_inputs(w, seed=1):
             elem = inputs.lorentzian_omega(n_all, seed, w.extra["gamma"], w.extra["omega_max"])
         else:
             elem = np.full(n_all, w.params["omega0"])
+    elif w.model == configs.KSI:
+        # phases as for KS; initial frequencies psi = 0.1 (2u - 1) from the FHN stream of the seed
+        y0 = np.stack([inputs.ks_phases(n_all, seed), 0.05 * inputs.fhn_circle(n_all, seed)[0]])
+        elem = np.full(n_all, w.params["omega0"])
     elif w.model == configs.FHN:
         y0 = inputs.fhn_circle(n_all, seed)
     else:
@@ -71,6 +75,8 @@ def make_oracle(w, inp, rows=None):
     p = w.params
     if w.model == configs.KS:
         return ora.OracleNet.ks(ntot(w), rp, ci, p["K"], p["alpha"], inp["elem"])
+    if w.model == configs.KSI:
+        return ora.OracleNet.ksi(ntot(w), rp, ci, p["K"], p["alpha"], p["m"], p["eps"], inp["elem"])
     if w.model == configs.FHN:
         return ora.OracleNet.fhn(ntot(w), rp, ci, p["eps"], p["a"], p["sigma"], p["phi"])
     return ora.OracleNet.hh(ntot(w), rp, ci, inp["elem"], **p)
@@ -81,7 +87,7 @@ def make_gpu(w, inp, method=0):
     net = B.Net.from_workload(w, method=method)
     net.set_state(inp["y0"].astype(net.np_dtype))
     if inp["elem"] is not None:
-        which = B.PARAM_OMEGA if w.model == configs.KS else B.PARAM_IEXT
+        which = B.PARAM_OMEGA if w.model in (configs.KS, configs.KSI) else B.PARAM_IEXT
         net.set_param_array(which, inp["elem"].astype(net.np_dtype))
     return net
 

@@ -1,0 +1,61 @@
+"""Kuramoto-Sakaguchi with inertia (eq. (3) in full) on the DIRECT
+path: parity with the pinned oracle (tests/test_oracle_dynamics.py::test_ksi_*) on every topology
+kind, both dtypes; FAST is refused in this build."""
+from dataclasses import replace
+
+import numpy as np
+import pytest
+
+import harness as H
+from paper_2410_19075_b200 import binding as B, configs
+
+pytestmark = pytest.mark.gpu
+
+P6 = dict(K=0.32, alpha=0.45, m=1.0, eps=0.05, omega0=0.0)
+
+
+def _cases():
+    base = configs.get("6", n1=12)                                   # 3D ball of radius 2, 1728 elements
+    ring = replace(base, topo=configs.RING, n=1000, extent=(), radius=37, name="KSI ring N=1000 P=37",
+                   params=dict(P6, K=1.0, m=0.7, eps=0.2, omega0=0.3))
+    lat2 = replace(base, n=23 * 17, extent=(23, 17), radius=3, name="KSI 2D 23x17 radius 3")
+    rnd = replace(base, topo=configs.RANDOM_INDEGREE, n=3000, extent=(), radius=0, in_degree=20,
+                  name="KSI random graph N=3000 k=20", params=dict(P6, K=0.8))
+    out = []
+    for w in (base, ring, lat2, rnd):
+        out.append(w)
+        out.append(replace(w, dtype="f32", name=w.name.replace("f64", "f32") + " (f32)"))
+    return out
+
+
+@pytest.mark.parametrize("w", _cases(), ids=lambda w: w.name)
+def test_ksi_direct_matches_oracle(w):
+    inp = H.make_inputs(w, seed=4)
+    onet = H.make_oracle(w, inp)
+    net = H.make_gpu(w, inp)
+    launches, method = net.counters()
+    assert method == B.METHOD_DIRECT
+    rp, ci = net.get_topology()
+    rp0, ci0 = H.oracle_topology(w)
+    assert np.array_equal(rp, rp0) and np.array_equal(ci, ci0)
+    e_rhs = H.rel_maxnorm(net.eval_rhs(), onet.rhs(inp["y0"]))
+    assert e_rhs <= H.TOL_RHS[w.dtype], e_rhs
+    net.integrate(100, w.dt)
+    got = net.get_state().astype(np.float64)
+    ref = onet.rk4(inp["y0"], 100, w.dt)
+    assert np.abs(got - ref).max() <= H.TOL_TRAJ[w.dtype], np.abs(got - ref).max()
+    # observables see the phase variable
+    R, Psi = onet.global_order(ref[0])
+    assert abs(net.observable(B.OBS_GLOBAL_ORDER)[0] - R) < (1e-9 if w.dtype == "f64" else 1e-4)
+    net.close()
+
+
+def test_ksi_fast_is_refused_and_mass_must_be_positive():
+    w = configs.get("6", n1=12)
+    with pytest.raises(B.OscnetError) as ei:
+        B.Net.from_workload(w, method=B.METHOD_FAST)
+    assert ei.value.code == -5
+    bad = replace(w, params=dict(P6, m=0.0))
+    with pytest.raises(B.OscnetError) as ei:
+        B.Net.from_workload(bad)
+    assert ei.value.code == -1
