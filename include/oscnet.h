@@ -59,7 +59,7 @@ enum {
 };
 
 enum { NET_MODEL_KS = 0, NET_MODEL_FHN = 1, NET_MODEL_HH = 2,
-       NET_MODEL_KSI = 3 /* KS with inertia; NET_METHOD_DIRECT only in this build */ };
+       NET_MODEL_KSI = 3 /* KS with inertia; FAST on rings, DIRECT elsewhere in this build */ };
 enum { NET_TOPO_RING = 0, NET_TOPO_LATTICE = 1, NET_TOPO_CSR = 2, NET_TOPO_RANDOM_INDEGREE = 3 };
 enum { NET_F32 = 0, NET_F64 = 1 };
 
@@ -94,8 +94,9 @@ typedef struct {
  *   dphi_i/dt = psi_i
  *   dpsi_i/dt = ( -eps psi_i + omega_i + (K/Omega_i) sum_{j in row i} sin(phi_j - phi_i - alpha) ) / m
  * (K/Omega_i = the paper's mu; omega_i = omega0 until net_set_param_array(NET_PARAM_OMEGA), 0 in the
- * paper).  State [phi | psi].  Served by NET_METHOD_DIRECT (the per-link form of Alg. 1) on every
- * topology; NET_METHOD_FAST returns NET_ERR_UNSUPPORTED in this build. */
+ * paper).  State [phi | psi].  Rings (and batches of rings) run the persistent prefix-sum kernel
+ * (NET_METHOD_FAST); lattices and graphs are served by NET_METHOD_DIRECT (the per-link form of
+ * Alg. 1) and return NET_ERR_UNSUPPORTED for NET_METHOD_FAST in this build. */
 typedef struct {
     double K, alpha, m, eps, omega0;
 } net_ksi_params;

@@ -26,7 +26,8 @@ int32_t ring_run(net* h, const void* y_in, void* y_out, int64_t n_steps, double 
 
 int32_t fast_select(const net_desc* d) {
     const net_topology& t = d->topo;
-    if (d->model == NET_MODEL_KSI) return FAST_NONE;     // KS with inertia: DIRECT only in this build
+    // KS with inertia: the persistent ring kernel (same fields as KS); DIRECT on the other topologies
+    if (d->model == NET_MODEL_KSI) return ring_supported(d) ? FAST_RING_KS : FAST_NONE;
     if (t.kind == NET_TOPO_CSR || t.kind == NET_TOPO_RANDOM_INDEGREE)
         return csr_blocked_supported(d) ? FAST_CSR_BLOCKED : FAST_CSR_WARP;
     if (lattice_v3_supported(d)) return FAST_LATTICE3D_V3;

@@ -96,7 +96,9 @@ __device__ __forceinline__ void block_scan2(A& a, A& b, A& ta, A& tb, A (*wsum)[
 
 template <class T, int MODEL, int E, bool SINGLE>
 __global__ void __launch_bounds__(RING_THREADS) ring_persistent_kernel(RingArgs a, ModelParams mp) {
+    // KS: phi | FHN: (u, v) | KS with inertia (eq. (3) in full): (phi, psi = dphi/dt), fields as for KS
     constexpr int NV = MODEL == NET_MODEL_KS ? 1 : 2;
+    constexpr bool PHASE = MODEL == NET_MODEL_KS || MODEL == NET_MODEL_KSI;
     extern __shared__ __align__(16) unsigned char ring_smem[];
     __shared__ T wsumT[2][RING_THREADS / 32];
     __shared__ double wsumD[2][RING_THREADS / 32];
@@ -121,7 +123,7 @@ __global__ void __launch_bounds__(RING_THREADS) ring_persistent_kernel(RingArgs 
 #pragma unroll
     for (int e = 0; e < E; ++e) {
         ok[e] = i0 + e < n && threadIdx.x * E + e < chunk;
-        om[e] = (MODEL == NET_MODEL_KS && ok[e]) ? ep[i0 + e] : T(0);
+        om[e] = (PHASE && ok[e]) ? ep[i0 + e] : T(0);
 #pragma unroll
         for (int v = 0; v < NV; ++v) {
             y0[e][v] = ok[e] ? yin[v * ld + i0 + e] : T(0);
@@ -140,7 +142,7 @@ __global__ void __launch_bounds__(RING_THREADS) ring_persistent_kernel(RingArgs 
         T f0[E], f1[E];
 #pragma unroll
         for (int e = 0; e < E; ++e) {
-            if (MODEL == NET_MODEL_KS) {
+            if (PHASE) {
                 T s, c;
                 Math<T>::sincos(x[e][0], &s, &c);
                 f0[e] = ok[e] ? c : T(0);
@@ -241,10 +243,15 @@ __global__ void __launch_bounds__(RING_THREADS) ring_persistent_kernel(RingArgs 
 #pragma unroll
         for (int e = 0; e < E; ++e) {
             const T W0 = W0v[e], W1 = W1v[e];
-            if (MODEL == NET_MODEL_KS) {
+            if (PHASE) {
                 T C = W0, S = W1;
                 if (!a.include_self) { C -= f0[e]; S -= f1[e]; }
-                k[e][0] = ks_rhs_factorised<T>(mp, om[e], C, S, f0[e], f1[e], inv_deg);
+                const T torque = ks_rhs_factorised<T>(mp, om[e], C, S, f0[e], f1[e], inv_deg);
+                if (MODEL == NET_MODEL_KS) k[e][0] = torque;
+                else {      // m phi'' + eps phi' = torque
+                    k[e][0] = x[e][NV - 1];
+                    k[e][NV - 1] = (torque - T(mp.damp) * x[e][NV - 1]) * T(mp.inv_m);
+                }
             } else {
                 const T Cu = W0 - nwin * f0[e], Cv = W1 - nwin * f1[e];
                 fhn_rhs<T>(mp, f0[e], f1[e], Cu, Cv, inv_deg, &k[e][0], &k[e][NV - 1]);
@@ -304,7 +311,8 @@ static bool ring_plan(int64_t n, size_t esize, RingPlan* p, int gmax = 148) {
 bool ring_supported(const net_desc* d) {
     RingPlan p;
     const int batch = d->batch > 0 ? d->batch : 1;
-    return d->topo.kind == NET_TOPO_RING && (d->model == NET_MODEL_KS || d->model == NET_MODEL_FHN) &&
+    return d->topo.kind == NET_TOPO_RING &&
+           (d->model == NET_MODEL_KS || d->model == NET_MODEL_FHN || d->model == NET_MODEL_KSI) &&
            ring_plan(d->n / batch, d->dtype == NET_F32 ? 4 : 8, &p, batch > 1 ? 1 : 148);
 }
 
@@ -373,6 +381,8 @@ static int32_t ring_run_plan(net* h, const RingPlan& p, const void* y_in, void* 
     const bool f32 = h->desc.dtype == NET_F32;
     if (h->desc.model == NET_MODEL_KS)
         return f32 ? ring_launch_e<float, NET_MODEL_KS>(h, a, p) : ring_launch_e<double, NET_MODEL_KS>(h, a, p);
+    if (h->desc.model == NET_MODEL_KSI)
+        return f32 ? ring_launch_e<float, NET_MODEL_KSI>(h, a, p) : ring_launch_e<double, NET_MODEL_KSI>(h, a, p);
     return f32 ? ring_launch_e<float, NET_MODEL_FHN>(h, a, p) : ring_launch_e<double, NET_MODEL_FHN>(h, a, p);
 }
 

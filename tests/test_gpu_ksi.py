@@ -1,6 +1,6 @@
-"""Kuramoto-Sakaguchi with inertia (eq. (3) in full) on the DIRECT
-path: parity with the pinned oracle (tests/test_oracle_dynamics.py::test_ksi_*) on every topology
-kind, both dtypes; FAST is refused in this build."""
+"""Kuramoto-Sakaguchi with inertia (eq. (3) in full) : the persistent
+ring kernel (FAST) for rings, the per-link DIRECT form elsewhere; parity with the pinned oracle (tests/test_oracle_dynamics.py::test_ksi_*) on every topology
+kind, both dtypes; FAST is refused on lattices and graphs in this build."""
 from dataclasses import replace
 
 import numpy as np
@@ -34,7 +34,8 @@ def test_ksi_direct_matches_oracle(w):
     onet = H.make_oracle(w, inp)
     net = H.make_gpu(w, inp)
     launches, method = net.counters()
-    assert method == B.METHOD_DIRECT
+    # rings: the persistent prefix-sum kernel (FAST); other topologies: the per-link DIRECT form
+    assert method == (B.METHOD_FAST if w.topo == configs.RING else B.METHOD_DIRECT)
     rp, ci = net.get_topology()
     rp0, ci0 = H.oracle_topology(w)
     assert np.array_equal(rp, rp0) and np.array_equal(ci, ci0)
@@ -47,6 +48,21 @@ def test_ksi_direct_matches_oracle(w):
     # observables see the phase variable
     R, Psi = onet.global_order(ref[0])
     assert abs(net.observable(B.OBS_GLOBAL_ORDER)[0] - R) < (1e-9 if w.dtype == "f64" else 1e-4)
+    net.close()
+
+
+@pytest.mark.parametrize("method", [B.METHOD_FAST, B.METHOD_DIRECT])
+@pytest.mark.parametrize("batch", [1, 3])
+def test_ksi_ring_fast_and_direct_and_batches(method, batch):
+    ring = [w for w in _cases() if w.topo == configs.RING and w.dtype == "f64"][0]
+    w = replace(ring, n=700, batch=batch, name=ring.name + " x %d" % batch)
+    inp = H.make_inputs(w, seed=6)
+    onet = H.make_oracle(w, inp)
+    net = H.make_gpu(w, inp, method=method)
+    assert net.counters()[1] == method
+    assert H.rel_maxnorm(net.eval_rhs(), onet.rhs(inp["y0"])) <= H.TOL_RHS["f64"]
+    net.integrate(100, w.dt)
+    assert np.abs(net.get_state() - onet.rk4(inp["y0"], 100, w.dt)).max() <= H.TOL_TRAJ["f64"]
     net.close()
 
 
