@@ -128,7 +128,8 @@ class OracleNet:
     @classmethod
     def ksi(cls, n, row_ptr, col_idx, K, alpha, m, eps, omega=0.0):
         """Kuramoto-Sakaguchi with inertia, eq. (3) PAPER.md:79 in full; state [phi | phi']
-        (oracle of the next row, SURVEY.md 8(f).1 -- not on the GPU path yet)."""
+        (GPU: NET_MODEL_KSI).  Its phase variable is phi, so the observables
+        treat it as a phase model like KS (reading R9)."""
         return cls(MODEL_KSI, n, row_ptr, col_idx, [K, alpha, m, eps], omega)
 
     @classmethod
@@ -190,7 +191,8 @@ class OracleNet:
         last sample times.  Returns a dict with mean and (population) std of the
         global R over the window, the mean over i of the local R_i at the last
         sample, and mean and std over i of the mean phase velocity on
-        [t_a, t_b]: KS (phi(t_b)-phi(t_a))/(t_b-t_a); FHN/HH the sum of the
+        [t_a, t_b]: KS and KS with inertia (phase models: the state variable phi is the unwrapped
+        phase, reading R9) (phi(t_b)-phi(t_a))/(t_b-t_a); FHN/HH the sum of the
         increments of theta between consecutive samples, each wrapped to
         (-pi, pi], divided by (t_b-t_a).
         """
@@ -211,7 +213,7 @@ class OracleNet:
                 wind += d - 2.0 * np.pi * np.round(d / (2.0 * np.pi))
             theta_prev = theta
         T = (n_steps - s_a) * dt
-        if self.model == MODEL_KS:
+        if self.model in (MODEL_KS, MODEL_KSI):
             vel = (y[0] - y_a[0]) / T if T > 0 else np.zeros(self.n)
         else:
             vel = wind / T if T > 0 else np.zeros(self.n)

@@ -30,7 +30,7 @@
  *       on uniform states, zero-sum coupling, dense brute force.
  *   ora_rhs (HH)  : hand-computed rate values at V=-65 mV, rest state near the
  *       textbook -65 mV / m=0.0529 h=0.5961 n=0.3177, dense brute force.
- *   ora_rhs (KSI) : (oracle of the NEXT row; not on the GPU path yet) dense
+ *   ora_rhs (KSI) : (Kuramoto-Sakaguchi with inertia) dense
  *       brute force, in-phase state, momentum balance for alpha=0, damped closed form for K=0.
  *   ora_rk4       : 4th-order convergence against a 16x finer step; exactness
  *       for constant RHS.
@@ -233,7 +233,7 @@ static void rhs_ks(const ora_net* net, const double* y, double* f) {
  * Pins (tests/test_oracle_dynamics.py): dense brute force, in-phase state, momentum balance
  * sum_i psi_i' = -(eps/m) sum_i psi_i + sum_i omega_i / m for alpha = 0 on symmetric topologies, the
  * damped closed form for K = 0 within the RK4 truncation error, reduction to rhs_ks as m -> 0 is
- * NOT used (singular limit).  NOT YET on the GPU path: this is the oracle of the next row only. */
+ * NOT used (singular limit). */
 static void rhs_ksi(const ora_net* net, const double* y, double* f) {
     const int64_t n = net->n;
     const double K = net->p[0], alpha = net->p[1], m = net->p[2], eps = net->p[3];

@@ -288,6 +288,19 @@ static int32_t integrate_plain(net* h, int64_t n_steps, double dt) {
     return NET_OK;
 }
 
+// Every entry point runs on the device that owns the workspace, whatever device is current in
+// the calling thread (the previous device is restored on return).
+struct DevGuard {
+    int prev = -1, dev = -1;
+    explicit DevGuard(const net* h) {
+        if (!h) return;
+        dev = h->device;
+        if (cudaGetDevice(&prev) != cudaSuccess) { prev = -1; return; }
+        if (prev != dev) cudaSetDevice(dev); else prev = -1;
+    }
+    ~DevGuard() { if (prev >= 0) cudaSetDevice(prev); }
+};
+
 }  // namespace oscnet
 
 using namespace oscnet;
@@ -298,6 +311,7 @@ extern "C" {
 const char* net_version(void) { return "oscnet 0.1 sm_100a"; }
 
 int32_t net_probe_latency(net_t* h, double* out4) {
+    DevGuard guard_(h);
     if (!h || !out4) return set_err(h, NET_ERR_INVALID, "net or out4 is NULL");
     return ring_probe_latency(h, out4);
 }
@@ -333,9 +347,16 @@ int32_t net_create(const net_desc* user_desc, const void* params, size_t params_
     Layout L = make_layout(desc, (char*)d_workspace);
     if (workspace_bytes < L.total)
         return set_err(nullptr, NET_ERR_SIZE, "workspace %zu bytes < required %zu", workspace_bytes, L.total);
+    cudaPointerAttributes pattr;
+    if (cudaPointerGetAttributes(&pattr, d_workspace) != cudaSuccess || pattr.type != cudaMemoryTypeDevice) {
+        cudaGetLastError();
+        return set_err(nullptr, NET_ERR_INVALID, "d_workspace is not device memory");
+    }
     net* h = new (std::nothrow) net;
     if (!h) return set_err(nullptr, NET_ERR_INVALID, "out of host memory");
     memset(h, 0, sizeof(*h));
+    h->device = pattr.device;
+    DevGuard guard_(h);
     h->desc = *desc;
     h->desc.topo.row_ptr = nullptr;  // the caller's arrays are not kept
     h->desc.topo.col_idx = nullptr;
@@ -391,6 +412,7 @@ int32_t net_create(const net_desc* user_desc, const void* params, size_t params_
 }
 
 int32_t net_destroy(net_t* h) {
+    DevGuard guard_(h);
     if (!h) return NET_OK;
     drop_graph(h);
     delete h;
@@ -398,6 +420,7 @@ int32_t net_destroy(net_t* h) {
 }
 
 int32_t net_set_state(net_t* h, const void* src, int32_t src_is_device) {
+    DevGuard guard_(h);
     if (!h) return NET_ERR_INVALID;
     if (!src) return set_err(h, NET_ERR_INVALID, "src is NULL");
     h->s_valid = 0;
@@ -405,12 +428,14 @@ int32_t net_set_state(net_t* h, const void* src, int32_t src_is_device) {
 }
 
 int32_t net_get_state(net_t* h, void* dst, int32_t dst_is_device) {
+    DevGuard guard_(h);
     if (!h) return NET_ERR_INVALID;
     if (!dst) return set_err(h, NET_ERR_INVALID, "dst is NULL");
     return copy_state(h, h->b.y, dst, false, dst_is_device != 0);
 }
 
 int32_t net_set_param_array(net_t* h, int32_t which, const void* src, int32_t src_is_device) {
+    DevGuard guard_(h);
     if (!h) return NET_ERR_INVALID;
     if (!src) return set_err(h, NET_ERR_INVALID, "src is NULL");
     if (!((which == NET_PARAM_OMEGA && (h->desc.model == NET_MODEL_KS || h->desc.model == NET_MODEL_KSI)) ||
@@ -423,12 +448,14 @@ int32_t net_set_param_array(net_t* h, int32_t which, const void* src, int32_t sr
 }
 
 int32_t net_hh_steady_gates(net_t* h) {
+    DevGuard guard_(h);
     if (!h) return NET_ERR_INVALID;
     if (h->desc.model != NET_MODEL_HH) return set_err(h, NET_ERR_INVALID, "net_hh_steady_gates on a non-HH net");
     return hh_steady_gates(h);
 }
 
 int32_t net_integrate(net_t* h, int64_t n_steps, double dt) {
+    DevGuard guard_(h);
     if (!h) return NET_ERR_INVALID;
     if (n_steps < 0 || !(dt == dt)) return set_err(h, NET_ERR_INVALID, "n_steps < 0 or dt is NaN");
     if (n_steps == 0) return NET_OK;
@@ -436,6 +463,7 @@ int32_t net_integrate(net_t* h, int64_t n_steps, double dt) {
 }
 
 int32_t net_integrate_observed(net_t* h, int64_t n_steps, double dt, int64_t obs_every) {
+    DevGuard guard_(h);
     if (!h) return NET_ERR_INVALID;
     if (n_steps < 1 || obs_every < 1 || n_steps % obs_every != 0)
         return set_err(h, NET_ERR_INVALID, "need n_steps >= 1, obs_every >= 1 and n_steps %% obs_every == 0");
@@ -454,6 +482,7 @@ int32_t net_integrate_observed(net_t* h, int64_t n_steps, double dt, int64_t obs
 }
 
 int32_t net_eval_rhs(net_t* h, void* dst, int32_t dst_is_device) {
+    DevGuard guard_(h);
     if (!h) return NET_ERR_INVALID;
     if (!dst) return set_err(h, NET_ERR_INVALID, "dst is NULL");
     int32_t rc = ensure_s(h);
@@ -467,6 +496,7 @@ int32_t net_eval_rhs(net_t* h, void* dst, int32_t dst_is_device) {
 }
 
 int32_t net_observables(net_t* h, int32_t what, void* dst, int32_t dst_is_device) {
+    DevGuard guard_(h);
     if (!h) return NET_ERR_INVALID;
     if (!dst) return set_err(h, NET_ERR_INVALID, "dst is NULL");
     cudaMemcpyKind kind = dst_is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost;
@@ -520,6 +550,7 @@ int32_t net_observables(net_t* h, int32_t what, void* dst, int32_t dst_is_device
 
 int32_t net_get_topology(net_t* h, int64_t row_begin, int64_t row_count, int64_t* row_ptr,
                          int32_t* col_idx, int32_t dst_is_device) {
+    DevGuard guard_(h);
     if (!h) return NET_ERR_INVALID;
     if (!row_ptr || !col_idx) return set_err(h, NET_ERR_INVALID, "row_ptr / col_idx is NULL");
     if (row_begin < 0 || row_count < 0 || row_begin + row_count > h->n)
@@ -534,7 +565,9 @@ int32_t net_get_topology(net_t* h, int64_t row_begin, int64_t row_count, int64_t
         OSC_CUDA(h, cudaStreamSynchronize(h->stream));
         return NET_OK;
     }
-    // ring / lattice: expand chunk by chunk through the staging scratch
+    // ring / lattice: expand chunk by chunk through the staging scratch.  That region also holds
+    // the exchange fields of y on the lattice FAST paths: have them rebuilt before the next stage.
+    h->s_valid = 0;
     const int64_t deg = h->degree_uniform;
     const size_t per_row = sizeof(int32_t) * (size_t)(deg > 0 ? deg : 1) + sizeof(int64_t);
     int64_t chunk = (int64_t)((h->b.scratch_bytes - 256) / per_row);
@@ -589,6 +622,7 @@ int32_t net_get_kernel_family(net_t* h, int32_t* family) {
 }
 
 int32_t net_synchronize(net_t* h) {
+    DevGuard guard_(h);
     if (!h) return NET_ERR_INVALID;
     OSC_CUDA(h, cudaStreamSynchronize(h->stream));
     OSC_CUDA(h, cudaGetLastError());

@@ -159,6 +159,7 @@ struct net {
     int32_t esize;
     int64_t n, ld;
     cudaStream_t stream;
+    int device;            // ordinal of the device that owns the workspace
     oscnet::ModelParams mp;
     oscnet::TopoView tv;
     oscnet::Buffers b;

@@ -148,8 +148,10 @@ __global__ void __launch_bounds__(RING_THREADS) ring_persistent_kernel(RingArgs 
                 f0[e] = ok[e] ? c : T(0);
                 f1[e] = ok[e] ? s : T(0);
             } else {
-                f0[e] = x[e][0];            // zero where !ok (state loaded as zero)
-                f1[e] = x[e][NV - 1];
+                // padding lanes of a ragged last chunk carry no field: their registers drift away
+                // from zero under the RK4 update (fhn_rhs(0,0) = (0, a)), so mask like the phase models
+                f0[e] = ok[e] ? x[e][0] : T(0);
+                f1[e] = ok[e] ? x[e][NV - 1] : T(0);
             }
         }
         T p0[E], p1[E];
@@ -294,7 +296,10 @@ struct RingPlan { int E, G, chunk; bool single; size_t smem; };
 // query at launch agrees -- fewer elements per thread shorten the dependent chain of a stage)
 static bool ring_plan(int64_t n, size_t esize, RingPlan* p, int gmax = 148) {
     int emin = 1;
-    if (const char* e = getenv("OSCNET_RING_E")) emin = atoi(e) > 0 ? atoi(e) : 1;   // tuning aid
+    if (const char* e = getenv("OSCNET_RING_E")) {      // tuning aid: the chunk must stay a power of two
+        const int v = atoi(e);
+        if (v == 1 || v == 2 || v == 4 || v == 8) emin = v;
+    }
     for (int E = emin; E <= 8; E *= 2) {
         const int64_t chunk = (int64_t)RING_THREADS * E;
         const int64_t G = (n + chunk - 1) / chunk;

@@ -402,6 +402,26 @@ def test_ksi_uncoupled_damped_closed_form():
     np.testing.assert_allclose(y[0], phi, atol=1e-11)
 
 
+def test_ksi_statistics_use_the_unwrapped_phase_difference():
+    """Reading R9: KS-type phases are unwrapped, so the mean phase velocity of a phase model is
+    (phi(t_b) - phi(t_a)) / (t_b - t_a).  Pin: K = 0, where the damped closed form gives it exactly,
+    with |psi| obs_every dt > pi between samples -- the wrapped-increment sum (the FHN/HH rule)
+    would alias there, the unwrapped difference must not."""
+    n, m, eps, dt, steps, every = 6, 1.0, 0.5, 0.01, 800, 100
+    rp, ci = ora.topology_ring(n, 2)
+    om = np.array([4.0, -4.5, 5.0, 0.3, -0.2, 6.0])        # psi_inf = omega / eps = 8 ... 12 rad per unit time
+    net = ora.OracleNet.ksi(n, rp, ci, 0.0, 0.45, m, eps, om)
+    y0 = np.stack([RNG.uniform(-3, 3, n), RNG.normal(size=n)])
+    st = net.run_statistics(y0, steps, dt, every)
+    ta, tb = steps // 2 * dt, steps * dt
+    pinf = om / eps
+    phi = lambda t: y0[0] + pinf * t + (y0[1] - pinf) * (m / eps) * (1 - math.exp(-eps * t / m))
+    vel = (phi(tb) - phi(ta)) / (tb - ta)
+    assert np.abs(vel).max() * every * dt > math.pi          # the aliasing regime
+    np.testing.assert_allclose(st["vel"], vel, atol=1e-9)
+    assert abs(st["vel_mean"] - vel.mean()) < 1e-9 and abs(st["vel_std"] - vel.std()) < 1e-9
+
+
 def test_ksi_rk4_fourth_order_and_energy_dissipation():
     """Coupled case: halving dt divides the error against a 16x finer run by 16 +- 2; and for
     alpha = 0, omega = 0 the energy  E = (m/2) sum psi^2 - (K/(2 Omega)) sum_ij L_ij cos(phi_j - phi_i)
