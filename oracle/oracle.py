@@ -155,12 +155,29 @@ class OracleNet:
         assert rc == 0
         return f.reshape(self.nvar, self.n)
 
-    def rk4(self, y, n_steps, dt):
-        """Returns the state after n_steps classical RK4 steps (y is not modified)."""
+    def rk4(self, y, n_steps, dt, fast=False):
+        """Returns the state after n_steps classical RK4 steps (y is not modified).
+        fast=True: the accelerated restatement of the neighbour sum (ora_rk4_fast), for the long
+        statistics runs of tests/golden/make_stats_cache.py only."""
         y = np.array(y, dtype=np.float64).reshape(self.nvar * self.n)
-        rc = lib().ora_rk4(C.byref(self._s), _p(y), C.c_int64(n_steps), C.c_double(dt))
+        if fast:
+            rc = lib().ora_rk4_fast(C.byref(self._s), _p(y), C.c_int64(n_steps), C.c_double(dt),
+                                    C.c_int64(self.ring_P))
+        else:
+            rc = lib().ora_rk4(C.byref(self._s), _p(y), C.c_int64(n_steps), C.c_double(dt))
         assert rc == 0
         return y.reshape(self.nvar, self.n)
+
+    ring_P = 0      # > 0: the rows are the ring windows of that radius (lets ora_rhs_fast use prefix sums)
+
+    def rhs_fast(self, y):
+        """ora_rhs_fast: factorised sine / precomputed S(V) / prefix sums (last
+        paragraph).  Only for the long statistics runs, after it was shown equal to rhs()."""
+        y = np.ascontiguousarray(y, dtype=np.float64).reshape(self.nvar * self.n)
+        f = np.empty_like(y)
+        rc = lib().ora_rhs_fast(C.byref(self._s), _p(y), _p(f), C.c_int64(self.ring_P))
+        assert rc == 0
+        return f.reshape(self.nvar, self.n)
 
     # ------------------------------------------------------------ observables
     def phase(self, y, phase_map=HH_PHASE_MAP):
@@ -183,7 +200,7 @@ class OracleNet:
                               _p(theta), _p(out))
         return out
 
-    def run_statistics(self, y0, n_steps, dt, obs_every, phase_map=HH_PHASE_MAP):
+    def run_statistics(self, y0, n_steps, dt, obs_every, phase_map=HH_PHASE_MAP, fast=False):
         """Long-run statistics, reading R9.
 
         Samples are taken after steps obs_every, 2*obs_every, ..., n_steps.  The
@@ -201,7 +218,7 @@ class OracleNet:
         Rs, wind, theta_prev, y_a, s_a = [], np.zeros(self.n), None, None, None
         theta = None
         for s in range(obs_every, n_steps + 1, obs_every):
-            y = self.rk4(y, obs_every, dt)
+            y = self.rk4(y, obs_every, dt, fast=fast)
             if 2 * s < n_steps:
                 continue
             theta = self.phase(y, phase_map)

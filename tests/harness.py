@@ -5,7 +5,7 @@ from oracle import oracle as ora
 from paper_2410_19075_b200 import configs, inputs
 
 TOL_RHS = {"f64": 1e-12, "f32": 1e-5}      # max-norm relative, per variable (reading R11)
-TOL_TRAJ = {"f64": 1e-9, "f32": 1e-4}      # absolute after 100 steps (phases mod 2 pi)
+TOL_TRAJ = {"f64": 1e-9, "f32": 1e-4}      # absolute after 100 steps (fp32 phases mod 2 pi, reading R6)
 TOL_STATS = 1e-3
 
 
@@ -123,7 +123,11 @@ def perturb_gates(w, y0, seed=11):
 
 
 def traj_err(w, got, ref):
+    """Max-norm state error.  fp64: plain absolute difference (the north star's 1e-9 absolute; a
+    2 pi slip of a phase is an error).  fp32 phase models: the phase rows are compared modulo 2 pi
+    (reading R6: unwrapped fp32 phases of fast elements lose absolute precision, their position on
+    the circle does not)."""
     d = np.asarray(got, dtype=np.float64) - ref
-    if w.model == configs.KS:
-        d = d - 2 * np.pi * np.round(d / (2 * np.pi))
+    if w.dtype == "f32" and w.model in (configs.KS, configs.KSI):
+        d[0] = d[0] - 2 * np.pi * np.round(d[0] / (2 * np.pi))
     return np.abs(d).max()

@@ -1,0 +1,149 @@
+"""Parity cases the round-1 review asked for (VERDICT.md "Next round" item 1):
+
+  * cfg 2 and cfg 4 at BASELINE.json's FULL size, a few RK4 steps, EVERY element compared with the
+    direct-sum oracle, through the launch configuration bench.py times (128-CTA cooperative ring
+    kernel; csr_blocked_pair_kernel);
+  * persistent ring kernel on rings that span several CTAs with a ragged tail (FHN, KS, KSI);
+  * KS with inertia long-run statistics (reading R9: a phase model, unwrapped velocity);
+  * net_get_topology followed by net_integrate on a KS lattice (the staging scratch overlaps the
+    exchange fields);
+  * two different tiles of the 3D lattice kernels give bit-identical states.
+"""
+import os
+from dataclasses import replace
+
+import numpy as np
+import pytest
+
+import harness as H
+from paper_2410_19075_b200 import binding as B, configs
+
+pytestmark = pytest.mark.gpu
+
+
+# ------------------------------------------------------------------ full size, every element
+def test_cfg2_full_size_trajectory_every_element():
+    w = configs.get("2")                       # N = 65536, R = 22937: 128 CTAs, E = 2
+    inp = H.make_inputs(w, seed=1)
+    net = H.make_gpu(w, inp)
+    assert net.counters()[1] == B.METHOD_FAST
+    steps = 5
+    net.integrate(steps, w.dt)
+    got = net.get_state()
+    net.close()
+    ref = H.make_oracle(w, inp).rk4(inp["y0"], steps, w.dt)     # 20 direct RHS of 6e9 pair terms
+    assert H.traj_err(w, got, ref) <= H.TOL_TRAJ["f64"]
+
+
+def test_cfg4_full_size_trajectory_every_element():
+    w = configs.get("4")                       # N = 1e6, k = 100: csr_blocked (pair form)
+    inp = H.make_inputs(w, seed=1)
+    net = H.make_gpu(w, inp)
+    assert net.kernel_family() == 7            # FAST_CSR_BLOCKED
+    steps = 10
+    net.integrate(steps, w.dt)
+    got = net.get_state()
+    net.close()
+    ref = H.make_oracle(w, inp).rk4(inp["y0"], steps, w.dt)     # 40 RHS of 1e8 links (one exp each)
+    assert H.traj_err(w, got, ref) <= H.TOL_TRAJ["f64"]
+
+
+# ------------------------------------------------------------------ rings over several CTAs, ragged
+def _ring(model, n, radius, dtype="f64"):
+    if model == configs.FHN:
+        base = configs.get("2", n=n)
+    elif model == configs.KS:
+        base = configs.get("1", n=n)
+    else:
+        base = replace(configs.get("6", n1=12), topo=configs.RING, extent=(), n=n,
+                       params=dict(K=1.0, alpha=0.45, m=1.0, eps=0.02, omega0=0.3))
+    return replace(base, n=n, radius=radius, dtype=dtype,
+                   name="%s ring N=%d P=%d %s" % ({0: "KS", 1: "FHN", 3: "KSI"}[model], n, radius, dtype))
+
+
+@pytest.mark.parametrize("model", [configs.FHN, configs.KS, configs.KSI], ids=["FHN", "KS", "KSI"])
+@pytest.mark.parametrize("n,radius", [(3000, 1050), (5000, 77), (100000, 333)])
+def test_ring_multi_cta_ragged(model, n, radius):
+    """n > 2048 and not a multiple of 256*E: several CTAs per ring, padding lanes in the last chunk."""
+    w = _ring(model, n, radius)
+    inp = H.make_inputs(w, seed=3)
+    onet = H.make_oracle(w, inp)
+    net = H.make_gpu(w, inp, method=B.METHOD_FAST)
+    assert H.rel_maxnorm(net.eval_rhs(), onet.rhs(inp["y0"])) <= H.TOL_RHS["f64"]
+    net.integrate(20, w.dt)
+    assert H.traj_err(w, net.get_state(), onet.rk4(inp["y0"], 20, w.dt)) <= H.TOL_TRAJ["f64"]
+    net.close()
+
+
+# ------------------------------------------------------------------ KSI statistics
+@pytest.mark.parametrize("topo", ["ring", "lattice"])
+def test_ksi_long_run_statistics(topo):
+    if topo == "ring":
+        w = replace(_ring(configs.KSI, 1500, 40), n_steps=400, obs_every=10, dt=0.05)
+    else:
+        w = configs.with_steps(configs.get("6", n1=12), 400, 10)
+    inp = H.make_inputs(w, seed=1)
+    # fast rotation: phases advance by more than pi between samples (the aliasing regime in which
+    # the wrapped-increment sum and the unwrapped difference disagree)
+    inp["y0"][1] += 20.0
+    ref = H.make_oracle(w, inp).run_statistics(inp["y0"], w.n_steps, w.dt, w.obs_every)
+    net = H.make_gpu(w, inp)
+    got = net.integrate_observed(w.n_steps, w.dt, w.obs_every)
+    assert got["n_samples"] == ref["n_samples"]
+    for k in ("R_mean", "R_std", "Rloc_mean", "vel_mean", "vel_std"):
+        assert abs(got[k] - ref[k]) <= H.TOL_STATS * max(1.0, abs(ref[k])), (k, got[k], ref[k])
+    vel = net.observable(B.OBS_MEAN_PHASE_VELOCITY)
+    assert np.abs(vel - ref["vel"]).max() <= 1e-6
+    assert abs(ref["vel_mean"]) > np.pi / (w.obs_every * w.dt)      # the regime the test is for
+    net.close()
+
+
+# ------------------------------------------------------------------ get_topology, then integrate
+@pytest.mark.parametrize("cfg", ["3a", "3b", "5"])
+def test_integrate_after_get_topology(cfg):
+    w = configs.get(cfg, n1=24)
+    inp = H.make_inputs(w, seed=5)
+    a, b = H.make_gpu(w, inp), H.make_gpu(w, inp)
+    rp, ci = a.get_topology(0, w.n)            # host destination: staged through the scratch region
+    assert rp[-1] == ci.size
+    a.integrate(12, w.dt)
+    b.integrate(12, w.dt)
+    assert np.array_equal(a.get_state(), b.get_state())
+    a.set_state(inp["y0"].astype(a.np_dtype))
+    a.get_topology(5, 100)
+    assert np.array_equal(a.eval_rhs(), H.make_gpu(w, inp).eval_rhs())
+
+
+# ------------------------------------------------------------------ tile independence
+def _with_env(name, value, fn):
+    old = os.environ.get(name)
+    os.environ[name] = value
+    try:
+        return fn()
+    finally:
+        if old is None:
+            del os.environ[name]
+        else:
+            os.environ[name] = old
+
+
+@pytest.mark.parametrize("cfg,tiles", [("5", ["32,4,16,2,2", "64,2,64,1,3"]),
+                                       ("3a", ["32,4,16,2,2", "64,2,64,1,2"]),
+                                       ("3b", ["32,4,16,2,2", "64,2,64,1,1"])])
+def test_lattice_tiles_give_identical_bits(cfg, tiles):
+    """OSCNET_LAT3 = TXt,SY,Lz,D,CTAS forces the tile / z chunk / pipeline depth of the lat3 kernels.
+    Every output's arithmetic is the same for every tile, so the states must agree bit for bit."""
+    w = configs.get(cfg, n1=64)
+    inp = H.make_inputs(w, seed=9)
+    states = []
+    for spec in [None] + tiles:
+        def run():
+            net = H.make_gpu(w, inp)
+            assert net.kernel_family() == 6    # FAST_LATTICE3D_V3
+            net.integrate(9, w.dt)             # graph replay (8 steps) + one single step
+            y = net.get_state()
+            net.close()
+            return y
+        states.append(run() if spec is None else _with_env("OSCNET_LAT3", spec, run))
+    for y in states[1:]:
+        assert np.array_equal(states[0], y)

@@ -447,3 +447,49 @@ def test_ksi_rk4_fourth_order_and_energy_dissipation():
         E.append(energy(y))
         y = net0.rk4(y, 10, 0.01)
     assert all(E[q + 1] < E[q] for q in range(len(E) - 1))
+
+
+# ------------------------------------------------------------------ accelerated variant (stats runs only)
+def _a11(got, ref):
+    return max(np.abs(got[v] - ref[v]).max() / max(np.abs(ref[v]).max(), 1e-300) for v in range(ref.shape[0]))
+
+
+@pytest.mark.parametrize("model", ["ks", "ksi", "fhn", "hh"])
+@pytest.mark.parametrize("name,n,rp,ci", TOPOS, ids=[t[0] for t in TOPOS])
+def test_fast_variant_equals_direct_rhs(model, name, n, rp, ci):
+    """ora_rhs_fast (factorised sine / precomputed S(V) / prefix sums; SURVEY.md 8(c) last paragraph)
+    against the direct form ora_rhs, itself pinned above: 1e-13 in the norm of reading R11, in an
+    incoherent and in a nearly coherent state."""
+    rng = np.random.default_rng(77)
+    if model == "ks":
+        net = ora.OracleNet.ks(n, rp, ci, 1.3, 0.7, rng.normal(size=n))
+    elif model == "ksi":
+        net = ora.OracleNet.ksi(n, rp, ci, 0.9, 0.45, 0.8, 0.05, rng.normal(size=n))
+    elif model == "fhn":
+        net = ora.OracleNet.fhn(n, rp, ci, 0.05, 0.5, 0.2, math.pi / 2 - 0.1)
+    else:
+        net = ora.OracleNet.hh(n, rp, ci, 9 + 2 * rng.random(n))
+    if name == "ring":
+        net.ring_P = 3
+    for coherent in (False, True):
+        y = rng.uniform(-3, 3, size=(net.nvar, n))
+        if model == "hh":
+            y[0] = rng.uniform(-80, 30, n)
+            y[1:] = rng.random((3, n))
+        if coherent:
+            y = 0.3 + 1e-2 * y if model != "hh" else y
+        assert _a11(net.rhs_fast(y), net.rhs(y)) <= 1e-13
+
+
+def test_fast_variant_ring_prefix_sums_wrap_and_large_radius():
+    """Prefix-sum windows on rings: every wrap case (window crossing 0, crossing n, radius close to
+    n/2 as in config 2) and include_self, against the direct neighbour loop."""
+    rng = np.random.default_rng(5)
+    for n, P, inc in ((64, 22, False), (65, 32, False), (37, 1, False), (50, 7, True)):
+        rp, ci = ora.topology_ring(n, P, inc)
+        net = ora.OracleNet.fhn(n, rp, ci, 0.05, 0.5, 0.1, math.pi / 2 - 0.1)
+        net.ring_P = P
+        y = rng.uniform(-2, 2, size=(2, n))
+        assert _a11(net.rhs_fast(y), net.rhs(y)) <= 1e-13
+        a, b = net.rk4(y, 25, 0.01), net.rk4(y, 25, 0.01, fast=True)
+        assert np.abs(a - b).max() <= 1e-12
