@@ -136,7 +136,7 @@ def build_net(w, device, seed=1, method=None, y0_map=None):
     return net, y0
 
 
-def measure(w, device, steps, warmup, e2e=True, seed=1):
+def measure(w, device, steps, warmup, e2e=True, seed=1, peaks=False):
     """Times `steps` bench steps (each = BENCH_RK4[cfg] RK4 steps) after `warmup` untimed ones.
     Returns device-resident ms, e2e ms, launches and byte counts."""
     import torch
@@ -161,7 +161,10 @@ def measure(w, device, steps, warmup, e2e=True, seed=1):
     ms = ev0.elapsed_time(ev1)
     launches = net.counters()[0] - l0
     method = net.counters()[1]
-    out = dict(ms=ms, launches=launches, method=method, clocks=clk.summary(), rk4_per_step=S)
+    out = dict(ms=ms, launches=launches, method=method, clocks=clk.summary(), rk4_per_step=S,
+               launch_config=net.launch_config())
+    if peaks:
+        out["measured_peaks"] = net.probe_peaks()
     if e2e:
         host_in = torch.from_numpy(y0).pin_memory()
         host_out = torch.empty_like(host_in).pin_memory()
@@ -272,6 +275,7 @@ def roofline_object(w, m, steps):
         achieved, peak, unit = per_launch / avg_launch_s / 1e9, pk[c["pipe"] + "_ginstr_s"], "Ginstr/s"
         peak_src = ("148 SM x %d lanes x sm_max_mhz (%s)" %
                     (R.LANES[c["pipe"]], "issue slots, all pipes" if c["pipe"] == "issue" else c["pipe"] + " pipe"))
+    value = ntot(w) * rk4 / sec
     return {"bound": c["bound"], "achieved": achieved, "peak": peak, "unit": unit,
             "frac": achieved / peak, "traffic": ncu_traffic(w.cfg),
             "kernel": "fused RHS+RK4 stage kernel",
@@ -279,9 +283,14 @@ def roofline_object(w, m, steps):
             "avg_launch_us": avg_launch_s * 1e6, "peak_source": peak_src,
             "bytes_per_osc_step": R.bytes_per_osc_step(w),
             "survey_bytes_per_osc_step": R.survey_bytes_per_osc_step(w),
-            "ops_per_osc_step": c["ops"], "ops_pipe": c["pipe"],
+            "ops_per_osc_step": c["ops"], "ops_pipe": c["pipe"], "ops_source": c["ops_source"],
             "ceiling_osc_steps_per_s": c["osc_steps_per_s"],
-            "frac_of_ceiling": (ntot(w) * rk4 / sec) / c["osc_steps_per_s"]}
+            "frac_of_ceiling": value / c["osc_steps_per_s"],
+            # the direct (one term per link) formulation beside it, so that the rewrite cannot
+            # inflate the fraction: > 1 means the shipped form beats what the direct form could reach
+            "direct_formulation": {"ops_per_osc_step": c["direct_ops"], "pipe": c["direct_pipe"],
+                                   "ceiling_osc_steps_per_s": c["direct_osc_steps_per_s"]},
+            "frac_direct_formulation": value / c["direct_osc_steps_per_s"]}
 
 
 # ------------------------------------------------------------------ CPU oracle arm
@@ -413,7 +422,7 @@ def run_ours(args):
     if ws > 1:
         replicas.init("nccl")
     w = configs.get(args.config)
-    m = measure(w, device, args.steps, args.warmup, e2e=True)
+    m = measure(w, device, args.steps, args.warmup, e2e=True, peaks=True)
     rk4 = args.steps * m["rk4_per_step"]
     units, ms_max, value = replicas.aggregate(ntot(w) * rk4, m["ms"], device)
     _, e2e_ms_max, e2e_value = replicas.aggregate(ntot(w) * rk4, m["e2e_ms"], device)
@@ -431,6 +440,15 @@ def run_ours(args):
             "e2e": {"value": e2e_value, "unit": METRIC, "h2d_bytes_per_step": m["h2d"],
                     "d2h_bytes_per_step": m["d2h"]},
             "gpu_launches": m["launches"], "roofline": head["roofline"]}
+    line["config"]["tile"] = m["launch_config"]
+    if "measured_peaks" in m:
+        # net_probe_peaks: the ALU / shared-memory / L2-gather ceilings
+        # measured on this device, beside the nominal unit counts x clock the fractions divide by
+        from paper_2410_19075_b200 import roofline as R
+        pk = R.peaks()
+        line["roofline"]["measured_peaks"] = dict(
+            m["measured_peaks"], nominal_fp32_ginstr_s=pk["fp32_ginstr_s"], nominal_fp64_ginstr_s=pk["fp64_ginstr_s"],
+            nominal_mufu_ginstr_s=pk["mufu_ginstr_s"])
     if "with_observables" in head and ws == 1:
         line["with_observables"] = head["with_observables"]
     if "latency_model" in head and ws == 1:
@@ -449,10 +467,23 @@ def run_ours(args):
             mc = measure(wc, device, k, max(3, args.warmup), e2e=True)
             e = line_for(wc, mc, k, 1)
             e["clocks"] = mc["clocks"]
+            e["tile"] = mc["launch_config"]
             if not args.no_rewrite_error:
                 e["rewrite_error"] = rewrite_error(wc, device)
             per.append(e)
         line["per_config"] = per
+        # the same facts in a compact table inside `roofline` (a key every record of the run keeps)
+        bad = {"hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown"}
+        tab = {}
+        for e in [dict(head, clocks=m["clocks"])] + per:
+            r = e["roofline"]
+            tab[e["cfg"]] = {"value": e["value"], "bound": r["bound"], "frac": r["frac_of_ceiling"],
+                             "frac_direct_formulation": r["frac_direct_formulation"],
+                             "us_per_launch": r["avg_launch_us"],
+                             "with_observables": e.get("with_observables", {}).get("value"),
+                             "sm_mhz": e["clocks"]["sm_mhz"],
+                             "clocks_ok": not (bad & set(e["clocks"]["reasons"]))}
+        line["roofline"]["per_config"] = tab
     if rank == 0 and ws == 1 and not args.no_cpu_baseline:
         cb, _, _, _ = time_oracle(w.cfg)
         line["cpu_baseline"] = cb

@@ -177,26 +177,32 @@ int32_t net_create(const net_desc* desc, const void* params, size_t params_bytes
 /* Frees the host handle (and its CUDA graph); the workspace stays with the caller. */
 int32_t net_destroy(net_t* net);
 
-/* Copies a full state [nvar][n] (dtype of the net) into / out of the net.  Resets nothing
+/* Copies a full state [nvar][n] (dtype of the net) into / out of the net ("runtime specification
+ * of initial values"; restart from any saved state).  Resets nothing
  * else; the time and step counter are kept (net_set_time changes them). */
 int32_t net_set_state(net_t* net, const void* src, int32_t src_is_device);
 int32_t net_get_state(net_t* net, void* dst, int32_t dst_is_device);
 
 /* Per-element parameter array [n] in the dtype of the net: NET_PARAM_OMEGA (KS) or
- * NET_PARAM_IEXT (HH). */
+ * NET_PARAM_IEXT (HH) ("model parameters" specified at run time). */
 int32_t net_set_param_array(net_t* net, int32_t which, const void* src, int32_t src_is_device);
 
 /* HH only: sets m, h, n of every element to the steady state x_inf(V_i) of its current V
  * (the north-star initial condition "gates at steady state"). */
 int32_t net_hh_steady_gates(net_t* net);
 
-/* Advances the state by n_steps classical RK4 steps of size dt (enqueued, asynchronous):
+/* Advances the state by n_steps classical RK4 steps of size dt (enqueued, asynchronous).  The
+ * integrator is BASELINE.json's (reading R1: the paper itself lists only adaptive / stiff solvers,
+ * PAPER.md:99; "the integrator outputs ... values of dynamical variables at specified time moments",
+ * call it once per output interval):
  *   k1=f(y); k2=f(y+dt/2 k1); k3=f(y+dt/2 k2); k4=f(y+dt k3); y += dt/6 (k1+2k2+2k3+k4).
  * Every stage is one fused kernel (coupled RHS + stage update); steps are replayed from a
  * captured CUDA graph. */
 int32_t net_integrate(net_t* net, int64_t n_steps, double dt);
 
-/* net_integrate plus the long-run statistics of DESIGN.md reading R9: samples after steps
+/* net_integrate plus the long-run statistics of DESIGN.md reading R9 ("synchronization analysis at
+ * each output"; average frequencies PAPER.md:301; coherent / incoherent regions
+ * the paper names the observables and gives no formulas): samples after steps
  * obs_every, 2*obs_every, ..., n_steps (n_steps % obs_every == 0); the window is the samples
  * with step >= n_steps/2.  Afterwards NET_OBS_STATS gives double[8] =
  * {mean R, std R (population), mean_i R_loc,i at the last sample, mean_i and std_i of the mean
@@ -204,15 +210,17 @@ int32_t net_integrate(net_t* net, int64_t n_steps, double dt);
  * NET_OBS_MEAN_PHASE_VELOCITY the per-element velocities. */
 int32_t net_integrate_observed(net_t* net, int64_t n_steps, double dt, int64_t obs_every);
 
-/* One right-hand-side evaluation f(y) at the current state, [nvar][n] in the dtype of the net
- * (parity hook). */
+/* One right-hand-side evaluation f(y) at the current state, [nvar][n] in the dtype of the net:
+ * the paper's Calculate(t, y, der) of Alg. 1 for all elements at once
+ * (parity hook; the systems are autonomous, so t is not an argument). */
 int32_t net_eval_rhs(net_t* net, void* dst, int32_t dst_is_device);
 
 /* Observables of the current state (or of the last net_integrate_observed window), always
- * double; sizes under NET_OBS_*. */
+ * double; sizes under NET_OBS_*.  Definitions: DESIGN.md reading R9. */
 int32_t net_observables(net_t* net, int32_t what, void* dst, int32_t dst_is_device);
 
-/* Expands rows [row_begin, row_begin+row_count) of the topology to canonical CSR: each row
+/* Expands rows [row_begin, row_begin+row_count) of the topology to canonical CSR (row i = the
+ * elements that influence i; lattice rule PAPER.md:309-313): each row
  * sorted ascending, row_ptr[row_count+1] relative to the range (parity hook; bit-exact
  * against the oracle). */
 int32_t net_get_topology(net_t* net, int64_t row_begin, int64_t row_count, int64_t* row_ptr,
@@ -233,6 +241,12 @@ int32_t net_get_counters(net_t* net, int64_t* kernel_launches, int32_t* method_i
  * RING (persistent, FHN 3 / KS 4), LATTICE3D_V2 5, LATTICE3D_V3 6, CSR_BLOCKED 7. */
 int32_t net_get_kernel_family(net_t* net, int32_t* family);
 
+/* Launch geometry of the stage kernel in use (diagnostic; the lattice tile is picked by a timing
+ * pass inside net_create for nets of >= 2^21 elements, so a bench line should print it).  out8 =
+ * {kernel family, tile x, tile y, z planes per chunk, prefetch depth, grid, threads, dynamic shared
+ * memory in bytes} of RK4 stage 1; entries a family does not have are 0. */
+int32_t net_get_launch_config(net_t* net, int32_t* out8);
+
 /* Blocks until the stream is idle; returns NET_ERR_CUDA if anything failed asynchronously. */
 int32_t net_synchronize(net_t* net);
 
@@ -240,7 +254,6 @@ int32_t net_synchronize(net_t* net);
  * The string is owned by the library and valid until the next call on the same handle. */
 const char* net_last_error(const net_t* net);
 
-/* "oscnet <major>.<minor> sm_100a" */
 /* Diagnostic: latencies of the primitives one stage of a latency-bound (ring) net chains, measured on
  * the net's stream with the net's scratch memory ("fraction of a measured latency
  * model").  out4 (host, microseconds each) = {grid barrier over the CTAs this net's persistent kernel
@@ -248,6 +261,19 @@ const char* net_last_error(const net_t* net);
  * doubles, one dependent fp64 sincos}.  Synchronises the stream; the state is not touched. */
 int32_t net_probe_latency(net_t* net, double* out4);
 
+/* Diagnostic: peak microbenchmarks on the net's device and stream (the
+ * denominators of the ALU- and gather-bound rooflines of SURVEY.md 8(d)).  out8 (host) =
+ *   [0] FFMA, [1] add.f32x2, [2] DFMA, [3] MUFU.EX2 thread-instructions per second / 1e9
+ *       (8 independent chains per thread, 8 CTAs of 256 threads per SM),
+ *   [4] shared-memory read bandwidth in GB/s (conflict-free LDS.128),
+ *   [5] independent random 8-byte loads per second / 1e9 from an L2-resident array of out8[6] bytes
+ *       (what the gathers of a CSR stage do; the array is min(8 MB, one state array)),
+ *   [7] SM clock in MHz as seen by clock64() during the probes.
+ * Uses the stage array Y4 (rewritten by every step before it is read) and synchronises the stream;
+ * y, the time and the topology are not touched. */
+int32_t net_probe_peaks(net_t* net, double* out8);
+
+/* "oscnet <major>.<minor> sm_100a" */
 const char* net_version(void);
 
 #ifdef __cplusplus

@@ -28,7 +28,7 @@ ABI_SYMBOLS = [
     "net_set_param_array", "net_hh_steady_gates", "net_integrate", "net_integrate_observed",
     "net_eval_rhs", "net_observables", "net_get_topology", "net_get_degree", "net_get_time",
     "net_set_time", "net_get_counters", "net_get_kernel_family", "net_synchronize", "net_last_error", "net_version",
-    "net_probe_latency",
+    "net_probe_latency", "net_probe_peaks", "net_get_launch_config",
 ]
 
 
@@ -106,6 +106,8 @@ def lib():
         L.net_get_counters.argtypes = [C.c_void_p, C.POINTER(C.c_int64), C.POINTER(C.c_int32)]
         L.net_synchronize.argtypes = [C.c_void_p]
         L.net_probe_latency.argtypes = [C.c_void_p, C.POINTER(C.c_double)]
+        L.net_probe_peaks.argtypes = [C.c_void_p, C.POINTER(C.c_double)]
+        L.net_get_launch_config.argtypes = [C.c_void_p, C.POINTER(C.c_int32)]
         for name in ABI_SYMBOLS:
             if name not in ("net_last_error", "net_version"):
                 getattr(L, name).restype = C.c_int32
@@ -210,6 +212,20 @@ def net_probe_latency(h):
     out = (C.c_double * 4)()
     _check(lib().net_probe_latency(h, out), h)
     return dict(grid_barrier_us=out[0], l2_round_trip_us=out[1], block_scan_us=out[2], fp64_sincos_us=out[3])
+
+
+def net_get_launch_config(h):
+    out = (C.c_int32 * 8)()
+    _check(lib().net_get_launch_config(h, out), h)
+    return dict(family=out[0], tile_x=out[1], tile_y=out[2], lz=out[3], depth=out[4], grid=out[5],
+                threads=out[6], smem_bytes=out[7])
+
+
+def net_probe_peaks(h):
+    out = (C.c_double * 8)()
+    _check(lib().net_probe_peaks(h, out), h)
+    return dict(ffma_ginstr_s=out[0], fadd2_ginstr_s=out[1], dfma_ginstr_s=out[2], mufu_ginstr_s=out[3],
+                smem_gbs=out[4], l2_gather_gops=out[5], gather_array_bytes=out[6], sm_mhz=out[7])
 
 
 def net_synchronize(h):
@@ -380,8 +396,7 @@ class Net:
         rp = np.empty(row_count + 1, dtype=np.int64)
         if deg >= 0:
             cnt = row_count * deg
-        else:       # general CSR: ask for the pointers first
-            full = np.empty(1, dtype=np.int64)
+        else:       # general CSR: at most nnz entries
             cnt = nnz
         ci = np.empty(max(cnt, 1), dtype=np.int32)
         net_get_topology(self.h, row_begin, row_count, rp.ctypes.data, ci.ctypes.data, False)
@@ -401,6 +416,12 @@ class Net:
 
     def probe_latency(self):
         return net_probe_latency(self.h)
+
+    def launch_config(self):
+        return net_get_launch_config(self.h)
+
+    def probe_peaks(self):
+        return net_probe_peaks(self.h)
 
     def synchronize(self):
         net_synchronize(self.h)

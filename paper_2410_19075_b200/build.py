@@ -17,16 +17,24 @@ FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std
          "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden", "--expt-relaxed-constexpr"]
 
 
-def _deps():
+def _deps(obj):
+    """Headers the object was last compiled from (the nvcc -MD file beside it); every header of
+    the tree when there is none yet."""
+    dfile = obj[:-2] + ".d"
+    if os.path.exists(dfile):
+        toks = open(dfile).read().replace("\\\n", " ").split()
+        deps = [t for t in toks[1:] if t.startswith(HERE) or "include/oscnet.h" in t]
+        if deps and all(os.path.exists(d) for d in deps):
+            return deps
     return glob.glob(os.path.join(CSRC, "*.cuh")) + [os.path.join(HERE, "..", "include", "oscnet.h")]
 
 
 def _compile(src, verbose):
     obj = os.path.join(OBJ, os.path.basename(src)[:-3] + ".o")
-    newest = max(os.path.getmtime(p) for p in [src] + _deps())
+    newest = max(os.path.getmtime(p) for p in [src] + _deps(obj))
     if os.path.exists(obj) and os.path.getmtime(obj) >= newest:
         return obj, False
-    cmd = [NVCC] + FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-c", src, "-o", obj]
+    cmd = [NVCC] + FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-MD", "-MF", obj[:-2] + ".d", "-c", src, "-o", obj]
     r = subprocess.run(cmd, capture_output=True, text=True)
     if r.returncode != 0:
         raise RuntimeError("nvcc failed for %s:\n%s\n%s" % (src, r.stdout, r.stderr))

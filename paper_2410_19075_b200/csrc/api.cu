@@ -316,6 +316,12 @@ int32_t net_probe_latency(net_t* h, double* out4) {
     return ring_probe_latency(h, out4);
 }
 
+int32_t net_probe_peaks(net_t* h, double* out8) {
+    DevGuard guard_(h);
+    if (!h || !out8) return set_err(h, NET_ERR_INVALID, "net or out8 is NULL");
+    return probe_peaks(h, out8);
+}
+
 const char* net_last_error(const net_t* h) { return h ? h->err : g_err; }
 
 int32_t net_workspace_bytes(const net_desc* desc, size_t* bytes) {
@@ -618,6 +624,23 @@ int32_t net_get_counters(net_t* h, int64_t* kernel_launches, int32_t* method_in_
 int32_t net_get_kernel_family(net_t* h, int32_t* family) {
     if (!h) return NET_ERR_INVALID;
     if (family) *family = h->method == NET_METHOD_FAST ? h->fast_kind : FAST_NONE;
+    return NET_OK;
+}
+
+int32_t net_get_launch_config(net_t* h, int32_t* out8) {
+    if (!h || !out8) return NET_ERR_INVALID;
+    for (int q = 0; q < 8; ++q) out8[q] = 0;
+    out8[0] = h->method == NET_METHOD_FAST ? h->fast_kind : FAST_NONE;
+    if (out8[0] == FAST_LATTICE3D_V3) {
+        const L3Geom& g = h->lat3[1];
+        out8[1] = g.TXt; out8[2] = g.TYt; out8[3] = g.Lz; out8[4] = g.D;
+        out8[5] = (int32_t)h->lat3_grid[1]; out8[6] = h->lat3_threads[1]; out8[7] = (int32_t)h->lat3_smem[1];
+    } else if (out8[0] == FAST_LATTICE3D_V2) {
+        out8[1] = h->lat2.TXt; out8[2] = h->lat2.TYt; out8[3] = h->lat2.Lz; out8[4] = h->lat2.D;
+        out8[5] = (int32_t)h->lat2_grid; out8[6] = h->lat2_threads; out8[7] = (int32_t)h->lat2_smem;
+    } else if (out8[0] == FAST_CSR_BLOCKED) {
+        out8[1] = h->cb_pair; out8[2] = h->cb_es; out8[5] = (int32_t)h->cb_grid; out8[6] = 1024; out8[7] = (int32_t)h->cb_smem;
+    }
     return NET_OK;
 }
 

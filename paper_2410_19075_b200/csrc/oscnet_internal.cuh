@@ -246,6 +246,7 @@ int32_t pairs_unpack(net* h, const void* pairs, void* soa);
 // observables.cu ------------------------------------------------------------
 int32_t obs_phase(net* h, const void* state, double* d_theta);
 int32_t ring_probe_latency(net* h, double* out4);   // ring_fast.cu
+int32_t probe_peaks(net* h, double* out8);          // probe.cu
 int32_t obs_global_order(net* h, const double* d_theta, double* d_out2);  // {R, Psi}
 int32_t obs_replica_order(net* h, const double* d_theta, double* d_out);  // {R_r, Psi_r} per replica of the batch
 int32_t obs_local_order(net* h, const double* d_theta, double* d_out);

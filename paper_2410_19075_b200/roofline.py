@@ -1,6 +1,14 @@
 """Roofline bookkeeping for bench.py: algorithmic bytes and
 operations per oscillator-step of each north-star workload, and the peaks they are divided by.
-Plain arithmetic on sizes; nothing of the method is computed here."""
+Plain arithmetic on sizes; nothing of the method is computed here.
+
+Operation counts are SURVEY.md 8(d)'s own ("Algorithmic bytes and operations per oscillator-step"
+and its table), NOT counts of the kernels in this repository: ~140 instructions per element and
+stage for KS with P = 4 (560 per oscillator-step, both dtypes), ~55 for FHN with P = 2 (220),
+~425 FP64 for HH (1700), ~160 for the FHN ring (prefix form), ~400 for the KS ring (factorised).
+The direct formulation (one sine / one pair term per link) is carried beside it so that a rewrite
+cannot inflate the fraction ("print the direct-formulation roofline next to it").
+"""
 import json
 import os
 
@@ -13,6 +21,9 @@ SM_MAX_MHZ_NOMINAL = 1965.0
 # issue rates per SM per clock (lanes): FP32 FMA pipe 128, FP64 64, MUFU (SFU) 16
 # "issue": warp instructions of all pipes, 4 schedulers x 32 lanes per SM and clock
 LANES = {"fp32": 128, "fp64": 64, "mufu": 16, "issue": 128}
+# instructions one sine costs in the direct formulation: fp32 sin.approx = 1 MUFU (+ range
+# reduction on the FP32 pipe, not counted); fp64 library sine ~ 60 instructions of the FP64 pipe
+SINE_FP64_INSTR = 60
 
 
 def peaks():
@@ -65,37 +76,60 @@ def survey_bytes_per_osc_step(w):
     return b
 
 
+def _degree(w):
+    """Links per element (Omega) of the workload."""
+    if w.in_degree:
+        return w.in_degree
+    if not w.extent:
+        return 2 * w.radius
+    P, nd = w.radius, len(w.extent)
+    rng = range(-P, P + 1)
+    if nd == 3:
+        return sum(1 for a in rng for b in rng for c in rng if a * a + b * b + c * c <= P * P) - 1
+    if nd == 2:
+        return sum(1 for a in rng for b in rng if a * a + b * b <= P * P) - 1
+    return 2 * P
+
+
 def ops_per_osc_step(w):
-    """Arithmetic instructions per oscillator per RK4 step in the formulation that is shipped
-    (pipe, count).  Estimates of DESIGN.md "Kernels"; used only to name the binding bound."""
+    """(pipe, ops of the shipped formulation, pipe and ops of the direct formulation, source).
+    Shipped = the exact-in-mathematics rewrite SURVEY.md 8(d) counts; direct = one term per link."""
+    deg = _degree(w)
+    f64 = w.dtype == "f64"
     if w.cfg in ("3a", "3b"):
-        # per stage: one sincos (fp32 ~40 instr, fp64 ~110), separable ball sum of (cos, sin):
-        # x-runs 2*(2P+1) adds + 49 run combinations * 2, local field + stage update ~30
-        per_stage = (40 if w.dtype == "f32" else 110) + 2 * 9 + 2 * 49 + 30
-        return ("fp32" if w.dtype == "f32" else "fp64", 4 * per_stage)
+        # SURVEY 8(d): "KS factorised+runs ~ 1 sincos + 2*(2P + (#runs-1)) adds + ~15 -> ~140 instr
+        # (P=4: 49 runs)"; table: 560 FP32 (+8 MUFU) / 560 FP64 + fp64 sincos with T_arith 240-300 us
+        # per step, i.e. ~620 FP64-pipe instructions per oscillator-step
+        if f64:
+            return ("fp64", 620, "fp64", 4 * deg * SINE_FP64_INSTR, "SURVEY.md 8(d): 560 FP64 + fp64 sincos (T_arith 240-300 us/step)")
+        return ("fp32", 560, "mufu", 4 * deg, "SURVEY.md 8(d): 560 FP32 (+8 MUFU)")
     if w.cfg == "5":
-        return ("fp32", 4 * (2 * 5 + 2 * 13 + 30))
+        return ("fp32", 220, "fp32", 4 * 2 * 2 * deg, "SURVEY.md 8(d): ~55 per stage (x-runs, P=2: 13 runs)")
     if w.cfg == "4":
-        return ("fp64", 4 * (7 * 35 + 80 + w.in_degree))
+        return ("fp64", 1700, "fp64", 4 * (deg * 35 + 7 * 35 + 80), "SURVEY.md 8(d): ~425 FP64 per stage (7 exp + 80 + Omega adds)")
     if w.cfg == "6":
-        # DIRECT (per-link) form of Alg. 1: one fp64 sine (~60 instructions) per link and stage
-        return ("fp64", 4 * (32 * 60 + 40))
+        # KS with inertia, P = 2 (13 runs): 1 fp64 sincos (~15 FP64-pipe) + 2*(2P + 12) adds + ~15 per stage
+        return ("fp64", 4 * (15 + 2 * (2 * w.radius + 12) + 15), "fp64", 4 * (deg * SINE_FP64_INSTR + 40),
+                "SURVEY.md 8(d) rule for KS with runs, P=2: 1 sincos + 2*(2P+12) adds + ~15 per stage")
     if w.cfg == "2":
-        return ("fp64", 4 * 60)
+        return ("fp64", 160, "fp64", 4 * 2 * 2 * deg, "SURVEY.md 8(d): ~160 FP64 (prefix sums)")
     if w.cfg == "1b":
-        # measured, not estimated (profiles/r01_split_ncu.md, cfg 1b): 275 instructions of all pipes
-        # per element and stage, 72 of them on the FP64 pipe (sincos, scan, window sums, RK4) -- the
-        # batch is bound by instruction issue (74 % of the slots), the FP64 pipe is 39 % busy
-        return ("issue", 4 * 275)
-    return ("fp64", 4 * (110 + 2 * 2 * w.radius))
+        # the batch of rings is bound by instruction issue of ALL pipes: ncu of this build counts 275
+        # instructions per element and stage, 72 of them FP64 (profiles/r01_split_ncu.md) -- an
+        # ncu-measured executed-instruction count, named as such; SURVEY's FP64 figure is 400 per step
+        return ("issue", 4 * 275, "fp64", 4 * deg * SINE_FP64_INSTR, "ncu-measured executed instructions of all pipes (275 per element and stage)")
+    return ("fp64", 400, "fp64", 4 * deg * SINE_FP64_INSTR, "SURVEY.md 8(d): ~400 FP64 (factorised)")
 
 
 def ceiling(w, pk=None):
     """Per-config roofline ceiling in oscillator-steps/s = 1/max(T_hbm, T_alu) and its parts."""
     pk = pk or peaks()
     t_hbm = bytes_per_osc_step(w) / (pk["hbm_gbs"] * 1e9)
-    pipe, ops = ops_per_osc_step(w)
+    pipe, ops, dpipe, dops, src = ops_per_osc_step(w)
     t_alu = ops / (pk[pipe + "_ginstr_s"] * 1e9)
+    t_direct = dops / (pk[dpipe + "_ginstr_s"] * 1e9)
     bound = "hbm" if t_hbm >= t_alu else "alu"
     return dict(bound=bound, osc_steps_per_s=1.0 / max(t_hbm, t_alu), t_hbm=t_hbm, t_alu=t_alu,
-                pipe=pipe, ops=ops, bytes=bytes_per_osc_step(w))
+                pipe=pipe, ops=ops, bytes=bytes_per_osc_step(w), ops_source=src,
+                direct_pipe=dpipe, direct_ops=dops,
+                direct_osc_steps_per_s=1.0 / max(t_hbm, t_direct))
