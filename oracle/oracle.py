@@ -179,6 +179,34 @@ class OracleNet:
         assert rc == 0
         return f.reshape(self.nvar, self.n)
 
+    # ------------------------------------------------------------ Dormand-Prince 5(4)
+    def dp5_step(self, y, h):
+        """One uncontrolled DOPRI5 step: (5th-order solution, embedded error vector)."""
+        y = np.ascontiguousarray(y, dtype=np.float64).reshape(self.nvar * self.n)
+        y5, e = np.empty_like(y), np.empty_like(y)
+        rc = lib().ora_dp5_step(C.byref(self._s), _p(y), C.c_double(h), _p(y5), _p(e))
+        assert rc == 0
+        return y5.reshape(self.nvar, self.n), e.reshape(self.nvar, self.n)
+
+    def dp5(self, y, t0, t_end, rtol, atol, h0, max_attempts=1000000, log=False):
+        """Adaptive DOPRI5 from t0 to t_end (reading R15).  Returns (state, info):
+        info = dict(accepted, rejected, h_last, h_next, t[, h_log: attempted step sizes, negative
+        when rejected])."""
+        y = np.array(y, dtype=np.float64).reshape(self.nvar * self.n)
+        out = np.zeros(5)
+        cap = 1 << 16
+        hl = np.zeros(cap if log else 1)
+        rc = lib().ora_dp5(C.byref(self._s), _p(y), C.c_double(t0), C.c_double(t_end),
+                           C.c_double(rtol), C.c_double(atol), C.c_double(h0),
+                           C.c_int64(max_attempts), _p(out), _p(hl) if log else None,
+                           C.c_int64(cap if log else 0))
+        assert rc in (0, 1)
+        info = dict(accepted=int(out[0]), rejected=int(out[1]), h_last=out[2], h_next=out[3],
+                    t=out[4], exhausted=bool(rc))
+        if log:
+            info["h_log"] = hl[:min(cap, info["accepted"] + info["rejected"])].copy()
+        return y.reshape(self.nvar, self.n), info
+
     # ------------------------------------------------------------ observables
     def phase(self, y, phase_map=HH_PHASE_MAP):
         y = np.ascontiguousarray(y, dtype=np.float64).reshape(self.nvar * self.n)

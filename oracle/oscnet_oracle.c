@@ -592,3 +592,128 @@ int ora_rk4_fast(const ora_net* net, double* y, int64_t n_steps, double dt, int6
     free(buf);
     return 0;
 }
+
+/* ------------------------------------------------------------------ */
+/* Dormand-Prince 5(4) with step-size control (the    */
+/* solver the paper names first: "a Dormand-Prince solver  */
+/* of 3, 5, or 8 order [22] for non-stiff problems").  The paper prints */
+/* neither the tableau nor the controller; both are the textbook ones   */
+/* of its reference [22] (Hairer, Norsett, Wanner, "Solving Ordinary    */
+/* Differential Equations I", the code DOPRI5), reading R15:  */
+/*   stages  k1 = f(y)  (first-same-as-last: k1 of a step after an       */
+/*           accepted one is k7 of that step),                           */
+/*           k_s = f(y + h sum_{j<s} a_sj k_j),  s = 2..7,               */
+/*   y5   = y + h sum_j b_j k_j   (b = a_7., the 5th-order solution),    */
+/*   e    = h sum_j (b_j - bhat_j) k_j        (bhat: embedded 4th order) */
+/*   err  = sqrt( (1/n) sum_i (e_i / (atol + rtol max(|y_i|, |y5_i|)))^2 ) */
+/*   accept iff err <= 1;                                                */
+/*   h_new = h * min(facmax, max(0.2, 0.9 err^(-1/5))), facmax = 10, and */
+/*           1 for the step right after a rejection; err = 0 -> facmax.  */
+/*   the last step is shortened to land on t_end exactly                 */
+/*           (if t + 1.01 h >= t_end then h = t_end - t).                */
+/* The systems are autonomous, so the nodes c_s are not needed.          */
+/* Pins (tests/test_oracle_dp5.py): stability polynomial of one step on  */
+/* a linear problem (1 + z + ... + z^5/120 + z^6/600, textbook), the     */
+/* embedded error of that step, order 5 against a 16x finer run, exact   */
+/* for constant RHS, accepted/rejected sequence equal to a scalar DOPRI5 */
+/* written out by hand on one FHN element.                               */
+/* ------------------------------------------------------------------ */
+static const double DP_A[7][6] = {
+    {0, 0, 0, 0, 0, 0},
+    {1.0 / 5.0, 0, 0, 0, 0, 0},
+    {3.0 / 40.0, 9.0 / 40.0, 0, 0, 0, 0},
+    {44.0 / 45.0, -56.0 / 15.0, 32.0 / 9.0, 0, 0, 0},
+    {19372.0 / 6561.0, -25360.0 / 2187.0, 64448.0 / 6561.0, -212.0 / 729.0, 0, 0},
+    {9017.0 / 3168.0, -355.0 / 33.0, 46732.0 / 5247.0, 49.0 / 176.0, -5103.0 / 18656.0, 0},
+    {35.0 / 384.0, 0.0, 500.0 / 1113.0, 125.0 / 192.0, -2187.0 / 6784.0, 11.0 / 84.0}};
+static const double DP_E[7] = {71.0 / 57600.0, 0.0, -71.0 / 16695.0, 71.0 / 1920.0,
+                               -17253.0 / 339200.0, 22.0 / 525.0, -1.0 / 40.0};
+
+/* One step of size h from y with k1 given.  Writes y5 (the 5th-order solution), k7 = f(y5) into
+ * k[6], and the error vector e.  k = 7 arrays of nvar*n. */
+static void dp5_stages(const ora_net* net, const double* y, double h, double** k, double* y5,
+                       double* e, double* tmp) {
+    const int64_t len = (int64_t)ora_nvar(net->model) * net->n;
+    for (int s = 1; s < 7; ++s) {
+        double* dst = s == 6 ? y5 : tmp;
+        for (int64_t q = 0; q < len; ++q) {
+            double acc = 0.0;
+            for (int j = 0; j < s; ++j) acc += DP_A[s][j] * k[j][q];
+            dst[q] = y[q] + h * acc;
+        }
+        ora_rhs(net, dst, k[s]);
+    }
+    for (int64_t q = 0; q < len; ++q) {
+        double acc = 0.0;
+        for (int j = 0; j < 7; ++j) acc += DP_E[j] * k[j][q];
+        e[q] = h * acc;
+    }
+}
+
+/* A single step of fixed size (no control): y5 and the embedded error vector e (pin hook). */
+int ora_dp5_step(const ora_net* net, const double* y, double h, double* y5, double* e) {
+    int32_t nv = ora_nvar(net->model);
+    if (nv < 0) return -1;
+    const int64_t len = (int64_t)nv * net->n;
+    double* buf = (double*)malloc(sizeof(double) * (size_t)len * 8);
+    if (!buf) return -2;
+    double* k[7];
+    for (int j = 0; j < 7; ++j) k[j] = buf + j * len;
+    ora_rhs(net, y, k[0]);
+    dp5_stages(net, y, h, k, y5, e, buf + 7 * len);
+    free(buf);
+    return 0;
+}
+
+/* Integrates from t0 to t_end.  y is advanced in place.  out[0..4] = {accepted steps, rejected
+ * steps, last step size used, suggested next step size, t reached}.  h_log (may be NULL) receives
+ * the size of every ATTEMPTED step, negative when it was rejected, up to h_log_cap entries.
+ * Returns 0, or 1 if max_attempts was exhausted before t_end. */
+int ora_dp5(const ora_net* net, double* y, double t0, double t_end, double rtol, double atol,
+            double h0, int64_t max_attempts, double* out, double* h_log, int64_t h_log_cap) {
+    int32_t nv = ora_nvar(net->model);
+    if (nv < 0 || !(h0 > 0.0) || !(t_end >= t0)) return -1;
+    const int64_t len = (int64_t)nv * net->n;
+    double* buf = (double*)malloc(sizeof(double) * (size_t)len * 10);
+    if (!buf) return -2;
+    double* k[7];
+    for (int j = 0; j < 7; ++j) k[j] = buf + j * len;
+    double *y5 = buf + 7 * len, *e = buf + 8 * len, *tmp = buf + 9 * len;
+    double t = t0, h = h0, h_used = 0.0;
+    int64_t acc_n = 0, rej_n = 0, att = 0;
+    int after_reject = 0, rc = 0;
+    ora_rhs(net, y, k[0]);
+    while (t < t_end) {
+        if (att >= max_attempts) { rc = 1; break; }
+        int last = 0;
+        if (t + 1.01 * h >= t_end) { h = t_end - t; last = 1; }
+        dp5_stages(net, y, h, k, y5, e, tmp);
+        double s2 = 0.0;
+        for (int64_t q = 0; q < len; ++q) {
+            double sc = atol + rtol * fmax(fabs(y[q]), fabs(y5[q]));
+            double r = e[q] / sc;
+            s2 += r * r;
+        }
+        const double err = sqrt(s2 / (double)len);
+        const double facmax = after_reject ? 1.0 : 10.0;
+        double fac = err > 0.0 ? 0.9 * pow(err, -0.2) : facmax;
+        fac = fmin(facmax, fmax(0.2, fac));
+        if (h_log && att < h_log_cap) h_log[att] = err <= 1.0 ? h : -h;
+        ++att;
+        if (err <= 1.0) {
+            t = last ? t_end : t + h;
+            h_used = h;
+            memcpy(y, y5, sizeof(double) * (size_t)len);
+            double* sw = k[0]; k[0] = k[6]; k[6] = sw;      /* first same as last */
+            ++acc_n;
+            after_reject = 0;
+        } else {
+            ++rej_n;
+            after_reject = 1;
+        }
+        h *= fac;
+    }
+    out[0] = (double)acc_n; out[1] = (double)rej_n; out[2] = h_used; out[3] = h; out[4] = t;
+    free(buf);
+    return rc;
+}

@@ -3,6 +3,11 @@ import sys
 
 import pytest
 
+# the oracle's OpenMP loops run on tiny nets thousands of times per test: threads that spin while
+# the box is busy (a build, another oracle run) make those calls crawl
+os.environ.setdefault("OMP_WAIT_POLICY", "PASSIVE")
+os.environ.setdefault("GOMP_SPINCOUNT", "0")
+
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
