@@ -210,6 +210,24 @@ int32_t net_integrate(net_t* net, int64_t n_steps, double dt);
  * NET_OBS_MEAN_PHASE_VELOCITY the per-element velocities. */
 int32_t net_integrate_observed(net_t* net, int64_t n_steps, double dt, int64_t obs_every);
 
+/* Adaptive integration from the net's current time to t_end with the Dormand-Prince 5(4) pair and
+ * step-size control on the device -- the solver the paper recommends first ("a
+ * Dormand-Prince solver of 3, 5, or 8 order [22] for non-stiff problems").  The paper prints neither
+ * tableau nor controller; both are the textbook DOPRI5 of its reference [22] (reading R15):
+ *   err = sqrt(mean_i (e_i / (atol + rtol max(|y_i|, |y5_i|)))^2), accept iff err <= 1,
+ *   h <- h min(facmax, max(0.2, 0.9 err^(-1/5))), facmax = 10 (1 right after a rejection),
+ *   first-same-as-last, the last step cut to land on t_end exactly.
+ * h0 > 0 is the first step tried.  d_work: device memory, 256-byte aligned, at least
+ * net_adaptive_workspace_bytes (10 state-sized vectors), owned by the caller, free to reuse
+ * afterwards.  out5 (host) = {accepted steps, rejected steps, last step used, next step suggested,
+ * time reached}.  The error norm, the decision and the next step are computed on the device; the
+ * host reads the control block once per 8 attempts.  Synchronises the stream.  Returns
+ * NET_ERR_INVALID (state and time as reached) when max_attempts is exhausted before t_end.
+ * No dense output: call once per output time. */
+int32_t net_adaptive_workspace_bytes(net_t* net, size_t* bytes);
+int32_t net_integrate_adaptive(net_t* net, double t_end, double rtol, double atol, double h0,
+                               int64_t max_attempts, void* d_work, size_t work_bytes, double* out5);
+
 /* One right-hand-side evaluation f(y) at the current state, [nvar][n] in the dtype of the net:
  * the paper's Calculate(t, y, der) of Alg. 1 for all elements at once
  * (parity hook; the systems are autonomous, so t is not an argument). */

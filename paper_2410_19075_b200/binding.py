@@ -29,6 +29,7 @@ ABI_SYMBOLS = [
     "net_eval_rhs", "net_observables", "net_get_topology", "net_get_degree", "net_get_time",
     "net_set_time", "net_get_counters", "net_get_kernel_family", "net_synchronize", "net_last_error", "net_version",
     "net_probe_latency", "net_probe_peaks", "net_get_launch_config",
+    "net_adaptive_workspace_bytes", "net_integrate_adaptive",
 ]
 
 
@@ -108,6 +109,9 @@ def lib():
         L.net_probe_latency.argtypes = [C.c_void_p, C.POINTER(C.c_double)]
         L.net_probe_peaks.argtypes = [C.c_void_p, C.POINTER(C.c_double)]
         L.net_get_launch_config.argtypes = [C.c_void_p, C.POINTER(C.c_int32)]
+        L.net_adaptive_workspace_bytes.argtypes = [C.c_void_p, C.POINTER(C.c_size_t)]
+        L.net_integrate_adaptive.argtypes = [C.c_void_p, C.c_double, C.c_double, C.c_double, C.c_double,
+                                             C.c_int64, C.c_void_p, C.c_size_t, C.POINTER(C.c_double)]
         for name in ABI_SYMBOLS:
             if name not in ("net_last_error", "net_version"):
                 getattr(L, name).restype = C.c_int32
@@ -165,6 +169,20 @@ def net_integrate(h, n_steps, dt):
 
 def net_integrate_observed(h, n_steps, dt, obs_every):
     _check(lib().net_integrate_observed(h, n_steps, dt, obs_every), h)
+
+
+def net_adaptive_workspace_bytes(h):
+    out = C.c_size_t()
+    _check(lib().net_adaptive_workspace_bytes(h, C.byref(out)), h)
+    return out.value
+
+
+def net_integrate_adaptive(h, t_end, rtol, atol, h0, max_attempts, work_ptr, work_bytes):
+    out = (C.c_double * 5)()
+    rc = lib().net_integrate_adaptive(h, t_end, rtol, atol, h0, max_attempts, work_ptr, work_bytes, out)
+    info = dict(accepted=int(out[0]), rejected=int(out[1]), h_last=out[2], h_next=out[3], t=out[4])
+    _check(rc, h)
+    return info
 
 
 def net_eval_rhs(h, ptr, is_device):
@@ -368,6 +386,19 @@ class Net:
     # dynamics -----------------------------------------------------------------
     def integrate(self, n_steps, dt):
         net_integrate(self.h, int(n_steps), float(dt))
+
+    def integrate_adaptive(self, t_end, rtol, atol, h0, max_attempts=1000000):
+        """Dormand-Prince 5(4) from the net's time to t_end; returns the step statistics."""
+        torch = self.torch
+        need = net_adaptive_workspace_bytes(self.h)
+        if getattr(self, "_adaptive_work", None) is None or self._adaptive_work.numel() < need + 256:
+            with torch.cuda.device(self.device):
+                self._adaptive_work = torch.empty(need + 256, dtype=torch.uint8, device=self.device)
+                self._adaptive_work.record_stream(self.stream)
+            self.stream.wait_stream(torch.cuda.current_stream())
+        base = (self._adaptive_work.data_ptr() + 255) // 256 * 256
+        return net_integrate_adaptive(self.h, float(t_end), float(rtol), float(atol), float(h0),
+                                      int(max_attempts), base, need)
 
     def integrate_observed(self, n_steps, dt, obs_every):
         net_integrate_observed(self.h, int(n_steps), float(dt), int(obs_every))

@@ -247,6 +247,26 @@ static int32_t enqueue_step(net* h, double dt) {
     return NET_OK;
 }
 
+// Helpers of the adaptive integrator (adaptive.cu): vectors in the caller's layout [nvar][n] on the device.
+int32_t state_to_external(net* h, void* d_dst) { return copy_state(h, h->b.y, d_dst, false, true); }
+int32_t state_from_external(net* h, const void* d_src) {
+    h->s_valid = 0;
+    return copy_state(h, h->b.y, const_cast<void*>(d_src), true, true);
+}
+// k = f(x): x becomes the net's state (the caller restores its own afterwards), then the RHS-only
+// instance of the net's stage kernel family, exactly as net_eval_rhs runs it
+int32_t rhs_at(net* h, const void* d_x, void* d_k) {
+    int32_t rc = state_from_external(h, d_x);
+    if (rc) return rc;
+    if ((rc = ensure_s(h))) return rc;
+    StageArgs a = stage_args(h, 0, 0.0);
+    a.stage = STAGE_RHS_ONLY;
+    a.out = h->b.Y4;
+    a.s_out = nullptr;
+    if ((rc = run_stage(h, a))) return rc;
+    return copy_state(h, h->b.Y4, d_k, false, true);
+}
+
 constexpr int GRAPH_STEPS = 8;
 
 static int32_t integrate_plain(net* h, int64_t n_steps, double dt) {
@@ -485,6 +505,19 @@ int32_t net_integrate_observed(net_t* h, int64_t n_steps, double dt, int64_t obs
         ++n_samples;
     }
     return obs_window_finish(h, t0 + (double)s_a * dt, t0 + (double)n_steps * dt, n_samples);
+}
+
+int32_t net_adaptive_workspace_bytes(net_t* h, size_t* bytes) {
+    if (!h || !bytes) return set_err(h, NET_ERR_INVALID, "net or bytes is NULL");
+    *bytes = adaptive_workspace_bytes(h);
+    return NET_OK;
+}
+
+int32_t net_integrate_adaptive(net_t* h, double t_end, double rtol, double atol, double h0, int64_t max_attempts,
+                               void* d_work, size_t work_bytes, double* out5) {
+    DevGuard guard_(h);
+    if (!h || !out5) return set_err(h, NET_ERR_INVALID, "net or out5 is NULL");
+    return adaptive_integrate(h, t_end, rtol, atol, h0, max_attempts, d_work, work_bytes, out5);
 }
 
 int32_t net_eval_rhs(net_t* h, void* dst, int32_t dst_is_device) {

@@ -247,6 +247,13 @@ int32_t pairs_unpack(net* h, const void* pairs, void* soa);
 int32_t obs_phase(net* h, const void* state, double* d_theta);
 int32_t ring_probe_latency(net* h, double* out4);   // ring_fast.cu
 int32_t probe_peaks(net* h, double* out8);          // probe.cu
+// adaptive.cu (Dormand-Prince 5(4)) and its helpers in api.cu
+size_t adaptive_workspace_bytes(const net* h);
+int32_t adaptive_integrate(net* h, double t_end, double rtol, double atol, double h0, int64_t max_attempts,
+                           void* d_work, size_t work_bytes, double* out5);
+int32_t state_to_external(net* h, void* d_dst);
+int32_t state_from_external(net* h, const void* d_src);
+int32_t rhs_at(net* h, const void* d_x, void* d_k);
 int32_t obs_global_order(net* h, const double* d_theta, double* d_out2);  // {R, Psi}
 int32_t obs_replica_order(net* h, const double* d_theta, double* d_out);  // {R_r, Psi_r} per replica of the batch
 int32_t obs_local_order(net* h, const double* d_theta, double* d_out);
