@@ -60,7 +60,8 @@ enum {
 
 enum { NET_MODEL_KS = 0, NET_MODEL_FHN = 1, NET_MODEL_HH = 2,
        NET_MODEL_KSI = 3 /* KS with inertia; FAST on rings, DIRECT elsewhere in this build */ };
-enum { NET_TOPO_RING = 0, NET_TOPO_LATTICE = 1, NET_TOPO_CSR = 2, NET_TOPO_RANDOM_INDEGREE = 3 };
+enum { NET_TOPO_RING = 0, NET_TOPO_LATTICE = 1, NET_TOPO_CSR = 2, NET_TOPO_RANDOM_INDEGREE = 3,
+       NET_TOPO_COMPRESSED = 4 /* differentially compressed coupling matrix, Alg. 2 */ };
 enum { NET_F32 = 0, NET_F64 = 1 };
 
 /* How the coupling sum is evaluated.  DIRECT = one term per neighbour, gathered
@@ -131,8 +132,38 @@ typedef struct {
  *           (ptrs_are_device); copied into the workspace by net_create.
  *  RANDOM_INDEGREE: every row has exactly in_degree distinct sources != i, drawn by the
  *           integer counter-based rule of DESIGN.md reading R8 from `seed`; built on the device.
+ *  COMPRESSED: the differentially compressed matrix of Alg. 2 (`compressed`, from net_compress_csr
+ *           or built by the caller).  The device keeps V, D and the n row references -- O(max(BK, n))
+ *           memory -- and every stage EXTRACTs rows on the fly: rows whose difference
+ *           is empty are the common pattern shifted by i (offset loop, no per-row data); the others
+ *           merge V with their table entry ("lattice with defects").  Served by the per-link DIRECT
+ *           kernels.
  *  include_self (ring/lattice): also count the centre as a link (then Omega = 2P+1 / 33 / 257,
  *           the link counts the paper prints). */
+/* Differentially compressed coupling matrix (Alg. 2), on position sets instead
+ * of bit vectors: the common vector V = row 0; for every row i the difference
+ * d_i = XOR(ROL(L_i, i), V) (ROL moves the bit at position j to (j - i) mod n); the table D of the
+ * distinct differences; C_i = the entry of D that equals d_i.  EXTRACT: row i = the positions
+ * (p + i) mod n for p in XOR(V, D[C_i]).  "A full mesh topology has a common vector with all bits
+ * set and a difference table with a single entry having all bits unset".
+ * All arrays are HOST memory; positions are sorted ascending within V and within each entry. */
+typedef struct {
+    int64_t n;             /* rows (elements) */
+    int64_t v_len;         /* set bits of the common vector */
+    const int32_t* v_pos;  /* [v_len] */
+    int64_t k;             /* entries of the difference table */
+    const int64_t* d_ptr;  /* [k + 1] */
+    const int32_t* d_pos;  /* [d_ptr[k]] */
+    const int32_t* c;      /* [n] row -> entry of the table */
+} net_compressed;
+
+/* COMPRESS of Alg. 2 on the host (done once per matrix, as in the paper: "performed only once",
+ * PAPER.md:173): rows given as CSR (host pointers; rows need not be sorted).  The result is owned
+ * by the library until net_compressed_free; net_create copies what it needs into the workspace.
+ * Cost O(nnz) expected (hashed table lookup). */
+int32_t net_compress_csr(int64_t n, const int64_t* row_ptr, const int32_t* col_idx, net_compressed** out);
+int32_t net_compressed_free(net_compressed* c);
+
 typedef struct {
     int32_t kind;
     int32_t ndim;
@@ -145,6 +176,7 @@ typedef struct {
     int32_t ptrs_are_device;
     int32_t in_degree;
     uint64_t seed;
+    const net_compressed* compressed;   /* NET_TOPO_COMPRESSED: the matrix (host); else NULL */
 } net_topology;
 
 typedef struct {

@@ -16,7 +16,7 @@ LIB_PATH = os.path.join(HERE, "liboscnet.so")
 
 NET_OK = 0
 MODEL_KS, MODEL_FHN, MODEL_HH, MODEL_KSI = 0, 1, 2, 3
-TOPO_RING, TOPO_LATTICE, TOPO_CSR, TOPO_RANDOM_INDEGREE = 0, 1, 2, 3
+TOPO_RING, TOPO_LATTICE, TOPO_CSR, TOPO_RANDOM_INDEGREE, TOPO_COMPRESSED = 0, 1, 2, 3, 4
 F32, F64 = 0, 1
 METHOD_AUTO, METHOD_DIRECT, METHOD_FAST = 0, 1, 2
 PARAM_OMEGA, PARAM_IEXT = 0, 1
@@ -30,6 +30,7 @@ ABI_SYMBOLS = [
     "net_set_time", "net_get_counters", "net_get_kernel_family", "net_synchronize", "net_last_error", "net_version",
     "net_probe_latency", "net_probe_peaks", "net_get_launch_config",
     "net_adaptive_workspace_bytes", "net_integrate_adaptive",
+    "net_compress_csr", "net_compressed_free",
 ]
 
 
@@ -59,7 +60,14 @@ class Topology(C.Structure):
     _fields_ = [("kind", C.c_int32), ("ndim", C.c_int32), ("extent", C.c_int64 * 3),
                 ("radius", C.c_int32), ("include_self", C.c_int32), ("row_ptr", C.c_void_p),
                 ("col_idx", C.c_void_p), ("nnz", C.c_int64), ("ptrs_are_device", C.c_int32),
-                ("in_degree", C.c_int32), ("seed", C.c_uint64)]
+                ("in_degree", C.c_int32), ("seed", C.c_uint64), ("compressed", C.c_void_p)]
+
+
+class Compressed(C.Structure):
+    """net_compressed: V, D, C of Alg. 2 (host arrays)."""
+    _fields_ = [("n", C.c_int64), ("v_len", C.c_int64), ("v_pos", C.POINTER(C.c_int32)),
+                ("k", C.c_int64), ("d_ptr", C.POINTER(C.c_int64)), ("d_pos", C.POINTER(C.c_int32)),
+                ("c", C.POINTER(C.c_int32))]
 
 
 class Desc(C.Structure):
@@ -112,6 +120,8 @@ def lib():
         L.net_adaptive_workspace_bytes.argtypes = [C.c_void_p, C.POINTER(C.c_size_t)]
         L.net_integrate_adaptive.argtypes = [C.c_void_p, C.c_double, C.c_double, C.c_double, C.c_double,
                                              C.c_int64, C.c_void_p, C.c_size_t, C.POINTER(C.c_double)]
+        L.net_compress_csr.argtypes = [C.c_int64, C.c_void_p, C.c_void_p, C.POINTER(C.POINTER(Compressed))]
+        L.net_compressed_free.argtypes = [C.POINTER(Compressed)]
         for name in ABI_SYMBOLS:
             if name not in ("net_last_error", "net_version"):
                 getattr(L, name).restype = C.c_int32
@@ -169,6 +179,42 @@ def net_integrate(h, n_steps, dt):
 
 def net_integrate_observed(h, n_steps, dt, obs_every):
     _check(lib().net_integrate_observed(h, n_steps, dt, obs_every), h)
+
+
+class CompressedMatrix:
+    """Owner of a net_compressed returned by net_compress_csr (freed with the object)."""
+
+    def __init__(self, ptr):
+        self.ptr = ptr
+
+    @property
+    def s(self):
+        return self.ptr.contents
+
+    def arrays(self):
+        """(V, d_ptr, d_pos, C) as numpy copies."""
+        s = self.s
+        dptr = np.ctypeslib.as_array(s.d_ptr, shape=(s.k + 1,)).copy()
+        return (np.ctypeslib.as_array(s.v_pos, shape=(max(s.v_len, 1),))[:s.v_len].copy(), dptr,
+                np.ctypeslib.as_array(s.d_pos, shape=(max(int(dptr[-1]), 1),))[:int(dptr[-1])].copy(),
+                np.ctypeslib.as_array(s.c, shape=(s.n,)).copy())
+
+    def __del__(self):
+        try:
+            if self.ptr:
+                lib().net_compressed_free(self.ptr)
+                self.ptr = None
+        except Exception:
+            pass
+
+
+def net_compress_csr(row_ptr, col_idx):
+    """COMPRESS of Alg. 2 on host CSR arrays (int64 row_ptr, int32 col_idx)."""
+    rp = np.ascontiguousarray(row_ptr, dtype=np.int64)
+    ci = np.ascontiguousarray(col_idx, dtype=np.int32)
+    out = C.POINTER(Compressed)()
+    _check(lib().net_compress_csr(len(rp) - 1, rp.ctypes.data, ci.ctypes.data, C.byref(out)))
+    return CompressedMatrix(out)
 
 
 def net_adaptive_workspace_bytes(h):
@@ -306,6 +352,10 @@ class Net:
                 t.row_ptr, t.col_idx = rp.data_ptr(), ci.data_ptr()
                 t.nnz, t.ptrs_are_device = int(ci.numel()), 1
             self._keep += [rp, ci]
+        if t.kind == TOPO_COMPRESSED:
+            cm = topo["compressed"]
+            t.compressed = C.cast(cm.ptr, C.c_void_p)
+            self._keep.append(cm)
         self.desc = d
         self.params = make_params(model, params)
         with torch.cuda.device(self.device):

@@ -65,6 +65,14 @@ static int32_t validate(net* h, const net_desc* d) {
             if (d->n < 2 || t.in_degree < 0 || (int64_t)t.in_degree > d->n - 1)
                 return set_err(h, NET_ERR_INVALID, "random graph: need n >= 2 and 0 <= in_degree <= n-1");
             break;
+        case NET_TOPO_COMPRESSED: {
+            const net_compressed* c = t.compressed;
+            if (!c || !c->c || !c->d_ptr || (c->v_len > 0 && !c->v_pos)) return set_err(h, NET_ERR_INVALID, "compressed matrix: NULL struct or arrays");
+            if (c->n != d->n) return set_err(h, NET_ERR_INVALID, "compressed matrix: n %lld != desc n %lld", (long long)c->n, (long long)d->n);
+            if (c->k < 1 || c->v_len < 0 || c->v_len > d->n || c->d_ptr[0] != 0 || c->d_ptr[c->k] < 0)
+                return set_err(h, NET_ERR_INVALID, "compressed matrix: bad table sizes");
+            break;
+        }
         default: return set_err(h, NET_ERR_INVALID, "unknown topology kind %d", t.kind);
     }
     return NET_OK;
@@ -119,6 +127,14 @@ static Layout make_layout(const net_desc* d, char* base) {
         size_t nnz = t.kind == NET_TOPO_CSR ? (size_t)t.nnz : (size_t)d->n * (size_t)t.in_degree;
         L.b.row_ptr = (int64_t*)P(sizeof(int64_t) * (size_t)(d->n + 1));
         L.b.col_idx = (int32_t*)P(sizeof(int32_t) * (nnz + 1));
+    }
+    if (t.kind == NET_TOPO_COMPRESSED) {
+        const net_compressed* c = t.compressed;
+        L.b.cmp_v = (int32_t*)P(sizeof(int32_t) * (size_t)(c->v_len + 1));
+        L.b.cmp_dptr = (int64_t*)P(sizeof(int64_t) * (size_t)(c->k + 1));
+        L.b.cmp_dpos = (int32_t*)P(sizeof(int32_t) * (size_t)(c->d_ptr[c->k] + 1));
+        L.b.cmp_c = (int32_t*)P(sizeof(int32_t) * (size_t)d->n);
+        L.b.cmp_deg = (int32_t*)P(sizeof(int32_t) * (size_t)c->k);
     }
     L.b.flag = (int32_t*)P(64);
     L.b.obs_theta_prev = (double*)P(sizeof(double) * d->n);
@@ -386,6 +402,7 @@ int32_t net_create(const net_desc* user_desc, const void* params, size_t params_
     h->desc = *desc;
     h->desc.topo.row_ptr = nullptr;  // the caller's arrays are not kept
     h->desc.topo.col_idx = nullptr;
+    h->desc.topo.compressed = nullptr;
     h->nvar = model_nvar(desc->model);
     h->esize = desc->dtype == NET_F32 ? 4 : 8;
     h->n = desc->n;
@@ -405,9 +422,11 @@ int32_t net_create(const net_desc* user_desc, const void* params, size_t params_
     // the caller's topology pointers are needed once, by the builder
     h->desc.topo.row_ptr = desc->topo.row_ptr;
     h->desc.topo.col_idx = desc->topo.col_idx;
+    h->desc.topo.compressed = desc->topo.compressed;
     rc = topo_build(h);
     h->desc.topo.row_ptr = nullptr;
     h->desc.topo.col_idx = nullptr;
+    h->desc.topo.compressed = nullptr;
     if (rc == NET_OK) rc = fast_prepare(h);
     cudaError_t e = cudaSuccess;
     if (rc == NET_OK) {
@@ -602,6 +621,29 @@ int32_t net_get_topology(net_t* h, int64_t row_begin, int64_t row_count, int64_t
         for (int64_t r = 0; r <= row_count; ++r) row_ptr[r] -= base;
         if (cnt > 0) OSC_CUDA(h, cudaMemcpyAsync(col_idx, h->b.col_idx + base, sizeof(int32_t) * cnt, cudaMemcpyDeviceToHost, h->stream));
         OSC_CUDA(h, cudaStreamSynchronize(h->stream));
+        return NET_OK;
+    }
+    if (h->tv.kind == NET_TOPO_COMPRESSED) {
+        // EXTRACT chunk by chunk through the staging scratch (rows of at most cmp_maxdeg entries)
+        const size_t per_row = sizeof(int32_t) * (size_t)(h->tv.cmp_maxdeg > 0 ? h->tv.cmp_maxdeg : 1) + sizeof(int64_t);
+        int64_t chunk = (int64_t)((h->b.scratch_bytes - 512) / per_row);
+        if (chunk < 1) return set_err(h, NET_ERR_SIZE, "staging scratch too small for one row");
+        int64_t base = 0;
+        row_ptr[0] = 0;
+        for (int64_t r0 = 0; r0 < row_count; r0 += chunk) {
+            const int64_t rows = row_count - r0 < chunk ? row_count - r0 : chunk;
+            int64_t* d_ptr = (int64_t*)h->b.scratch;
+            int32_t* d_idx = (int32_t*)((char*)h->b.scratch + round_up((int64_t)sizeof(int64_t) * (rows + 1), 256));
+            int32_t rc = topo_expand(h, row_begin + r0, rows, d_ptr, d_idx);
+            if (rc) return rc;
+            OSC_CUDA(h, cudaMemcpyAsync(row_ptr + r0 + 1, d_ptr + 1, sizeof(int64_t) * rows, cudaMemcpyDeviceToHost, h->stream));
+            OSC_CUDA(h, cudaStreamSynchronize(h->stream));
+            const int64_t cnt = row_ptr[r0 + rows];
+            if (cnt > 0) OSC_CUDA(h, cudaMemcpyAsync(col_idx + base, d_idx, sizeof(int32_t) * cnt, cudaMemcpyDeviceToHost, h->stream));
+            OSC_CUDA(h, cudaStreamSynchronize(h->stream));
+            for (int64_t r = 1; r <= rows; ++r) row_ptr[r0 + r] += base;
+            base += cnt;
+        }
         return NET_OK;
     }
     // ring / lattice: expand chunk by chunk through the staging scratch.  That region also holds

@@ -82,6 +82,9 @@ static int32_t launch_topo(net* h, const StageArgs& a) {
         case NET_TOPO_CSR:
             direct_stage_kernel<T, MODEL, NET_TOPO_CSR><<<g, b, 0, h->stream>>>(a, h->mp, h->tv);
             break;
+        case NET_TOPO_COMPRESSED:
+            direct_stage_kernel<T, MODEL, NET_TOPO_COMPRESSED><<<g, b, 0, h->stream>>>(a, h->mp, h->tv);
+            break;
         default:
             direct_stage_kernel<T, MODEL, NET_TOPO_RANDOM_INDEGREE><<<g, b, 0, h->stream>>>(a, h->mp, h->tv);
             break;

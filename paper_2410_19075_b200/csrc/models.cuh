@@ -134,6 +134,32 @@ __device__ __forceinline__ int for_each_neighbor(const TopoView& tv, int64_t n, 
             f(((int64_t)zz * ny + yy) * nx + xx);
         }
         return tv.noff;
+    } else if (TOPO == NET_TOPO_COMPRESSED) {
+        // EXTRACT of Alg. 2: row i = (p + i) mod n for p in XOR(V, D[C_i])
+        const int c = tv.cmp_c[i];
+        int64_t b = tv.cmp_dptr[c];
+        const int64_t be = tv.cmp_dptr[c + 1];
+        const int ae = tv.cmp_vlen;
+        if (b == be) {                      // empty difference: the common pattern shifted by i
+            for (int a = 0; a < ae; ++a) {
+                int64_t j = i + tv.cmp_v[a];
+                if (j >= n) j -= n;
+                f(j);
+            }
+            return ae;
+        }
+        int a = 0, deg = 0;                 // symmetric difference of two sorted position lists
+        while (a < ae || b < be) {
+            const int32_t pv = a < ae ? tv.cmp_v[a] : 0x7fffffff;
+            const int32_t pd = b < be ? tv.cmp_dpos[b] : 0x7fffffff;
+            if (pv == pd) { ++a; ++b; continue; }
+            int64_t j = i + (pv < pd ? pv : pd);
+            if (pv < pd) ++a; else ++b;
+            if (j >= n) j -= n;
+            f(j);
+            ++deg;
+        }
+        return deg;
     } else if (TOPO == NET_TOPO_CSR) {
         int64_t b = tv.row_ptr[i], e = tv.row_ptr[i + 1];
         for (int64_t q = b; q < e; ++q) f((int64_t)tv.col_idx[q]);

@@ -170,6 +170,7 @@ int32_t obs_local_order(net* h, const double* d_theta, double* d_out) {
         case NET_TOPO_RING: local_order_kernel<NET_TOPO_RING><<<g, 256, 0, h->stream>>>(h->tv, h->n, h->b.obs_tmp, d_out); break;
         case NET_TOPO_LATTICE: local_order_kernel<NET_TOPO_LATTICE><<<g, 256, 0, h->stream>>>(h->tv, h->n, h->b.obs_tmp, d_out); break;
         case NET_TOPO_CSR: local_order_kernel<NET_TOPO_CSR><<<g, 256, 0, h->stream>>>(h->tv, h->n, h->b.obs_tmp, d_out); break;
+        case NET_TOPO_COMPRESSED: local_order_kernel<NET_TOPO_COMPRESSED><<<g, 256, 0, h->stream>>>(h->tv, h->n, h->b.obs_tmp, d_out); break;
         default: local_order_kernel<NET_TOPO_RANDOM_INDEGREE><<<g, 256, 0, h->stream>>>(h->tv, h->n, h->b.obs_tmp, d_out); break;
     }
     h->launches += 2;

@@ -36,6 +36,13 @@ struct TopoView {
     const int32_t* off;    // lattice: noff x (dx,dy,dz), sorted by (dz,dy,dx)
     const int64_t* row_ptr;
     const int32_t* col_idx;
+    // NET_TOPO_COMPRESSED (Alg. 2): common vector, difference table, row references, degree per entry
+    const int32_t* cmp_v;
+    const int64_t* cmp_dptr;
+    const int32_t* cmp_dpos;
+    const int32_t* cmp_c;
+    const int32_t* cmp_deg;
+    int32_t cmp_vlen, cmp_k, cmp_maxdeg;
 };
 
 // RK4 in the low-traffic form: four state-sized arrays
@@ -79,6 +86,11 @@ struct Buffers {
     int32_t* off;                 // lattice offsets
     int64_t* row_ptr;
     int32_t* col_idx;
+    int32_t* cmp_v;               // NET_TOPO_COMPRESSED: V, D (ptr, pos), C, degree per table entry
+    int64_t* cmp_dptr;
+    int32_t* cmp_dpos;
+    int32_t* cmp_c;
+    int32_t* cmp_deg;
     int32_t* flag;                // device error/validation flag (4 ints)
     // observables
     double* obs_theta_prev;       // n

@@ -3,6 +3,8 @@
 // (parity hook).  Integer-only; results are bit-exact by construction.
 // Rules: PAPER.md:299-301 (ring), :309-313 (disc / ball, index map), :147 (orientation);
 // random graph: DESIGN.md reading R8.
+#include <stdlib.h>
+
 #include "oscnet_internal.cuh"
 
 namespace oscnet {
@@ -197,6 +199,65 @@ __global__ void copy_rows_kernel(const int64_t* row_ptr, const int32_t* col_idx,
     for (int64_t e = tid; e < cnt; e += stride) out_idx[e] = col_idx[base + e];
 }
 
+// NET_TOPO_COMPRESSED: degrees of a row range (EXTRACT counts), then the rows themselves, sorted
+__global__ void compressed_degree_kernel(TopoView tv, int64_t row_begin, int64_t row_count, int64_t* out_ptr) {
+    for (int64_t r = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; r <= row_count; r += (int64_t)gridDim.x * blockDim.x)
+        out_ptr[r] = r == 0 ? 0 : tv.cmp_deg[tv.cmp_c[row_begin + r - 1]];
+}
+
+// in-place inclusive scan of ptr[0..count] by one CTA (count + 1 values; ptr[0] = 0)
+__global__ void __launch_bounds__(1024) scan_i64_kernel(int64_t* ptr, int64_t count) {
+    __shared__ int64_t wsum[32];
+    __shared__ int64_t carry_s;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    if (threadIdx.x == 0) carry_s = 0;
+    __syncthreads();
+    for (int64_t base = 0; base <= count; base += 1024) {
+        const int64_t s = base + threadIdx.x;
+        int64_t v = s <= count ? ptr[s] : 0;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            int64_t u = __shfl_up_sync(0xffffffffu, v, o);
+            if (lane >= o) v += u;
+        }
+        if (lane == 31) wsum[warp] = v;
+        __syncthreads();
+        int64_t off = carry_s;
+        for (int w = 0; w < warp; ++w) off += wsum[w];
+        v += off;
+        if (s <= count) ptr[s] = v;
+        __syncthreads();
+        if (threadIdx.x == 1023) carry_s = v;
+        __syncthreads();
+    }
+}
+
+__global__ void compressed_expand_kernel(TopoView tv, int64_t n, int64_t row_begin, int64_t row_count,
+                                         const int64_t* out_ptr, int32_t* col_idx) {
+    for (int64_t r = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; r < row_count; r += (int64_t)gridDim.x * blockDim.x) {
+        const int64_t i = row_begin + r;
+        int32_t* row = col_idx + out_ptr[r];
+        const int c = tv.cmp_c[i];
+        int64_t b = tv.cmp_dptr[c];
+        const int64_t be = tv.cmp_dptr[c + 1];
+        int a = 0, have = 0;
+        // positions p ascend; (p + i) mod n ascends too except at the single wrap: entries that wrap
+        // (p + i >= n) are smaller than all that do not, so they are written first
+        for (int pass = 0; pass < 2; ++pass) {
+            a = 0; b = tv.cmp_dptr[c];
+            while (a < tv.cmp_vlen || b < be) {
+                const int32_t pv = a < tv.cmp_vlen ? tv.cmp_v[a] : 0x7fffffff;
+                const int32_t pd = b < be ? tv.cmp_dpos[b] : 0x7fffffff;
+                if (pv == pd) { ++a; ++b; continue; }
+                const int64_t j = i + (pv < pd ? pv : pd);
+                if (pv < pd) ++a; else ++b;
+                if (pass == 0 && j >= n) row[have++] = (int32_t)(j - n);
+                if (pass == 1 && j < n) row[have++] = (int32_t)j;
+            }
+        }
+    }
+}
+
 static unsigned grid_for(int64_t items) {
     int64_t b = (items + 255) / 256;
     if (b < 1) b = 1;
@@ -252,6 +313,48 @@ int32_t topo_build(net* h) {
         tv.col_idx = h->b.col_idx;
         h->nnz = t.nnz;
         h->degree_uniform = f[2] ? -1 : f[1];
+    } else if (t.kind == NET_TOPO_COMPRESSED) {
+        // V, D, C of Alg. 2 go to the workspace as they are; validated on the host
+        const net_compressed* c = t.compressed;
+        const int64_t n = h->n, dtot = c->d_ptr[c->k];
+        for (int64_t q = 0; q < c->v_len; ++q)
+            if (c->v_pos[q] < 0 || c->v_pos[q] >= n || (q > 0 && c->v_pos[q] <= c->v_pos[q - 1]))
+                return set_err(h, NET_ERR_TOPOLOGY, "compressed matrix: common vector not sorted / out of range");
+        int32_t* deg = (int32_t*)malloc(sizeof(int32_t) * (size_t)c->k);
+        if (!deg) return set_err(h, NET_ERR_INVALID, "out of host memory");
+        int32_t maxdeg = 0;
+        for (int64_t e = 0; e < c->k; ++e) {
+            const int64_t b = c->d_ptr[e], be = c->d_ptr[e + 1];
+            if (be < b || be > dtot) { free(deg); return set_err(h, NET_ERR_TOPOLOGY, "compressed matrix: d_ptr not monotone"); }
+            int64_t common = 0, a = 0;
+            for (int64_t q = b; q < be; ++q) {
+                const int32_t p = c->d_pos[q];
+                if (p < 0 || p >= n || (q > b && p <= c->d_pos[q - 1])) { free(deg); return set_err(h, NET_ERR_TOPOLOGY, "compressed matrix: table entry not sorted / out of range"); }
+                while (a < c->v_len && c->v_pos[a] < p) ++a;
+                if (a < c->v_len && c->v_pos[a] == p) ++common;
+            }
+            deg[e] = (int32_t)(c->v_len + (be - b) - 2 * common);      // |V xor D_e|
+            if (deg[e] > maxdeg) maxdeg = deg[e];
+        }
+        int64_t nnz = 0;
+        bool uniform = true;
+        for (int64_t i = 0; i < n; ++i) {
+            if (c->c[i] < 0 || c->c[i] >= c->k) { free(deg); return set_err(h, NET_ERR_TOPOLOGY, "compressed matrix: row reference outside the table"); }
+            nnz += deg[c->c[i]];
+            uniform = uniform && deg[c->c[i]] == deg[c->c[0]];
+        }
+        OSC_CUDA(h, cudaMemcpyAsync(h->b.cmp_v, c->v_pos, sizeof(int32_t) * c->v_len, cudaMemcpyHostToDevice, st));
+        OSC_CUDA(h, cudaMemcpyAsync(h->b.cmp_dptr, c->d_ptr, sizeof(int64_t) * (c->k + 1), cudaMemcpyHostToDevice, st));
+        if (dtot > 0) OSC_CUDA(h, cudaMemcpyAsync(h->b.cmp_dpos, c->d_pos, sizeof(int32_t) * dtot, cudaMemcpyHostToDevice, st));
+        OSC_CUDA(h, cudaMemcpyAsync(h->b.cmp_c, c->c, sizeof(int32_t) * n, cudaMemcpyHostToDevice, st));
+        OSC_CUDA(h, cudaMemcpyAsync(h->b.cmp_deg, deg, sizeof(int32_t) * c->k, cudaMemcpyHostToDevice, st));
+        OSC_CUDA(h, cudaStreamSynchronize(st));
+        h->degree_uniform = uniform ? deg[c->c[0]] : -1;
+        free(deg);
+        tv.cmp_v = h->b.cmp_v; tv.cmp_dptr = h->b.cmp_dptr; tv.cmp_dpos = h->b.cmp_dpos;
+        tv.cmp_c = h->b.cmp_c; tv.cmp_deg = h->b.cmp_deg;
+        tv.cmp_vlen = (int32_t)c->v_len; tv.cmp_k = (int32_t)c->k; tv.cmp_maxdeg = maxdeg;
+        h->nnz = nnz;
     } else {  // RANDOM_INDEGREE
         random_indegree_kernel<<<grid_for(h->n), 256, 0, st>>>(h->n, t.in_degree, t.seed, h->b.col_idx);
         uniform_row_ptr_kernel<<<grid_for(h->n + 1), 256, 0, st>>>(h->b.row_ptr, h->n, t.in_degree);
@@ -269,6 +372,14 @@ int32_t topo_build(net* h) {
 int32_t topo_expand(net* h, int64_t row_begin, int64_t row_count, int64_t* d_row_ptr,
                     int32_t* d_col_idx) {
     cudaStream_t st = h->stream;
+    if (h->tv.kind == NET_TOPO_COMPRESSED) {
+        compressed_degree_kernel<<<grid_for(row_count + 1), 256, 0, st>>>(h->tv, row_begin, row_count, d_row_ptr);
+        scan_i64_kernel<<<1, 1024, 0, st>>>(d_row_ptr, row_count);
+        if (row_count > 0) compressed_expand_kernel<<<grid_for(row_count), 256, 0, st>>>(h->tv, h->n, row_begin, row_count, d_row_ptr, d_col_idx);
+        h->launches += 3;
+        OSC_CUDA(h, cudaGetLastError());
+        return NET_OK;
+    }
     if (h->tv.kind == NET_TOPO_RING || h->tv.kind == NET_TOPO_LATTICE) {
         int32_t deg = h->degree_uniform;
         uniform_row_ptr_kernel<<<grid_for(row_count + 1), 256, 0, st>>>(d_row_ptr, row_count, deg);
