@@ -12,8 +12,8 @@ import numpy as np
 
 from .build import build
 
-MODEL_KS, MODEL_FHN, MODEL_HH, MODEL_KSI = 0, 1, 2, 3
-NVAR = {MODEL_KS: 1, MODEL_FHN: 2, MODEL_HH: 4, MODEL_KSI: 2}
+MODEL_KS, MODEL_FHN, MODEL_HH, MODEL_KSI, MODEL_FHN2, MODEL_HHS = 0, 1, 2, 3, 4, 5
+NVAR = {MODEL_KS: 1, MODEL_FHN: 2, MODEL_HH: 4, MODEL_KSI: 2, MODEL_FHN2: 2, MODEL_HHS: 5}
 
 _lib = None
 
@@ -30,6 +30,8 @@ def lib():
         _lib = C.CDLL(build())
         _lib.ora_lattice_degree.restype = C.c_int64
         _lib.ora_lattice_degree.argtypes = [C.c_int32, C.c_int32, C.c_int32]
+        _lib.ora_gauss.restype = C.c_double
+        _lib.ora_gauss.argtypes = [C.c_uint64, C.c_int64, C.c_int64]
     return _lib
 
 
@@ -143,6 +145,35 @@ class OracleNet:
         return cls(MODEL_HH, n, row_ptr, col_idx,
                    [p[k] for k in ("gNa", "gK", "gL", "ENa", "EK", "EL", "C", "g_syn",
                                    "E_syn", "theta_syn", "k_syn")], I_ext)
+
+    @classmethod
+    def fhn2(cls, n, row_ptr, col_idx, eps, a, sigma, I_app=0.0):
+        """FitzHugh-Nagumo exactly as eq. (2) PAPER.md:70-75 (x-only coupling, I_app); the delay and
+        the noise belong to the integrator (fhn2_rk4).  SURVEY.md 8(f).4, reading R17."""
+        return cls(MODEL_FHN2, n, row_ptr, col_idx, [eps, a, sigma, I_app])
+
+    @classmethod
+    def hhs(cls, n, row_ptr, col_idx, I_ext, a_s=2.0, b_s=0.5, **kw):
+        """Hodgkin-Huxley with the synaptic gating ODE of eq. (1) (reading R18); state [V|m|h|n|s]."""
+        p = dict(HH_DEFAULT)
+        p.update(kw)
+        return cls(MODEL_HHS, n, row_ptr, col_idx,
+                   [p[k] for k in ("gNa", "gK", "gL", "ENa", "EK", "EL", "C", "g_syn",
+                                   "E_syn", "theta_syn", "k_syn")] + [a_s, b_s], I_ext)
+
+    def fhn2_rk4(self, y, n_steps, dt, m=0, D=0.0, seed=0, hist=None):
+        """RK4 steps of eq. (2) with delay tau = m dt and noise amplitude D (ora_fhn2_rk4).
+        hist: None to start from the constant initial function, or the dict a previous call returned
+        to continue.  Returns (state, hist)."""
+        y = np.array(y, dtype=np.float64).reshape(2 * self.n)
+        if hist is None:
+            hist = dict(step=0, x=np.zeros((m + 2) * self.n), d=np.zeros((m + 2) * self.n))
+        rc = lib().ora_fhn2_rk4(C.byref(self._s), _p(y), C.c_int64(n_steps), C.c_double(dt),
+                                C.c_int64(m), C.c_double(D), C.c_uint64(seed),
+                                C.c_int64(hist["step"]), _p(hist["x"]), _p(hist["d"]))
+        assert rc == 0
+        hist = dict(hist, step=hist["step"] + n_steps)
+        return y.reshape(2, self.n), hist
 
     @property
     def nvar(self):
@@ -267,6 +298,11 @@ class OracleNet:
                     Rloc_mean=float(self.local_order(theta).mean()),
                     vel_mean=float(vel.mean()), vel_std=float(vel.std()),
                     n_samples=int(Rs.size), vel=vel, y=y)
+
+
+def gauss(seed, i, n):
+    """Standard normal deviate (i, n) of the counter-based stream `seed` (ora_gauss)."""
+    return float(lib().ora_gauss(C.c_uint64(seed), C.c_int64(i), C.c_int64(n)))
 
 
 def hh_steady_gates(V):

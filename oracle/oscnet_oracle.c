@@ -49,6 +49,8 @@
 #define ORA_MODEL_FHN 1
 #define ORA_MODEL_HH 2
 #define ORA_MODEL_KSI 3   /* Kuramoto-Sakaguchi with inertia, eq. (3) in full (next row) */
+#define ORA_MODEL_FHN2 4  /* FitzHugh-Nagumo exactly as eq. (2): x-only coupling, delay, noise, I_app (8(f).4) */
+#define ORA_MODEL_HHS 5   /* Hodgkin-Huxley with the synaptic gating ODE of eq. (1) (8(f).4) */
 
 /* ------------------------------------------------------------------ */
 /* Topology: canonical CSR, rows = in-neighbour lists (PAPER.md:147:    */
@@ -198,7 +200,7 @@ typedef struct {
 
 int32_t ora_nvar(int32_t model) {
     return model == ORA_MODEL_KS ? 1 : model == ORA_MODEL_FHN ? 2 : model == ORA_MODEL_HH ? 4 :
-           model == ORA_MODEL_KSI ? 2 : -1;
+           model == ORA_MODEL_KSI ? 2 : model == ORA_MODEL_FHN2 ? 2 : model == ORA_MODEL_HHS ? 5 : -1;
 }
 
 /* Kuramoto-Sakaguchi (eq. (3) with m=0, eps=1, mu=1/Omega, PAPER.md:79, :107;
@@ -332,9 +334,69 @@ static void rhs_hh(const ora_net* net, const double* y, double* f) {
     }
 }
 
-/* One full right-hand-side evaluation f(y); y and f are nvar*n SoA. */
+/* FitzHugh-Nagumo exactly as the paper prints it, eq. (2) PAPER.md:70-75:
+ *   eps dx_i/dt = x_i - x_i^3/3 - y_i + sum_j L_ij s_ij (x_j(t - tau) - x_i) + I_app
+ *       dy_i/dt = x_i + a + D n(t)
+ * with uniform coupling strength s_ij = sigma / Omega_i (reading R17).  This function is the
+ * deterministic part given the DELAYED fast variable xd_j = x_j(t - tau) of every element (xd = x
+ * itself when tau = 0); the noise term is added by the integrator (ora_fhn2_rk4).
+ * p = {eps, a, sigma, I_app}. */
+static void rhs_fhn2(const ora_net* net, const double* y, const double* xd, double* f) {
+    const int64_t n = net->n;
+    const double eps = net->p[0], a = net->p[1], sigma = net->p[2], Iapp = net->p[3];
+    const double* x = y;
+    const double* v = y + n;
+#pragma omp parallel for schedule(static)
+    for (int64_t i = 0; i < n; ++i) {
+        double Cx = 0.0;
+        int64_t links_amount = 0;
+        for (int64_t e = net->row_ptr[i]; e < net->row_ptr[i + 1]; ++e, ++links_amount)
+            Cx += xd[net->col_idx[e]] - x[i];
+        double s = links_amount > 0 ? sigma / (double)links_amount : 0.0;
+        f[i] = (x[i] - x[i] * x[i] * x[i] / 3.0 - v[i] + s * Cx + Iapp) / eps;
+        f[n + i] = x[i] + a;
+    }
+}
+
+/* Hodgkin-Huxley element with the synaptic gating ODE of eq. (1) ("ds_ik/dt =
+ * p_ik(U_i, s_ik, n_j)", s_ik "the synaptic conductivity from the k-th to the i-th neuron").
+ * Reading R18: p depends on the presynaptic voltage only, so all links leaving element k share
+ * one gating variable s_k with first-order kinetics driven by the same sigmoid as rhs_hh:
+ *   ds_k/dt = a_s S(V_k) (1 - s_k) - b_s s_k,   S(V) = 1/(1+exp(-(V-theta_syn)/k_syn)),
+ *   I_syn,i = (g_syn/Omega_i)(E_syn - V_i) sum_{k in row i} s_k.
+ * State SoA [V | m | h | n | s].  p = HH's eleven parameters, then a_s (p[11]), b_s (p[12]). */
+static void rhs_hhs(const ora_net* net, const double* y, double* f) {
+    const int64_t n = net->n;
+    const double gNa = net->p[0], gK = net->p[1], gL = net->p[2];
+    const double ENa = net->p[3], EK = net->p[4], EL = net->p[5], C = net->p[6];
+    const double gsyn = net->p[7], Esyn = net->p[8], th = net->p[9], ks = net->p[10];
+    const double as = net->p[11], bs = net->p[12];
+    const double *V = y, *m = y + n, *h = y + 2 * n, *g = y + 3 * n, *sg = y + 4 * n;
+#pragma omp parallel for schedule(static)
+    for (int64_t i = 0; i < n; ++i) {
+        double ssum = 0.0;
+        int64_t links_amount = 0;
+        for (int64_t e = net->row_ptr[i]; e < net->row_ptr[i + 1]; ++e, ++links_amount)
+            ssum += sg[net->col_idx[e]];
+        double Isyn = links_amount > 0 ? (gsyn / (double)links_amount) * (Esyn - V[i]) * ssum : 0.0;
+        double am, bm, ah, bh, an, bn;
+        hh_rates(V[i], &am, &bm, &ah, &bh, &an, &bn);
+        double INa = gNa * m[i] * m[i] * m[i] * h[i] * (V[i] - ENa);
+        double IK = gK * g[i] * g[i] * g[i] * g[i] * (V[i] - EK);
+        double IL = gL * (V[i] - EL);
+        f[i] = (net->elem_param[i] - INa - IK - IL + Isyn) / C;
+        f[n + i] = am * (1.0 - m[i]) - bm * m[i];
+        f[2 * n + i] = ah * (1.0 - h[i]) - bh * h[i];
+        f[3 * n + i] = an * (1.0 - g[i]) - bn * g[i];
+        f[4 * n + i] = as * (1.0 / (1.0 + exp(-(V[i] - th) / ks))) * (1.0 - sg[i]) - bs * sg[i];
+    }
+}
+
+/* One full right-hand-side evaluation f(y); y and f are nvar*n SoA.  (FHN2: without delay.) */
 int ora_rhs(const ora_net* net, const double* y, double* f) {
     switch (net->model) {
+        case ORA_MODEL_FHN2: rhs_fhn2(net, y, y, f); return 0;
+        case ORA_MODEL_HHS: rhs_hhs(net, y, f); return 0;
         case ORA_MODEL_KS: rhs_ks(net, y, f); return 0;
         case ORA_MODEL_FHN: rhs_fhn(net, y, f); return 0;
         case ORA_MODEL_HH: rhs_hh(net, y, f); return 0;
@@ -395,7 +457,7 @@ void ora_phase(int32_t model, int64_t n, const double* y, const double* pm, doub
     for (int64_t i = 0; i < n; ++i) {
         if (model == ORA_MODEL_KS || model == ORA_MODEL_KSI)
             theta[i] = y[i];
-        else if (model == ORA_MODEL_FHN)
+        else if (model == ORA_MODEL_FHN || model == ORA_MODEL_FHN2)
             theta[i] = atan2(y[n + i], y[i]);
         else
             theta[i] = atan2(y[3 * n + i] - pm[1], (y[i] - pm[0]) / pm[2]);
@@ -716,4 +778,89 @@ int ora_dp5(const ora_net* net, double* y, double t0, double t_end, double rtol,
     out[0] = (double)acc_n; out[1] = (double)rej_n; out[2] = h_used; out[3] = h; out[4] = t;
     free(buf);
     return rc;
+}
+
+
+/* ------------------------------------------------------------------ */
+/* Eq. (2) with delay tau and noise D n(t) under fixed-step RK4        */
+/* (reading R17).  The paper's own solvers keep       */
+/* "data from previous time steps and perform interpolation"           */
+/* (PAPER.md:101); with a fixed step that becomes:                     */
+/*   tau = m dt, m >= 0 an integer;                                     */
+/*   history: x_j and dx_j/dt at the step times t_n (dx/dt = the k1 of  */
+/*     that step), m + 2 slots, slot of step q = q mod (m + 2); before  */
+/*     the first step every slot holds the initial x with derivative 0  */
+/*     (constant initial function);                                     */
+/*   the RK4 stages at t_n, t_n + dt/2, t_n + dt/2, t_n + dt see        */
+/*     x_j(t_n - tau) = H[n-m],                                          */
+/*     x_j(t_n + dt/2 - tau) = cubic Hermite midpoint of H[n-m], H[n-m+1] */
+/*        = (xa + xb)/2 + dt/8 (da - db),                               */
+/*     x_j(t_n + dt - tau) = H[n-m+1]                                    */
+/*     (while n < m the interval [t_n - tau, t_n + dt - tau] lies in     */
+/*     t <= 0 and the midpoint is the constant initial value: dx/dt has  */
+/*     a jump at t = 0, the stored derivative there is the right one)    */
+/*     (m = 0: the stage values themselves, an ordinary coupling);      */
+/*   noise: additive Gaussian white noise on y by Euler-Maruyama after  */
+/*     the deterministic step, y_i += D sqrt(dt) xi(seed, i, n), with   */
+/*     xi from a counter-based generator (ora_gauss) so that any other  */
+/*     implementation of the same rule draws the same numbers.          */
+/* ------------------------------------------------------------------ */
+
+/* Standard normal deviate number (i, n) of stream `seed`: two 53-bit uniforms from the splitmix64
+ * finaliser of reading R8, Box-Muller cosine branch.
+ *   a = mix(mix(seed + G (i+1)) + G (2n+1)), b = mix(mix(seed + G (i+1)) + G (2n+2)),
+ *   u1 = ((a >> 11) + 1) / 2^53 in (0, 1], u2 = (b >> 11) / 2^53 in [0, 1),
+ *   xi = sqrt(-2 ln u1) cos(2 pi u2). */
+double ora_gauss(uint64_t seed, int64_t i, int64_t n) {
+    const uint64_t G = 0x9E3779B97F4A7C15ULL;
+    const uint64_t hi = ora_mix64(seed + G * (uint64_t)(i + 1));
+    const uint64_t a = ora_mix64(hi + G * (uint64_t)(2 * n + 1));
+    const uint64_t b = ora_mix64(hi + G * (uint64_t)(2 * n + 2));
+    const double u1 = ((double)(a >> 11) + 1.0) * (1.0 / 9007199254740992.0);
+    const double u2 = (double)(b >> 11) * (1.0 / 9007199254740992.0);
+    return sqrt(-2.0 * log(u1)) * cos(6.283185307179586476925286766559 * u2);
+}
+
+/* n_steps RK4 steps of ORA_MODEL_FHN2 with delay m dt.  hist_x, hist_d: (m + 2) * n doubles each,
+ * owned by the caller and carried from call to call; step0 = number of steps taken before this
+ * call (0: the history is initialised here).  D = 0: no noise. */
+int ora_fhn2_rk4(const ora_net* net, double* y, int64_t n_steps, double dt, int64_t m, double D,
+                 uint64_t seed, int64_t step0, double* hist_x, double* hist_d) {
+    if (net->model != ORA_MODEL_FHN2 || m < 0) return -1;
+    const int64_t n = net->n, len = 2 * n, S = m + 2;
+    double* buf = (double*)malloc(sizeof(double) * (size_t)(5 * len + n));
+    if (!buf) return -2;
+    double *k1 = buf, *k2 = buf + len, *k3 = buf + 2 * len, *k4 = buf + 3 * len, *tmp = buf + 4 * len;
+    double* xd = buf + 5 * len;
+    if (step0 == 0)
+        for (int64_t q = 0; q < S; ++q)
+            for (int64_t i = 0; i < n; ++i) { hist_x[q * n + i] = y[i]; hist_d[q * n + i] = 0.0; }
+    for (int64_t st = step0; st < step0 + n_steps; ++st) {
+        const int64_t qa = ((st - m) % S + S) % S, qb = ((st - m + 1) % S + S) % S, qn = st % S;
+        const double *xa = hist_x + qa * n, *da = hist_d + qa * n;
+        const double *xb = hist_x + qb * n, *db = hist_d + qb * n;
+        /* stage 1 at t_n */
+        for (int64_t i = 0; i < n; ++i) hist_x[qn * n + i] = y[i];       /* x at t_n (qa == qn when m = 0) */
+        rhs_fhn2(net, y, m > 0 ? xa : y, k1);
+        for (int64_t i = 0; i < n; ++i) hist_d[qn * n + i] = k1[i];      /* dx/dt at t_n */
+        /* stages 2, 3 at t_n + dt/2 */
+        if (m > 0)
+            for (int64_t i = 0; i < n; ++i)      /* st < m: the whole interval lies in t <= 0, constant history */
+                xd[i] = st < m ? xa[i] : 0.5 * (xa[i] + xb[i]) + 0.125 * dt * (da[i] - db[i]);
+        for (int64_t q = 0; q < len; ++q) tmp[q] = y[q] + 0.5 * dt * k1[q];
+        rhs_fhn2(net, tmp, m > 0 ? xd : tmp, k2);
+        for (int64_t q = 0; q < len; ++q) tmp[q] = y[q] + 0.5 * dt * k2[q];
+        rhs_fhn2(net, tmp, m > 0 ? xd : tmp, k3);
+        /* stage 4 at t_n + dt */
+        for (int64_t q = 0; q < len; ++q) tmp[q] = y[q] + dt * k3[q];
+        rhs_fhn2(net, tmp, m > 0 ? xb : tmp, k4);
+        for (int64_t q = 0; q < len; ++q)
+            y[q] = y[q] + (dt / 6.0) * (k1[q] + 2.0 * k2[q] + 2.0 * k3[q] + k4[q]);
+        if (D != 0.0) {
+            const double amp = D * sqrt(dt);
+            for (int64_t i = 0; i < n; ++i) y[n + i] += amp * ora_gauss(seed, i, st);
+        }
+    }
+    free(buf);
+    return 0;
 }
