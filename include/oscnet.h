@@ -31,7 +31,8 @@
  *    call as NET_ERR_CUDA.
  *  - State layout: structure of arrays [nvar][n], element type = the dtype of
  *    the net (float or double), contiguous (variable v of element i at
- *    v*n + i).  nvar: KS 1 (phi); FHN 2 (u, v); HH 4 (V, m, h, n).
+ *    v*n + i).  nvar: KS 1 (phi); FHN 2 (u, v); HH 4 (V, m, h, n); KSI 2 (phi, psi); FHN2 2 (x, y);
+ *    HHS 5 (V, m, h, n, s).
  *  - Element numbering of lattices: site (i,j,k) is element k*nx*ny + j*nx + i
  *    (PAPER.md:309 "jN1+i", :311 "kN1^2+jN1+i").
  *  - CSR orientation: row i lists the elements j that influence i
@@ -59,7 +60,9 @@ enum {
 };
 
 enum { NET_MODEL_KS = 0, NET_MODEL_FHN = 1, NET_MODEL_HH = 2,
-       NET_MODEL_KSI = 3 /* KS with inertia; FAST on rings, DIRECT elsewhere in this build */ };
+       NET_MODEL_KSI = 3,  /* KS with inertia, eq. (3) in full */
+       NET_MODEL_FHN2 = 4, /* FHN exactly as eq. (2): x-only coupling, delay, noise, I_app (DIRECT kernels) */
+       NET_MODEL_HHS = 5   /* HH with the synaptic gating ODE of eq. (1) (DIRECT kernels) */ };
 enum { NET_TOPO_RING = 0, NET_TOPO_LATTICE = 1, NET_TOPO_CSR = 2, NET_TOPO_RANDOM_INDEGREE = 3,
        NET_TOPO_COMPRESSED = 4 /* differentially compressed coupling matrix, Alg. 2 */ };
 enum { NET_F32 = 0, NET_F64 = 1 };
@@ -110,6 +113,24 @@ typedef struct {
     double eps, a, sigma, phi;
 } net_fhn_params;
 
+/* FitzHugh-Nagumo exactly as the paper prints it, eq. (2), nvar = 2, state [x | y]:
+ *   eps dx_i/dt = x_i - x_i^3/3 - y_i + (sigma/Omega_i) sum_{j in row i} (x_j(t - tau) - x_i) + I_app
+ *       dy_i/dt = x_i + a + D n_i(t)
+ * (uniform coupling strength s_ij = sigma/Omega_i).  Under the fixed-step RK4 of net_integrate
+ * (reading R17): tau = net_desc.delay_steps * dt; the library keeps x and dx/dt of the last
+ * delay_steps + 2 step times in the workspace ("maintaining data from previous time steps and
+ * performing interpolation") and the half-step stages read the cubic Hermite midpoint;
+ * before the first step the history is the constant initial x (net_set_state resets it).  The noise
+ * is additive Gaussian white noise on y by Euler-Maruyama: after every step
+ * y_i += D sqrt(dt) xi(seed, i, step) with xi from the counter-based generator of reading R17
+ * (splitmix64 finaliser, Box-Muller), so that runs are reproducible and comparable across
+ * implementations.  net_eval_rhs gives the deterministic right-hand side without delay.
+ * net_integrate_adaptive is refused while delay_steps > 0 or D != 0. */
+typedef struct {
+    double eps, a, sigma, I_app, D;
+    uint64_t seed;
+} net_fhn2_params;
+
 /* Hodgkin-Huxley type element, eq. (1), standard squid-axon
  * channels and an instantaneous sigmoidal synapse (mV, ms, uA/cm^2, mS/cm^2, uF/cm^2):
  *   C dV_i/dt = I_ext,i - gNa m^3 h (V-ENa) - gK n^4 (V-EK) - gL (V-EL)
@@ -122,6 +143,17 @@ typedef struct {
     double I_ext0;
     double V_c, n_c, V_s;
 } net_hh_params;
+
+/* Hodgkin-Huxley element with the synaptic gating ODE of eq. (1) ("ds_ik/dt = p_ik(U_i, s_ik, n_j)",
+ * PAPER.md:54), nvar = 5, state [V | m | h | n | s].  Reading R18: the kinetics depend on the
+ * presynaptic voltage only, so all links leaving element k share one gating variable s_k:
+ *   ds_k/dt = a_s S(V_k)(1 - s_k) - b_s s_k,  I_syn,i = (g_syn/Omega_i)(E_syn - V_i) sum_{k in row i} s_k
+ * (S the sigmoid of net_hh_params; everything else as NET_MODEL_HH).  net_hh_steady_gates also sets
+ * s to its steady state a_s S/(a_s S + b_s). */
+typedef struct {
+    net_hh_params hh;
+    double a_s, b_s;
+} net_hhs_params;
 
 /* Coupling topology (static during a run).
  *  RING:    n elements on a circle, each coupled to `radius` neighbours on both sides.
@@ -193,6 +225,8 @@ typedef struct {
                      * n * batch <= 2^31 - 1. */
     int32_t method; /* NET_METHOD_* */
     net_topology topo;
+    int32_t delay_steps; /* NET_MODEL_FHN2: tau = delay_steps * dt (0 = no delay); else 0 */
+    int32_t reserved_;
 } net_desc;
 
 /* Bytes of device workspace net_create needs for this description (pure function). */

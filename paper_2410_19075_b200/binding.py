@@ -15,13 +15,13 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(HERE, "liboscnet.so")
 
 NET_OK = 0
-MODEL_KS, MODEL_FHN, MODEL_HH, MODEL_KSI = 0, 1, 2, 3
+MODEL_KS, MODEL_FHN, MODEL_HH, MODEL_KSI, MODEL_FHN2, MODEL_HHS = 0, 1, 2, 3, 4, 5
 TOPO_RING, TOPO_LATTICE, TOPO_CSR, TOPO_RANDOM_INDEGREE, TOPO_COMPRESSED = 0, 1, 2, 3, 4
 F32, F64 = 0, 1
 METHOD_AUTO, METHOD_DIRECT, METHOD_FAST = 0, 1, 2
 PARAM_OMEGA, PARAM_IEXT = 0, 1
 OBS_PHASE, OBS_GLOBAL_ORDER, OBS_LOCAL_ORDER, OBS_MEAN_PHASE_VELOCITY, OBS_STATS, OBS_REPLICA_ORDER = 0, 1, 2, 3, 4, 5
-NVAR = {MODEL_KS: 1, MODEL_FHN: 2, MODEL_HH: 4, MODEL_KSI: 2}
+NVAR = {MODEL_KS: 1, MODEL_FHN: 2, MODEL_HH: 4, MODEL_KSI: 2, MODEL_FHN2: 2, MODEL_HHS: 5}
 
 ABI_SYMBOLS = [
     "net_workspace_bytes", "net_create", "net_destroy", "net_set_state", "net_get_state",
@@ -53,6 +53,15 @@ class HHParams(C.Structure):
                  "I_ext0", "V_c", "n_c", "V_s")]
 
 
+class FHN2Params(C.Structure):
+    _fields_ = [("eps", C.c_double), ("a", C.c_double), ("sigma", C.c_double), ("I_app", C.c_double),
+                ("D", C.c_double), ("seed", C.c_uint64)]
+
+
+class HHSParams(C.Structure):
+    _fields_ = [("hh", HHParams), ("a_s", C.c_double), ("b_s", C.c_double)]
+
+
 HH_PHASE_MAP = dict(V_c=-20.0, n_c=0.55, V_s=100.0)
 
 
@@ -72,7 +81,8 @@ class Compressed(C.Structure):
 
 class Desc(C.Structure):
     _fields_ = [("model", C.c_int32), ("dtype", C.c_int32), ("n", C.c_int64), ("batch", C.c_int32),
-                ("method", C.c_int32), ("topo", Topology)]
+                ("method", C.c_int32), ("topo", Topology), ("delay_steps", C.c_int32),
+                ("reserved_", C.c_int32)]
 
 
 class OscnetError(RuntimeError):
@@ -304,9 +314,14 @@ def make_params(model, p):
         return KSIParams(p["K"], p["alpha"], p["m"], p["eps"], p.get("omega0", 0.0))
     if model == MODEL_FHN:
         return FHNParams(p["eps"], p["a"], p["sigma"], p["phi"])
+    if model == MODEL_FHN2:
+        return FHN2Params(p["eps"], p["a"], p["sigma"], p.get("I_app", 0.0), p.get("D", 0.0), int(p.get("seed", 0)))
     q = dict(HH_PHASE_MAP, I_ext0=0.0)
     q.update(p)
-    return HHParams(*[q[k] for k, _ in HHParams._fields_])
+    hh = HHParams(*[q[k] for k, _ in HHParams._fields_])
+    if model == MODEL_HHS:
+        return HHSParams(hh, p.get("a_s", 2.0), p.get("b_s", 0.5))
+    return hh
 
 
 def _np_dtype(dtype):
@@ -317,7 +332,7 @@ class Net:
     """Owns a workspace tensor and a handle; methods mirror the C ABI."""
 
     def __init__(self, model, dtype, n, topo, params, method=METHOD_AUTO, device="cuda:0",
-                 stream=None, batch=1):
+                 stream=None, batch=1, delay_steps=0):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("oscnet needs a CUDA device (no CPU fallback)")
@@ -330,6 +345,7 @@ class Net:
         self.torch_dtype = torch.float32 if dtype == F32 else torch.float64
         d = Desc()
         d.model, d.dtype, d.n, d.batch, d.method = model, dtype, int(n), int(batch), method
+        d.delay_steps = int(delay_steps)
         t = d.topo
         t.kind = topo["kind"]
         ext = list(topo.get("extent", ())) + [1, 1, 1]
@@ -381,7 +397,8 @@ class Net:
         else:
             topo = dict(kind=TOPO_RANDOM_INDEGREE, in_degree=w.in_degree, seed=w.topo_seed)
         return cls(w.model, dtype, w.n, topo, w.params, method=method, device=device,
-                   stream=stream, batch=getattr(w, "batch", 1))
+                   stream=stream, batch=getattr(w, "batch", 1),
+                   delay_steps=w.extra.get("delay_steps", 0))
 
     def close(self):
         if getattr(self, "h", None):

@@ -8,7 +8,7 @@ No arithmetic of the method lives here.
 import math
 from dataclasses import dataclass, field, replace
 
-KS, FHN, HH, KSI = 0, 1, 2, 3
+KS, FHN, HH, KSI, FHN2, HHS = 0, 1, 2, 3, 4, 5
 RING, LATTICE, CSR, RANDOM_INDEGREE = 0, 1, 2, 3
 
 
@@ -33,7 +33,7 @@ class Workload:
 
     @property
     def nvar(self):
-        return {KS: 1, FHN: 2, HH: 4, KSI: 2}[self.model]
+        return {KS: 1, FHN: 2, HH: 4, KSI: 2, FHN2: 2, HHS: 5}[self.model]
 
 
 _FHN2 = dict(eps=0.05, a=0.5, sigma=0.1, phi=math.pi / 2 - 0.1)

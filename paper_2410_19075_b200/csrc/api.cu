@@ -25,7 +25,8 @@ int32_t cuda_err(net* h, cudaError_t e, const char* what) {
 }
 
 static int model_nvar(int model) {
-    return model == NET_MODEL_KS ? 1 : model == NET_MODEL_FHN ? 2 : model == NET_MODEL_HH ? 4 : model == NET_MODEL_KSI ? 2 : -1;
+    return model == NET_MODEL_KS ? 1 : model == NET_MODEL_FHN ? 2 : model == NET_MODEL_HH ? 4 : model == NET_MODEL_KSI ? 2 :
+           model == NET_MODEL_FHN2 ? 2 : model == NET_MODEL_HHS ? 5 : -1;
 }
 
 static int32_t validate(net* h, const net_desc* d) {
@@ -38,6 +39,8 @@ static int32_t validate(net* h, const net_desc* d) {
         return set_err(h, NET_ERR_UNSUPPORTED, "batch = %d: this build batches ring nets only", d->batch);
     if (d->n * (int64_t)d->batch > 2147483647LL) return set_err(h, NET_ERR_INVALID, "n * batch exceeds 2^31-1");
     if (d->method < NET_METHOD_AUTO || d->method > NET_METHOD_FAST) return set_err(h, NET_ERR_INVALID, "unknown method %d", d->method);
+    if (d->delay_steps < 0 || d->delay_steps > (1 << 20) || (d->delay_steps > 0 && d->model != NET_MODEL_FHN2))
+        return set_err(h, NET_ERR_INVALID, "delay_steps = %d: need 0 <= delay_steps <= 2^20, and only NET_MODEL_FHN2 has a delay", d->delay_steps);
     const net_topology& t = d->topo;
     switch (t.kind) {
         case NET_TOPO_RING:
@@ -116,6 +119,10 @@ static Layout make_layout(const net_desc* d, char* base) {
     L.state_bytes = state;
     L.b.y = P(state); L.b.Y2 = P(state); L.b.Y3 = P(state); L.b.Y4 = P(state);
     L.b.elem_param = P((size_t)ld * es);
+    if (d->model == NET_MODEL_FHN2) {
+        L.b.hist_x = P((size_t)(d->delay_steps + 2) * ld * es);
+        L.b.hist_d = P((size_t)(d->delay_steps + 2) * ld * es);
+    }
     if (d->model == NET_MODEL_HH && (fk == FAST_CSR_WARP || fk == FAST_CSR_BLOCKED)) {
         L.b.s_y = P((size_t)ld * es); L.b.s_Y2 = P((size_t)ld * es);
         L.b.s_Y3 = P((size_t)ld * es); L.b.s_Y4 = P((size_t)ld * es);
@@ -163,12 +170,17 @@ static void fill_params(net* h, const void* params) {
         const net_ksi_params* p = (const net_ksi_params*)params;
         mp.K = p->K; mp.alpha = p->alpha; mp.sin_a = sin(p->alpha); mp.cos_a = cos(p->alpha);
         mp.inv_m = 1.0 / p->m; mp.damp = p->eps;
+    } else if (h->desc.model == NET_MODEL_FHN2) {
+        const net_fhn2_params* p = (const net_fhn2_params*)params;
+        mp.inv_eps = 1.0 / p->eps; mp.a = p->a; mp.sigma = p->sigma; mp.I_app = p->I_app;
+        mp.noise_D = p->D; mp.noise_seed = p->seed;
     } else if (h->desc.model == NET_MODEL_FHN) {
         const net_fhn_params* p = (const net_fhn_params*)params;
         mp.inv_eps = 1.0 / p->eps; mp.a = p->a; mp.sigma = p->sigma;
         mp.buu = cos(p->phi); mp.buv = sin(p->phi); mp.bvu = -sin(p->phi); mp.bvv = cos(p->phi);
     } else {
-        const net_hh_params* p = (const net_hh_params*)params;
+        const net_hh_params* p = (const net_hh_params*)params;     // HHS: the same struct comes first
+        if (h->desc.model == NET_MODEL_HHS) { mp.a_s = ((const net_hhs_params*)params)->a_s; mp.b_s = ((const net_hhs_params*)params)->b_s; }
         mp.gNa = p->gNa; mp.gK = p->gK; mp.gL = p->gL; mp.ENa = p->ENa; mp.EK = p->EK; mp.EL = p->EL;
         mp.inv_C = 1.0 / p->C; mp.g_syn = p->g_syn; mp.E_syn = p->E_syn; mp.theta_syn = p->theta_syn;
         mp.inv_k_syn = 1.0 / p->k_syn; mp.V_c = p->V_c; mp.n_c = p->n_c; mp.inv_V_s = 1.0 / p->V_s;
@@ -225,6 +237,7 @@ static void drop_graph(net* h) {
 }
 
 static int32_t run_stage(net* h, const StageArgs& a) {
+    if (h->desc.model == NET_MODEL_FHN2) return delay_stage(h, a);
     if (h->method == NET_METHOD_FAST) return fast_stage(h, a);
     return direct_stage(h, a);
 }
@@ -260,6 +273,7 @@ static int32_t enqueue_step(net* h, double dt) {
         int32_t rc = run_stage(h, stage_args(h, s, dt));
         if (rc) return rc;
     }
+    h->hist_step += 1;      // NET_MODEL_FHN2: slot of the history ring, counter of the noise stream
     return NET_OK;
 }
 
@@ -294,7 +308,8 @@ static int32_t integrate_plain(net* h, int64_t n_steps, double dt) {
     if (!handled) {
         int64_t left = n_steps;
         // the legacy default stream cannot be captured: plain launches there
-        const bool can_capture = h->stream != nullptr && h->stream != cudaStreamLegacy;
+        // (FHN2: the history slots and the noise counter change from step to step -- plain launches)
+        const bool can_capture = h->stream != nullptr && h->stream != cudaStreamLegacy && h->desc.model != NET_MODEL_FHN2;
         if (left >= GRAPH_STEPS && can_capture) {
             if (!h->graph_exec || h->graph_dt != dt) {
                 drop_graph(h);
@@ -379,7 +394,9 @@ int32_t net_create(const net_desc* user_desc, const void* params, size_t params_
     const net_desc* desc = &nd;                 // n = total elements of the batch from here on
     size_t want = desc->model == NET_MODEL_KS ? sizeof(net_ks_params)
                 : desc->model == NET_MODEL_KSI ? sizeof(net_ksi_params)
-                : desc->model == NET_MODEL_FHN ? sizeof(net_fhn_params) : sizeof(net_hh_params);
+                : desc->model == NET_MODEL_FHN ? sizeof(net_fhn_params)
+                : desc->model == NET_MODEL_FHN2 ? sizeof(net_fhn2_params)
+                : desc->model == NET_MODEL_HHS ? sizeof(net_hhs_params) : sizeof(net_hh_params);
     if (desc->model == NET_MODEL_KSI && params && params_bytes == want && !(((const net_ksi_params*)params)->m > 0.0))
         return set_err(nullptr, NET_ERR_INVALID, "KS with inertia: need m > 0");
     if (!params || params_bytes != want)
@@ -440,7 +457,7 @@ int32_t net_create(const net_desc* user_desc, const void* params, size_t params_
     if (rc == NET_OK) {
         double v0 = desc->model == NET_MODEL_KS ? ((const net_ks_params*)params)->omega0
                   : desc->model == NET_MODEL_KSI ? ((const net_ksi_params*)params)->omega0
-                  : desc->model == NET_MODEL_HH ? ((const net_hh_params*)params)->I_ext0 : 0.0;
+                  : (desc->model == NET_MODEL_HH || desc->model == NET_MODEL_HHS) ? ((const net_hh_params*)params)->I_ext0 : 0.0;
         rc = fill_elem_param(h, v0);
     }
     if (rc == NET_OK) {
@@ -469,7 +486,9 @@ int32_t net_set_state(net_t* h, const void* src, int32_t src_is_device) {
     if (!h) return NET_ERR_INVALID;
     if (!src) return set_err(h, NET_ERR_INVALID, "src is NULL");
     h->s_valid = 0;
-    return copy_state(h, h->b.y, const_cast<void*>(src), true, src_is_device != 0);
+    int32_t rc = copy_state(h, h->b.y, const_cast<void*>(src), true, src_is_device != 0);
+    if (rc == NET_OK && h->desc.model == NET_MODEL_FHN2) rc = delay_reset_history(h);   // constant initial function
+    return rc;
 }
 
 int32_t net_get_state(net_t* h, void* dst, int32_t dst_is_device) {
@@ -484,7 +503,7 @@ int32_t net_set_param_array(net_t* h, int32_t which, const void* src, int32_t sr
     if (!h) return NET_ERR_INVALID;
     if (!src) return set_err(h, NET_ERR_INVALID, "src is NULL");
     if (!((which == NET_PARAM_OMEGA && (h->desc.model == NET_MODEL_KS || h->desc.model == NET_MODEL_KSI)) ||
-          (which == NET_PARAM_IEXT && h->desc.model == NET_MODEL_HH)))
+          (which == NET_PARAM_IEXT && (h->desc.model == NET_MODEL_HH || h->desc.model == NET_MODEL_HHS))))
         return set_err(h, NET_ERR_INVALID, "parameter array %d does not belong to model %d", which, h->desc.model);
     OSC_CUDA(h, cudaMemcpyAsync(h->b.elem_param, src, (size_t)h->n * h->esize,
                                 src_is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, h->stream));
@@ -495,7 +514,7 @@ int32_t net_set_param_array(net_t* h, int32_t which, const void* src, int32_t sr
 int32_t net_hh_steady_gates(net_t* h) {
     DevGuard guard_(h);
     if (!h) return NET_ERR_INVALID;
-    if (h->desc.model != NET_MODEL_HH) return set_err(h, NET_ERR_INVALID, "net_hh_steady_gates on a non-HH net");
+    if (h->desc.model != NET_MODEL_HH && h->desc.model != NET_MODEL_HHS) return set_err(h, NET_ERR_INVALID, "net_hh_steady_gates on a non-HH net");
     return hh_steady_gates(h);
 }
 
@@ -536,6 +555,8 @@ int32_t net_integrate_adaptive(net_t* h, double t_end, double rtol, double atol,
                                void* d_work, size_t work_bytes, double* out5) {
     DevGuard guard_(h);
     if (!h || !out5) return set_err(h, NET_ERR_INVALID, "net or out5 is NULL");
+    if (h->desc.model == NET_MODEL_FHN2 && (h->desc.delay_steps > 0 || h->mp.noise_D != 0.0))
+        return set_err(h, NET_ERR_UNSUPPORTED, "net_integrate_adaptive: eq. (2) with delay or noise runs under the fixed-step integrator only");
     return adaptive_integrate(h, t_end, rtol, atol, h0, max_attempts, d_work, work_bytes, out5);
 }
 

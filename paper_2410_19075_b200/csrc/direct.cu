@@ -18,7 +18,7 @@ __global__ void __launch_bounds__(256) direct_stage_kernel(StageArgs a, ModelPar
     const T dt = (T)a.dt;
     for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n;
          i += (int64_t)gridDim.x * blockDim.x) {
-        constexpr int NV = MODEL == NET_MODEL_KS ? 1 : (MODEL == NET_MODEL_FHN || MODEL == NET_MODEL_KSI) ? 2 : 4;
+        constexpr int NV = MODEL == NET_MODEL_KS ? 1 : (MODEL == NET_MODEL_FHN || MODEL == NET_MODEL_KSI) ? 2 : MODEL == NET_MODEL_HHS ? 5 : 4;
         T k[NV], xin[NV];
 #pragma unroll
         for (int v = 0; v < NV; ++v) xin[v] = in[v * ld + i];
@@ -48,6 +48,13 @@ __global__ void __launch_bounds__(256) direct_stage_kernel(StageArgs a, ModelPar
             });
             T inv = deg > 0 ? T(1) / T(deg) : T(0);
             fhn_rhs<T>(mp, xin[0], xin[1], Cu, Cv, inv, &k[0], &k[1]);
+        } else if (MODEL == NET_MODEL_HHS) {
+            // eq. (1) with the gating ODE (reading R18): the links carry the presynaptic gate s_j
+            T ssum = 0;
+            int deg = for_each_neighbor<TOPO>(tv, n, i, [&](int64_t j) { ssum += in[4 * ld + j]; });
+            T inv = deg > 0 ? T(1) / T(deg) : T(0);
+            hh_rhs<T>(mp, xin[0], xin[1], xin[2], xin[3], ep[i], ssum, inv, &k[0], &k[1], &k[2], &k[3]);
+            k[NV - 1] = T(mp.a_s) * hh_syn_activation<T>(mp, xin[0]) * (T(1) - xin[NV - 1]) - T(mp.b_s) * xin[NV - 1];
         } else {
             T ssum = 0;
             int deg = for_each_neighbor<TOPO>(tv, n, i, [&](int64_t j) {
@@ -100,6 +107,7 @@ static int32_t launch_model(net* h, const StageArgs& a) {
         case NET_MODEL_KS: return launch_topo<T, NET_MODEL_KS>(h, a);
         case NET_MODEL_FHN: return launch_topo<T, NET_MODEL_FHN>(h, a);
         case NET_MODEL_KSI: return launch_topo<T, NET_MODEL_KSI>(h, a);
+        case NET_MODEL_HHS: return launch_topo<T, NET_MODEL_HHS>(h, a);
         default: return launch_topo<T, NET_MODEL_HH>(h, a);
     }
 }
@@ -129,7 +137,7 @@ int32_t hh_compute_s(net* h, const void* V, void* s) {
 }
 
 template <class T>
-__global__ void hh_gates_kernel(T* __restrict__ y, int64_t n, int64_t ld) {
+__global__ void hh_gates_kernel(T* __restrict__ y, int64_t n, int64_t ld, int with_s, ModelParams mp) {
     for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n;
          i += (int64_t)gridDim.x * blockDim.x) {
         T am, bm, ah, bh, an, bn;
@@ -137,6 +145,10 @@ __global__ void hh_gates_kernel(T* __restrict__ y, int64_t n, int64_t ld) {
         y[ld + i] = am / (am + bm);
         y[2 * ld + i] = ah / (ah + bh);
         y[3 * ld + i] = an / (an + bn);
+        if (with_s) {       // HHS: gating variable at a_s S/(a_s S + b_s)
+            const T S = hh_syn_activation<T>(mp, y[i]);
+            y[4 * ld + i] = T(mp.a_s) * S / (T(mp.a_s) * S + T(mp.b_s));
+        }
     }
 }
 
@@ -144,9 +156,9 @@ int32_t hh_steady_gates(net* h) {
     int64_t blocks = (h->n + 255) / 256;
     if (blocks > 148 * 16) blocks = 148 * 16;
     if (h->desc.dtype == NET_F32)
-        hh_gates_kernel<float><<<(unsigned)blocks, 256, 0, h->stream>>>((float*)h->b.y, h->n, h->ld);
+        hh_gates_kernel<float><<<(unsigned)blocks, 256, 0, h->stream>>>((float*)h->b.y, h->n, h->ld, h->desc.model == NET_MODEL_HHS, h->mp);
     else
-        hh_gates_kernel<double><<<(unsigned)blocks, 256, 0, h->stream>>>((double*)h->b.y, h->n, h->ld);
+        hh_gates_kernel<double><<<(unsigned)blocks, 256, 0, h->stream>>>((double*)h->b.y, h->n, h->ld, h->desc.model == NET_MODEL_HHS, h->mp);
     h->launches += 1;
     OSC_CUDA(h, cudaGetLastError());
     return NET_OK;

@@ -26,6 +26,7 @@ int32_t ring_run(net* h, const void* y_in, void* y_out, int64_t n_steps, double 
 
 int32_t fast_select(const net_desc* d) {
     const net_topology& t = d->topo;
+    if (d->model == NET_MODEL_FHN2 || d->model == NET_MODEL_HHS) return FAST_NONE;   // per-link DIRECT kernels
     // KS with inertia: the persistent ring kernel (same fields as KS); DIRECT on the other topologies
     if (d->model == NET_MODEL_KSI) return ring_supported(d) ? FAST_RING_KS : FAST_NONE;
     if (t.kind == NET_TOPO_CSR || t.kind == NET_TOPO_RANDOM_INDEGREE)

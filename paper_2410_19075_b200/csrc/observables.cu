@@ -17,7 +17,7 @@ __global__ void phase_kernel(const T* __restrict__ y, int64_t n, int64_t ld, int
          i += (int64_t)gridDim.x * blockDim.x) {
         double th;
         if (model == NET_MODEL_KS || model == NET_MODEL_KSI) th = (double)y[i];
-        else if (model == NET_MODEL_FHN) th = atan2((double)y[ld + i], (double)y[i]);
+        else if (model == NET_MODEL_FHN || model == NET_MODEL_FHN2) th = atan2((double)y[ld + i], (double)y[i]);
         else th = atan2((double)y[3 * ld + i] - mp.n_c, ((double)y[i] - mp.V_c) * mp.inv_V_s);
         theta[i] = th;
     }

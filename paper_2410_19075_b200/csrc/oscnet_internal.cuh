@@ -21,6 +21,9 @@ struct ModelParams {
     // HH
     double gNa, gK, gL, ENa, EK, EL, inv_C, g_syn, E_syn, theta_syn, inv_k_syn;
     double V_c, n_c, inv_V_s;
+    // HHS (gating ODE) and FHN2 (eq. (2): applied current, noise amplitude)
+    double a_s, b_s, I_app, noise_D;
+    unsigned long long noise_seed;
 };
 
 // Topology as seen by kernels.
@@ -101,6 +104,7 @@ struct Buffers {
     double* obs_loc;              // n
     double* obs_partial;          // reduction partials (4096 doubles)
     double* obs_acc;              // small accumulator block (16 doubles)
+    void *hist_x, *hist_d;        // NET_MODEL_FHN2: (delay_steps + 2) slots of ld elements each (x, dx/dt at step times)
     void* scratch;                // method-specific scratch
     size_t scratch_bytes;
 };
@@ -192,6 +196,7 @@ struct net {
     double stats[8];
     int stats_valid;
     int s_valid;           // HH fast path: s_y consistent with y
+    int64_t hist_step;     // NET_MODEL_FHN2: steps taken since the history was reset (net_set_state)
     oscnet::Lat3 lat;      // FAST_LATTICE3D launch geometry
     unsigned lat_grid;
     int lat_threads;
@@ -259,6 +264,9 @@ int32_t pairs_unpack(net* h, const void* pairs, void* soa);
 int32_t obs_phase(net* h, const void* state, double* d_theta);
 int32_t ring_probe_latency(net* h, double* out4);   // ring_fast.cu
 int32_t probe_peaks(net* h, double* out8);          // probe.cu
+// delay.cu (NET_MODEL_FHN2: eq. (2) with delay and noise)
+int32_t delay_stage(net* h, const StageArgs& a);
+int32_t delay_reset_history(net* h);
 // adaptive.cu (Dormand-Prince 5(4)) and its helpers in api.cu
 size_t adaptive_workspace_bytes(const net* h);
 int32_t adaptive_integrate(net* h, double t_end, double rtol, double atol, double h0, int64_t max_attempts,
