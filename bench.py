@@ -219,8 +219,6 @@ def rewrite_error(w, device):
     import numpy as np
     from paper_2410_19075_b200 import binding as B, configs
     out = {}
-    if w.model == configs.KSI:                 # DIRECT only in this build: no rewrite to measure
-        return {"note": "served by the DIRECT (per-link) form; no rewrite"}
     states = [("incoherent", None)]
     if w.model != configs.HH:                  # HH gates are set to their steady state of V by the library
         states.append(("coherent", lambda y: (y * 1e-2 + 0.3).astype(y.dtype)))

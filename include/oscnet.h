@@ -56,7 +56,7 @@ enum {
     NET_ERR_SIZE = -2,        /* workspace too small or misaligned (needs 256-byte alignment) */
     NET_ERR_TOPOLOGY = -3,    /* CSR not monotone / index out of range / self-loop where forbidden */
     NET_ERR_CUDA = -4,        /* a CUDA call failed; message holds cudaGetErrorString */
-    NET_ERR_UNSUPPORTED = -5  /* valid request this build does not implement (e.g. batch > 1 on a lattice) */
+    NET_ERR_UNSUPPORTED = -5  /* valid request this build does not implement (e.g. NET_METHOD_FAST on a 2D lattice) */
 };
 
 enum { NET_MODEL_KS = 0, NET_MODEL_FHN = 1, NET_MODEL_HH = 2,
@@ -220,8 +220,10 @@ typedef struct {
                      * per-element parameters.  Every array that is [..][n] for batch = 1 becomes
                      * [..][batch][n] (replica-major, n contiguous); element ids in net_get_topology
                      * and the observables run over 0 .. batch*n - 1 (the coupling matrix of the batch
-                     * is block diagonal; global observables are ensemble values).  batch > 1 is
-                     * built for NET_TOPO_RING; other topologies return NET_ERR_UNSUPPORTED.
+                     * is block diagonal; global observables are ensemble values).  The topology
+                     * describes ONE replica.  Rings of <= 2048 elements run one CTA of the persistent
+                     * kernel per replica (FAST); batches of lattices and graphs run the per-link DIRECT
+                     * kernels; NET_TOPO_COMPRESSED is not batched (NET_ERR_UNSUPPORTED).
                      * n * batch <= 2^31 - 1. */
     int32_t method; /* NET_METHOD_* */
     net_topology topo;

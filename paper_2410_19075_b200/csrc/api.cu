@@ -35,8 +35,8 @@ static int32_t validate(net* h, const net_desc* d) {
     if (d->dtype != NET_F32 && d->dtype != NET_F64) return set_err(h, NET_ERR_INVALID, "unknown dtype %d", d->dtype);
     if (d->n < 1 || d->n > 2147483647LL) return set_err(h, NET_ERR_INVALID, "n = %lld outside [1, 2^31-1] (col_idx is int32)", (long long)d->n);
     if (d->batch < 1) return set_err(h, NET_ERR_INVALID, "batch = %d < 1", d->batch);
-    if (d->batch > 1 && d->topo.kind != NET_TOPO_RING)
-        return set_err(h, NET_ERR_UNSUPPORTED, "batch = %d: this build batches ring nets only", d->batch);
+    if (d->batch > 1 && d->topo.kind == NET_TOPO_COMPRESSED)
+        return set_err(h, NET_ERR_UNSUPPORTED, "batch = %d: compressed matrices are not batched in this build", d->batch);
     if (d->n * (int64_t)d->batch > 2147483647LL) return set_err(h, NET_ERR_INVALID, "n * batch exceeds 2^31-1");
     if (d->method < NET_METHOD_AUTO || d->method > NET_METHOD_FAST) return set_err(h, NET_ERR_INVALID, "unknown method %d", d->method);
     if (d->delay_steps < 0 || d->delay_steps > (1 << 20) || (d->delay_steps > 0 && d->model != NET_MODEL_FHN2))
@@ -635,7 +635,9 @@ int32_t net_get_topology(net_t* h, int64_t row_begin, int64_t row_count, int64_t
     if (row_begin < 0 || row_count < 0 || row_begin + row_count > h->n)
         return set_err(h, NET_ERR_INVALID, "row range outside [0, n]");
     if (dst_is_device) return topo_expand(h, row_begin, row_count, row_ptr, col_idx);
-    if (h->tv.kind == NET_TOPO_CSR || h->tv.kind == NET_TOPO_RANDOM_INDEGREE) {
+    if ((h->tv.kind == NET_TOPO_CSR || h->tv.kind == NET_TOPO_RANDOM_INDEGREE) && h->desc.batch > 1 && h->degree_uniform < 0)
+        return set_err(h, NET_ERR_UNSUPPORTED, "net_get_topology to host memory: batches of graphs with non-uniform rows (use a device destination)");
+    if ((h->tv.kind == NET_TOPO_CSR || h->tv.kind == NET_TOPO_RANDOM_INDEGREE) && h->desc.batch == 1) {
         OSC_CUDA(h, cudaMemcpyAsync(row_ptr, h->b.row_ptr + row_begin, sizeof(int64_t) * (row_count + 1), cudaMemcpyDeviceToHost, h->stream));
         OSC_CUDA(h, cudaStreamSynchronize(h->stream));
         int64_t base = row_ptr[0], cnt = row_ptr[row_count] - base;

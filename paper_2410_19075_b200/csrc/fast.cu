@@ -27,8 +27,10 @@ int32_t ring_run(net* h, const void* y_in, void* y_out, int64_t n_steps, double 
 int32_t fast_select(const net_desc* d) {
     const net_topology& t = d->topo;
     if (d->model == NET_MODEL_FHN2 || d->model == NET_MODEL_HHS) return FAST_NONE;   // per-link DIRECT kernels
+    if (d->batch > 1 && t.kind != NET_TOPO_RING) return FAST_NONE;   // batches of lattices / graphs: block-diagonal DIRECT form
     // KS with inertia: the persistent ring kernel (same fields as KS); DIRECT on the other topologies
-    if (d->model == NET_MODEL_KSI) return ring_supported(d) ? FAST_RING_KS : FAST_NONE;
+    if (d->model == NET_MODEL_KSI)
+        return ring_supported(d) ? FAST_RING_KS : lattice_v3_supported(d) ? FAST_LATTICE3D_V3 : FAST_NONE;
     if (t.kind == NET_TOPO_CSR || t.kind == NET_TOPO_RANDOM_INDEGREE)
         return csr_blocked_supported(d) ? FAST_CSR_BLOCKED : FAST_CSR_WARP;
     if (lattice_v3_supported(d)) return FAST_LATTICE3D_V3;
@@ -62,7 +64,7 @@ int32_t fast_prepare(net* h) {
     }
     if (h->fast_kind == FAST_LATTICE3D_V3) {
         rc = lattice_v3_prepare(h);
-        if (rc == NET_ERR_UNSUPPORTED) {     // same layout, second-generation kernels
+        if (rc == NET_ERR_UNSUPPORTED && h->desc.model != NET_MODEL_KSI) {     // same layout, second-generation kernels
             h->fast_kind = FAST_LATTICE3D_V2;
             rc = NET_OK;
         }

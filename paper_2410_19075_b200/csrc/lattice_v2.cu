@@ -21,7 +21,7 @@ bool lattice_v2_supported(const net_desc* d) {
     const net_topology& t = d->topo;
     if (t.kind != NET_TOPO_LATTICE || t.ndim != 3) return false;
     if (t.radius != 2 && t.radius != 4) return false;
-    if (d->model != NET_MODEL_KS && d->model != NET_MODEL_FHN) return false;
+    if (d->model != NET_MODEL_KS && d->model != NET_MODEL_FHN && d->model != NET_MODEL_KSI) return false;
     // rows must be whole 16-byte vectors of the per-thread column group (X = 2 columns)
     return t.extent[0] % 2 == 0;
 }
@@ -34,9 +34,11 @@ size_t lattice_v2_state_bytes(const net_desc* d) {
 }
 
 size_t lattice_v2_scratch_bytes(const net_desc* d) {
-    if (d->model != NET_MODEL_KS) return 0;
+    if (d->model != NET_MODEL_KS && d->model != NET_MODEL_KSI) return 0;
     const size_t es = d->dtype == NET_F32 ? 4 : 8;
-    return 2 * ((padded_pairs(d) * 2 * es + 255) / 256 * 256) + 512;     // E_a, E_b
+    size_t b = 2 * ((padded_pairs(d) * 2 * es + 255) / 256 * 256) + 512;     // E_a, E_b
+    if (d->model == NET_MODEL_KSI) b += (size_t)round_up(d->n, 64) * es + 256;   // coupling term of the stage input
+    return b;
 }
 
 int32_t lattice_v2_prepare(net* h) {
@@ -156,7 +158,7 @@ int32_t pairs_unpack(net* h, const void* pairs, void* soa) {
 }
 
 int32_t lattice_v2_refresh_exchange(net* h) {
-    if (h->desc.model != NET_MODEL_KS) return NET_OK;
+    if (h->desc.model != NET_MODEL_KS && h->desc.model != NET_MODEL_KSI) return NET_OK;
     return h->ks_planar ? pad_fill<2>(h, h->b.y, h->E_a) : pad_fill<1>(h, h->b.y, h->E_a);
 }
 
@@ -173,7 +175,7 @@ int32_t lattice_v3_entry_f64_fhn(net* h, int stage, double dt, void* rhs_out);
 int32_t lattice_v3_entry_f64_ks(net* h, int stage, double dt, void* rhs_out);
 
 static int32_t l3_dispatch(net* h, int stage, double dt, void* rhs_out) {
-    const bool ks = h->desc.model == NET_MODEL_KS;
+    const bool ks = h->desc.model == NET_MODEL_KS || h->desc.model == NET_MODEL_KSI;   // KSI: the KS kernels' RHS instance
     if (h->desc.dtype == NET_F32)
         return ks ? lattice_v3_entry_f32_ks(h, stage, dt, rhs_out) : lattice_v3_entry_f32_fhn(h, stage, dt, rhs_out);
     return ks ? lattice_v3_entry_f64_ks(h, stage, dt, rhs_out) : lattice_v3_entry_f64_fhn(h, stage, dt, rhs_out);
@@ -183,15 +185,17 @@ bool lattice_v3_supported(const net_desc* d) {
     if (!lattice_v2_supported(d)) return false;
     if (getenv("OSCNET_NO_LAT3")) return false;
     // KS operand tiles are rows of scalars: whole 16-byte vectors
-    if (d->model == NET_MODEL_KS && d->dtype == NET_F32 && d->topo.extent[0] % 4 != 0) return false;
+    if ((d->model == NET_MODEL_KS || d->model == NET_MODEL_KSI) && d->dtype == NET_F32 && d->topo.extent[0] % 4 != 0) return false;
     return true;
 }
 
 int32_t lattice_v3_prepare(net* h) {
-    if (h->desc.model == NET_MODEL_KS) {
+    if (h->desc.model == NET_MODEL_KS || h->desc.model == NET_MODEL_KSI) {
         char* s = (char*)h->b.scratch;
+        const size_t eb = (padded_pairs(&h->desc) * 2 * h->esize + 255) / 256 * 256;
         h->E_a = s;
-        h->E_b = s + (padded_pairs(&h->desc) * 2 * h->esize + 255) / 256 * 256;
+        h->E_b = s + eb;
+        h->ksi_c = s + 2 * eb + 256;          // KSI: omega + (K/Omega) sum sin(...) of the stage input
     }
     int32_t rc = l3_dispatch(h, -1, 0.0, nullptr);
     if (rc) return rc;
@@ -203,7 +207,69 @@ int32_t lattice_v3_prepare(net* h) {
     return NET_OK;
 }
 
+// Kuramoto-Sakaguchi with inertia (eq. (3) in full; the paper's own performance model,
+// PAPER.md:327, :337-343) on the field-split lattice kernels: psi is a LOCAL variable, the coupling
+// is the KS one, so a stage is (1) the RHS instance of lat3s_kernel on the exchange field E of the
+// stage input -- c_i = omega_i + (K/Omega) sum_j sin(phi_j - phi_i - alpha), run sums and all --
+// and (2) one pointwise kernel: phi' = psi, psi' = (c - eps psi)/m, the RK4 stage update of both
+// variables, and E = (cos, sin) of the new phi with its periodic ghost images for the next stage.
+template <class T>
+__global__ void __launch_bounds__(256) ksi_update_kernel(StageArgs a, ModelParams mp, const T* __restrict__ c,
+                                                        T* __restrict__ E, int nx, int ny, int nz, int HX, int P, long long plane) {
+    const int64_t n = a.n, ld = a.ld;
+    const T* __restrict__ in = (const T*)a.in;
+    const int stage = a.stage;
+    const T dt = (T)a.dt;
+    const int nxp = nx + 2 * HX, nyp = ny + 2 * P;
+    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+        const T xin[2] = {in[i], in[ld + i]};
+        const T k[2] = {xin[1], (c[i] - T(mp.damp) * xin[1]) * T(mp.inv_m)};
+        T o[2];
+#pragma unroll
+        for (int v = 0; v < 2; ++v) {
+            T y = 0, y2 = 0, y3 = 0;
+            if (stage != STAGE_RHS_ONLY) y = ((const T*)a.y)[v * ld + i];
+            if (stage == 3) { y2 = ((const T*)a.Y2)[v * ld + i]; y3 = ((const T*)a.Y3)[v * ld + i]; }
+            o[v] = stage_combine<T>(stage, dt, k[v], y, y2, y3, xin[v]);
+            ((T*)a.out)[v * ld + i] = o[v];
+        }
+        if (stage == STAGE_RHS_ONLY) continue;
+        T sn, cs;
+        sincos_stage<T>(o[0], &sn, &cs);
+        const int x = (int)(i % nx);
+        const int64_t r = i / nx;
+        const int y = (int)(r % ny), z = (int)(r / ny);
+        const int64_t ip = ((int64_t)z * nyp + (y + P)) * nxp + (x + HX);
+        const int gxs = x < HX ? nx : (x >= nx - HX ? -nx : 0);      // periodic images this element also owns
+        const int gys = y < P ? ny : (y >= ny - P ? -ny : 0);
+        auto put = [&](int64_t at) { E[at] = cs; E[plane + at] = sn; };
+        put(ip);
+        if (gxs) put(ip + gxs);
+        if (gys) {
+            put(ip + (int64_t)gys * nxp);
+            if (gxs) put(ip + (int64_t)gys * nxp + gxs);
+        }
+    }
+}
+
+static int32_t ksi_lattice_stage(net* h, const StageArgs& sa) {
+    int32_t rc = l3_dispatch(h, 4, 0.0, h->ksi_c);           // RHS instance of the KS kernel on E_a = E(stage input)
+    if (rc) return rc;
+    const TopoView& tv = h->tv;
+    const int HX = l2_gx(h->desc.dtype, tv.P);
+    const long long plane = (long long)(tv.nx + 2 * HX) * (tv.ny + 2 * tv.P) * tv.nz;
+    const unsigned g = l2_grid_for(h->n);
+    if (h->desc.dtype == NET_F32)
+        ksi_update_kernel<float><<<g, 256, 0, h->stream>>>(sa, h->mp, (const float*)h->ksi_c, (float*)h->E_a, tv.nx, tv.ny, tv.nz, HX, tv.P, plane);
+    else
+        ksi_update_kernel<double><<<g, 256, 0, h->stream>>>(sa, h->mp, (const double*)h->ksi_c, (double*)h->E_a, tv.nx, tv.ny, tv.nz, HX, tv.P, plane);
+    h->launches += 1;
+    OSC_CUDA(h, cudaGetLastError());
+    return NET_OK;
+}
+
 int32_t lattice_v3_stage(net* h, const StageArgs& sa) {
+    if (h->desc.model == NET_MODEL_KSI) return ksi_lattice_stage(h, sa);
     return l3_dispatch(h, sa.stage == STAGE_RHS_ONLY ? 4 : sa.stage, sa.dt, sa.out);
 }
 

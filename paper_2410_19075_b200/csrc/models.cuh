@@ -108,7 +108,21 @@ __device__ __forceinline__ void hh_rhs(const ModelParams& mp, T V, T m, T h, T g
 // --------------------------------------------------------------- neighbours
 // Calls f(j) for every in-neighbour j of element i, and returns the in-degree.
 template <int TOPO, class F>
+__device__ __forceinline__ int for_each_neighbor_local(const TopoView& tv, int64_t n, int64_t i, F&& f);
+
+// A batch of B replicas of a net of rn elements is ONE net of B * rn elements whose coupling matrix is
+// block diagonal: element i belongs to replica i / rn, its neighbours are
+// those of its local index inside that replica.  The topology arrays describe ONE replica.
+template <int TOPO, class F>
 __device__ __forceinline__ int for_each_neighbor(const TopoView& tv, int64_t n, int64_t i, F&& f) {
+    const int64_t rn = tv.ring_n;
+    if (TOPO == NET_TOPO_RING || rn == n) return for_each_neighbor_local<TOPO>(tv, n, i, f);
+    const int64_t base = i / rn * rn;
+    return for_each_neighbor_local<TOPO>(tv, rn, i - base, [&](int64_t j) { f(base + j); });
+}
+
+template <int TOPO, class F>
+__device__ __forceinline__ int for_each_neighbor_local(const TopoView& tv, int64_t n, int64_t i, F&& f) {
     if (TOPO == NET_TOPO_RING) {
         int P = tv.P;
         const int64_t rn = tv.ring_n, base = i / rn * rn;    // a batch is block diagonal: rings of rn elements

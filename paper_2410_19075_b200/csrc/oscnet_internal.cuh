@@ -208,6 +208,7 @@ struct net {
     int lat2_threads;
     size_t lat2_smem;
     void *E_a, *E_b;       // KS on FAST_LATTICE3D_V2: (cos, sin) pairs of the stage states
+    void* ksi_c;           // KSI on FAST_LATTICE3D_V3: coupling term of the stage input (n scalars)
     CUtensorMap tm3_st[4]; // FAST_LATTICE3D_V3: stencil maps (FHN y,Y2,Y3,Y4; KS E_a,E_b)
     CUtensorMap tm3_op[4]; // operand maps (FHN y,Y2 centre boxes; KS y,Y2,Y3,omega scalars)
     oscnet::L3Geom lat3[5]; // per stage (0-3, RHS)

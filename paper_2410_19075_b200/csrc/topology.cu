@@ -147,15 +147,16 @@ __global__ void expand_rows_kernel(TopoView tv, int64_t n, int64_t row_begin, in
                 put(base + j);
             }
         } else {
-            int x = (int)(i % tv.nx);
-            int64_t q = i / tv.nx;
+            const int64_t rbase = i / tv.ring_n * tv.ring_n, il = i - rbase;      // replica of a batch
+            int x = (int)(il % tv.nx);
+            int64_t q = il / tv.nx;
             int y = (int)(q % tv.ny), z = (int)(q / tv.ny);
             for (int o = 0; o < tv.noff; ++o) {
                 int xx = x + tv.off[3 * o], yy = y + tv.off[3 * o + 1], zz = z + tv.off[3 * o + 2];
                 xx += (xx < 0) ? tv.nx : 0; xx -= (xx >= tv.nx) ? tv.nx : 0;
                 yy += (yy < 0) ? tv.ny : 0; yy -= (yy >= tv.ny) ? tv.ny : 0;
                 zz += (zz < 0) ? tv.nz : 0; zz -= (zz >= tv.nz) ? tv.nz : 0;
-                put(((int64_t)zz * tv.ny + yy) * tv.nx + xx);
+                put(rbase + ((int64_t)zz * tv.ny + yy) * tv.nx + xx);
             }
         }
     }
@@ -189,14 +190,20 @@ __global__ void expand_ring_kernel(int64_t n, int32_t P, int32_t include_self, i
     }
 }
 
+// rn = rows of one replica (the arrays describe one replica; a batch repeats them block-diagonally)
 __global__ void copy_rows_kernel(const int64_t* row_ptr, const int32_t* col_idx, int64_t row_begin,
-                                 int64_t row_count, int64_t* out_ptr, int32_t* out_idx) {
-    const int64_t base = row_ptr[row_begin];
-    const int64_t cnt = row_ptr[row_begin + row_count] - base;
+                                 int64_t row_count, int64_t* out_ptr, int32_t* out_idx, int64_t rn) {
+    const int64_t nnz1 = row_ptr[rn];
+    auto gptr = [&](int64_t i) { return (i / rn) * nnz1 + row_ptr[i % rn]; };     // row_ptr of the whole batch
+    const int64_t base = gptr(row_begin);
     int64_t tid = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
     int64_t stride = (int64_t)gridDim.x * blockDim.x;
-    for (int64_t r = tid; r <= row_count; r += stride) out_ptr[r] = row_ptr[row_begin + r] - base;
-    for (int64_t e = tid; e < cnt; e += stride) out_idx[e] = col_idx[base + e];
+    for (int64_t r = tid; r <= row_count; r += stride) out_ptr[r] = gptr(row_begin + r) - base;
+    for (int64_t r = tid; r < row_count; r += stride) {
+        const int64_t i = row_begin + r, rep = i / rn, il = i % rn;
+        int32_t* dst = out_idx + (gptr(i) - base);
+        for (int64_t e = row_ptr[il]; e < row_ptr[il + 1]; ++e) dst[e - row_ptr[il]] = (int32_t)(rep * rn + col_idx[e]);
+    }
 }
 
 // NET_TOPO_COMPRESSED: degrees of a row range (EXTRACT counts), then the rows themselves, sorted
@@ -275,6 +282,7 @@ int32_t topo_build(net* h) {
     tv.P = t.radius;
     tv.include_self = t.include_self ? 1 : 0;
     tv.ring_n = h->n / (h->desc.batch > 0 ? h->desc.batch : 1);
+    const int64_t rn = tv.ring_n, nb = h->desc.batch > 0 ? h->desc.batch : 1;     // elements of one replica, replicas
     cudaStream_t st = h->stream;
     OSC_CUDA(h, cudaMemsetAsync(h->b.flag, 0, 4 * sizeof(int32_t), st));
     if (t.kind == NET_TOPO_RING) {
@@ -297,11 +305,11 @@ int32_t topo_build(net* h) {
         h->nnz = h->n * (int64_t)tv.noff;
     } else if (t.kind == NET_TOPO_CSR) {
         cudaMemcpyKind kind = t.ptrs_are_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
-        OSC_CUDA(h, cudaMemcpyAsync(h->b.row_ptr, t.row_ptr, sizeof(int64_t) * (h->n + 1), kind, st));
+        OSC_CUDA(h, cudaMemcpyAsync(h->b.row_ptr, t.row_ptr, sizeof(int64_t) * (rn + 1), kind, st));
         if (t.nnz > 0)
             OSC_CUDA(h, cudaMemcpyAsync(h->b.col_idx, t.col_idx, sizeof(int32_t) * t.nnz, kind, st));
-        csr_validate_kernel<<<grid_for(t.nnz > h->n ? t.nnz : h->n), 256, 0, st>>>(h->b.row_ptr, h->b.col_idx, h->n, t.nnz, h->b.flag);
-        csr_degree_kernel<<<grid_for(h->n), 256, 0, st>>>(h->b.row_ptr, h->n, h->b.flag);
+        csr_validate_kernel<<<grid_for(t.nnz > rn ? t.nnz : rn), 256, 0, st>>>(h->b.row_ptr, h->b.col_idx, rn, t.nnz, h->b.flag);
+        csr_degree_kernel<<<grid_for(rn), 256, 0, st>>>(h->b.row_ptr, rn, h->b.flag);
         h->launches += 2;
         OSC_CUDA(h, cudaGetLastError());
         int32_t f[4];
@@ -311,12 +319,12 @@ int32_t topo_build(net* h) {
         if (f[0] & 2) return set_err(h, NET_ERR_TOPOLOGY, "CSR col_idx has an index outside [0, n)");
         tv.row_ptr = h->b.row_ptr;
         tv.col_idx = h->b.col_idx;
-        h->nnz = t.nnz;
+        h->nnz = t.nnz * nb;
         h->degree_uniform = f[2] ? -1 : f[1];
     } else if (t.kind == NET_TOPO_COMPRESSED) {
         // V, D, C of Alg. 2 go to the workspace as they are; validated on the host
         const net_compressed* c = t.compressed;
-        const int64_t n = h->n, dtot = c->d_ptr[c->k];
+        const int64_t n = rn, dtot = c->d_ptr[c->k];
         for (int64_t q = 0; q < c->v_len; ++q)
             if (c->v_pos[q] < 0 || c->v_pos[q] >= n || (q > 0 && c->v_pos[q] <= c->v_pos[q - 1]))
                 return set_err(h, NET_ERR_TOPOLOGY, "compressed matrix: common vector not sorted / out of range");
@@ -356,8 +364,8 @@ int32_t topo_build(net* h) {
         tv.cmp_vlen = (int32_t)c->v_len; tv.cmp_k = (int32_t)c->k; tv.cmp_maxdeg = maxdeg;
         h->nnz = nnz;
     } else {  // RANDOM_INDEGREE
-        random_indegree_kernel<<<grid_for(h->n), 256, 0, st>>>(h->n, t.in_degree, t.seed, h->b.col_idx);
-        uniform_row_ptr_kernel<<<grid_for(h->n + 1), 256, 0, st>>>(h->b.row_ptr, h->n, t.in_degree);
+        random_indegree_kernel<<<grid_for(rn), 256, 0, st>>>(rn, t.in_degree, t.seed, h->b.col_idx);
+        uniform_row_ptr_kernel<<<grid_for(rn + 1), 256, 0, st>>>(h->b.row_ptr, rn, t.in_degree);
         h->launches += 2;
         OSC_CUDA(h, cudaGetLastError());
         tv.k_uniform = t.in_degree;
@@ -389,7 +397,7 @@ int32_t topo_expand(net* h, int64_t row_begin, int64_t row_count, int64_t* d_row
             expand_rows_kernel<<<grid_for(row_count), 256, 0, st>>>(h->tv, h->n, row_begin, row_count, deg, d_col_idx);
         h->launches += 2;
     } else {
-        copy_rows_kernel<<<grid_for(row_count * 8 + 1), 256, 0, st>>>(h->b.row_ptr, h->b.col_idx, row_begin, row_count, d_row_ptr, d_col_idx);
+        copy_rows_kernel<<<grid_for(row_count + 1), 256, 0, st>>>(h->b.row_ptr, h->b.col_idx, row_begin, row_count, d_row_ptr, d_col_idx, h->tv.ring_n);
         h->launches += 1;
     }
     OSC_CUDA(h, cudaGetLastError());

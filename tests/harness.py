@@ -41,21 +41,25 @@ def make_inputs(w, seed=1):
     return dict(y0=rnd(y0), elem=None if elem is None else rnd(elem))
 
 
+def _single_topology(w, row_begin=0, row_count=None):
+    if w.topo == configs.RING:
+        return ora.topology_ring(w.n, w.radius, False, row_begin, row_count)
+    if w.topo == configs.LATTICE:
+        return ora.topology_lattice(w.extent, w.radius, False, row_begin, row_count)
+    return ora.topology_random_indegree(w.n, w.in_degree, w.topo_seed, row_begin, row_count)
+
+
 def oracle_topology(w, row_begin=0, row_count=None):
-    if w.topo == configs.RING and getattr(w, "batch", 1) > 1:
-        # the batch as one block-diagonal net: ring r owns elements r*n .. (r+1)*n - 1
-        rp1, ci1 = ora.topology_ring(w.n, w.radius, False, 0, None)
+    if getattr(w, "batch", 1) > 1:
+        # the batch as one block-diagonal net: replica r owns elements r*n .. (r+1)*n - 1
+        rp1, ci1 = _single_topology(w)
         B = w.batch
         ci = np.concatenate([ci1.astype(np.int64) + r * w.n for r in range(B)]).astype(np.int32)
         rp = np.concatenate([[0], np.cumsum(np.tile(np.diff(rp1), B))]).astype(np.int64)
         row_count = ntot(w) - row_begin if row_count is None else row_count
         lo, hi = rp[row_begin], rp[row_begin + row_count]
         return rp[row_begin:row_begin + row_count + 1] - lo, ci[lo:hi]
-    if w.topo == configs.RING:
-        return ora.topology_ring(w.n, w.radius, False, row_begin, row_count)
-    if w.topo == configs.LATTICE:
-        return ora.topology_lattice(w.extent, w.radius, False, row_begin, row_count)
-    return ora.topology_random_indegree(w.n, w.in_degree, w.topo_seed, row_begin, row_count)
+    return _single_topology(w, row_begin, row_count)
 
 
 def make_oracle(w, inp, rows=None):

@@ -63,10 +63,42 @@ def test_replica_equals_the_ring_integrated_alone():
         assert np.array_equal(got[:, r, :], alone)      # same kernel, same arithmetic: bit-identical
 
 
-def test_batch_on_other_topologies_is_refused():
+@pytest.mark.parametrize("cfg,kw,batch", [("5", dict(n1=10), 3), ("3b", dict(n1=9), 2), ("4", dict(n=700), 4),
+                                          ("6", dict(n1=8), 2), ("3a", dict(n1=12), 2)])
+def test_batches_of_lattices_and_graphs(cfg, kw, batch):
+    """batch > 1 on every topology kind (batch is a property of net_create): the
+    block-diagonal net on the per-link kernels; topology bit-exact, RHS and 100 steps within the
+    north star's tolerances against the oracle on the block-diagonal CSR, replica = the net alone."""
+    w = replace(configs.get(cfg, **kw), batch=batch)
+    inp = H.make_inputs(w, seed=6)
+    onet = H.make_oracle(w, inp)
+    net = H.make_gpu(w, inp)
+    assert net.counters()[1] == B.METHOD_DIRECT
+    rp, ci = net.get_topology()
+    rp0, ci0 = H.oracle_topology(w)
+    assert np.array_equal(rp, rp0) and np.array_equal(ci, ci0)
+    a, b = net.get_topology(w.n - 3, 7)                    # a range that straddles two replicas
+    a0, b0 = H.oracle_topology(w, w.n - 3, 7)
+    assert np.array_equal(a, a0) and np.array_equal(b, b0)
+    assert H.rel_maxnorm(net.eval_rhs(), onet.rhs(inp["y0"]), H.rhs_floor(w)) <= H.TOL_RHS[w.dtype]
+    net.integrate(100, w.dt)
+    got = net.get_state()
+    assert H.traj_err(w, got, onet.rk4(inp["y0"], 100, w.dt)) <= H.TOL_TRAJ[w.dtype]
+    w1 = replace(w, batch=1)
+    r = batch - 1
+    sl = slice(r * w.n, (r + 1) * w.n)
+    inp1 = dict(y0=inp["y0"][:, sl].copy(), elem=None if inp["elem"] is None else inp["elem"][sl].copy())
+    n1 = H.make_gpu(w1, inp1, method=B.METHOD_DIRECT)
+    n1.integrate(100, w.dt)
+    assert np.array_equal(got[:, sl], n1.get_state())      # same kernel, same arithmetic: bit-identical
+    rep = net.observable(B.OBS_REPLICA_ORDER).reshape(batch, 2)
+    assert abs(rep[r, 0] - n1.observable(B.OBS_GLOBAL_ORDER)[0]) < 1e-12
+
+
+def test_batch_refusals():
     w = replace(configs.get("5", n1=16), batch=2)
-    with pytest.raises(B.OscnetError) as ei:
-        B.Net.from_workload(w)
+    with pytest.raises(B.OscnetError) as ei:               # the tiled lattice kernels take one lattice
+        B.Net.from_workload(w, method=B.METHOD_FAST)
     assert ei.value.code == -5
     w = replace(configs.get("1"), batch=0)
     with pytest.raises(B.OscnetError) as ei:

@@ -1,6 +1,7 @@
-"""Kuramoto-Sakaguchi with inertia (eq. (3) in full) : the persistent
-ring kernel (FAST) for rings, the per-link DIRECT form elsewhere; parity with the pinned oracle (tests/test_oracle_dynamics.py::test_ksi_*) on every topology
-kind, both dtypes; FAST is refused on lattices and graphs in this build."""
+"""Kuramoto-Sakaguchi with inertia (eq. (3) in full): the persistent
+ring kernel (FAST) for rings, the field-split lattice kernels (FAST) for 3D balls of radius 2 / 4, the
+per-link DIRECT form elsewhere; parity with the pinned oracle (tests/test_oracle_dynamics.py::test_ksi_*)
+on every topology kind, both dtypes."""
 from dataclasses import replace
 
 import numpy as np
@@ -34,8 +35,10 @@ def test_ksi_direct_matches_oracle(w):
     onet = H.make_oracle(w, inp)
     net = H.make_gpu(w, inp)
     launches, method = net.counters()
-    # rings: the persistent prefix-sum kernel (FAST); other topologies: the per-link DIRECT form
-    assert method == (B.METHOD_FAST if w.topo == configs.RING else B.METHOD_DIRECT)
+    # rings: the persistent prefix-sum kernel; 3D balls: the field-split lattice kernels (both FAST);
+    # 2D lattices and graphs: the per-link DIRECT form
+    fast = w.topo == configs.RING or (w.topo == configs.LATTICE and len(w.extent) == 3)
+    assert method == (B.METHOD_FAST if fast else B.METHOD_DIRECT)
     rp, ci = net.get_topology()
     rp0, ci0 = H.oracle_topology(w)
     assert np.array_equal(rp, rp0) and np.array_equal(ci, ci0)
@@ -66,11 +69,36 @@ def test_ksi_ring_fast_and_direct_and_batches(method, batch):
     net.close()
 
 
-def test_ksi_fast_is_refused_and_mass_must_be_positive():
-    w = configs.get("6", n1=12)
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("n1,radius", [(12, 2), (20, 4), (36, 2)])
+def test_ksi_lattice_fast_and_direct(n1, radius, dtype):
+    """The paper's performance model (Fig. 6c) on the field-split lattice kernels: RHS instance of the
+    KS kernel + one pointwise update of (phi, psi); FAST against the oracle and against DIRECT."""
+    w = replace(configs.get("6", n1=n1), radius=radius, dtype=dtype,
+                name="KSI 3D %d^3 radius %d %s" % (n1, radius, dtype))
+    inp = H.make_inputs(w, seed=5)
+    onet = H.make_oracle(w, inp)
+    fast = H.make_gpu(w, inp, method=B.METHOD_FAST)
+    assert fast.kernel_family() == 6
+    direct = H.make_gpu(w, inp, method=B.METHOD_DIRECT)
+    ref = onet.rhs(inp["y0"])
+    assert H.rel_maxnorm(fast.eval_rhs(), ref) <= H.TOL_RHS[dtype]
+    assert H.rel_maxnorm(fast.eval_rhs(), direct.eval_rhs()) <= 2 * H.TOL_RHS[dtype]
+    fast.integrate(37, w.dt)
+    fast.integrate(63, w.dt)
+    got = fast.get_state().astype(np.float64)
+    assert H.traj_err(w, got, onet.rk4(inp["y0"], 100, w.dt)) <= H.TOL_TRAJ[dtype]
+    # RHS after steps: the exchange field of the current state is the one the last stage left
+    assert H.rel_maxnorm(fast.eval_rhs(), onet.rhs(got)) <= 10 * H.TOL_RHS[dtype]
+    fast.close(); direct.close()
+
+
+def test_ksi_fast_is_refused_on_graphs_and_mass_must_be_positive():
+    w = replace(configs.get("6", n1=12), topo=configs.RANDOM_INDEGREE, n=3000, extent=(), radius=0, in_degree=20)
     with pytest.raises(B.OscnetError) as ei:
         B.Net.from_workload(w, method=B.METHOD_FAST)
     assert ei.value.code == -5
+    w = configs.get("6", n1=12)
     bad = replace(w, params=dict(P6, m=0.0))
     with pytest.raises(B.OscnetError) as ei:
         B.Net.from_workload(bad)
