@@ -252,13 +252,14 @@ static int32_t l3_configure_tile(net* h) {
     if ((rc = l3_configure_stage<T, MODEL, P, L3_S2>(h))) return rc;
     if ((rc = l3_configure_stage<T, MODEL, P, L3_S3>(h))) return rc;
     if ((rc = l3_configure_stage<T, MODEL, P, L3_RHS>(h))) return rc;
+    if ((rc = l3_configure_stage<T, MODEL, P, L3_LOC>(h))) return rc;
     // the tile is the same for every stage (only D differs), so one set of maps serves all
     const L3Geom& g = h->lat3[0];
     const uint64_t nxp = (uint64_t)g.nx + 2 * HX, nyp = (uint64_t)g.ny + 2 * P;
     void* st_src[4] = {h->b.y, h->b.Y2, h->b.Y3, h->b.Y4};
     if (KS) { st_src[0] = h->E_a; st_src[1] = h->E_b; }
     constexpr bool PLANAR = L3Sh<T, MODEL, P>::SPLIT;   // (cos | sin) planes instead of pairs (lat3s_kernel.cuh)
-    for (int st = 0; st < 5; ++st) h->lat3[st].plane = (long long)(nxp * nyp * (uint64_t)g.nz);
+    for (int st = 0; st < 6; ++st) h->lat3[st].plane = (long long)(nxp * nyp * (uint64_t)g.nz);
     for (int k = 0; k < (KS ? 2 : 4); ++k) {
         if (PLANAR) rc = l3_encode_planes(h, &h->tm3_st[k], st_src[k], (int)sizeof(T), nxp, nyp, (uint64_t)g.nz, (uint32_t)g.PW, (uint32_t)g.PH);
         else rc = l3_encode(h, &h->tm3_st[k], st_src[k], 8, nxp * U8, nyp, (uint64_t)g.nz, (uint32_t)(g.PW * U8), (uint32_t)g.PH);
@@ -295,6 +296,7 @@ static L3Params<T> l3_params(const net* h, int stage, double dt) {
     p.cvu = (T)(s * mp.bvu); p.cvv = (T)(s * mp.bvv);
     p.ie = (T)mp.inv_eps; p.ie3 = (T)(-mp.inv_eps / 3.0); p.a = (T)mp.a;
     p.kd = (T)(mp.K * inv_deg); p.ca = (T)mp.cos_a; p.sa = (T)mp.sin_a;
+    p.inv_nb = (T)(1.0 / n_ball);
     p.include_self = h->tv.include_self;
     return p;
 }
@@ -340,6 +342,9 @@ static int32_t l3_stage(net* h, int stage, double dt, void* rhs_out) {
             op[0] = to[1];                     // Z lives in Y2
             if (KS) op[1] = to[3];
             return l3_launch_stage<T, MODEL, P, L3_S3>(h, a, dt, tm[KS ? 1 : 3], op);
+        case 5:     // local order parameter: KS reads E(y) = E_a, FHN the unit phasor field staged in Y3
+            a.out = rhs_out;
+            return l3_launch_stage<T, MODEL, P, L3_LOC>(h, a, dt, tm[KS ? 0 : 2], op);
         default:
             a.out = rhs_out;
             if (KS) op[0] = to[3];

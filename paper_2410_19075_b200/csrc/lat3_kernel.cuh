@@ -26,12 +26,15 @@
 
 namespace oscnet {
 
-enum { L3_S0 = 0, L3_S1 = 1, L3_S2 = 2, L3_S3 = 3, L3_RHS = 4 };
+// L3_LOC: not a stage of the integrator -- the local order parameter of reading R9 through the same
+// ball-sum machinery: the stencil source is the unit phasor field
+// (cos theta, sin theta), the finisher writes |ball sum incl. the centre| / n_ball.
+enum { L3_S0 = 0, L3_S1 = 1, L3_S2 = 2, L3_S3 = 3, L3_RHS = 4, L3_LOC = 5 };
 
 // operand tiles per finished plane.  FHN (pair tiles): stage 0: - | 1: y | 2: y, Y2 | 3: Z | RHS: -
 // KS (scalar tiles, omega last): stage 0, 1: y, omega | 2: y, Y2, Y3, omega | 3: Z, omega | RHS: omega
 template <int MODEL, int STAGE> struct L3Ops {
-    static constexpr int N = MODEL == NET_MODEL_FHN
+    static constexpr int N = STAGE == L3_LOC ? 0 : MODEL == NET_MODEL_FHN
         ? (STAGE == L3_S1 || STAGE == L3_S3 ? 1 : STAGE == L3_S2 ? 2 : 0)
         : (STAGE == L3_S2 ? 4 : STAGE == L3_RHS ? 1 : 2);
 };
@@ -42,6 +45,7 @@ template <class T> struct L3Params {   // model constants in the arithmetic type
     T cuu, cuv, cvu, cvv;      // FHN: (sigma/Omega) b, the u row also divided by eps
     T ie, ie3, a;              // FHN: 1/eps, -1/(3 eps), a
     T kd, ca, sa;              // KS: K/Omega, cos alpha, sin alpha
+    T inv_nb;                  // L3_LOC: 1 / (lattice points of the ball including the centre)
     int include_self;
 };
 
@@ -237,6 +241,16 @@ lat3_kernel(const __grid_constant__ CUtensorMap tm_st, const __grid_constant__ C
             for (int r = 0; r < TY; ++r) {
                 const int yy = yrow0 + r;
                 if (yy >= ny) continue;
+                if constexpr (STAGE == L3_LOC) {     // |sum of the unit phasors over the ball| / n_ball, plain scalar array
+                    T lo[X];
+#pragma unroll
+                    for (int e = 0; e < X; ++e) {
+                        const Pr W = acc[J % NACC][r][e];
+                        lo[e] = sqrt(W.x * W.x + W.y * W.y) * mp.inv_nb;
+                    }
+                    stg_vec<X>((T*)a.out + ((int64_t)zo * ny + yy) * nx + x, lo);
+                    continue;
+                }
                 const int64_t ip = (int64_t)zo * pxy + (int64_t)(yy + P) * nxp + (x + HX);     // padded pair arrays
                 const int gys = yy < P ? ny : (yy >= ny - P ? -ny : 0);
                 auto store_pairs = [&](T* base, const T (&vals)[2 * X]) {    // with the periodic images

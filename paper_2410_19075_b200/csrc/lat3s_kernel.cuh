@@ -208,6 +208,12 @@ lat3s_kernel(const __grid_constant__ CUtensorMap tm_st, const __grid_constant__ 
                 ldg_vec<X>(cc, cx);
                 ldg_vec<X>(cc + splane, cy);
                 T ov[X], zv[X], cv[X], sv[X];
+                if constexpr (STAGE == L3_LOC) {      // local order parameter: |ball sum incl. the centre| / n_ball
+#pragma unroll
+                    for (int e = 0; e < X; ++e) ov[e] = sqrt(ownv[e] * ownv[e] + other[e] * other[e]) * mp.inv_nb;
+                    stg_vec<X>((T*)a.out + il, ov);
+                    continue;
+                }
 #pragma unroll
                 for (int e = 0; e < X; ++e) {
                     const T own = ownv[e];

@@ -268,6 +268,54 @@ static int32_t ksi_lattice_stage(net* h, const StageArgs& sa) {
     return NET_OK;
 }
 
+// ------------------------------------------------------------------ local order parameter
+// R_i = |sum over the ball incl. i of e^{i theta_j}| / n_ball (reading R9) through the L3_LOC instance
+// of the lattice kernels instead of one gather per link.  KS / KSI: the unit phasor field is the
+// exchange field E(y) the stages keep anyway.  FHN: (u, v)/|(u, v)| of every padded position of y
+// (ghosts hold the periodic images already) is written to Y3, which is dead between steps.
+template <class T>
+__global__ void unit_pairs_kernel(const T* __restrict__ y, T* __restrict__ out, int64_t pairs) {
+    for (int64_t e = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; e < pairs; e += (int64_t)gridDim.x * blockDim.x) {
+        const T u = y[2 * e], v = y[2 * e + 1];
+        // theta = atan2(v, u); (cos, sin) theta = (u, v)/r, and (1, 0) at the origin as atan2(0, 0) = 0
+        const T r = sqrt(u * u + v * v);
+        out[2 * e] = r > T(0) ? u / r : T(1);
+        out[2 * e + 1] = r > T(0) ? v / r : T(0);
+    }
+}
+
+template <class T>
+__global__ void widen_kernel(const T* __restrict__ in, double* __restrict__ out, int64_t n) {
+    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) out[i] = (double)in[i];
+}
+
+bool lattice_v3_has_local_order(const net* h) {
+    return h->method == NET_METHOD_FAST && h->fast_kind == FAST_LATTICE3D_V3 && !getenv("OSCNET_NO_FAST_OBS");
+}
+
+int32_t lattice_v3_local_order(net* h, double* d_out) {
+    int32_t rc;
+    const bool f32 = h->desc.dtype == NET_F32;
+    if (h->desc.model == NET_MODEL_FHN) {
+        const int64_t pairs = (int64_t)padded_pairs(&h->desc);
+        if (f32) unit_pairs_kernel<float><<<l2_grid_for(pairs), 256, 0, h->stream>>>((const float*)h->b.y, (float*)h->b.Y3, pairs);
+        else unit_pairs_kernel<double><<<l2_grid_for(pairs), 256, 0, h->stream>>>((const double*)h->b.y, (double*)h->b.Y3, pairs);
+        h->launches += 1;
+    } else if (!h->s_valid) {
+        if ((rc = lattice_v2_refresh_exchange(h))) return rc;
+        h->s_valid = 1;
+    }
+    // fp32 nets: the kernel writes float (into Y4, rewritten by the next step), widened afterwards
+    void* out = f32 ? h->b.Y4 : (void*)d_out;
+    if ((rc = l3_dispatch(h, 5, 0.0, out))) return rc;
+    if (f32) {
+        widen_kernel<float><<<l2_grid_for(h->n), 256, 0, h->stream>>>((const float*)h->b.Y4, d_out, h->n);
+        h->launches += 1;
+    }
+    OSC_CUDA(h, cudaGetLastError());
+    return NET_OK;
+}
+
 int32_t lattice_v3_stage(net* h, const StageArgs& sa) {
     if (h->desc.model == NET_MODEL_KSI) return ksi_lattice_stage(h, sa);
     return l3_dispatch(h, sa.stage == STAGE_RHS_ONLY ? 4 : sa.stage, sa.dt, sa.out);

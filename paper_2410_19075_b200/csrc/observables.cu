@@ -163,8 +163,67 @@ int32_t obs_replica_order(net* h, const double* d_theta, double* d_out) {
     return NET_OK;
 }
 
+// Rings: the window sum of (cos, sin) theta over |j - i| <= P is a difference of prefix sums -- the
+// same machinery as the ring stage kernel.  In-place inclusive scan of the two
+// rows of cs (one CTA; the rings are small), then one thread per element.
+__global__ void __launch_bounds__(1024) ring_prefix_kernel(double* __restrict__ cs, int64_t n) {
+    __shared__ double wsum[2][32];
+    __shared__ double carry[2];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    if (threadIdx.x < 2) carry[threadIdx.x] = 0.0;
+    __syncthreads();
+    for (int64_t base = 0; base < n; base += 1024) {
+        const int64_t i = base + threadIdx.x;
+        double a = i < n ? cs[i] : 0.0, b = i < n ? cs[n + i] : 0.0;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const double ua = __shfl_up_sync(0xffffffffu, a, o), ub = __shfl_up_sync(0xffffffffu, b, o);
+            if (lane >= o) { a += ua; b += ub; }
+        }
+        if (lane == 31) { wsum[0][warp] = a; wsum[1][warp] = b; }
+        __syncthreads();
+        double oa = carry[0], ob = carry[1];
+        for (int w = 0; w < warp; ++w) { oa += wsum[0][w]; ob += wsum[1][w]; }
+        a += oa; b += ob;
+        if (i < n) { cs[i] = a; cs[n + i] = b; }
+        __syncthreads();
+        if (threadIdx.x == 1023) { carry[0] = a; carry[1] = b; }
+        __syncthreads();
+    }
+}
+
+// pre = inclusive prefix of (cos | sin) over all rings back to back; ring r = elements [r rn, (r+1) rn)
+__global__ void ring_local_order_kernel(const double* __restrict__ pre, int64_t n, int64_t rn, int P, double* __restrict__ out) {
+    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+        const int64_t base = i / rn * rn, il = i - base;
+        auto pref = [&](const double* p, int64_t j) { return j < 0 ? 0.0 : p[j]; };     // Pref(-1) = 0
+        double w[2];
+#pragma unroll
+        for (int f = 0; f < 2; ++f) {
+            const double* p = pre + (int64_t)f * n;
+            const double before = pref(p, base - 1), total = p[base + rn - 1] - before;   // this ring alone
+            int64_t lo = il - P, hi = il + P;                                             // window [lo, hi], self included
+            double s = 0.0;
+            if (lo < 0) { s += total - (p[base + lo + rn - 1] - before); lo = 0; }        // tail of the ring
+            if (hi >= rn) { s += p[base + hi - rn] - before; hi = rn - 1; }               // head of the ring
+            s += p[base + hi] - pref(p, base + lo - 1);
+            w[f] = s;
+        }
+        out[i] = sqrt(w[0] * w[0] + w[1] * w[1]) / (double)(2 * P + 1);
+    }
+}
+
 int32_t obs_local_order(net* h, const double* d_theta, double* d_out) {
+    // 3D lattices on the tiled kernels: the ball-sum instance of the stage kernel (lattice_v2.cu)
+    if (lattice_v3_has_local_order(h)) return lattice_v3_local_order(h, d_out);
     cossin_kernel<<<grid_for(h->n), 256, 0, h->stream>>>(d_theta, h->n, h->b.obs_tmp);
+    if (h->tv.kind == NET_TOPO_RING && 2 * (int64_t)h->tv.P + 1 <= h->tv.ring_n) {
+        ring_prefix_kernel<<<1, 1024, 0, h->stream>>>(h->b.obs_tmp, h->n);
+        ring_local_order_kernel<<<grid_for(h->n), 256, 0, h->stream>>>(h->b.obs_tmp, h->n, h->tv.ring_n, h->tv.P, d_out);
+        h->launches += 3;
+        OSC_CUDA(h, cudaGetLastError());
+        return NET_OK;
+    }
     unsigned g = grid_for(h->n);
     switch (h->tv.kind) {
         case NET_TOPO_RING: local_order_kernel<NET_TOPO_RING><<<g, 256, 0, h->stream>>>(h->tv, h->n, h->b.obs_tmp, d_out); break;

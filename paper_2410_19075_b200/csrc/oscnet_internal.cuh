@@ -211,10 +211,10 @@ struct net {
     void* ksi_c;           // KSI on FAST_LATTICE3D_V3: coupling term of the stage input (n scalars)
     CUtensorMap tm3_st[4]; // FAST_LATTICE3D_V3: stencil maps (FHN y,Y2,Y3,Y4; KS E_a,E_b)
     CUtensorMap tm3_op[4]; // operand maps (FHN y,Y2 centre boxes; KS y,Y2,Y3,omega scalars)
-    oscnet::L3Geom lat3[5]; // per stage (0-3, RHS)
-    unsigned lat3_grid[5];
-    int lat3_threads[5];
-    size_t lat3_smem[5];
+    oscnet::L3Geom lat3[6]; // per stage (0-3, RHS, local order parameter)
+    unsigned lat3_grid[6];
+    int lat3_threads[6];
+    size_t lat3_smem[6];
     char cb_geom[96];      // FAST_CSR_BLOCKED: CbGeom (csr_blocked.cu)
     unsigned cb_grid;
     int32_t cb_pair;       // 1 = pair form of the blocked CSR kernel (each CTA streams half of the s blocks)
@@ -278,6 +278,8 @@ int32_t rhs_at(net* h, const void* d_x, void* d_k);
 int32_t obs_global_order(net* h, const double* d_theta, double* d_out2);  // {R, Psi}
 int32_t obs_replica_order(net* h, const double* d_theta, double* d_out);  // {R_r, Psi_r} per replica of the batch
 int32_t obs_local_order(net* h, const double* d_theta, double* d_out);
+bool lattice_v3_has_local_order(const net* h);                 // lattice_v2.cu: ball-sum form of the local order parameter
+int32_t lattice_v3_local_order(net* h, double* d_out);
 int32_t obs_window_begin(net* h);
 int32_t obs_window_sample(net* h, int first);
 int32_t obs_window_finish(net* h, double t_a, double t_b, int64_t n_samples);
