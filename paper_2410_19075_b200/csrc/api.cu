@@ -534,6 +534,19 @@ int32_t net_integrate_observed(net_t* h, int64_t n_steps, double dt, int64_t obs
     int32_t rc = obs_window_begin(h);
     if (rc) return rc;
     const double t0 = h->t;
+    {   // phase models on the persistent ring kernel: one launch, samples taken inside it
+        int64_t first = (n_steps + 1) / 2;                              // smallest s with 2 s >= n_steps ...
+        first = (first + obs_every - 1) / obs_every * obs_every;        // ... that is a sample step
+        if (first < obs_every) first = obs_every;
+        bool handled = false;
+        if ((rc = ring_run_observed(h, n_steps, dt, obs_every, first, &handled))) return rc;
+        if (handled) {
+            h->step += n_steps;
+            h->t += (double)n_steps * dt;
+            if ((rc = obs_window_sample(h, first == n_steps))) return rc;      // the sample at n_steps
+            return obs_window_finish(h, t0 + (double)first * dt, t0 + (double)n_steps * dt, (n_steps - first) / obs_every + 1);
+        }
+    }
     int64_t n_samples = 0, s_a = -1;
     for (int64_t s = obs_every; s <= n_steps; s += obs_every) {
         if ((rc = integrate_plain(h, obs_every, dt))) return rc;

@@ -264,6 +264,7 @@ int32_t pairs_unpack(net* h, const void* pairs, void* soa);
 // observables.cu ------------------------------------------------------------
 int32_t obs_phase(net* h, const void* state, double* d_theta);
 int32_t ring_probe_latency(net* h, double* out4);   // ring_fast.cu
+int32_t ring_run_observed(net* h, int64_t n_steps, double dt, int64_t obs_every, int64_t s_a, bool* handled);
 int32_t probe_peaks(net* h, double* out8);          // probe.cu
 // delay.cu (NET_MODEL_FHN2: eq. (2) with delay and noise)
 int32_t delay_stage(net* h, const StageArgs& a);

@@ -30,6 +30,8 @@ namespace oscnet {
 
 constexpr int RING_THREADS = 256;
 constexpr int RING_GMAX = RING_THREADS;   // the chunk totals are scanned in one pass by one CTA
+constexpr int RING_NT_SINGLE = 256;       // threads of a single-CTA ring / of every ring of a batch unless OSCNET_RING_NT
+constexpr int RING_NT_BATCH = 128;        // says otherwise (measured, see ring_plan)
 
 struct RingArgs {
     const void* y_in;        // [nvar][ld] state the run starts from / RHS is evaluated on
@@ -43,6 +45,13 @@ struct RingArgs {
     int64_t n_steps;
     double dt;
     int32_t rhs_only;
+    // phase models: order-parameter samples taken inside the launch (net_integrate_observed).  The
+    // block totals of (cos phi, sin phi) that stage 0 of a step scans anyway ARE the sums of the
+    // global order parameter of the state at that step, so a sample costs one 16-byte store.
+    int64_t obs_every;       // 0: no sampling; else the state at steps obs_first, obs_first + obs_every, ... < n_steps
+    int64_t obs_first;
+    double* obs_cs;          // [sample][ring][2] = sum cos phi, sum sin phi over the ring
+    double* obs_ref;         // phi of every element at step obs_first (start of the velocity window)
 };
 
 __device__ __forceinline__ unsigned ld_acquire_u32(const unsigned* p) {
@@ -72,8 +81,8 @@ template <class T> __device__ __forceinline__ void st_l2(T* p, T v) { __stcg(p, 
 // barrier of its own before wsum is written again.  (A radix-4 warp scan with a tree over the
 // warp totals -- fewer dependent levels, more shuffles -- was measured slower: 0.35 against
 // 0.34 us per scan, config 1b 2.29e10 against 2.51e10.)
-template <class A, bool TAIL_SYNC>
-__device__ __forceinline__ void block_scan2(A& a, A& b, A& ta, A& tb, A (*wsum)[RING_THREADS / 32]) {
+template <class A, bool TAIL_SYNC, int NT = RING_THREADS>
+__device__ __forceinline__ void block_scan2(A& a, A& b, A& ta, A& tb, A (*wsum)[NT / 32]) {
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) {
@@ -84,7 +93,7 @@ __device__ __forceinline__ void block_scan2(A& a, A& b, A& ta, A& tb, A (*wsum)[
     __syncthreads();
     A oa = 0, ob = 0, sa = 0, sb = 0;
 #pragma unroll
-    for (int w = 0; w < RING_THREADS / 32; ++w) {
+    for (int w = 0; w < NT / 32; ++w) {
         const A va = wsum[0][w], vb = wsum[1][w];
         if (w < warp) { oa += va; ob += vb; }
         sa += va; sb += vb;
@@ -94,14 +103,20 @@ __device__ __forceinline__ void block_scan2(A& a, A& b, A& ta, A& tb, A (*wsum)[
     if (TAIL_SYNC) __syncthreads();
 }
 
-template <class T, int MODEL, int E, bool SINGLE>
-__global__ void __launch_bounds__(RING_THREADS) ring_persistent_kernel(RingArgs a, ModelParams mp) {
+// NT: threads per CTA.  Multi-CTA rings always run RING_THREADS; single-CTA rings (config 1 and the
+// batches) may run fewer, wider threads: fewer warps shorten the scan over the warp totals and the
+// CTA barriers, more elements per thread lengthen the serial part (sincos, thread-local prefix).
+// OBS: the launch takes order-parameter samples (a separate instance: the plain kernel carries none
+// of it -- the first version, with the test inside the one kernel, cost config 1 20 %).
+template <class T, int MODEL, int E, bool SINGLE, int NT = RING_THREADS, bool OBS = false>
+__global__ void __launch_bounds__(NT) ring_persistent_kernel(RingArgs a, ModelParams mp) {
     // KS: phi | FHN: (u, v) | KS with inertia (eq. (3) in full): (phi, psi = dphi/dt), fields as for KS
     constexpr int NV = MODEL == NET_MODEL_KS ? 1 : 2;
     constexpr bool PHASE = MODEL == NET_MODEL_KS || MODEL == NET_MODEL_KSI;
     extern __shared__ __align__(16) unsigned char ring_smem[];
-    __shared__ T wsumT[2][RING_THREADS / 32];
-    __shared__ double wsumD[2][RING_THREADS / 32];
+    static_assert(SINGLE || NT == RING_THREADS, "multi-CTA rings scan the chunk totals with RING_THREADS threads");
+    __shared__ T wsumT[2][NT / 32];
+    __shared__ double wsumD[2][NT / 32];
     __shared__ double BT[2][RING_GMAX + 1];
 
     const int64_t n = a.n, ld = a.ld;
@@ -133,6 +148,7 @@ __global__ void __launch_bounds__(RING_THREADS) ring_persistent_kernel(RingArgs 
     }
 
     const int64_t n_stage = a.rhs_only ? 1 : 4 * a.n_steps;
+    [[maybe_unused]] int64_t next_sample = a.obs_first, n_sampled = 0;
     for (int64_t q = 0; q < n_stage; ++q) {
         const int stage = (int)(q & 3);
         const int buf = (int)(q & 1);
@@ -159,8 +175,28 @@ __global__ void __launch_bounds__(RING_THREADS) ring_persistent_kernel(RingArgs 
 #pragma unroll
         for (int e = 1; e < E; ++e) { p0[e] = p0[e - 1] + f0[e]; p1[e] = p1[e - 1] + f1[e]; }
         T s0 = p0[E - 1], s1 = p1[E - 1], t0, t1;
-        block_scan2<T, false>(s0, s1, t0, t1, wsumT);       // a CTA barrier follows before wsumT is reused
+        block_scan2<T, false, NT>(s0, s1, t0, t1, wsumT);   // a CTA barrier follows before wsumT is reused
         const T ex0 = s0 - p0[E - 1], ex1 = s1 - p1[E - 1];   // exclusive offset of this thread
+        // order-parameter sample of the state this step starts from
+        [[maybe_unused]] bool sample_now = false;
+        [[maybe_unused]] int64_t sample_k = 0;
+        if constexpr (OBS && PHASE) {
+            if (stage == 0 && (q >> 2) == next_sample) {
+                const int64_t sidx = q >> 2;
+                sample_now = true;
+                sample_k = n_sampled++;
+                next_sample += a.obs_every;
+                if (SINGLE && threadIdx.x == 0) {
+                    double* o = a.obs_cs + (sample_k * (int64_t)gridDim.x + blockIdx.x) * 2;
+                    o[0] = (double)t0; o[1] = (double)t1;
+                }
+                if (sidx == a.obs_first) {
+#pragma unroll
+                    for (int e = 0; e < E; ++e)
+                        if (ok[e]) a.obs_ref[goff + i0 + e] = (double)y0[e][0];
+                }
+            }
+        }
 #pragma unroll
         for (int e = 0; e < E; ++e) {
             if (ok[e]) {
@@ -206,9 +242,11 @@ __global__ void __launch_bounds__(RING_THREADS) ring_persistent_kernel(RingArgs 
         if (!SINGLE) {
             const double v0 = c0, v1 = c1;
             double u0, u1;
-            block_scan2<double, false>(c0, c1, u0, u1, wsumD);  // the __syncthreads after BT
+            block_scan2<double, false, NT>(c0, c1, u0, u1, wsumD);  // the __syncthreads after BT
             if (threadIdx.x < G) { BT[0][threadIdx.x] = c0 - v0; BT[1][threadIdx.x] = c1 - v1; }
             if (threadIdx.x == 0) { BT[0][G] = u0; BT[1][G] = u1; }
+            if constexpr (OBS)
+                if (sample_now && blockIdx.x == 0 && threadIdx.x == 0) { a.obs_cs[sample_k * 2] = u0; a.obs_cs[sample_k * 2 + 1] = u1; }
             __syncthreads();
         }
         // window sums, local field, RK4 update.  W(i) = Pref(i+P) - Pref(i-P-1) with the ring wrap
@@ -290,7 +328,7 @@ __global__ void __launch_bounds__(RING_THREADS) ring_persistent_kernel(RingArgs 
 }
 
 // ------------------------------------------------------------------ host side
-struct RingPlan { int E, G, chunk; bool single; size_t smem; };
+struct RingPlan { int E, G, chunk, nt; bool single; size_t smem; };
 
 // gmax: CTAs that can be co-resident (one per SM always can; two per SM when the occupancy
 // query at launch agrees -- fewer elements per thread shorten the dependent chain of a stage)
@@ -304,8 +342,25 @@ static bool ring_plan(int64_t n, size_t esize, RingPlan* p, int gmax = 148) {
         const int64_t chunk = (int64_t)RING_THREADS * E;
         const int64_t G = (n + chunk - 1) / chunk;
         if (G <= gmax && G <= RING_GMAX) {
-            p->E = E; p->G = (int)G; p->chunk = (int)chunk; p->single = G == 1;
-            p->smem = p->single ? 2 * (size_t)chunk * esize : 0;
+            p->E = E; p->G = (int)G; p->chunk = (int)chunk; p->single = G == 1; p->nt = RING_THREADS;
+            // single-CTA rings: fewer, wider threads where the ring fits (instantiated: 32 x 8,
+            // 64 x {4, 8}, 128 x {2, 4, 8}).  Default RING_NT_SINGLE, OSCNET_RING_NT overrides.
+            if (p->single) {
+                // measured on B200 (OSCNET_RING_NT sweep, bench configs 1 / 1b, osc-steps/s):
+                //   threads      256      128      64       32 (one warp, 8 elements per lane)
+                //   one ring   1.08e8   9.3e7    6.3e7    2.7e7   -- the fp64 sincos of 8 elements per lane is
+                //                                                   issue-bound in one warp; more warps win
+                //   1184 rings 2.51e10  3.42e10  3.44e10  1.83e10 -- the batch is bound by instruction issue:
+                //                                                   fewer warps = less scan work per element
+                int want = gmax == 1 ? RING_NT_BATCH : RING_NT_SINGLE;
+                if (const char* e = getenv("OSCNET_RING_NT")) want = atoi(e);
+                if (want == 32 || want == 64 || want == 128) {
+                    const int emin_nt = want == 32 ? 8 : want == 64 ? 4 : 2;
+                    for (int E2 = emin_nt; E2 <= 8; E2 *= 2)
+                        if ((int64_t)want * E2 >= n) { p->nt = want; p->E = E2; p->chunk = want * E2; break; }
+                }
+            }
+            p->smem = p->single ? 2 * (size_t)p->chunk * esize : 0;
             return true;
         }
     }
@@ -321,15 +376,23 @@ bool ring_supported(const net_desc* d) {
            ring_plan(d->n / batch, d->dtype == NET_F32 ? 4 : 8, &p, batch > 1 ? 1 : 148);
 }
 
-size_t ring_scratch_bytes(const net_desc* d) {
-    const size_t es = d->dtype == NET_F32 ? 4 : 8;
-    const size_t npad = (size_t)round_up(d->n, 64);
-    return 2 * (2 * npad * es) + 2 * (2 * RING_GMAX * sizeof(double)) + 256 + 1024;
+constexpr size_t RING_OBS_BYTES = 32u << 20;     // order-parameter samples taken inside a launch (16 bytes per sample and ring)
+
+static size_t ring_work_bytes(int64_t n_total, size_t es) {
+    const size_t npad = (size_t)round_up(n_total, 64);
+    return (2 * (2 * npad * es) + 2 * (2 * RING_GMAX * sizeof(double)) + 256 + 1024 + 255) / 256 * 256;
 }
 
-template <class T, int MODEL, int E, bool SINGLE>
+size_t ring_scratch_bytes(const net_desc* d) {
+    return ring_work_bytes(d->n, d->dtype == NET_F32 ? 4 : 8) + RING_OBS_BYTES;
+}
+
+template <class T, int MODEL, int E, bool SINGLE, int NT = RING_THREADS>
 static int32_t ring_launch_t(net* h, RingArgs& a, const RingPlan& p) {
-    auto kern = ring_persistent_kernel<T, MODEL, E, SINGLE>;
+    constexpr bool PHASE = MODEL == NET_MODEL_KS || MODEL == NET_MODEL_KSI;
+    auto kern = ring_persistent_kernel<T, MODEL, E, SINGLE, NT, false>;
+    if constexpr (PHASE)
+        if (a.obs_every > 0) kern = ring_persistent_kernel<T, MODEL, E, SINGLE, NT, true>;
     if (p.smem > 48 * 1024)
         OSC_CUDA(h, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.smem));
     if (!SINGLE && p.G > 148) {      // more than one CTA per SM: must all be resident
@@ -342,7 +405,7 @@ static int32_t ring_launch_t(net* h, RingArgs& a, const RingPlan& p) {
     if (!SINGLE) OSC_CUDA(h, cudaMemsetAsync(a.bar, 0, sizeof(unsigned), h->stream));
     void* params[] = {&a, &h->mp};
     if (SINGLE)      // one CTA per ring of the batch
-        OSC_CUDA(h, cudaLaunchKernel((const void*)kern, dim3((unsigned)h->desc.batch), dim3(RING_THREADS), params, p.smem, h->stream));
+        OSC_CUDA(h, cudaLaunchKernel((const void*)kern, dim3((unsigned)h->desc.batch), dim3(NT), params, p.smem, h->stream));
     else
         OSC_CUDA(h, cudaLaunchCooperativeKernel((const void*)kern, dim3(p.G), dim3(RING_THREADS), params, p.smem, h->stream));
     h->launches += 1;
@@ -351,6 +414,12 @@ static int32_t ring_launch_t(net* h, RingArgs& a, const RingPlan& p) {
 
 template <class T, int MODEL>
 static int32_t ring_launch_e(net* h, RingArgs& a, const RingPlan& p) {
+    if (p.single && p.nt == 32) return ring_launch_t<T, MODEL, 8, true, 32>(h, a, p);
+    if (p.single && p.nt == 64)
+        return p.E == 4 ? ring_launch_t<T, MODEL, 4, true, 64>(h, a, p) : ring_launch_t<T, MODEL, 8, true, 64>(h, a, p);
+    if (p.single && p.nt == 128)
+        return p.E == 2 ? ring_launch_t<T, MODEL, 2, true, 128>(h, a, p)
+             : p.E == 4 ? ring_launch_t<T, MODEL, 4, true, 128>(h, a, p) : ring_launch_t<T, MODEL, 8, true, 128>(h, a, p);
     if (p.single) {
         switch (p.E) {
             case 1: return ring_launch_t<T, MODEL, 1, true>(h, a, p);
@@ -368,9 +437,13 @@ static int32_t ring_launch_e(net* h, RingArgs& a, const RingPlan& p) {
 }
 
 // y_in -> y_out over n_steps RK4 steps (rhs_only: y_out = f(y_in))
-static int32_t ring_run_plan(net* h, const RingPlan& p, const void* y_in, void* y_out, int64_t n_steps, double dt, int rhs_only) {
+static int32_t ring_run_plan(net* h, const RingPlan& p, const void* y_in, void* y_out, int64_t n_steps, double dt, int rhs_only,
+                             int64_t obs_every = 0, int64_t obs_first = 0) {
     RingArgs a;
     memset(&a, 0, sizeof(a));
+    a.obs_every = obs_every; a.obs_first = obs_first;
+    a.obs_cs = (double*)((char*)h->b.scratch + ring_work_bytes(h->n, h->esize));
+    a.obs_ref = h->b.obs_ref;
     a.y_in = y_in; a.y_out = y_out; a.elem_param = h->b.elem_param;
     a.n = h->tv.ring_n; a.ld = h->ld; a.npad = round_up(h->n, 64);
     a.P = h->tv.P; a.include_self = h->tv.include_self; a.chunk = p.chunk; a.G = p.G;
@@ -482,6 +555,49 @@ int32_t ring_probe_latency(net* h, double* out) {
     cudaEventDestroy(e1);
     h->launches += 9;
     return rc;
+}
+
+// sum R, sum R^2 and the count of the samples a launch took, added to the statistics accumulators
+// (observables.cu: acc[0], acc[1], acc[2]); R = |sum over the rings of (C, S)| / n_total
+__global__ void __launch_bounds__(256) ring_obs_accumulate_kernel(const double* __restrict__ cs, int64_t samples, int rings, double inv_n, double* acc) {
+    __shared__ double red[2][256];
+    double s1 = 0.0, s2 = 0.0;
+    for (int64_t k = threadIdx.x; k < samples; k += 256) {
+        double C = 0.0, S = 0.0;
+        for (int r = 0; r < rings; ++r) { C += cs[(k * rings + r) * 2]; S += cs[(k * rings + r) * 2 + 1]; }
+        const double R = sqrt(C * C + S * S) * inv_n;
+        s1 += R; s2 += R * R;
+    }
+    red[0][threadIdx.x] = s1; red[1][threadIdx.x] = s2;
+    __syncthreads();
+    for (int o = 128; o > 0; o >>= 1) {
+        if (threadIdx.x < o) { red[0][threadIdx.x] += red[0][threadIdx.x + o]; red[1][threadIdx.x] += red[1][threadIdx.x + o]; }
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) { acc[0] += red[0][0]; acc[1] += red[1][0]; acc[2] += (double)samples; }
+}
+
+// net_integrate_observed of a phase model on the persistent ring kernel: ONE launch for all steps;
+// the samples at steps s_a, s_a + obs_every, ... < n_steps are taken inside it.  *handled = false:
+// this net / run does not qualify (the caller samples between launches as before).
+int32_t ring_run_observed(net* h, int64_t n_steps, double dt, int64_t obs_every, int64_t s_a, bool* handled) {
+    *handled = false;
+    RingPlan p;
+    if (!(h->method == NET_METHOD_FAST && h->fast_kind == FAST_RING_KS) || n_steps > (1 << 20)) return NET_OK;
+    if (!ring_plan(h->tv.ring_n, h->esize, &p, h->desc.batch > 1 ? 1 : 148)) return NET_OK;
+    const int64_t samples = (n_steps - s_a) / obs_every;          // steps s_a ... n_steps - obs_every
+    const int rings = p.single ? h->desc.batch : 1;
+    if ((size_t)samples * rings * 16 > RING_OBS_BYTES || getenv("OSCNET_NO_FAST_OBS")) return NET_OK;
+    int32_t rc = ring_run_plan(h, p, h->b.y, h->b.y, n_steps, dt, 0, obs_every, s_a);
+    if (rc) return rc;
+    if (samples > 0) {
+        const double* cs = (const double*)((char*)h->b.scratch + ring_work_bytes(h->n, h->esize));
+        ring_obs_accumulate_kernel<<<1, 256, 0, h->stream>>>(cs, samples, rings, 1.0 / (double)h->n, h->b.obs_acc);
+        h->launches += 1;
+        OSC_CUDA(h, cudaGetLastError());
+    }
+    *handled = true;
+    return NET_OK;
 }
 
 int32_t ring_run(net* h, const void* y_in, void* y_out, int64_t n_steps, double dt, int rhs_only) {

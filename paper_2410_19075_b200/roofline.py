@@ -113,11 +113,6 @@ def ops_per_osc_step(w):
                 "SURVEY.md 8(d) rule for KS with runs, P=2: 1 sincos + 2*(2P+12) adds + ~15 per stage")
     if w.cfg == "2":
         return ("fp64", 160, "fp64", 4 * 2 * 2 * deg, "SURVEY.md 8(d): ~160 FP64 (prefix sums)")
-    if w.cfg == "1b":
-        # the batch of rings is bound by instruction issue of ALL pipes: ncu of this build counts 275
-        # instructions per element and stage, 72 of them FP64 (profiles/r01_split_ncu.md) -- an
-        # ncu-measured executed-instruction count, named as such; SURVEY's FP64 figure is 400 per step
-        return ("issue", 4 * 275, "fp64", 4 * deg * SINE_FP64_INSTR, "ncu-measured executed instructions of all pipes (275 per element and stage)")
     return ("fp64", 400, "fp64", 4 * deg * SINE_FP64_INSTR, "SURVEY.md 8(d): ~400 FP64 (factorised)")
 
 
