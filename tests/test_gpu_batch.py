@@ -56,11 +56,23 @@ def test_replica_equals_the_ring_integrated_alone():
     for r in (0, 3):
         sl = slice(r * w.n, (r + 1) * w.n)
         inp1 = dict(y0=inp["y0"][:, sl].copy(), elem=inp["elem"][sl].copy())
-        n1 = H.make_gpu(w1, inp1, method=B.METHOD_FAST)
-        n1.integrate(50, w.dt)
-        alone = n1.get_state()
-        n1.close()
-        assert np.array_equal(got[:, r, :], alone)      # same kernel, same arithmetic: bit-identical
+        # a batch runs 128 threads per ring, a single ring 256 (measured, ring_fast.cu: ring_plan): with
+        # the same thread count the two are the same kernel and the same arithmetic -- bit-identical;
+        # with the defaults only the order of the scan differs
+        import os
+        os.environ["OSCNET_RING_NT"] = "128"
+        try:
+            n1 = H.make_gpu(w1, inp1, method=B.METHOD_FAST)
+            n1.integrate(50, w.dt)
+            alone = n1.get_state()
+            n1.close()
+        finally:
+            del os.environ["OSCNET_RING_NT"]
+        assert np.array_equal(got[:, r, :], alone)
+        n2 = H.make_gpu(w1, inp1, method=B.METHOD_FAST)
+        n2.integrate(50, w.dt)
+        assert np.abs(got[:, r, :] - n2.get_state()).max() <= 1e-12
+        n2.close()
 
 
 @pytest.mark.parametrize("cfg,kw,batch", [("5", dict(n1=10), 3), ("3b", dict(n1=9), 2), ("4", dict(n=700), 4),
