@@ -42,6 +42,7 @@ struct RingArgs {
     unsigned int* bar;       // grid barrier counter (zeroed before the launch)
     int64_t n, ld, npad;     // n: elements per ring (a batch holds several rings back to back)
     int32_t P, include_self, chunk, G, chunk_shift;
+    int32_t barrier_flags;   // 1: flag-array grid barrier, 0: shared counter
     int64_t n_steps;
     double dt;
     int32_t rhs_only;
@@ -63,12 +64,26 @@ __device__ __forceinline__ void red_release_add_u32(unsigned* p, unsigned v) {
     asm volatile("red.release.gpu.global.add.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
 }
 
-// All CTAs arrive; returns when `target` arrivals have been counted.
-__device__ __forceinline__ void grid_barrier(unsigned* bar, unsigned target) {
+__device__ __forceinline__ void st_release_u32(unsigned* p, unsigned v) {
+    asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+
+// Grid barrier over G co-resident CTAs (cooperative launch), G <= RING_THREADS.
+// Counter form (default): one red.release.add per CTA on a shared counter, thread 0 polls it.
+// Flag form (OSCNET_RING_BARRIER=flags, tried in round 2 to avoid the read-modify-write that L2
+// serialises over G arrivals): CTA b publishes the epoch in its own word flags[b] (one release
+// store); thread t < G of every CTA polls flags[t] (acquire), all G words in parallel.  Measured
+// over 128 CTAs (net_probe_latency): 5.47 us against 1.21 us for the counter -- 16 384 polling
+// threads with acquire loads cost far more than 128 serialised reds; config 2 2.3e9 against 5.7e9
+// osc-steps/s.  Kept only as the record of that measurement.
+__device__ __forceinline__ void grid_barrier(unsigned* bar, unsigned epoch, int G, int flags_form) {
     __syncthreads();
-    if (threadIdx.x == 0) {
+    if (flags_form) {
+        if (threadIdx.x == 0) st_release_u32(bar + blockIdx.x, epoch);
+        if ((int)threadIdx.x < G) while (ld_acquire_u32(bar + threadIdx.x) < epoch) {}
+    } else if (threadIdx.x == 0) {
         red_release_add_u32(bar, 1u);
-        while (ld_acquire_u32(bar) < target) {}
+        while (ld_acquire_u32(bar) < epoch * (unsigned)G) {}
     }
     __syncthreads();
 }
@@ -211,7 +226,7 @@ __global__ void __launch_bounds__(NT) ring_persistent_kernel(RingArgs a, ModelPa
         }
         // ---- B: every chunk's prefix is visible
         if (SINGLE) __syncthreads();
-        else grid_barrier(a.bar, (unsigned)((q + 1) * G));
+        else grid_barrier(a.bar, (unsigned)(q + 1), G, a.barrier_flags);
         // the chunk totals and the 4 E prefix values of this thread are requested together: both
         // are in flight during the same L2 round trip
         double c0 = 0.0, c1 = 0.0;
@@ -402,7 +417,7 @@ static int32_t ring_launch_t(net* h, RingArgs& a, const RingPlan& p) {
         OSC_CUDA(h, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, RING_THREADS, p.smem));
         if ((int64_t)occ * sms < p.G) return NET_ERR_UNSUPPORTED;
     }
-    if (!SINGLE) OSC_CUDA(h, cudaMemsetAsync(a.bar, 0, sizeof(unsigned), h->stream));
+    if (!SINGLE) OSC_CUDA(h, cudaMemsetAsync(a.bar, 0, sizeof(unsigned) * RING_GMAX, h->stream));
     void* params[] = {&a, &h->mp};
     if (SINGLE)      // one CTA per ring of the batch
         OSC_CUDA(h, cudaLaunchKernel((const void*)kern, dim3((unsigned)h->desc.batch), dim3(NT), params, p.smem, h->stream));
@@ -436,12 +451,18 @@ static int32_t ring_launch_e(net* h, RingArgs& a, const RingPlan& p) {
     }
 }
 
+static int ring_barrier_flags() {
+    const char* e = getenv("OSCNET_RING_BARRIER");
+    return e && e[0] == 'f';
+}
+
 // y_in -> y_out over n_steps RK4 steps (rhs_only: y_out = f(y_in))
 static int32_t ring_run_plan(net* h, const RingPlan& p, const void* y_in, void* y_out, int64_t n_steps, double dt, int rhs_only,
                              int64_t obs_every = 0, int64_t obs_first = 0) {
     RingArgs a;
     memset(&a, 0, sizeof(a));
     a.obs_every = obs_every; a.obs_first = obs_first;
+    a.barrier_flags = ring_barrier_flags();
     a.obs_cs = (double*)((char*)h->b.scratch + ring_work_bytes(h->n, h->esize));
     a.obs_ref = h->b.obs_ref;
     a.y_in = y_in; a.y_out = y_out; a.elem_param = h->b.elem_param;
@@ -469,8 +490,8 @@ static int32_t ring_run_plan(net* h, const RingPlan& p, const void* y_in, void* 
 // (SURVEY.md 8(d)): block scan -> grid barrier -> one L2 round trip -> scan of the totals ->
 // local field (KS: one fp64 sincos).  These kernels time exactly those primitives, as the ring
 // kernel uses them, so that bench.py can quote the stage time against a measured floor.
-__global__ void __launch_bounds__(RING_THREADS) probe_barrier_kernel(unsigned* bar, int iters, int G) {
-    for (int it = 0; it < iters; ++it) grid_barrier(bar, (unsigned)(it + 1) * (unsigned)G);
+__global__ void __launch_bounds__(RING_THREADS) probe_barrier_kernel(unsigned* bar, int iters, int G, int flags_form) {
+    for (int it = 0; it < iters; ++it) grid_barrier(bar, (unsigned)(it + 1), G, flags_form);
 }
 __global__ void probe_ring_init_kernel(unsigned* ring, unsigned n, unsigned stride) {
     for (unsigned i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) ring[i] = (i + stride) % n;
@@ -510,10 +531,10 @@ int32_t ring_probe_latency(net* h, double* out) {
     const int G = p.G;
     char* s = (char*)h->b.scratch;
     const unsigned N = 1u << 20;                                     // 4 MB ring of indices, L2 resident
-    if (h->b.scratch_bytes < (size_t)N * 4 + 1024) return set_err(h, NET_ERR_SIZE, "scratch too small for the probes");
+    if (h->b.scratch_bytes < (size_t)N * 4 + 4096) return set_err(h, NET_ERR_SIZE, "scratch too small for the probes");
     unsigned* ring = (unsigned*)s;
     unsigned* bar = (unsigned*)(s + (size_t)N * 4);
-    double* sink = (double*)(s + (size_t)N * 4 + 256);
+    double* sink = (double*)(s + (size_t)N * 4 + 2048);      // past the RING_GMAX barrier words
     cudaStream_t st = h->stream;
     cudaEvent_t e0, e1;
     OSC_CUDA(h, cudaEventCreate(&e0));
@@ -536,9 +557,9 @@ int32_t ring_probe_latency(net* h, double* out) {
     out[0] = 0.0;
     if (G > 1) {
         rc = timed([&]() -> int32_t {
-            OSC_CUDA(h, cudaMemsetAsync(bar, 0, sizeof(unsigned), st));
-            int it = iters, g = G;
-            void* params[] = {&bar, &it, &g};
+            OSC_CUDA(h, cudaMemsetAsync(bar, 0, sizeof(unsigned) * RING_GMAX, st));
+            int it = iters, g = G, ff = ring_barrier_flags();
+            void* params[] = {&bar, &it, &g, &ff};
             OSC_CUDA(h, cudaLaunchCooperativeKernel((const void*)probe_barrier_kernel, dim3(G), dim3(RING_THREADS), params, 0, st));
             return NET_OK;
         }, &out[0]);
