@@ -21,7 +21,9 @@ __global__ void __launch_bounds__(CSR_THREADS) csr_warp_stage_kernel(StageArgs a
     __shared__ int degs[CSR_ROWS];
     const int64_t n = a.n, ld = a.ld;
     const T* __restrict__ in = (const T*)a.in;
-    const T* __restrict__ gsrc = MODEL == NET_MODEL_HH ? (const T*)a.s_in : in;
+    // gathered quantity: HH the precomputed S(V_j); HHS the presynaptic gate s_j (state variable 4);
+    // KS / KSI the phase; FHN u (and v)
+    const T* __restrict__ gsrc = MODEL == NET_MODEL_HH ? (const T*)a.s_in : MODEL == NET_MODEL_HHS ? in + 4 * ld : in;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     constexpr int NW = CSR_THREADS / 32;
     const int ku = tv.k_uniform;
@@ -37,7 +39,7 @@ __global__ void __launch_bounds__(CSR_THREADS) csr_warp_stage_kernel(StageArgs a
             else { b = tv.row_ptr[i]; e = tv.row_ptr[i + 1]; }
             T s0 = 0, s1 = 0;
             T pa = 0;
-            if (MODEL == NET_MODEL_KS) pa = in[i] + T(mp.alpha);
+            if (MODEL == NET_MODEL_KS || MODEL == NET_MODEL_KSI) pa = in[i] + T(mp.alpha);
             // warp-uniform trip count; up to four independent gathers in flight per lane
 #pragma unroll 1
             for (int64_t qb = b + lane; qb - lane < e; qb += 128) {
@@ -52,7 +54,7 @@ __global__ void __launch_bounds__(CSR_THREADS) csr_warp_stage_kernel(StageArgs a
                 }
 #pragma unroll
                 for (int u = 0; u < 4; ++u) {
-                    if (MODEL == NET_MODEL_KS) s0 += j[u] >= 0 ? Math<T>::sin(g[u] - pa) : T(0);
+                    if (MODEL == NET_MODEL_KS || MODEL == NET_MODEL_KSI) s0 += j[u] >= 0 ? Math<T>::sin(g[u] - pa) : T(0);
                     else {
                         s0 += g[u];
                         if (MODEL == NET_MODEL_FHN) s1 += g2[u];
@@ -76,7 +78,7 @@ __global__ void __launch_bounds__(CSR_THREADS) csr_warp_stage_kernel(StageArgs a
             const int r = threadIdx.x;
             const int64_t i = row0 + r;
             if (i < n) {
-                constexpr int NV = MODEL == NET_MODEL_KS ? 1 : MODEL == NET_MODEL_FHN ? 2 : 4;
+                constexpr int NV = MODEL == NET_MODEL_KS ? 1 : (MODEL == NET_MODEL_FHN || MODEL == NET_MODEL_KSI) ? 2 : MODEL == NET_MODEL_HHS ? 5 : 4;
                 T xin[NV], k[NV];
 #pragma unroll
                 for (int v = 0; v < NV; ++v) xin[v] = in[v * ld + i];
@@ -85,6 +87,9 @@ __global__ void __launch_bounds__(CSR_THREADS) csr_warp_stage_kernel(StageArgs a
                 const T* ep = (const T*)a.elem_param;
                 if (MODEL == NET_MODEL_KS) {
                     k[0] = ks_rhs_direct<T>(mp, ep[i], sums[0][r], inv);
+                } else if (MODEL == NET_MODEL_KSI) {       // eq. (3) in full: psi is a local variable
+                    k[0] = xin[NV - 1];
+                    k[NV - 1] = (ks_rhs_direct<T>(mp, ep[i], sums[0][r], inv) - T(mp.damp) * xin[NV - 1]) * T(mp.inv_m);
                 } else if (MODEL == NET_MODEL_FHN) {
                     T Cu = sums[0][r] - T(deg) * xin[0];
                     T Cv = sums[NS - 1][r] - T(deg) * xin[1];
@@ -92,6 +97,8 @@ __global__ void __launch_bounds__(CSR_THREADS) csr_warp_stage_kernel(StageArgs a
                 } else {
                     hh_rhs<T>(mp, xin[0], xin[1], xin[2], xin[3], ep[i], sums[0][r], inv, &k[0],
                               &k[1], &k[2], &k[3]);
+                    if (MODEL == NET_MODEL_HHS)            // gating ODE of eq. (1), reading R18
+                        k[NV - 1] = T(mp.a_s) * hh_syn_activation<T>(mp, xin[0]) * (T(1) - xin[NV - 1]) - T(mp.b_s) * xin[NV - 1];
                 }
                 const int stage = a.stage;
                 const T dt = (T)a.dt;
@@ -119,6 +126,8 @@ static int32_t launch(net* h, const StageArgs& a) {
     switch (h->desc.model) {
         case NET_MODEL_KS: csr_warp_stage_kernel<T, NET_MODEL_KS><<<g, CSR_THREADS, 0, h->stream>>>(a, h->mp, h->tv); break;
         case NET_MODEL_FHN: csr_warp_stage_kernel<T, NET_MODEL_FHN><<<g, CSR_THREADS, 0, h->stream>>>(a, h->mp, h->tv); break;
+        case NET_MODEL_KSI: csr_warp_stage_kernel<T, NET_MODEL_KSI><<<g, CSR_THREADS, 0, h->stream>>>(a, h->mp, h->tv); break;
+        case NET_MODEL_HHS: csr_warp_stage_kernel<T, NET_MODEL_HHS><<<g, CSR_THREADS, 0, h->stream>>>(a, h->mp, h->tv); break;
         default: csr_warp_stage_kernel<T, NET_MODEL_HH><<<g, CSR_THREADS, 0, h->stream>>>(a, h->mp, h->tv); break;
     }
     h->launches += 1;

@@ -26,11 +26,14 @@ int32_t ring_run(net* h, const void* y_in, void* y_out, int64_t n_steps, double 
 
 int32_t fast_select(const net_desc* d) {
     const net_topology& t = d->topo;
-    if (d->model == NET_MODEL_FHN2 || d->model == NET_MODEL_HHS) return FAST_NONE;   // per-link DIRECT kernels
+    if (d->model == NET_MODEL_FHN2) return FAST_NONE;                  // eq. (2) with delay: per-link kernels (delay.cu)
     if (d->batch > 1 && t.kind != NET_TOPO_RING) return FAST_NONE;   // batches of lattices / graphs: block-diagonal DIRECT form
-    // KS with inertia: the persistent ring kernel (same fields as KS); DIRECT on the other topologies
+    const bool graph = t.kind == NET_TOPO_CSR || t.kind == NET_TOPO_RANDOM_INDEGREE;
+    if (d->model == NET_MODEL_HHS) return graph ? FAST_CSR_WARP : FAST_NONE;     // gate s_j gathered per link
+    // KS with inertia: the persistent ring kernel (same fields as KS), the field-split lattice kernels,
+    // warp-per-row gathers on graphs (psi is a local variable); DIRECT elsewhere
     if (d->model == NET_MODEL_KSI)
-        return ring_supported(d) ? FAST_RING_KS : lattice_v3_supported(d) ? FAST_LATTICE3D_V3 : FAST_NONE;
+        return ring_supported(d) ? FAST_RING_KS : lattice_v3_supported(d) ? FAST_LATTICE3D_V3 : graph ? FAST_CSR_WARP : FAST_NONE;
     if (t.kind == NET_TOPO_CSR || t.kind == NET_TOPO_RANDOM_INDEGREE)
         return csr_blocked_supported(d) ? FAST_CSR_BLOCKED : FAST_CSR_WARP;
     if (lattice_v3_supported(d)) return FAST_LATTICE3D_V3;

@@ -94,6 +94,8 @@ def test_hhs_gating_ode_matches_oracle(kind, dtype):
     y1 = y0.copy()
     y1[1:] = np.clip(y1[1:] * rng.uniform(0.5, 1.5, size=(4, n)), 0, 1).astype(npdt)
     net.set_state(y1.astype(npdt))
+    # graphs: warp-per-row gathers of the gate (FAST); rings and lattices: the per-link form
+    assert net.counters()[1] == (B.METHOD_FAST if kind == "graph" else B.METHOD_DIRECT)
     assert H.rel_maxnorm(net.eval_rhs(), onet.rhs(y1)) <= H.TOL_RHS[dtype]
     net.integrate(100, 0.01)
     got, ref = net.get_state().astype(np.float64), onet.rk4(y1, 100, 0.01)

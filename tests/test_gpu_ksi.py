@@ -35,9 +35,9 @@ def test_ksi_direct_matches_oracle(w):
     onet = H.make_oracle(w, inp)
     net = H.make_gpu(w, inp)
     launches, method = net.counters()
-    # rings: the persistent prefix-sum kernel; 3D balls: the field-split lattice kernels (both FAST);
-    # 2D lattices and graphs: the per-link DIRECT form
-    fast = w.topo == configs.RING or (w.topo == configs.LATTICE and len(w.extent) == 3)
+    # rings: the persistent prefix-sum kernel; 3D balls: the field-split lattice kernels; graphs:
+    # warp-per-row gathers (all FAST); 2D lattices: the per-link DIRECT form
+    fast = w.topo != configs.LATTICE or len(w.extent) == 3
     assert method == (B.METHOD_FAST if fast else B.METHOD_DIRECT)
     rp, ci = net.get_topology()
     rp0, ci0 = H.oracle_topology(w)
@@ -93,8 +93,8 @@ def test_ksi_lattice_fast_and_direct(n1, radius, dtype):
     fast.close(); direct.close()
 
 
-def test_ksi_fast_is_refused_on_graphs_and_mass_must_be_positive():
-    w = replace(configs.get("6", n1=12), topo=configs.RANDOM_INDEGREE, n=3000, extent=(), radius=0, in_degree=20)
+def test_ksi_fast_is_refused_on_2d_lattices_and_mass_must_be_positive():
+    w = replace(configs.get("6", n1=12), n=23 * 17, extent=(23, 17), radius=3)
     with pytest.raises(B.OscnetError) as ei:
         B.Net.from_workload(w, method=B.METHOD_FAST)
     assert ei.value.code == -5
