@@ -28,9 +28,11 @@ if ROOT not in sys.path:
 
 METRIC = "oscillator-steps/s"
 HEADLINE = "5"
-PER_CONFIG = ("1", "1b", "2", "3a", "3b", "4", "5", "6")   # 1b: config 1 as a batch of nets (extra, SURVEY.md 8(d) iii)
+# 1b: config 1 as a batch of nets (extra, SURVEY.md 8(d) iii); 6 / 6b / 6c: the paper's own performance model
+# (KS with inertia, Fig. 6c) at its radii P = 2 / 4 / 6 (extras)
+PER_CONFIG = ("1", "1b", "2", "3a", "3b", "4", "5", "6", "6b", "6c")
 # RK4 steps per bench step (= per net_integrate call)
-BENCH_RK4 = {"6": 10, "1": 1000, "1b": 1000, "2": 200, "3a": 10, "3b": 10, "4": 100, "5": 10}
+BENCH_RK4 = {"6": 10, "6b": 10, "6c": 10, "1": 1000, "1b": 1000, "2": 200, "3a": 10, "3b": 10, "4": 100, "5": 10}
 
 
 def ntot(w):

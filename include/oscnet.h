@@ -98,9 +98,9 @@ typedef struct {
  *   dphi_i/dt = psi_i
  *   dpsi_i/dt = ( -eps psi_i + omega_i + (K/Omega_i) sum_{j in row i} sin(phi_j - phi_i - alpha) ) / m
  * (K/Omega_i = the paper's mu; omega_i = omega0 until net_set_param_array(NET_PARAM_OMEGA), 0 in the
- * paper).  State [phi | psi].  Rings (and batches of rings) run the persistent prefix-sum kernel
- * (NET_METHOD_FAST); lattices and graphs are served by NET_METHOD_DIRECT (the per-link form of
- * Alg. 1) and return NET_ERR_UNSUPPORTED for NET_METHOD_FAST in this build. */
+ * paper).  State [phi | psi].  NET_METHOD_FAST: rings (and batches of rings) run the persistent
+ * prefix-sum kernel, 3D balls of radius 2 / 4 / 6 the field-split lattice kernels, graphs the
+ * warp-per-row gathers; 1D / 2D lattices are served by NET_METHOD_DIRECT (the per-link form of Alg. 1). */
 typedef struct {
     double K, alpha, m, eps, omega0;
 } net_ksi_params;

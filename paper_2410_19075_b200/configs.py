@@ -54,14 +54,16 @@ def get(cfg, n=None, n1=None, batch=None):
         n = n or 256
         return Workload("1", "KS ring N=%d P=64 f64" % n, KS, RING, n, "f64", 0.025, 1000, 1,
                         dict(K=1.0, alpha=math.pi / 2 - 0.05, omega0=0.0), radius=64)
-    if cfg == "6":
+    if cfg in ("6", "6b", "6c"):
         # extra, not a BASELINE.json config: the paper's own performance model (PAPER.md:327, :337-343,
         # Fig. 6c): Kuramoto-Sakaguchi with inertia on a 3D ball, m = 1, eps = 0.05, mu = 0.01,
-        # alpha = 0.45, N1 = 100, P = 2 (K = mu * Omega with Omega = 32, self link excluded, reading R4)
+        # alpha = 0.45, N1 = 100, at its three radii P = 2 / 4 / 6 (cfg 6 / 6b / 6c); K = mu * Omega with
+        # Omega = 32 / 256 / 924 links, self link excluded (reading R4)
         n1 = n1 or 100
-        return Workload("6", "KS with inertia 3D %d^3 radius 2 f64" % n1, KSI, LATTICE, n1 ** 3, "f64",
-                        0.05, 200, 10, dict(K=0.32, alpha=0.45, m=1.0, eps=0.05, omega0=0.0),
-                        extent=(n1, n1, n1), radius=2)
+        P, deg = {"6": (2, 32), "6b": (4, 256), "6c": (6, 924)}[cfg]
+        return Workload(cfg, "KS with inertia 3D %d^3 radius %d f64" % (n1, P), KSI, LATTICE, n1 ** 3, "f64",
+                        0.05, 200, 10, dict(K=0.01 * deg, alpha=0.45, m=1.0, eps=0.05, omega0=0.0),
+                        extent=(n1, n1, n1), radius=P)
     if cfg == "2":
         n = n or 65536
         R = int(math.floor(0.35 * n))          # reading R5

@@ -15,6 +15,9 @@ template <> struct L3Shape<float, 2> { static constexpr int X = 2, TY = 4; };
 template <> struct L3Shape<float, 4> { static constexpr int X = 2, TY = 2; };
 template <> struct L3Shape<double, 2> { static constexpr int X = 2, TY = 2; };
 template <> struct L3Shape<double, 4> { static constexpr int X = 2, TY = 1; };
+// radius 6 (the paper's largest): field-split kernel only (KS / KS with inertia)
+template <> struct L3Shape<float, 6> { static constexpr int X = 2, TY = 2; };
+template <> struct L3Shape<double, 6> { static constexpr int X = 2, TY = 2; };
 constexpr int L3_MAXT = 288;     // up to 8 consumer warps + the producer warp
 constexpr int L3_MINB = 1;
 // KS runs the field-split kernel (lat3s_kernel.cuh): two lanes per 2 x 2 block of outputs, the
@@ -27,7 +30,7 @@ template <class T, int MODEL, int P> struct L3Sh {
     // fp32 field-split: 7 consumer warps + producer, two CTAs per SM => 128 registers per thread
     // (fp64 at 160 threads x 3 CTAs, 128 registers: 1.10e10 against 1.08e10 on cfg 3b -- not kept)
     static constexpr int MAXT = (SPLIT && sizeof(T) == 4) ? 256 : L3_MAXT;
-    static constexpr int MINB = (SPLIT && sizeof(T) == 4) ? 2 : L3_MINB;
+    static constexpr int MINB = (SPLIT && sizeof(T) == 4 && P <= 4) ? 2 : L3_MINB;   // P = 6: 13 open planes, one CTA per SM
 };
 
 // Field-split kernel: extra columns of the staged box that make the shared-memory row pitch
@@ -101,7 +104,8 @@ static auto l3_kernel_ptr() {
     if constexpr (S::SPLIT) {
         // fp64, P = 4: rotating accumulators (small code, no spills); fp32: compile-time phases
         // measured faster (cfg 3a 2.26e10 vs 1.97e10)
-        return lat3s_kernel<T, P, STAGE, S::TY, S::MAXT, S::MINB, (P > 2 && sizeof(T) == 8)>;
+        // P = 6: rotating accumulators for both dtypes (13 copies of the plane body otherwise)
+        return lat3s_kernel<T, P, STAGE, S::TY, S::MAXT, S::MINB, (P > 4 || (P > 2 && sizeof(T) == 8))>;
     } else {
         return lat3_kernel<T, MODEL, P, STAGE, S::X, S::TY, L3_MAXT, L3_MINB, (P > 2 && sizeof(T) == 4)>;
     }
@@ -435,6 +439,13 @@ static int32_t l3_configure(net* h) {
     if (best >= 0) { h->l3_force_tx = best_c.tx; h->l3_force_sy = best_c.sy; h->l3_force_ctas = best_c.ctas; }
     else h->l3_force_tx = h->l3_force_sy = h->l3_force_ctas = 0;
     return l3_configure_tile<T, MODEL, P>(h);
+}
+
+// entry point of one (dtype, model, radius), for radii that have a translation unit of their own
+template <class T, int MODEL, int P>
+static int32_t l3_entry_p(net* h, int stage, double dt, void* rhs_out) {
+    if (h->tv.P != P) return NET_ERR_UNSUPPORTED;
+    return stage < 0 ? l3_configure<T, MODEL, P>(h) : l3_stage<T, MODEL, P>(h, stage, dt, rhs_out);
 }
 
 // entry point of one (dtype, model): configure (stage < 0) or launch

@@ -20,8 +20,9 @@ static size_t padded_pairs(const net_desc* d) {
 bool lattice_v2_supported(const net_desc* d) {
     const net_topology& t = d->topo;
     if (t.kind != NET_TOPO_LATTICE || t.ndim != 3) return false;
-    if (t.radius != 2 && t.radius != 4) return false;
     if (d->model != NET_MODEL_KS && d->model != NET_MODEL_FHN && d->model != NET_MODEL_KSI) return false;
+    // radius 2, 4: every kernel generation; radius 6 (the paper's largest): the field-split kernel (KS, KSI)
+    if (t.radius != 2 && t.radius != 4 && !(t.radius == 6 && d->model != NET_MODEL_FHN)) return false;
     // rows must be whole 16-byte vectors of the per-thread column group (X = 2 columns)
     return t.extent[0] % 2 == 0;
 }
@@ -173,9 +174,13 @@ int32_t lattice_v3_entry_f32_fhn(net* h, int stage, double dt, void* rhs_out);
 int32_t lattice_v3_entry_f32_ks(net* h, int stage, double dt, void* rhs_out);
 int32_t lattice_v3_entry_f64_fhn(net* h, int stage, double dt, void* rhs_out);
 int32_t lattice_v3_entry_f64_ks(net* h, int stage, double dt, void* rhs_out);
+int32_t lattice_v3_entry_f32_ks6(net* h, int stage, double dt, void* rhs_out);
+int32_t lattice_v3_entry_f64_ks6(net* h, int stage, double dt, void* rhs_out);
 
 static int32_t l3_dispatch(net* h, int stage, double dt, void* rhs_out) {
     const bool ks = h->desc.model == NET_MODEL_KS || h->desc.model == NET_MODEL_KSI;   // KSI: the KS kernels' RHS instance
+    if (ks && h->tv.P == 6)
+        return h->desc.dtype == NET_F32 ? lattice_v3_entry_f32_ks6(h, stage, dt, rhs_out) : lattice_v3_entry_f64_ks6(h, stage, dt, rhs_out);
     if (h->desc.dtype == NET_F32)
         return ks ? lattice_v3_entry_f32_ks(h, stage, dt, rhs_out) : lattice_v3_entry_f32_fhn(h, stage, dt, rhs_out);
     return ks ? lattice_v3_entry_f64_ks(h, stage, dt, rhs_out) : lattice_v3_entry_f64_fhn(h, stage, dt, rhs_out);

@@ -107,10 +107,12 @@ def ops_per_osc_step(w):
         return ("fp32", 220, "fp32", 4 * 2 * 2 * deg, "SURVEY.md 8(d): ~55 per stage (x-runs, P=2: 13 runs)")
     if w.cfg == "4":
         return ("fp64", 1700, "fp64", 4 * (deg * 35 + 7 * 35 + 80), "SURVEY.md 8(d): ~425 FP64 per stage (7 exp + 80 + Omega adds)")
-    if w.cfg == "6":
-        # KS with inertia, P = 2 (13 runs): 1 fp64 sincos (~15 FP64-pipe) + 2*(2P + 12) adds + ~15 per stage
-        return ("fp64", 4 * (15 + 2 * (2 * w.radius + 12) + 15), "fp64", 4 * (deg * SINE_FP64_INSTR + 40),
-                "SURVEY.md 8(d) rule for KS with runs, P=2: 1 sincos + 2*(2P+12) adds + ~15 per stage")
+    if w.cfg in ("6", "6b", "6c"):
+        # KS with inertia: 1 fp64 sincos (~15 FP64-pipe) + 2*(2P + (#runs - 1)) adds + ~15 per stage;
+        # x-runs of the ball: 13 (P = 2), 49 (P = 4), 113 (P = 6)
+        runs = {2: 13, 4: 49, 6: 113}[w.radius]
+        return ("fp64", 4 * (15 + 2 * (2 * w.radius + runs - 1) + 15), "fp64", 4 * (deg * SINE_FP64_INSTR + 40),
+                "SURVEY.md 8(d) rule for KS with runs: 1 sincos + 2*(2P + #runs - 1) adds + ~15 per stage")
     if w.cfg == "2":
         return ("fp64", 160, "fp64", 4 * 2 * 2 * deg, "SURVEY.md 8(d): ~160 FP64 (prefix sums)")
     return ("fp64", 400, "fp64", 4 * deg * SINE_FP64_INSTR, "SURVEY.md 8(d): ~400 FP64 (factorised)")

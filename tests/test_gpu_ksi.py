@@ -70,7 +70,7 @@ def test_ksi_ring_fast_and_direct_and_batches(method, batch):
 
 
 @pytest.mark.parametrize("dtype", ["f64", "f32"])
-@pytest.mark.parametrize("n1,radius", [(12, 2), (20, 4), (36, 2)])
+@pytest.mark.parametrize("n1,radius", [(12, 2), (20, 4), (36, 2), (16, 6)])
 def test_ksi_lattice_fast_and_direct(n1, radius, dtype):
     """The paper's performance model (Fig. 6c) on the field-split lattice kernels: RHS instance of the
     KS kernel + one pointwise update of (phi, psi); FAST against the oracle and against DIRECT."""

@@ -147,3 +147,22 @@ def test_lattice_tiles_give_identical_bits(cfg, tiles):
         states.append(run() if spec is None else _with_env("OSCNET_LAT3", spec, run))
     for y in states[1:]:
         assert np.array_equal(states[0], y)
+
+
+# ------------------------------------------------------------------ radius 6 (the paper's largest)
+@pytest.mark.parametrize("cfg,extent", [("3b", (16, 16, 16)), ("3a", (20, 16, 14)), ("3b", (26, 14, 18))])
+def test_ks_lattice_radius_6_on_the_field_split_kernel(cfg, extent):
+    """925 links including the centre: the field-split kernel with 13 open planes."""
+    n = extent[0] * extent[1] * extent[2]
+    w = replace(configs.get(cfg, n1=16), extent=extent, n=n, radius=6, name="KS 3D %dx%dx%d radius 6 %s" % (*extent, cfg))
+    inp = H.make_inputs(w, seed=7)
+    onet = H.make_oracle(w, inp)
+    net = H.make_gpu(w, inp, method=B.METHOD_FAST)
+    assert net.kernel_family() == 6 and net.degree()[1] == 924
+    assert H.rel_maxnorm(net.eval_rhs(), onet.rhs(inp["y0"])) <= H.TOL_RHS[w.dtype]
+    net.integrate(100, w.dt)
+    y = net.get_state()
+    assert H.traj_err(w, y, onet.rk4(inp["y0"], 100, w.dt)) <= H.TOL_TRAJ[w.dtype]
+    th = onet.phase(y.astype(np.float64))
+    np.testing.assert_allclose(net.observable(B.OBS_LOCAL_ORDER), onet.local_order(th), atol=1e-12 if w.dtype == "f64" else 2e-6)
+    net.close()
