@@ -100,3 +100,27 @@ def test_latency_probe_is_a_ring_diagnostic_and_leaves_the_state_alone():
         lat.probe_latency()
     assert ei.value.code == -5
     lat.close()
+
+
+def test_probe_peaks_and_launch_config_leave_the_state_alone():
+    """net_probe_peaks: positive, physically plausible numbers; the state,
+    the time and the results of the net are untouched.  net_get_launch_config names the kernel family."""
+    import harness as H
+    from paper_2410_19075_b200 import configs
+    w = configs.get("3b", n1=24)
+    inp = H.make_inputs(w, seed=3)
+    a, b = H.make_gpu(w, inp), H.make_gpu(w, inp)
+    a.integrate(5, w.dt)
+    b.integrate(5, w.dt)
+    pk = a.probe_peaks()
+    assert 5e3 < pk["ffma_ginstr_s"] < 6e4 and 2e3 < pk["dfma_ginstr_s"] < 3e4
+    assert 0.3 < pk["dfma_ginstr_s"] / pk["ffma_ginstr_s"] < 0.7          # FP64 at half the FP32 rate
+    assert 0.3 < pk["fadd2_ginstr_s"] / pk["ffma_ginstr_s"] < 0.7         # packed adds: half the instruction rate
+    assert 500 < pk["mufu_ginstr_s"] < 1e4 and pk["l2_gather_gops"] > 10 and pk["smem_gbs"] > 1e3
+    assert 500 < pk["sm_mhz"] < 3000
+    assert a.time() == b.time()
+    a.integrate(5, w.dt)
+    b.integrate(5, w.dt)
+    assert np.array_equal(a.get_state(), b.get_state())
+    lc = a.launch_config()
+    assert lc["family"] == a.kernel_family() == 6 and lc["tile_x"] > 0 and lc["threads"] % 32 == 0

@@ -94,3 +94,25 @@ def test_lattice_with_defects_adds_few_entries():
     assert base <= len(D) <= base + len(edited)
     a, b = cp.extract_all(V, D, C, n)
     assert np.array_equal(a, rp2) and np.array_equal(b, ci2)
+
+
+def test_round_trip_property_based():
+    """Hypothesis: for any rows (any n <= 24, any subsets), EXTRACT(COMPRESS(L)) = L, rows that are
+    circular shifts of row 0 share the empty entry, and the table never has more entries than rows."""
+    from hypothesis import given, settings, strategies as st
+
+    @settings(max_examples=150, deadline=None)
+    @given(st.integers(1, 24).flatmap(lambda n: st.tuples(st.just(n), st.lists(
+        st.sets(st.integers(0, n - 1)), min_size=n, max_size=n))))
+    def check(arg):
+        n, sets = arg
+        rows = [np.array(sorted(s), dtype=np.int64) for s in sets]
+        rp, ci = _csr(rows)
+        V, D, C = cp.compress(rp, ci)
+        assert len(D) <= n and np.array_equal(V, rows[0])
+        for i in range(n):
+            assert np.array_equal(cp.extract(i, V, D, C, n), rows[i])
+            if np.array_equal(np.sort((rows[0] + i) % n), rows[i]):
+                assert len(D[C[i]]) == 0
+
+    check()
