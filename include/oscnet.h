@@ -238,7 +238,13 @@ int32_t net_workspace_bytes(const net_desc* desc, size_t* bytes);
  * (offset tables / CSR / random graph) and zeroes the state.  `params` points to the
  * net_*_params struct of desc->model (params_bytes = its sizeof).  d_workspace: device memory,
  * 256-byte aligned, >= net_workspace_bytes; owned by the caller and must outlive the handle.
- * cuda_stream: a cudaStream_t (NULL = legacy default stream).  On failure *out is NULL. */
+ * cuda_stream: a cudaStream_t (NULL = legacy default stream).  On failure *out is NULL.
+ * Cost: 3D lattice nets of >= 2^21 elements on the tiled kernels time the ten best-scoring tiles at
+ * three pipeline depths on one RK4 step each (about 500 launches on zeroed buffers, 0.1 - 1 s) and keep
+ * the fastest; the arithmetic of every output is the same for every tile, so results do not depend on
+ * the pick (tests/test_gpu_round2.py::test_lattice_tiles_give_identical_bits).  The pick is reported
+ * by net_get_launch_config.  Environment: OSCNET_NO_AUTOTUNE = take the best-scoring tile untimed;
+ * OSCNET_LAT3 = "tile_x,strips,planes_per_chunk,depth,ctas" = that geometry. */
 int32_t net_create(const net_desc* desc, const void* params, size_t params_bytes,
                    void* d_workspace, size_t workspace_bytes, void* cuda_stream, net_t** out);
 
