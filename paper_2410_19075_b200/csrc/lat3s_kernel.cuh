@@ -198,7 +198,7 @@ lat3s_kernel(const __grid_constant__ CUtensorMap tm_st, const __grid_constant__ 
                 const int ostride = g.op_stride / (int)sizeof(T);    // scalars between operand tiles
                 const int64_t il = (int64_t)zo * nxy + (int64_t)yy * nx + x;                    // plain scalar arrays
                 const int64_t ip = (int64_t)zo * pxy + (int64_t)(yy + P) * nxp + (x + HX);     // padded planes
-                const int gys = yy < P ? ny : (yy >= ny - P ? -ny : 0);
+                [[maybe_unused]] const int gys = yy < P ? ny : (yy >= ny - P ? -ny : 0);
                 T o0[X], o1[X], o2[X], o3[X];
                 if (NT >= 1) ldg_vec<X>(ob, o0);
                 if (NT >= 2) ldg_vec<X>(ob + ostride, o1);
@@ -207,7 +207,7 @@ lat3s_kernel(const __grid_constant__ CUtensorMap tm_st, const __grid_constant__ 
                 T cx[X], cy[X];
                 ldg_vec<X>(cc, cx);
                 ldg_vec<X>(cc + splane, cy);
-                T ov[X], zv[X], cv[X], sv[X];
+                [[maybe_unused]] T ov[X], zv[X], cv[X], sv[X];
                 if constexpr (STAGE == L3_LOC) {      // local order parameter: |ball sum incl. the centre| / n_ball
 #pragma unroll
                     for (int e = 0; e < X; ++e) ov[e] = sqrt(ownv[e] * ownv[e] + other[e] * other[e]) * mp.inv_nb;
