@@ -238,6 +238,20 @@ class OracleNet:
             info["h_log"] = hl[:min(cap, info["accepted"] + info["rejected"])].copy()
         return y.reshape(self.nvar, self.n), info
 
+    def dp5_dense(self, y, t0, t_out, rtol, atol, h0, max_attempts=1000000):
+        """Adaptive DOPRI5 with dense output (ora_dp5_dense): the states at the ascending times t_out
+        (the last one is also the end of the integration).  Returns (out[n_out][nvar][n], info)."""
+        y = np.array(y, dtype=np.float64).reshape(self.nvar * self.n)
+        t_out = np.ascontiguousarray(t_out, dtype=np.float64)
+        out = np.empty((len(t_out), self.nvar * self.n))
+        st = np.zeros(5)
+        rc = lib().ora_dp5_dense(C.byref(self._s), _p(y), C.c_double(t0), C.c_int64(len(t_out)), _p(t_out),
+                                 _p(out), C.c_double(rtol), C.c_double(atol), C.c_double(h0),
+                                 C.c_int64(max_attempts), _p(st))
+        assert rc in (0, 1)
+        info = dict(accepted=int(st[0]), rejected=int(st[1]), h_last=st[2], h_next=st[3], t=st[4])
+        return out.reshape(len(t_out), self.nvar, self.n), info
+
     # ------------------------------------------------------------ observables
     def phase(self, y, phase_map=HH_PHASE_MAP):
         y = np.ascontiguousarray(y, dtype=np.float64).reshape(self.nvar * self.n)

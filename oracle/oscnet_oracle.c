@@ -781,6 +781,84 @@ int ora_dp5(const ora_net* net, double* y, double t0, double t_end, double rtol,
 }
 
 
+/* Dense output of DOPRI5 ("our approach interpolates the solution for dense output", PAPER.md:416;
+ * SURVEY.md 8(f).2 "dense output optional").  The continuous extension of the paper's reference [22]
+ * (Hairer, Norsett, Wanner, code DOPRI5, routine CONTD5): after an accepted step from (t, y) to
+ * (t + h, y5) with stages k1..k7, for theta = (t_out - t)/h in (0, 1]:
+ *   r1 = y, r2 = y5 - y, r3 = h k1 - r2, r4 = r2 - h k7 - r3,
+ *   r5 = h (d1 k1 + d3 k3 + d4 k4 + d5 k5 + d6 k6 + d7 k7),
+ *   y(t + theta h) = r1 + theta (r2 + (1 - theta)(r3 + theta (r4 + (1 - theta) r5)))
+ * (fourth-order accurate; equals y at theta = 0 and y5 at theta = 1).  The step control is that of
+ * ora_dp5, the steps are NOT shortened to hit the output times (only t_out[n_out-1] = t_end is hit).
+ * t_out ascending, t0 < t_out[0]; out = n_out states of nvar*n.  stats as ora_dp5's out. */
+static const double DP_D[7] = {-12715105075.0 / 11282082432.0, 0.0, 87487479700.0 / 32700410799.0,
+                               -10690763975.0 / 1880347072.0, 701980252875.0 / 199316789632.0,
+                               -1453857185.0 / 822651844.0, 69997945.0 / 29380423.0};
+
+int ora_dp5_dense(const ora_net* net, double* y, double t0, int64_t n_out, const double* t_out, double* out,
+                  double rtol, double atol, double h0, int64_t max_attempts, double* stats) {
+    int32_t nv = ora_nvar(net->model);
+    if (nv < 0 || !(h0 > 0.0) || n_out < 1 || !(t_out[0] > t0)) return -1;
+    for (int64_t q = 1; q < n_out; ++q) if (!(t_out[q] > t_out[q - 1])) return -1;
+    const double t_end = t_out[n_out - 1];
+    const int64_t len = (int64_t)nv * net->n;
+    double* buf = (double*)malloc(sizeof(double) * (size_t)len * 10);
+    if (!buf) return -2;
+    double* k[7];
+    for (int j = 0; j < 7; ++j) k[j] = buf + j * len;
+    double *y5 = buf + 7 * len, *e = buf + 8 * len, *tmp = buf + 9 * len;
+    double t = t0, h = h0, h_used = 0.0;
+    int64_t acc_n = 0, rej_n = 0, att = 0, next = 0;
+    int after_reject = 0, rc = 0;
+    ora_rhs(net, y, k[0]);
+    while (t < t_end) {
+        if (att >= max_attempts) { rc = 1; break; }
+        int last = 0;
+        if (t + 1.01 * h >= t_end) { h = t_end - t; last = 1; }
+        dp5_stages(net, y, h, k, y5, e, tmp);
+        double s2 = 0.0;
+        for (int64_t q = 0; q < len; ++q) {
+            double sc = atol + rtol * fmax(fabs(y[q]), fabs(y5[q]));
+            double r = e[q] / sc;
+            s2 += r * r;
+        }
+        const double err = sqrt(s2 / (double)len);
+        const double facmax = after_reject ? 1.0 : 10.0;
+        double fac = err > 0.0 ? 0.9 * pow(err, -0.2) : facmax;
+        fac = fmin(facmax, fmax(0.2, fac));
+        ++att;
+        if (err <= 1.0) {
+            const double t_new = last ? t_end : t + h;
+            while (next < n_out && t_out[next] <= t_new) {       /* output times inside this step */
+                const double th = last && next == n_out - 1 ? 1.0 : (t_out[next] - t) / h, th1 = 1.0 - th;
+                double* o = out + next * len;
+                for (int64_t q = 0; q < len; ++q) {
+                    const double r2 = y5[q] - y[q], r3 = h * k[0][q] - r2, r4 = r2 - h * k[6][q] - r3;
+                    double r5 = 0.0;
+                    for (int j = 0; j < 7; ++j) r5 += DP_D[j] * k[j][q];
+                    r5 *= h;
+                    o[q] = y[q] + th * (r2 + th1 * (r3 + th * (r4 + th1 * r5)));
+                }
+                ++next;
+            }
+            t = t_new;
+            h_used = h;
+            memcpy(y, y5, sizeof(double) * (size_t)len);
+            double* sw = k[0]; k[0] = k[6]; k[6] = sw;
+            ++acc_n;
+            after_reject = 0;
+        } else {
+            ++rej_n;
+            after_reject = 1;
+        }
+        h *= fac;
+    }
+    stats[0] = (double)acc_n; stats[1] = (double)rej_n; stats[2] = h_used; stats[3] = h; stats[4] = t;
+    free(buf);
+    return rc;
+}
+
+
 /* ------------------------------------------------------------------ */
 /* Eq. (2) with delay tau and noise D n(t) under fixed-step RK4        */
 /* (reading R17).  The paper's own solvers keep       */

@@ -146,3 +146,55 @@ def test_global_error_scales_with_the_tolerance():
         errs.append(np.abs(y - ref).max())
     assert errs[0] > errs[1] > errs[2] and errs[2] < 1e-5
     assert errs[0] / errs[2] > 1e2
+
+
+# ------------------------------------------------------------------ dense output
+def test_dense_output_end_points_and_step_sequence():
+    """theta = 1 gives the step's own solution, so the last output equals ora_dp5's state and the
+    step statistics are those of the run without outputs (the outputs do not steer the steps)."""
+    n = 8
+    rp, ci = ora.topology_ring(n, 2)
+    rng = np.random.default_rng(5)
+    net = ora.OracleNet.ks(n, rp, ci, 1.0, 0.3, rng.normal(size=n))
+    y0 = rng.uniform(-3, 3, size=(1, n))
+    ref, rinfo = net.dp5(y0, 0.0, 4.0, 1e-7, 1e-10, 0.05)
+    t_out = np.array([0.3, 0.31, 1.7, 2.0, 3.999, 4.0])
+    out, info = net.dp5_dense(y0, 0.0, t_out, 1e-7, 1e-10, 0.05)
+    assert (info["accepted"], info["rejected"]) == (rinfo["accepted"], rinfo["rejected"])
+    assert np.array_equal(out[-1], ref)
+    # every output is close to the solution at its own time (RK4 with a tiny step as the reference)
+    for q, t in enumerate(t_out):
+        fine = net.rk4(y0, int(round(t / 1e-4)), 1e-4)
+        assert np.abs(out[q] - fine).max() < 5e-7, (t, np.abs(out[q] - fine).max())
+
+
+def test_dense_output_is_the_contd5_polynomial_and_fourth_order():
+    """One uncontrolled-size step on a linear problem (y' = lam y through the psi row of an uncoupled
+    KSI net): the interpolant equals CONTD5 written out here with the published d coefficients, is
+    exact at both ends, and its error against exp(lam t) inside the step falls by ~2^5 per halving."""
+    net, lam = _ksi_uncoupled()
+    y = np.array([[0.0, 0.0, 0.0], [1.0, -2.0, 0.5]])
+    d = [-12715105075 / 11282082432, 0.0, 87487479700 / 32700410799, -10690763975 / 1880347072,
+         701980252875 / 199316789632, -1453857185 / 822651844, 69997945 / 29380423]
+    A = [[], [1 / 5], [3 / 40, 9 / 40], [44 / 45, -56 / 15, 32 / 9],
+         [19372 / 6561, -25360 / 2187, 64448 / 6561, -212 / 729],
+         [9017 / 3168, -355 / 33, 46732 / 5247, 49 / 176, -5103 / 18656],
+         [35 / 384, 0.0, 500 / 1113, 125 / 192, -2187 / 6784, 11 / 84]]
+    errs = []
+    for h in (0.8, 0.4):
+        # rtol huge: the first step of size h is accepted whatever its error; outputs inside it
+        ths = np.array([0.25, 0.5, 0.9, 1.0])
+        out, info = net.dp5_dense(y, 0.0, ths * h, 1e30, 1e30, h)
+        assert info["accepted"] == 1
+        ks = []
+        for s in range(7):
+            ks.append(lam * (1 + h * sum(A[s][j] * ks[j] for j in range(s))))
+        y5 = 1 + h * sum(A[6][j] * ks[j] for j in range(6))
+        r2 = y5 - 1; r3 = h * ks[0] - r2; r4 = r2 - h * ks[6] - r3
+        r5 = h * sum(d[j] * ks[j] for j in range(7))
+        for q, th in enumerate(ths):
+            poly = 1 + th * (r2 + (1 - th) * (r3 + th * (r4 + (1 - th) * r5)))
+            np.testing.assert_allclose(out[q][1], poly * y[1], rtol=1e-13)
+        np.testing.assert_allclose(out[-1][1], y5 * y[1], rtol=1e-15)
+        errs.append(abs(out[1][1][0] - math.exp(lam * 0.5 * h)))
+    assert 20 <= errs[0] / errs[1] <= 45, errs
