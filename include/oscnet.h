@@ -297,10 +297,22 @@ int32_t net_integrate_observed(net_t* net, int64_t n_steps, double dt, int64_t o
  * time reached}.  The error norm, the decision and the next step are computed on the device; the
  * host reads the control block once per 8 attempts.  Synchronises the stream.  Returns
  * NET_ERR_INVALID (state and time as reached) when max_attempts is exhausted before t_end.
- * No dense output: call once per output time. */
+ * Dense output: net_integrate_adaptive_dense below. */
 int32_t net_adaptive_workspace_bytes(net_t* net, size_t* bytes);
 int32_t net_integrate_adaptive(net_t* net, double t_end, double rtol, double atol, double h0,
                                int64_t max_attempts, void* d_work, size_t work_bytes, double* out5);
+
+/* net_integrate_adaptive with dense output ("the integrator outputs ... values of dynamical variables
+ * at specified time moments"; "our approach interpolates the solution for dense output",
+ * PAPER.md:416): the states at the strictly ascending HOST times t_out[0 .. n_out), t_out[0] > the
+ * net's time, are written to d_out [n_out][nvar][n] (DEVICE, dtype of the net); the run ends at
+ * t_out[n_out - 1].  Interpolant: the continuous extension of DOPRI5 (routine CONTD5 of the paper's
+ * reference [22]; fourth order, exact at both ends of a step), evaluated on the device right after
+ * each accepted step.  The output times never shorten a step: the step sequence is that of
+ * net_integrate_adaptive.  d_work: at least net_adaptive_workspace_bytes + 8 n_out rounded up to 256. */
+int32_t net_integrate_adaptive_dense(net_t* net, int64_t n_out, const double* t_out, void* d_out,
+                                     double rtol, double atol, double h0, int64_t max_attempts,
+                                     void* d_work, size_t work_bytes, double* out5);
 
 /* One right-hand-side evaluation f(y) at the current state, [nvar][n] in the dtype of the net:
  * the paper's Calculate(t, y, der) of Alg. 1 for all elements at once

@@ -30,7 +30,7 @@ ABI_SYMBOLS = [
     "net_set_time", "net_get_counters", "net_get_kernel_family", "net_synchronize", "net_last_error", "net_version",
     "net_probe_latency", "net_probe_peaks", "net_get_launch_config",
     "net_adaptive_workspace_bytes", "net_integrate_adaptive",
-    "net_compress_csr", "net_compressed_free",
+    "net_compress_csr", "net_compressed_free", "net_integrate_adaptive_dense",
 ]
 
 
@@ -130,6 +130,8 @@ def lib():
         L.net_adaptive_workspace_bytes.argtypes = [C.c_void_p, C.POINTER(C.c_size_t)]
         L.net_integrate_adaptive.argtypes = [C.c_void_p, C.c_double, C.c_double, C.c_double, C.c_double,
                                              C.c_int64, C.c_void_p, C.c_size_t, C.POINTER(C.c_double)]
+        L.net_integrate_adaptive_dense.argtypes = [C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p, C.c_double, C.c_double,
+                                                   C.c_double, C.c_int64, C.c_void_p, C.c_size_t, C.POINTER(C.c_double)]
         L.net_compress_csr.argtypes = [C.c_int64, C.c_void_p, C.c_void_p, C.POINTER(C.POINTER(Compressed))]
         L.net_compressed_free.argtypes = [C.POINTER(Compressed)]
         for name in ABI_SYMBOLS:
@@ -466,6 +468,27 @@ class Net:
         base = (self._adaptive_work.data_ptr() + 255) // 256 * 256
         return net_integrate_adaptive(self.h, float(t_end), float(rtol), float(atol), float(h0),
                                       int(max_attempts), base, need)
+
+    def integrate_adaptive_dense(self, t_out, rtol, atol, h0, max_attempts=1000000):
+        """Dormand-Prince 5(4) to t_out[-1] with dense output at the ascending times t_out; returns
+        (states [n_out][nvar][n] as a numpy array, step statistics)."""
+        torch = self.torch
+        t_out = np.ascontiguousarray(t_out, dtype=np.float64)
+        need = net_adaptive_workspace_bytes(self.h) + (8 * len(t_out) + 255) // 256 * 256
+        with torch.cuda.device(self.device):
+            work = torch.empty(need + 256, dtype=torch.uint8, device=self.device)
+            out = torch.empty((len(t_out), self.nvar, self.n), dtype=self.torch_dtype, device=self.device)
+        work.record_stream(self.stream)
+        out.record_stream(self.stream)
+        self.stream.wait_stream(torch.cuda.current_stream())
+        base = (work.data_ptr() + 255) // 256 * 256
+        st = (C.c_double * 5)()
+        rc = lib().net_integrate_adaptive_dense(self.h, len(t_out), t_out.ctypes.data, out.data_ptr(), float(rtol),
+                                                float(atol), float(h0), int(max_attempts), base, need, st)
+        _check(rc, self.h)
+        torch.cuda.current_stream().wait_stream(self.stream)
+        info = dict(accepted=int(st[0]), rejected=int(st[1]), h_last=st[2], h_next=st[3], t=st[4])
+        return out.cpu().numpy(), info
 
     def integrate_observed(self, n_steps, dt, obs_every):
         net_integrate_observed(self.h, int(n_steps), float(dt), int(obs_every))

@@ -25,8 +25,8 @@ constexpr int DP5_THREADS = 256;
 constexpr int DP5_MAXBLOCKS = 1184;
 
 struct Dp5Ctrl {
-    double t, h, t_end, rtol, atol, err, h_used;
-    long long accepted, rejected, attempts, max_attempts;
+    double t, h, t_end, rtol, atol, err, h_used, t_prev;
+    long long accepted, rejected, attempts, max_attempts, next_out;
     int done, after_reject, last, accept;
     unsigned ticket;
     int pad_;
@@ -40,6 +40,10 @@ __constant__ double DP5_A[7][6] = {
     {19372.0 / 6561.0, -25360.0 / 2187.0, 64448.0 / 6561.0, -212.0 / 729.0, 0, 0},
     {9017.0 / 3168.0, -355.0 / 33.0, 46732.0 / 5247.0, 49.0 / 176.0, -5103.0 / 18656.0, 0},
     {35.0 / 384.0, 0.0, 500.0 / 1113.0, 125.0 / 192.0, -2187.0 / 6784.0, 11.0 / 84.0}};
+// continuous extension CONTD5 of the paper's reference [22] (dense output)
+__constant__ double DP5_D[7] = {-12715105075.0 / 11282082432.0, 0.0, 87487479700.0 / 32700410799.0,
+                                -10690763975.0 / 1880347072.0, 701980252875.0 / 199316789632.0,
+                                -1453857185.0 / 822651844.0, 69997945.0 / 29380423.0};
 __constant__ double DP5_E[7] = {71.0 / 57600.0, 0.0, -71.0 / 16695.0, 71.0 / 1920.0,
                                 -17253.0 / 339200.0, 22.0 / 525.0, -1.0 / 40.0};
 
@@ -123,6 +127,7 @@ __global__ void __launch_bounds__(DP5_THREADS) dp5_error_kernel(Dp5Ctrl* c, Dp5V
         c->attempts += 1;
         if (err <= 1.0) {           // (a NaN error is a rejection with the smallest factor)
             c->accept = 1;
+            c->t_prev = c->t;
             c->t = c->last ? c->t_end : c->t + c->h;
             c->h_used = c->h;
             c->accepted += 1;
@@ -134,6 +139,32 @@ __global__ void __launch_bounds__(DP5_THREADS) dp5_error_kernel(Dp5Ctrl* c, Dp5V
             if (!(err == err)) fac = 0.2;
         }
         c->h *= fac;
+    }
+}
+
+// Dense output (runs between the decision and the commit of an accepted step): every requested time
+// in (t_prev, t] gets the CONTD5 interpolant
+//   y(t_prev + theta h) = r1 + theta (r2 + (1 - theta)(r3 + theta (r4 + (1 - theta) r5))),
+//   r1 = y, r2 = y5 - y, r3 = h k1 - r2, r4 = r2 - h k7 - r3, r5 = h sum_j d_j k_j.
+// All blocks walk the same list of pending times (read-only here); dp5_end_kernel advances next_out.
+template <class T>
+__global__ void __launch_bounds__(DP5_THREADS) dp5_dense_kernel(const Dp5Ctrl* c, Dp5Vecs v, int64_t len,
+                                                                const double* __restrict__ t_out, long long n_out, T* out) {
+    if (c->done || !c->accept) return;
+    const double h = c->h_used, t0 = c->t_prev, t1 = c->t;
+    for (long long o = c->next_out; o < n_out && t_out[o] <= t1; ++o) {
+        const double th = (c->last && o == n_out - 1) ? 1.0 : (t_out[o] - t0) / h, th1 = 1.0 - th;
+        T* dst = out + o * len;
+        for (int64_t q = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; q < len; q += (int64_t)gridDim.x * blockDim.x) {
+            const double y = (double)((const T*)v.y)[q], y5 = (double)((const T*)v.y5)[q];
+            const double k1 = (double)((const T*)v.k[0])[q], k7 = (double)((const T*)v.k[6])[q];
+            const double r2 = y5 - y, r3 = h * k1 - r2, r4 = r2 - h * k7 - r3;
+            double r5 = 0.0;
+#pragma unroll
+            for (int j = 0; j < 7; ++j) r5 += DP5_D[j] * (double)((const T*)v.k[j])[q];
+            r5 *= h;
+            dst[q] = (T)(y + th * (r2 + th1 * (r3 + th * (r4 + th1 * r5))));
+        }
     }
 }
 
@@ -154,9 +185,14 @@ __global__ void __launch_bounds__(DP5_THREADS) dp5_commit_kernel(Dp5Ctrl* c, Dp5
 }
 
 // after every block of the commit kernel has run (next kernel on the stream)
-__global__ void dp5_end_kernel(Dp5Ctrl* c) {
+__global__ void dp5_end_kernel(Dp5Ctrl* c, const double* __restrict__ t_out, long long n_out) {
     if (c->done) return;
-    if (c->accept && !(c->t < c->t_end)) c->done = 1;
+    if (c->accept) {
+        long long o = c->next_out;
+        while (o < n_out && t_out[o] <= c->t) ++o;      // the outputs dp5_dense_kernel has just written
+        c->next_out = o;
+        if (!(c->t < c->t_end)) c->done = 1;
+    }
     c->accept = 0;
 }
 
@@ -168,9 +204,10 @@ size_t adaptive_workspace_bytes(const net* h) {
     return 10 * dp5_vec_bytes(h) + 256 + sizeof(double) * DP5_MAXBLOCKS + 256;
 }
 
+// t_out (device, ascending, n_out >= 0 entries, the last one = t_end) / d_out: dense output, or null
 template <class T>
 static int32_t dp5_run(net* h, double t_end, double rtol, double atol, double h0, int64_t max_attempts,
-                       char* work, double* out5) {
+                       char* work, double* out5, const double* d_t_out, long long n_out, void* d_out) {
     const size_t vb = dp5_vec_bytes(h);
     Dp5Vecs v;
     v.y = work; v.y5 = work + vb; v.tmp = work + 2 * vb;
@@ -196,9 +233,10 @@ static int32_t dp5_run(net* h, double t_end, double rtol, double atol, double h0
                 if ((rc = rhs_at(h, s == 6 ? v.y5 : v.tmp, v.k[s]))) return rc;
             }
             dp5_error_kernel<T><<<grid, DP5_THREADS, 0, st>>>(d_c, v, len, partial);
+            if (n_out > 0) dp5_dense_kernel<T><<<grid, DP5_THREADS, 0, st>>>(d_c, v, len, d_t_out, n_out, (T*)d_out);
             dp5_commit_kernel<T><<<grid, DP5_THREADS, 0, st>>>(d_c, v, len);
-            dp5_end_kernel<<<1, 1, 0, st>>>(d_c);
-            h->launches += 10;
+            dp5_end_kernel<<<1, 1, 0, st>>>(d_c, d_t_out, n_out);
+            h->launches += n_out > 0 ? 11 : 10;
         }
         OSC_CUDA(h, cudaGetLastError());
         OSC_CUDA(h, cudaMemcpyAsync(&c, d_c, sizeof(c), cudaMemcpyDeviceToHost, st));
@@ -220,8 +258,30 @@ int32_t adaptive_integrate(net* h, double t_end, double rtol, double atol, doubl
     if (!d_work || ((uintptr_t)d_work & 255) != 0 || work_bytes < adaptive_workspace_bytes(h))
         return set_err(h, NET_ERR_SIZE, "net_integrate_adaptive: work buffer missing, misaligned or smaller than net_adaptive_workspace_bytes");
     if (t_end == h->t) { out5[0] = out5[1] = out5[2] = 0.0; out5[3] = h0; out5[4] = h->t; return NET_OK; }
-    return h->desc.dtype == NET_F32 ? dp5_run<float>(h, t_end, rtol, atol, h0, max_attempts, (char*)d_work, out5)
-                                    : dp5_run<double>(h, t_end, rtol, atol, h0, max_attempts, (char*)d_work, out5);
+    return h->desc.dtype == NET_F32 ? dp5_run<float>(h, t_end, rtol, atol, h0, max_attempts, (char*)d_work, out5, nullptr, 0, nullptr)
+                                    : dp5_run<double>(h, t_end, rtol, atol, h0, max_attempts, (char*)d_work, out5, nullptr, 0, nullptr);
+}
+
+// Dense output: the states at the ascending host times t_out[0 .. n_out) (the last one ends the run)
+// go to d_out [n_out][nvar][n] (device, dtype of the net).  The times travel to the tail of the work
+// buffer; the steps are those of adaptive_integrate (outputs never shorten a step).
+int32_t adaptive_integrate_dense(net* h, int64_t n_out, const double* t_out, void* d_out, double rtol, double atol, double h0,
+                                 int64_t max_attempts, void* d_work, size_t work_bytes, double* out5) {
+    if (n_out < 1 || !t_out || !d_out) return set_err(h, NET_ERR_INVALID, "net_integrate_adaptive_dense: need n_out >= 1, t_out and d_out");
+    if (!(t_out[0] > h->t)) return set_err(h, NET_ERR_INVALID, "net_integrate_adaptive_dense: t_out[0] must lie after the net's time");
+    for (int64_t q = 1; q < n_out; ++q)
+        if (!(t_out[q] > t_out[q - 1])) return set_err(h, NET_ERR_INVALID, "net_integrate_adaptive_dense: t_out must ascend strictly");
+    if (!(h0 > 0.0) || !(rtol >= 0.0) || !(atol >= 0.0) || !(rtol + atol > 0.0) || max_attempts < 1)
+        return set_err(h, NET_ERR_INVALID, "net_integrate_adaptive_dense: need h0 > 0, rtol, atol >= 0 (not both 0), max_attempts >= 1");
+    const size_t need = adaptive_workspace_bytes(h) + (size_t)round_up(n_out * (int64_t)sizeof(double), 256);
+    if (!d_work || ((uintptr_t)d_work & 255) != 0 || work_bytes < need)
+        return set_err(h, NET_ERR_SIZE, "net_integrate_adaptive_dense: work buffer missing, misaligned or smaller than net_adaptive_workspace_bytes + 8 n_out (rounded up to 256)");
+    double* d_t = (double*)((char*)d_work + adaptive_workspace_bytes(h));
+    OSC_CUDA(h, cudaMemcpyAsync(d_t, t_out, sizeof(double) * n_out, cudaMemcpyHostToDevice, h->stream));
+    OSC_CUDA(h, cudaStreamSynchronize(h->stream));     // t_out is the caller's (pageable) memory
+    const double t_end = t_out[n_out - 1];
+    return h->desc.dtype == NET_F32 ? dp5_run<float>(h, t_end, rtol, atol, h0, max_attempts, (char*)d_work, out5, d_t, n_out, d_out)
+                                    : dp5_run<double>(h, t_end, rtol, atol, h0, max_attempts, (char*)d_work, out5, d_t, n_out, d_out);
 }
 
 }  // namespace oscnet

@@ -573,6 +573,15 @@ int32_t net_integrate_adaptive(net_t* h, double t_end, double rtol, double atol,
     return adaptive_integrate(h, t_end, rtol, atol, h0, max_attempts, d_work, work_bytes, out5);
 }
 
+int32_t net_integrate_adaptive_dense(net_t* h, int64_t n_out, const double* t_out, void* d_out, double rtol, double atol,
+                                     double h0, int64_t max_attempts, void* d_work, size_t work_bytes, double* out5) {
+    DevGuard guard_(h);
+    if (!h || !out5) return set_err(h, NET_ERR_INVALID, "net or out5 is NULL");
+    if (h->desc.model == NET_MODEL_FHN2 && (h->desc.delay_steps > 0 || h->mp.noise_D != 0.0))
+        return set_err(h, NET_ERR_UNSUPPORTED, "net_integrate_adaptive_dense: eq. (2) with delay or noise runs under the fixed-step integrator only");
+    return adaptive_integrate_dense(h, n_out, t_out, d_out, rtol, atol, h0, max_attempts, d_work, work_bytes, out5);
+}
+
 int32_t net_eval_rhs(net_t* h, void* dst, int32_t dst_is_device) {
     DevGuard guard_(h);
     if (!h) return NET_ERR_INVALID;

@@ -273,6 +273,8 @@ int32_t delay_reset_history(net* h);
 size_t adaptive_workspace_bytes(const net* h);
 int32_t adaptive_integrate(net* h, double t_end, double rtol, double atol, double h0, int64_t max_attempts,
                            void* d_work, size_t work_bytes, double* out5);
+int32_t adaptive_integrate_dense(net* h, int64_t n_out, const double* t_out, void* d_out, double rtol, double atol, double h0,
+                                 int64_t max_attempts, void* d_work, size_t work_bytes, double* out5);
 int32_t state_to_external(net* h, void* d_dst);
 int32_t state_from_external(net* h, const void* d_src);
 int32_t rhs_at(net* h, const void* d_x, void* d_k);

@@ -71,3 +71,35 @@ def test_dp5_f32_and_errors():
     with pytest.raises(B.OscnetError) as ei:
         net.integrate_adaptive(50.0, 1e-10, 1e-12, 1e-6, max_attempts=5)
     assert "max_attempts" in str(ei.value)
+
+
+@pytest.mark.parametrize("name,w,method", [("cfg 1 ring", configs.get("1"), 0), ("cfg 3b lattice 16^3", configs.get("3b", n1=16), 0),
+                                           ("cfg 4 graph N=5000", configs.get("4", n=5000), 0),
+                                           ("cfg 5 lattice 24^3 f32", configs.get("5", n1=24), 0)],
+                         ids=["ring", "lattice", "graph", "lattice_f32"])
+def test_dp5_dense_output_matches_oracle(name, w, method):
+    """Dense output (CONTD5 interpolant evaluated on the device after each accepted step) at output
+    times that fall inside steps, several in one step, and on the end point; the step sequence is the
+    one of the run without outputs."""
+    inp = H.make_inputs(w, seed=3)
+    T = 2.0 if w.dtype == "f64" else 0.4
+    t_out = np.array([0.013, 0.0131, 0.25, 0.5, 0.77, 0.9999, 1.0]) * T
+    rtol, atol = (1e-6, 1e-9) if w.dtype == "f64" else (1e-4, 1e-6)
+    ref, rinfo = H.make_oracle(w, inp).dp5_dense(inp["y0"], 0.0, t_out, rtol, atol, 0.01)
+    net = H.make_gpu(w, inp, method)
+    out, info = net.integrate_adaptive_dense(t_out, rtol, atol, 0.01)
+    if w.dtype == "f64":
+        assert (info["accepted"], info["rejected"]) == (rinfo["accepted"], rinfo["rejected"])
+        for q in range(len(t_out)):
+            assert H.traj_err(w, out[q], ref[q]) <= H.TOL_TRAJ["f64"], q
+        # theta = 1: y + (y5 - y), the state itself up to one rounding
+        np.testing.assert_allclose(out[-1], net.get_state(), rtol=1e-14, atol=1e-13)
+    else:
+        assert abs(info["accepted"] - rinfo["accepted"]) <= 1
+        assert np.abs(out.astype(np.float64) - ref).max() <= 1e-3
+    assert net.time()[0] == t_out[-1]
+    with pytest.raises(B.OscnetError):
+        net.integrate_adaptive_dense(np.array([t_out[-1] + 1.0, t_out[-1] + 0.5]), rtol, atol, 0.01)   # not ascending
+    with pytest.raises(B.OscnetError):
+        net.integrate_adaptive_dense(np.array([t_out[-1]]), rtol, atol, 0.01)                           # not after the net's time
+    net.close()
