@@ -17,10 +17,14 @@
 
 namespace {
 
-struct Owned {
-    net_compressed pub;                // first member: the pointer handed out
+struct Storage {
     std::vector<int32_t> v, dpos, c;
     std::vector<int64_t> dptr;
+};
+// standard-layout: a pointer to `pub` (what the caller holds) is a pointer to the Owned
+struct Owned {
+    net_compressed pub;
+    Storage* st;
 };
 
 uint64_t hash_positions(const std::vector<int32_t>& d) {
@@ -40,8 +44,11 @@ int32_t net_compress_csr(int64_t n, const int64_t* row_ptr, const int32_t* col_i
     *out = nullptr;
     if (n < 1 || n > 2147483647LL || !row_ptr || (row_ptr[n] > 0 && !col_idx))
         return set_err(nullptr, NET_ERR_INVALID, "net_compress_csr: bad n or NULL arrays");
-    Owned* o = new (std::nothrow) Owned;
-    if (!o) return set_err(nullptr, NET_ERR_INVALID, "out of host memory");
+    Owned* owned = new (std::nothrow) Owned;
+    Storage* o = new (std::nothrow) Storage;
+    if (!owned || !o) { delete owned; delete o; return set_err(nullptr, NET_ERR_INVALID, "out of host memory"); }
+    owned->st = o;
+    auto drop = [&]() { delete o; delete owned; };
     try {
         std::vector<int32_t> shifted, d;
         auto rol = [&](int64_t i) {              // ROL(L_i, i) as a sorted position list
@@ -57,15 +64,15 @@ int32_t net_compress_csr(int64_t n, const int64_t* row_ptr, const int32_t* col_i
             shifted.erase(std::unique(shifted.begin(), shifted.end()), shifted.end());
             return true;
         };
-        if (row_ptr[0] != 0) { delete o; return set_err(nullptr, NET_ERR_TOPOLOGY, "net_compress_csr: row_ptr[0] != 0"); }
-        if (!rol(0)) { delete o; return set_err(nullptr, NET_ERR_TOPOLOGY, "net_compress_csr: index outside [0, n)"); }
+        if (row_ptr[0] != 0) { drop(); return set_err(nullptr, NET_ERR_TOPOLOGY, "net_compress_csr: row_ptr[0] != 0"); }
+        if (!rol(0)) { drop(); return set_err(nullptr, NET_ERR_TOPOLOGY, "net_compress_csr: index outside [0, n)"); }
         o->v = shifted;                          // V <- L_0
         o->c.resize((size_t)n);
         o->dptr.push_back(0);
         std::unordered_multimap<uint64_t, int32_t> index;
         for (int64_t i = 0; i < n; ++i) {
-            if (row_ptr[i + 1] < row_ptr[i]) { delete o; return set_err(nullptr, NET_ERR_TOPOLOGY, "net_compress_csr: row_ptr not monotone"); }
-            if (!rol(i)) { delete o; return set_err(nullptr, NET_ERR_TOPOLOGY, "net_compress_csr: index outside [0, n)"); }
+            if (row_ptr[i + 1] < row_ptr[i]) { drop(); return set_err(nullptr, NET_ERR_TOPOLOGY, "net_compress_csr: row_ptr not monotone"); }
+            if (!rol(i)) { drop(); return set_err(nullptr, NET_ERR_TOPOLOGY, "net_compress_csr: index outside [0, n)"); }
             d.clear();                           // d = XOR(ROL(L_i, i), V)
             std::set_symmetric_difference(shifted.begin(), shifted.end(), o->v.begin(), o->v.end(), std::back_inserter(d));
             const uint64_t key = hash_positions(d);
@@ -84,23 +91,29 @@ int32_t net_compress_csr(int64_t n, const int64_t* row_ptr, const int32_t* col_i
             o->c[(size_t)i] = found;
         }
     } catch (...) {
-        delete o;
+        drop();
         return set_err(nullptr, NET_ERR_INVALID, "net_compress_csr: out of host memory");
     }
     if (o->dpos.empty()) o->dpos.push_back(0);   // keep data() non-null
-    if (o->v.empty()) o->v.push_back(0), o->pub.v_len = 0; else o->pub.v_len = (int64_t)o->v.size();
-    o->pub.n = n;
-    o->pub.v_pos = o->v.data();
-    o->pub.k = (int64_t)o->dptr.size() - 1;
-    o->pub.d_ptr = o->dptr.data();
-    o->pub.d_pos = o->dpos.data();
-    o->pub.c = o->c.data();
-    *out = &o->pub;
+    net_compressed& pub = owned->pub;
+    pub.v_len = (int64_t)o->v.size();
+    if (o->v.empty()) o->v.push_back(0);         // keep data() non-null
+    pub.n = n;
+    pub.v_pos = o->v.data();
+    pub.k = (int64_t)o->dptr.size() - 1;
+    pub.d_ptr = o->dptr.data();
+    pub.d_pos = o->dpos.data();
+    pub.c = o->c.data();
+    *out = &owned->pub;
     return NET_OK;
 }
 
 int32_t net_compressed_free(net_compressed* c) {
-    if (c) delete reinterpret_cast<Owned*>(c);
+    if (c) {
+        Owned* owned = reinterpret_cast<Owned*>(c);
+        delete owned->st;
+        delete owned;
+    }
     return NET_OK;
 }
 
