@@ -37,8 +37,9 @@
  *   ora_rk4       : 4th-order convergence against a 16x finer step; exactness
  *       for constant RHS.
  *   ora_local_order, phase maps : R=1 for identical phases, splay state R=0.
- *   Long-run order-parameter statistics: PARITY UNPINNED in absolute terms
- *       (the paper prints no value); they are only compared GPU-vs-oracle.
+ *   Long-run order-parameter statistics of the coupled configs: PARITY UNPINNED in absolute
+ *       terms (the paper prints no value); they are only compared GPU-vs-oracle.  The procedure
+ *       (oracle.py: run_statistics) is pinned on the K = 0 closed form.
  */
 #include <math.h>
 #include <stdint.h>

@@ -493,3 +493,27 @@ def test_fast_variant_ring_prefix_sums_wrap_and_large_radius():
         assert _a11(net.rhs_fast(y), net.rhs(y)) <= 1e-13
         a, b = net.rk4(y, 25, 0.01), net.rk4(y, 25, 0.01, fast=True)
         assert np.abs(a - b).max() <= 1e-12
+
+
+def test_run_statistics_against_the_uncoupled_closed_form():
+    """The long-run statistics PROCEDURE of reading R9 pinned in absolute terms on the one case with a
+    closed form: K = 0, phi_i(t) = phi_i(0) + omega_i t.  Window = samples with step >= n_steps / 2,
+    population std of R, local order parameter at the last sample over row + self, velocity over
+    [t_a, t_b] -- each recomputed here with numpy from the closed form, not with the oracle."""
+    n, P = 40, 3
+    rp, ci = ora.topology_ring(n, P)
+    rng = np.random.default_rng(8)
+    om = rng.normal(size=n)
+    phi0 = rng.uniform(-np.pi, np.pi, n)
+    net = ora.OracleNet.ks(n, rp, ci, 0.0, 0.4, om)
+    n_steps, dt, every = 90, 0.05, 10
+    st = net.run_statistics(phi0.reshape(1, n), n_steps, dt, every)
+    steps = [s for s in range(every, n_steps + 1, every) if 2 * s >= n_steps]
+    assert st["n_samples"] == len(steps) == 5
+    R = np.array([abs(np.exp(1j * (phi0 + om * s * dt)).mean()) for s in steps])
+    assert abs(st["R_mean"] - R.mean()) < 1e-12 and abs(st["R_std"] - R.std()) < 1e-12
+    z = np.exp(1j * (phi0 + om * n_steps * dt))
+    loc = np.array([abs(sum(z[(i + d) % n] for d in range(-P, P + 1))) / (2 * P + 1) for i in range(n)])
+    assert abs(st["Rloc_mean"] - loc.mean()) < 1e-12
+    np.testing.assert_allclose(st["vel"], om, rtol=0, atol=1e-12)
+    assert abs(st["vel_mean"] - om.mean()) < 1e-12 and abs(st["vel_std"] - om.std()) < 1e-12
