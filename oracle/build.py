@@ -16,9 +16,12 @@ def build(force: bool = False) -> str:
             and os.path.getmtime(LIB) >= os.path.getmtime(SRC)):
         return LIB
     # -O2, no -ffast-math: the oracle's arithmetic is exactly what is written.
+    # (written beside and renamed into place: a process that has the old object mapped keeps it)
+    tmp = LIB + ".tmp%d" % os.getpid()
     cmd = ["gcc", "-O2", "-std=c99", "-fPIC", "-shared", "-fopenmp",
-           "-ffp-contract=off", SRC, "-o", LIB, "-lm"]
+           "-ffp-contract=off", SRC, "-o", tmp, "-lm"]
     subprocess.check_call(cmd)
+    os.replace(tmp, LIB)
     return LIB
 
 
