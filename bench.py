@@ -293,6 +293,119 @@ def roofline_object(w, m, steps):
             "frac_direct_formulation": value / c["direct_osc_steps_per_s"]}
 
 
+# ------------------------------------------------------------------ SURVEY.md 8(f) rows, measured
+def measure_next_rows(device, steps):
+    """The rows SURVEY.md 8(f) lists as next, each measured on a synthetic workload of the paper's
+    shape (3D ball of radius 2 on 100^3 = 10^6 elements, fp64, the size of the paper's own performance
+    tests) with the metric of the bench and the roofline of its formulation:
+      dp5        adaptive Dormand-Prince 5(4) (net_integrate_adaptive) on the KS lattice: N x accepted
+                 steps / s; bytes per attempt = 6 RHS evaluations (read state, write k: 2 words each)
+                 + the stage combinations (sum_{s=1..6} (s + 2) words) + error norm (9) + commit (4);
+      compressed the coupling matrix of Alg. 2 (net_compress_csr of the lattice's CSR, EXTRACT inside
+                 the per-link kernels) beside the same net given as a lattice (offset table) and as
+                 plain CSR, all on the per-link DIRECT form: the paper's "decompression increases
+                 computing time 2-5 folds compared to uncompressed bit arrays" (PAPER.md:175);
+      delay      eq. (2) with delay 5 dt and noise (NET_MODEL_FHN2), per-link form.
+    The per-link forms are bound by the FP64 sines / the gathers of the direct formulation."""
+    import numpy as np
+    import torch
+    from paper_2410_19075_b200 import binding as B, configs, inputs, roofline as R
+    pk = R.peaks()
+    out = {}
+    n1, P = 100, 2
+    n = n1 ** 3
+    from dataclasses import replace
+    w = replace(configs.get("3b", n1=n1), radius=P, name="KS 3D %d^3 radius %d f64" % (n1, P))
+    y0, elem = make_inputs(w, 1)
+
+    def run_fixed(net, rk4_steps, reps):
+        for _ in range(3):
+            net.integrate(rk4_steps, w.dt)
+        net.synchronize()
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        ev0.record(net.stream)
+        for _ in range(reps):
+            net.integrate(rk4_steps, w.dt)
+        ev1.record(net.stream)
+        torch.cuda.synchronize()
+        return n * rk4_steps * reps / (ev0.elapsed_time(ev1) * 1e-3)
+
+    def ks_net(topo, method):
+        net = B.Net(w.model, B.F64, n, topo, w.params, method=method, device=device)
+        net.set_state(y0)
+        net.set_param_array(B.PARAM_OMEGA, elem)
+        return net
+
+    lattice = dict(kind=B.TOPO_LATTICE, extent=w.extent, radius=P)
+    # ---- Dormand-Prince 5(4)
+    net = ks_net(lattice, B.METHOD_AUTO)
+    net.integrate_adaptive(1.0, 1e-8, 1e-11, 0.05)      # warm-up and the controller settles
+    net.synchronize()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    t0 = net.time()[0]
+    ev0.record(net.stream)
+    info = net.integrate_adaptive(t0 + 10.0 * max(1, steps // 5), 1e-8, 1e-11, 0.05)
+    ev1.record(net.stream)
+    torch.cuda.synchronize()
+    sec = ev0.elapsed_time(ev1) * 1e-3
+    attempts = info["accepted"] + info["rejected"]
+    words = 6 * 2 + sum(s + 2 for s in range(1, 7)) + 9 + 4
+    gbs = attempts * n * words * 8 / sec / 1e9
+    out["dp5"] = {"workload": w.name + ", rtol 1e-8, atol 1e-11", "value": n * info["accepted"] / sec, "unit": METRIC,
+                  "accepted": info["accepted"], "rejected": info["rejected"], "ms_per_attempt": sec * 1e3 / max(1, attempts),
+                  "roofline": {"bound": "hbm", "achieved": gbs, "peak": pk["hbm_gbs"], "unit": "GB/s", "frac": gbs / pk["hbm_gbs"],
+                               "bytes_per_element_and_attempt": words * 8,
+                               "note": "state-sized vectors of the integrator only (58 words per element and attempt); the 6 "
+                                       "RHS launches inside are the lattice kernels of config 3b; every evaluation also pays two "
+                                       "layout copies (DESIGN.md section 5)"}}
+    net.close()
+    # ---- compressed matrix against the same topology as offset table and as plain CSR (all DIRECT)
+    net = ks_net(lattice, B.METHOD_DIRECT)
+    v_lat = run_fixed(net, 4, max(2, steps // 2))
+    rp, ci = net.get_topology()
+    net.close()
+    t_c = time.perf_counter()
+    cm = B.net_compress_csr(rp, ci)
+    t_c = time.perf_counter() - t_c
+    net = ks_net(dict(kind=B.TOPO_CSR, row_ptr=rp, col_idx=ci), B.METHOD_DIRECT)
+    v_csr = run_fixed(net, 4, max(2, steps // 2))
+    net.close()
+    net = ks_net(dict(kind=B.TOPO_COMPRESSED, compressed=cm), B.METHOD_DIRECT)
+    v_cmp = run_fixed(net, 4, max(2, steps // 2))
+    net.close()
+    v, dptr, dpos, c = cm.arrays()
+    deg = len(ci) // n
+    sine_ceiling = pk["fp64_ginstr_s"] * 1e9 / (4 * deg * R.SINE_FP64_INSTR)
+    out["compressed"] = {"workload": w.name + " as a compressed coupling matrix (Alg. 2), per-link form", "value": v_cmp,
+                         "unit": METRIC, "same_topology_as_offset_table": v_lat, "same_topology_as_csr": v_csr,
+                         "slowdown_vs_csr": v_csr / v_cmp, "table_entries": int(len(dptr) - 1),
+                         "compressed_bytes": int(4 * (len(v) + len(dpos) + len(c)) + 8 * len(dptr)),
+                         "csr_bytes": int(4 * len(ci) + 8 * len(rp)), "host_compress_s": t_c,
+                         "roofline": {"bound": "alu", "achieved": v_cmp * 4 * deg * R.SINE_FP64_INSTR / 1e9,
+                                      "peak": pk["fp64_ginstr_s"], "unit": "Ginstr/s",
+                                      "frac": v_cmp / sine_ceiling,
+                                      "note": "direct formulation: one fp64 sine (~60 FP64-pipe instructions) per link and stage"}}
+    # ---- eq. (2) with delay and noise (per-link form)
+    th = inputs.fhn_circle(n, 1)
+    P2 = dict(eps=0.05, a=0.5, sigma=0.3, I_app=0.0)
+    for name, m, D in (("delay", 5, 0.05), ("no_delay", 0, 0.0)):
+        net = B.Net(B.MODEL_FHN2, B.F64, n, lattice, dict(P2, D=D, seed=3), device=device, delay_steps=m)
+        net.set_state(th)
+        val = run_fixed(net, 4, max(2, steps // 2))
+        net.close()
+        if name == "delay":
+            # per stage and element: deg gathers of the delayed x (midpoint stages: 4 history values per link)
+            out["delay"] = {"workload": "eq. (2) FHN 3D %d^3 radius %d f64, delay 5 dt, noise" % (n1, P), "value": val, "unit": METRIC}
+        else:
+            out["delay"]["without_delay_and_noise"] = val
+    out["delay"]["roofline"] = {"bound": "gathers (L1 / L2; lattice neighbours are local)", "unit": "gathers/s",
+                                "achieved": out["delay"]["value"] * deg * (1 + 4 + 4 + 1),
+                                "note": "per oscillator-step: deg x (1 + 4 + 4 + 1) history values gathered per link "
+                                        "(stage 0 and 3 one slot, the midpoint stages two slots of x and dx/dt); compare with "
+                                        "roofline.measured_peaks.l2_gather_gops x 1e9"}
+    return out
+
+
 # ------------------------------------------------------------------ CPU oracle arm
 SAMPLE = {"1": dict(), "2": dict(n=16384), "3a": dict(n1=64), "3b": dict(n1=64),
           "4": dict(n=200_000), "5": dict(n1=160)}
@@ -484,6 +597,8 @@ def run_ours(args):
                              "sm_mhz": e["clocks"]["sm_mhz"],
                              "clocks_ok": not (bad & set(e["clocks"]["reasons"]))}
         line["roofline"]["per_config"] = tab
+    if rank == 0 and ws == 1 and not args.no_per_config:
+        line["next_rows"] = measure_next_rows(device, args.steps)
     if rank == 0 and ws == 1 and not args.no_cpu_baseline:
         cb, _, _, _ = time_oracle(w.cfg)
         line["cpu_baseline"] = cb
