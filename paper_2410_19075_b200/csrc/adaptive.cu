@@ -13,6 +13,7 @@
 // reads the control block back once per batch (no round trip per step).  Attempts enqueued after
 // t_end was reached leave every vector untouched.
 #include <math.h>
+#include <stdlib.h>
 
 #include "oscnet_internal.cuh"
 
@@ -225,12 +226,18 @@ static int32_t dp5_run(net* h, double t_end, double rtol, double atol, double h0
     int32_t rc;
     if ((rc = state_to_external(h, v.y))) return rc;              // y (caller layout [nvar][n]) <- the net's state
     if ((rc = rhs_at(h, v.y, v.k[0]))) return rc;                 // k1 = f(y)
-    while (true) {
+    // One batch of DP5_BATCH attempts.  Every kernel takes the step size, the time and the decision
+    // from the device control block, so a batch is the same work whatever the state: it is captured
+    // once into a CUDA graph and replayed (about 50 launches and 24 copies per attempt would
+    // otherwise be bound by the host's launch rate: 0.41 ms against 0.35 ms per attempt on 10^6
+    // elements).  The legacy default stream cannot be captured: plain launches there.
+    auto enqueue_batch = [&]() -> int32_t {
         for (int a = 0; a < DP5_BATCH; ++a) {
             dp5_begin_kernel<<<1, 1, 0, st>>>(d_c);
             for (int s = 1; s < 7; ++s) {
                 dp5_stage_kernel<T><<<grid, DP5_THREADS, 0, st>>>(d_c, v, s, len);
-                if ((rc = rhs_at(h, s == 6 ? v.y5 : v.tmp, v.k[s]))) return rc;
+                int32_t r = rhs_at(h, s == 6 ? v.y5 : v.tmp, v.k[s]);
+                if (r) return r;
             }
             dp5_error_kernel<T><<<grid, DP5_THREADS, 0, st>>>(d_c, v, len, partial);
             if (n_out > 0) dp5_dense_kernel<T><<<grid, DP5_THREADS, 0, st>>>(d_c, v, len, d_t_out, n_out, (T*)d_out);
@@ -238,6 +245,30 @@ static int32_t dp5_run(net* h, double t_end, double rtol, double atol, double h0
             dp5_end_kernel<<<1, 1, 0, st>>>(d_c, d_t_out, n_out);
             h->launches += n_out > 0 ? 11 : 10;
         }
+        return NET_OK;
+    };
+    struct GraphHolder {
+        cudaGraph_t g = nullptr;
+        cudaGraphExec_t e = nullptr;
+        ~GraphHolder() { if (e) cudaGraphExecDestroy(e); if (g) cudaGraphDestroy(g); }
+    } gh;
+    int64_t per_batch = 0;
+    if (st != nullptr && st != cudaStreamLegacy && !getenv("OSCNET_DP5_NO_GRAPH")) {
+        const int64_t before = h->launches;
+        OSC_CUDA(h, cudaStreamBeginCapture(st, cudaStreamCaptureModeThreadLocal));
+        rc = enqueue_batch();
+        const cudaError_t e = cudaStreamEndCapture(st, &gh.g);
+        per_batch = h->launches - before;
+        h->launches = before;                      // the capture itself launched nothing
+        if (rc) return rc;
+        if (e != cudaSuccess) return cuda_err(h, e, "cudaStreamEndCapture(dp5)");
+        OSC_CUDA(h, cudaGraphInstantiate(&gh.e, gh.g, 0));
+    }
+    while (true) {
+        if (gh.e) {
+            OSC_CUDA(h, cudaGraphLaunch(gh.e, st));
+            h->launches += per_batch;
+        } else if ((rc = enqueue_batch())) return rc;
         OSC_CUDA(h, cudaGetLastError());
         OSC_CUDA(h, cudaMemcpyAsync(&c, d_c, sizeof(c), cudaMemcpyDeviceToHost, st));
         OSC_CUDA(h, cudaStreamSynchronize(st));

@@ -2,6 +2,7 @@
 // the CUDA-graph step driver and the observable entry points.
 #include <math.h>
 #include <stdarg.h>
+#include <stdlib.h>
 
 #include <new>
 
@@ -262,7 +263,7 @@ static int32_t ensure_s(net* h) {
     if (h->s_valid) return NET_OK;
     int32_t rc = NET_OK;
     if (h->b.s_y) rc = hh_compute_s(h, h->b.y, h->b.s_y);
-    if (rc == NET_OK) rc = fast_refresh_exchange(h);
+    if (rc == NET_OK) rc = fast_refresh_exchange(h, nullptr);
     if (rc) return rc;
     h->s_valid = 1;
     return NET_OK;
@@ -286,7 +287,21 @@ int32_t state_from_external(net* h, const void* d_src) {
 // k = f(x): x becomes the net's state (the caller restores its own afterwards), then the RHS-only
 // instance of the net's stage kernel family, exactly as net_eval_rhs runs it
 int32_t rhs_at(net* h, const void* d_x, void* d_k) {
-    int32_t rc = state_from_external(h, d_x);
+    int32_t rc;
+    // same layout inside and outside (no padding between the variables, no interleaved pairs): the
+    // stage kernels read x and write k in place, only the exchange fields of x are rebuilt
+    if (!h->pairs && h->n == h->ld && h->desc.model != NET_MODEL_FHN2 && !getenv("OSCNET_DP5_COPIES")) {
+        h->s_valid = 0;                                   // the exchange fields no longer belong to y
+        if (h->b.s_y && (rc = hh_compute_s(h, d_x, h->b.s_y))) return rc;
+        if (h->method == NET_METHOD_FAST && (rc = fast_refresh_exchange(h, d_x))) return rc;
+        StageArgs a = stage_args(h, 0, 0.0);
+        a.stage = STAGE_RHS_ONLY;
+        a.in = d_x;
+        a.out = d_k;
+        a.s_out = nullptr;
+        return run_stage(h, a);
+    }
+    rc = state_from_external(h, d_x);
     if (rc) return rc;
     if ((rc = ensure_s(h))) return rc;
     StageArgs a = stage_args(h, 0, 0.0);

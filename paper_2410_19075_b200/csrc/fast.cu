@@ -16,7 +16,7 @@ size_t lattice_v2_scratch_bytes(const net_desc* d);
 size_t lattice_v2_state_bytes(const net_desc* d);
 int32_t lattice_v2_prepare(net* h);
 int32_t lattice_v2_stage(net* h, const StageArgs& a);
-int32_t lattice_v2_refresh_exchange(net* h);
+int32_t lattice_v2_refresh_exchange(net* h, const void* state);
 bool lattice_v3_supported(const net_desc* d);
 int32_t lattice_v3_prepare(net* h);
 int32_t lattice_v3_stage(net* h, const StageArgs& a);
@@ -108,8 +108,8 @@ int32_t fast_stage(net* h, const StageArgs& a) {
     return set_err(h, NET_ERR_UNSUPPORTED, "fast kernel family %d has no stage kernel", h->fast_kind);
 }
 
-int32_t fast_refresh_exchange(net* h) {
-    if (h->fast_kind == FAST_LATTICE3D_V2 || h->fast_kind == FAST_LATTICE3D_V3) return lattice_v2_refresh_exchange(h);
+int32_t fast_refresh_exchange(net* h, const void* state) {
+    if (h->fast_kind == FAST_LATTICE3D_V2 || h->fast_kind == FAST_LATTICE3D_V3) return lattice_v2_refresh_exchange(h, state);
     return NET_OK;
 }
 

@@ -158,9 +158,11 @@ int32_t pairs_unpack(net* h, const void* pairs, void* soa) {
     return NET_OK;
 }
 
-int32_t lattice_v2_refresh_exchange(net* h) {
+// exchange field E_a = (cos, sin) of the phase row of `state` ([nvar][ld]; nullptr = the net's y)
+int32_t lattice_v2_refresh_exchange(net* h, const void* state) {
     if (h->desc.model != NET_MODEL_KS && h->desc.model != NET_MODEL_KSI) return NET_OK;
-    return h->ks_planar ? pad_fill<2>(h, h->b.y, h->E_a) : pad_fill<1>(h, h->b.y, h->E_a);
+    const void* src = state ? state : h->b.y;
+    return h->ks_planar ? pad_fill<2>(h, src, h->E_a) : pad_fill<1>(h, src, h->E_a);
 }
 
 }  // namespace oscnet
@@ -307,7 +309,7 @@ int32_t lattice_v3_local_order(net* h, double* d_out) {
         else unit_pairs_kernel<double><<<l2_grid_for(pairs), 256, 0, h->stream>>>((const double*)h->b.y, (double*)h->b.Y3, pairs);
         h->launches += 1;
     } else if (!h->s_valid) {
-        if ((rc = lattice_v2_refresh_exchange(h))) return rc;
+        if ((rc = lattice_v2_refresh_exchange(h, nullptr))) return rc;
         h->s_valid = 1;
     }
     // fp32 nets: the kernel writes float (into Y4, rewritten by the next step), widened afterwards

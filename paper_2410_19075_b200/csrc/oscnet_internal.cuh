@@ -257,7 +257,7 @@ size_t fast_state_bytes(const net_desc* d, int32_t fast_kind);   // 0 = the defa
 int32_t fast_prepare(net* h);                             // once, at the end of net_create
 int32_t fast_stage(net* h, const StageArgs& a);
 int32_t fast_integrate(net* h, int64_t n_steps, double dt, bool* handled);  // persistent kernels
-int32_t fast_refresh_exchange(net* h);                    // exchange fields of y (after set_state)
+int32_t fast_refresh_exchange(net* h, const void* state);   // exchange fields of `state` (nullptr: of y, after set_state)
 int32_t pairs_pack(net* h, const void* soa, void* pairs);    // SoA [2][ld] -> padded pairs (+ ghosts)
 int32_t pairs_unpack(net* h, const void* pairs, void* soa);
 
