@@ -323,7 +323,6 @@ static int32_t l3_stage(net* h, int stage, double dt, void* rhs_out) {
     const Buffers& b = h->b;
     L3Ptrs a;
     memset(&a, 0, sizeof(a));
-    a.ksi_stage = -1;
     CUtensorMap op[4] = {h->tm3_op[0], h->tm3_op[0], h->tm3_op[0], h->tm3_op[0]};
     const CUtensorMap* tm = h->tm3_st;
     const CUtensorMap* to = h->tm3_op;     // FHN: y, Y2 | KS: y, Y2, Y3, omega
@@ -347,19 +346,6 @@ static int32_t l3_stage(net* h, int stage, double dt, void* rhs_out) {
             op[0] = to[1];                     // Z lives in Y2
             if (KS) op[1] = to[3];
             return l3_launch_stage<T, MODEL, P, L3_S3>(h, a, dt, tm[KS ? 1 : 3], op);
-        case 10: case 11: case 12: case 13: {
-            // KS with inertia, RK4 stage s = stage - 10, fused into the RHS instance: stencil source
-            // E_a (s even) / E_b (s odd), E of the new phase into the other one -- after stage 3 E_a = E(y)
-            const int s = stage - 10;
-            void* bufs[5] = {b.y, b.Y2, b.Y3, b.Y4, b.y};
-            a.ksi_stage = s;
-            a.k_in = bufs[s]; a.out = bufs[s + 1];
-            a.k_y = b.y; a.k_Y2 = b.Y2; a.k_Y3 = b.Y3;
-            a.k_ld = h->ld; a.k_dt = dt; a.k_damp = h->mp.damp; a.k_inv_m = h->mp.inv_m;
-            a.Eout = (s & 1) ? h->E_a : h->E_b;
-            if (KS) op[0] = to[3];
-            return l3_launch_stage<T, MODEL, P, L3_RHS>(h, a, dt, tm[s & 1], op);
-        }
         case 5:     // local order parameter: KS reads E(y) = E_a, FHN the unit phasor field staged in Y3
             a.out = rhs_out;
             return l3_launch_stage<T, MODEL, P, L3_LOC>(h, a, dt, tm[KS ? 0 : 2], op);

@@ -230,47 +230,6 @@ lat3s_kernel(const __grid_constant__ CUtensorMap tm_st, const __grid_constant__ 
                     ov[e] = o;
                     if constexpr (STAGE != L3_RHS) sincos_stage<T>(o, &sv[e], &cv[e]);
                 }
-                if constexpr (STAGE == L3_RHS) {
-                    if (a.ksi_stage >= 0) {
-                        // KS with inertia (eq. (3) in full) fused into this instance: ov = the
-                        // torque omega + (K/Omega) sum sin(...); phi' = psi, psi' = (torque - eps psi)/m; RK4
-                        // stage update of both variables (the 4-array form of the per-link kernels); E of
-                        // the new phi with its ghost images for the next stage
-                        const int64_t ld = a.k_ld;
-                        const T* in = (const T*)a.k_in;
-                        const T* yb = (const T*)a.k_y;
-                        T psi[X], phin[X], y0v[X], y1v[X], a2[X], b2[X], a3[X], b3[X], op[X], oq[X];
-                        ldg_vec<X>(in + ld + il, psi);
-                        ldg_vec<X>(yb + il, y0v);
-                        ldg_vec<X>(yb + ld + il, y1v);
-                        if (a.ksi_stage == 3) {
-                            ldg_vec<X>(in + il, phin);
-                            ldg_vec<X>((const T*)a.k_Y2 + il, a2); ldg_vec<X>((const T*)a.k_Y2 + ld + il, b2);
-                            ldg_vec<X>((const T*)a.k_Y3 + il, a3); ldg_vec<X>((const T*)a.k_Y3 + ld + il, b3);
-                        }
-                        const T dt = (T)a.k_dt;
-#pragma unroll
-                        for (int e = 0; e < X; ++e) {
-                            const T kphi = psi[e], kpsi = (ov[e] - T(a.k_damp) * psi[e]) * T(a.k_inv_m);
-                            const bool s3 = a.ksi_stage == 3;
-                            op[e] = stage_combine<T>(a.ksi_stage, dt, kphi, y0v[e], s3 ? a2[e] : T(0), s3 ? a3[e] : T(0), s3 ? phin[e] : T(0));
-                            oq[e] = stage_combine<T>(a.ksi_stage, dt, kpsi, y1v[e], s3 ? b2[e] : T(0), s3 ? b3[e] : T(0), psi[e]);
-                            sincos_stage<T>(op[e], &sv[e], &cv[e]);
-                        }
-                        stg_vec<X>((T*)a.out + il, op);
-                        stg_vec<X>((T*)a.out + ld + il, oq);
-                        T* Ec = (T*)a.Eout;
-                        T* Es = Ec + g.plane;
-                        auto store_planes = [&](int64_t at) { stg_vec<X>(Ec + at, cv); stg_vec<X>(Es + at, sv); };
-                        store_planes(ip);
-                        if (gxs != 0) store_planes(ip + gxs);
-                        if (gys != 0) {
-                            store_planes(ip + (int64_t)gys * nxp);
-                            if (gxs != 0) store_planes(ip + (int64_t)gys * nxp + gxs);
-                        }
-                        continue;
-                    }
-                }
                 stg_vec<X>((T*)a.out + il, ov);
                 if constexpr (STAGE == L3_S2) stg_vec<X>((T*)a.out2 + il, zv);
                 if constexpr (STAGE != L3_RHS) {

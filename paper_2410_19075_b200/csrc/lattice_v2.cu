@@ -260,13 +260,6 @@ __global__ void __launch_bounds__(256) ksi_update_kernel(StageArgs a, ModelParam
 }
 
 static int32_t ksi_lattice_stage(net* h, const StageArgs& sa) {
-    // Tried in round 2 (OSCNET_KSI_FUSED): ONE launch per stage, the update of (phi, psi) fused into
-    // the finisher of the RHS instance (lat3s_kernel.cuh, a.ksi_stage >= 0), psi and the RK4 operands
-    // read from global memory by the consumer warps.  Measured SLOWER than the two launches below --
-    // config 6 / 6b / 6c: 7.5e9 / 5.7e9 / 2.1e9 against 1.11e10 / 6.45e9 / 3.17e9 osc-steps/s: global
-    // loads in the consumer warps of a kernel that runs ~12 warps per SM stall the whole pipeline
-    // (which is why the stage kernels take every operand as a TMA tile).  Kept as the record.
-    if (sa.stage != STAGE_RHS_ONLY && getenv("OSCNET_KSI_FUSED")) return l3_dispatch(h, 10 + sa.stage, sa.dt, nullptr);
     int32_t rc = l3_dispatch(h, 4, 0.0, h->ksi_c);           // RHS instance of the KS kernel on E_a = E(stage input)
     if (rc) return rc;
     const TopoView& tv = h->tv;

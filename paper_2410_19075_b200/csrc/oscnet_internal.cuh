@@ -165,12 +165,6 @@ struct L3Ptrs {
     void* out;                 // FHN: padded pairs; KS: plain scalars
     void* out2;                // stage 2: Z
     void* Eout;                // KS: padded (cos, sin) pairs of the output state
-    // KS with inertia fused into the RHS instance of the field-split kernel (ksi_stage >= 0): the
-    // finisher reads the local variable psi and the RK4 operands from global memory ([2][ld] arrays)
-    const void *k_in, *k_y, *k_Y2, *k_Y3;
-    long long k_ld;
-    double k_dt, k_damp, k_inv_m;
-    int ksi_stage;             // -1: plain RHS instance; 0..3: RK4 stage of NET_MODEL_KSI
 };
 
 }  // namespace oscnet

@@ -104,24 +104,3 @@ def test_ksi_fast_is_refused_on_2d_lattices_and_mass_must_be_positive():
         B.Net.from_workload(bad)
     assert ei.value.code == -1
 
-
-def test_ksi_lattice_fused_stage_form_matches_the_two_launch_form():
-    """OSCNET_KSI_FUSED: the update of (phi, psi) inside the finisher of the lattice RHS instance
-    (measured slower, kept as the record of that measurement): same results as the default form."""
-    import os
-    w = configs.get("6", n1=16)
-    inp = H.make_inputs(w, seed=8)
-    ref = H.make_oracle(w, inp).rk4(inp["y0"], 40, w.dt)
-    os.environ["OSCNET_KSI_FUSED"] = "1"
-    try:
-        net = H.make_gpu(w, inp, method=B.METHOD_FAST)
-        net.integrate(40, w.dt)
-        fused = net.get_state()
-        assert H.rel_maxnorm(net.eval_rhs(), H.make_oracle(w, inp).rhs(fused)) <= 10 * H.TOL_RHS["f64"]
-        net.close()
-    finally:
-        del os.environ["OSCNET_KSI_FUSED"]
-    net = H.make_gpu(w, inp, method=B.METHOD_FAST)
-    net.integrate(40, w.dt)
-    assert H.traj_err(w, fused, ref) <= H.TOL_TRAJ["f64"]
-    assert np.abs(fused - net.get_state()).max() <= 1e-12
