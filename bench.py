@@ -534,6 +534,10 @@ def run_ours(args):
     device = "cuda:%d" % local_rank
     if ws > 1:
         replicas.init("nccl")
+    if args.next_rows:
+        if rank == 0:
+            print(json.dumps({"next_rows": measure_next_rows(device, args.steps)}), flush=True)
+        return 0
     w = configs.get(args.config)
     m = measure(w, device, args.steps, args.warmup, e2e=True, peaks=True)
     rk4 = args.steps * m["rk4_per_step"]
@@ -621,6 +625,8 @@ def main():
     ap.add_argument("--no-per-config", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-rewrite-error", action="store_true")
+    ap.add_argument("--next-rows", action="store_true",
+                    help="measure only the SURVEY.md 8(f) rows (next_rows of the full line) and print them")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     return run_reference(args) if args.impl == "reference" else run_ours(args)
