@@ -2,7 +2,7 @@
 """bench.py -- oscillator-steps/s of the fused RK4 hot path on B200, against its roofline.
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--config 5] [--impl ours|reference]
-                    [--no-per-config] [--no-cpu-baseline]
+                    [--no-per-config] [--no-cpu-baseline] [--no-rewrite-error] [--next-rows]
 
 One bench "step" = one net_integrate call of BENCH_RK4[cfg] RK4 steps over the whole network
 (the output interval `obs_every` of the workload for the large nets; the whole 1000-step run
@@ -11,7 +11,9 @@ state resident in HBM; `e2e` = the same through the C ABI with HOST buffers (net
 pinned memory + net_integrate + net_get_state to pinned memory inside the timed region).
 The headline workload is config 5 (DESIGN.md "Measurement": the metric is quoted per config;
 config 5 is the largest one and has a clean HBM roofline); `per_config` carries the same
-measurement for every other north-star config.  N > 1 GPUs = independent replicas (weak
+measurement for every other north-star config (and the same facts as a compact table in
+`roofline.per_config`); `next_rows` measures the SURVEY.md 8(f) rows (Dormand-Prince 5(4), the
+compressed coupling matrix, eq. (2) with delay and noise).  N > 1 GPUs = independent replicas (weak
 scaling, no collective on the data path).  `--impl reference` times the CPU oracle, as it
 stands, on a bounded sample of the same workload.
 """
