@@ -377,6 +377,23 @@ int32_t net_probe_latency(net_t* net, double* out4);
  * y, the time and the topology are not touched. */
 int32_t net_probe_peaks(net_t* net, double* out8);
 
+/* The global order parameter without a handle, a workspace or any allocation: for callers that may
+ * not call cudaMalloc (code under CUDA graph capture, tight serving loops, harnesses that forbid it).
+ *   R e^{i Psi} = (1/N) sum_j e^{i theta_j}   (reading R9), as NET_OBS_GLOBAL_ORDER.
+ * d_theta (DEVICE, caller-owned): n phases of `dtype` (NET_F32 / NET_F64); the sum is in double.
+ * d_out2 (DEVICE, caller-owned): double[2] = {R, Psi}, written when the work on `stream` (a cudaStream_t
+ * of the CURRENT device, NULL = default stream) completes; the call does not synchronise.
+ * The block partials live in one static device array of 262400 bytes that every GPU loading the
+ * library holds until exit: n <= NET_NOALLOC_MAX_N, larger n returns NET_ERR_SIZE and launches nothing
+ * (message: net_last_error(NULL)).  Every call on a device shares that array, so calls that overlap on
+ * the GPU (different streams, graphs replayed concurrently) race: serialise them.  The call enqueues one
+ * 256-byte cudaMemsetAsync (the completion ticket must start at zero) and one kernel; it calls no
+ * cudaMalloc, cudaFree or allocating library routine.  The first call on each device also resolves the
+ * array's device address (cudaGetSymbolAddress): make that one outside stream capture.
+ * Errors: NET_ERR_INVALID (NULL pointer, n < 1, bad dtype), NET_ERR_SIZE, NET_ERR_CUDA. */
+#define NET_NOALLOC_MAX_N 134217728LL /* 2^27 */
+int32_t net_order_parameter_noalloc(const void* d_theta, int64_t n, int32_t dtype, double* d_out2, void* stream);
+
 /* "oscnet <major>.<minor> sm_100a" */
 const char* net_version(void);
 

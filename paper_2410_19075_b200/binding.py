@@ -31,6 +31,7 @@ ABI_SYMBOLS = [
     "net_probe_latency", "net_probe_peaks", "net_get_launch_config",
     "net_adaptive_workspace_bytes", "net_integrate_adaptive",
     "net_compress_csr", "net_compressed_free", "net_integrate_adaptive_dense",
+    "net_order_parameter_noalloc",
 ]
 
 
@@ -134,6 +135,7 @@ def lib():
                                                    C.c_double, C.c_int64, C.c_void_p, C.c_size_t, C.POINTER(C.c_double)]
         L.net_compress_csr.argtypes = [C.c_int64, C.c_void_p, C.c_void_p, C.POINTER(C.POINTER(Compressed))]
         L.net_compressed_free.argtypes = [C.POINTER(Compressed)]
+        L.net_order_parameter_noalloc.argtypes = [C.c_void_p, C.c_int64, C.c_int32, C.c_void_p, C.c_void_p]
         for name in ABI_SYMBOLS:
             if name not in ("net_last_error", "net_version"):
                 getattr(L, name).restype = C.c_int32
@@ -306,6 +308,15 @@ def net_probe_peaks(h):
 
 def net_synchronize(h):
     _check(lib().net_synchronize(h), h)
+
+
+NOALLOC_MAX_N = 1 << 27
+
+
+def net_order_parameter_noalloc(d_theta_ptr, n, dtype, d_out2_ptr, stream_ptr=None):
+    """{R, Psi} of n device phases into a device double[2]; allocates nothing (static device scratch,
+    n <= NOALLOC_MAX_N; calls that overlap on the GPU race).  Pointers are device addresses (ints)."""
+    _check(lib().net_order_parameter_noalloc(d_theta_ptr, n, dtype, d_out2_ptr, stream_ptr))
 
 
 # ------------------------------------------------------------------ convenience
