@@ -161,7 +161,9 @@ static int32_t l3_enumerate(int nx, int ny, int want_tx, int want_sy, F&& f) {
 
 // Geometry of one stage.  Tiles: the (TXt, SY) with the best lane / cover efficiency among
 // those whose staged boxes TMA can take; pipeline depth D: the deepest that still leaves
-// `want_ctas` CTAs per SM; z chunks: fewest waves.  OSCNET_LAT3 = "TXt,SY,Lz,D,CTAS" overrides.
+// `want_ctas` CTAs per SM; grid: fewest planes on the longest CTA.  OSCNET_LAT3 = "TXt,SY,Lz,D,CTAS[,A]"
+// overrides (Lz > 0: chunks of Lz planes, no tail -- or, with A < Lz, that many chunks shortened to A
+// planes and a tail over the rest; Lz < 0: -Lz CTAs with equal spans of the whole space).
 template <class T, int MODEL, int P, int STAGE>
 static int32_t l3_configure_stage(net* h) {
     typedef L3Sh<T, MODEL, P> S;
@@ -174,8 +176,8 @@ static int32_t l3_configure_stage(net* h) {
     L3Geom g;
     memset(&g, 0, sizeof(g));
     g.nx = tv.nx; g.ny = tv.ny; g.nz = tv.nz;
-    int want_tx = 0, want_sy = 0, want_lz = 0, want_d = 0, want_ctas = 0;
-    if (const char* e = getenv("OSCNET_LAT3")) sscanf(e, "%d,%d,%d,%d,%d", &want_tx, &want_sy, &want_lz, &want_d, &want_ctas);
+    int want_tx = 0, want_sy = 0, want_lz = 0, want_d = 0, want_ctas = 0, want_a = 0;
+    if (const char* e = getenv("OSCNET_LAT3")) sscanf(e, "%d,%d,%d,%d,%d,%d", &want_tx, &want_sy, &want_lz, &want_d, &want_ctas, &want_a);
     if (want_ctas <= 0) want_ctas = h->l3_force_ctas > 0 ? h->l3_force_ctas : 2;
     // operand / stencil rows must be whole 16-byte vectors: scalar f32 tiles need TXt % 4 == 0
     const int xq = (KS && sizeof(T) == 4) ? 4 : X;
@@ -224,20 +226,43 @@ static int32_t l3_configure_stage(net* h) {
     int occ = 0;
     OSC_CUDA(h, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, threads, smem));
     if (occ < 1) return NET_ERR_UNSUPPORTED;
+    // Grid (l3_span in lat3_kernel.cuh): chunk-aligned CTAs, tiles x chunks of them, marching in step;
+    // where they leave part of a single wave empty, shorter chunks plus a tail of equal spans over the
+    // planes left at the top of the columns.  Cost = waves x planes of the longest CTA, every segment
+    // paying its 2P lead-in planes (+ 4 for the pipeline restart).  l3_force_tail < 0: aligned only.
     const int64_t slots = (int64_t)occ * sms, tiles = (int64_t)g.tiles_x * g.tiles_y;
-    int64_t best_cost = -1;
+    const int64_t SP = tiles * g.nz;                                         // tile-planes of one stage
+    const int HZ = 2 * P + 4;
+    int64_t best_cost = -1, grid = tiles;
+    g.Lz = g.nz; g.nchunks = 1;
+    const bool allow_tail = h->l3_force_tail >= 0 && want_lz == 0 && !getenv("OSCNET_LAT3_NO_TAIL");
     for (int nch = 1; nch <= g.nz; ++nch) {
         const int Lz = (g.nz + nch - 1) / nch;
         const int chunks = (g.nz + Lz - 1) / Lz;
-        const int64_t waves = (tiles * chunks + slots - 1) / slots;
-        const int64_t cost = waves * (Lz + 2 * P + 4);
-        if (best_cost < 0 || cost < best_cost) { best_cost = cost; g.Lz = Lz; g.nchunks = chunks; }
+        const int64_t m = tiles * chunks;
+        const int64_t waves = (m + slots - 1) / slots;
+        const int64_t cost = waves * (Lz + HZ);
+        if (best_cost < 0 || cost < best_cost) { best_cost = cost; g.Lz = Lz; g.nchunks = chunks; grid = m; }
+        if (!allow_tail || m >= slots) continue;
+        const int64_t gt = slots - m;                                        // CTAs of the tail
+        for (int a = Lz - 1; a >= 1 && 2 * a >= Lz; --a) {
+            const int64_t r = g.nz - (int64_t)chunks * a;
+            if (r <= 0) continue;
+            const int64_t Lt = (tiles * r + gt - 1) / gt;
+            const int64_t segs = 1 + (Lt + r - 2) / r;
+            const int64_t tail = Lt + segs * HZ, c2 = a + HZ > tail ? a + HZ : tail;
+            if (c2 < best_cost) { best_cost = c2; g.Lz = a; g.nchunks = chunks; grid = slots; }
+        }
     }
-    if (want_lz > 0) { g.Lz = want_lz; g.nchunks = (g.nz + g.Lz - 1) / g.Lz; }
+    if (want_lz > 0) {
+        g.Lz = want_lz; g.nchunks = (g.nz + g.Lz - 1) / g.Lz; grid = tiles * g.nchunks;
+        if (want_a > 0 && want_a < want_lz && tiles * g.nchunks < slots && (int64_t)g.nchunks * want_a < g.nz) { g.Lz = want_a; grid = slots; }
+    }
+    if (want_lz < 0 && -(int64_t)want_lz <= SP) { g.Lz = 0; g.nchunks = 0; grid = -want_lz; }   // equal spans over everything
     h->lat3[STAGE] = g;
     h->lat3_threads[STAGE] = threads;
     h->lat3_smem[STAGE] = smem;
-    h->lat3_grid[STAGE] = (unsigned)(tiles * g.nchunks);
+    h->lat3_grid[STAGE] = (unsigned)grid;
     if (getenv("OSCNET_VERBOSE"))
         fprintf(stderr, "lat3 stage %d: tile %dx%d (QX %d SY %d, %d consumer warps) tiles %dx%d Lz %d chunks %d D %d smem %zu occ %d grid %u\n",
                 STAGE, g.TXt, g.TYt, g.QX, g.SY, g.ncw, g.tiles_x, g.tiles_y, g.Lz, g.nchunks, g.D, smem, occ, h->lat3_grid[STAGE]);
@@ -366,11 +391,11 @@ static int32_t l3_stage(net* h, int stage, double dt, void* rhs_out) {
 template <class T, int MODEL, int P>
 static int32_t l3_configure(net* h) {
     typedef L3Sh<T, MODEL, P> S;
-    h->l3_force_tx = h->l3_force_sy = h->l3_force_ctas = 0;
+    h->l3_force_tx = h->l3_force_sy = h->l3_force_ctas = h->l3_force_tail = 0;
     int32_t rc = l3_configure_tile<T, MODEL, P>(h);
     if (rc) return rc;
     if (getenv("OSCNET_LAT3") || getenv("OSCNET_NO_AUTOTUNE") || h->n < (1 << 21)) return NET_OK;
-    struct Cand { int tx, sy; double score; int ctas; };
+    struct Cand { int tx, sy; double score; int ctas, tail; };
     constexpr int KMAX = 10;
     Cand cand[KMAX];
     int nc = 0;
@@ -380,10 +405,10 @@ static int32_t l3_configure(net* h) {
                 if (score > cand[q].score) { cand[q].sy = SY; cand[q].score = score; }
                 return;
             }
-        if (nc < KMAX) { cand[nc++] = Cand{TXt, SY, score, 2}; return; }
+        if (nc < KMAX) { cand[nc++] = Cand{TXt, SY, score, 2, 0}; return; }
         int worst = 0;
         for (int q = 1; q < nc; ++q) if (cand[q].score < cand[worst].score) worst = q;
-        if (score > cand[worst].score) cand[worst] = Cand{TXt, SY, score, 2};
+        if (score > cand[worst].score) cand[worst] = Cand{TXt, SY, score, 2, 0};
     });
     const size_t sb = h->state_bytes;
     OSC_CUDA(h, cudaMemsetAsync(h->b.y, 0, sb, h->stream));
@@ -403,7 +428,7 @@ static int32_t l3_configure(net* h) {
     int best = -1;
     const int64_t launches_before = h->launches;
     auto time_cand = [&](const Cand& c, float* ms_out) -> bool {
-        h->l3_force_tx = c.tx; h->l3_force_sy = c.sy; h->l3_force_ctas = c.ctas;
+        h->l3_force_tx = c.tx; h->l3_force_sy = c.sy; h->l3_force_ctas = c.ctas; h->l3_force_tail = c.tail;
         if (l3_configure_tile<T, MODEL, P>(h) != NET_OK) return false;
         float ms = 0.f;
         bool ok = true;
@@ -418,26 +443,38 @@ static int32_t l3_configure(net* h) {
             if (rep >= 1 && (rep == 1 || one < ms)) ms = one;
         }
         if (getenv("OSCNET_VERBOSE"))
-            fprintf(stderr, "lat3 autotune: tile %dx%d ctas %d score %.3f -> %.3f ms%s\n", c.tx, c.sy * S::TY, c.ctas, c.score, ms, ok ? "" : " (failed)");
+            fprintf(stderr, "lat3 autotune: tile %dx%d ctas %d %s grid %u (%d x %d planes) score %.3f -> %.3f ms%s\n", c.tx, c.sy * S::TY, c.ctas,
+                    c.tail < 0 ? "aligned" : "tail ok", h->lat3_grid[0], h->lat3[0].nchunks, h->lat3[0].Lz, c.score, ms, ok ? "" : " (failed)");
         *ms_out = ms;
         return ok;
     };
     // every tile at three pipeline depths (the deepest that leaves 2, 3, 4 CTAs' worth of shared
     // memory): deeper is not better -- cfg 3a, tile 40x8: D = 2 2.3e10, D = 4 2.0e10 osc-steps/s
-    Cand best_c = Cand{0, 0, 0.0, 0};
+    // and with / without a tail of spans in the last wave (the tail fills the SMs a chunk-aligned grid
+    // leaves half empty, but its CTAs do not march in step with their neighbours: cfg 3b gains, cfg 5 loses)
+    Cand best_c = Cand{0, 0, 0.0, 0, 0};
     for (int q = 0; q < nc; ++q)
-        for (int ctas = 2; ctas <= 4; ++ctas) {
-            Cand c = cand[q];
-            c.ctas = ctas;
-            float ms;
-            if (time_cand(c, &ms) && (best < 0 || ms < best_ms)) { best = q; best_ms = ms; best_c = c; }
-        }
+        for (int ctas = 2; ctas <= 4; ++ctas)
+            for (int tail = -1; tail <= 0; ++tail) {
+                Cand c = cand[q];
+                c.ctas = ctas; c.tail = tail;
+                if (tail == 0) {             // same grid as the aligned pick: nothing new to time
+                    h->l3_force_tx = c.tx; h->l3_force_sy = c.sy; h->l3_force_ctas = c.ctas; h->l3_force_tail = -1;
+                    if (l3_configure_tile<T, MODEL, P>(h) != NET_OK) continue;
+                    const unsigned ga = h->lat3_grid[0];
+                    const int la = h->lat3[0].Lz;
+                    h->l3_force_tail = 0;
+                    if (l3_configure_tile<T, MODEL, P>(h) != NET_OK || (h->lat3_grid[0] == ga && h->lat3[0].Lz == la)) continue;
+                }
+                float ms;
+                if (time_cand(c, &ms) && (best < 0 || ms < best_ms)) { best = q; best_ms = ms; best_c = c; }
+            }
     cudaEventDestroy(e0);
     cudaEventDestroy(e1);
     h->launches = launches_before;
     if (cudaGetLastError() != cudaSuccess) best = -1;
-    if (best >= 0) { h->l3_force_tx = best_c.tx; h->l3_force_sy = best_c.sy; h->l3_force_ctas = best_c.ctas; }
-    else h->l3_force_tx = h->l3_force_sy = h->l3_force_ctas = 0;
+    if (best >= 0) { h->l3_force_tx = best_c.tx; h->l3_force_sy = best_c.sy; h->l3_force_ctas = best_c.ctas; h->l3_force_tail = best_c.tail; }
+    else h->l3_force_tx = h->l3_force_sy = h->l3_force_ctas = h->l3_force_tail = 0;
     return l3_configure_tile<T, MODEL, P>(h);
 }
 

@@ -61,6 +61,41 @@ __device__ __forceinline__ double2 pfma(double2 a, double2 b, double2 c) {
     return make_double2(fma(a.x, b.x, c.x), fma(a.y, b.y, c.y));
 }
 
+// Work distribution.  The first tiles * nchunks CTAs each take one chunk of Lz planes of one tile
+// column, chunk-major, so that all of them march through the same planes at the same time: the halo
+// rows and columns a tile shares with its neighbours are then fetched from HBM once and served from L2
+// to the others (measured on cfg 3a: 296 equal spans cut tile-major, every SM busy, run 28 % SLOWER
+// than 250 aligned half columns that leave 46 SMs with one CTA instead of two).  Where the chunks do not
+// fill the grid's last wave, they are shortened (nchunks * Lz < nz) and the planes left at the top of
+// every column, linearised tile-major, are cut into equal spans for the remaining CTAs of the wave; a
+// span that crosses into the next column is run as segments, each with its own 2P lead-in planes, the
+// pipeline state carrying over.  nchunks = 0: the whole space as equal spans.
+struct L3Span { long long begin, end; int r, zbase; };   // positions u: tile u / r, plane zbase + u % r
+struct L3Seg { int x0, y0, z0, len; };
+__device__ __forceinline__ L3Span l3_span(const L3Geom& g, int nz) {
+    const int tiles = g.tiles_x * g.tiles_y;
+    const int m = tiles * g.nchunks;
+    const int bid = (int)blockIdx.x;
+    if (bid < m) {
+        const int tile = bid % tiles, k = bid / tiles;
+        const int zb = k * g.Lz;
+        const int len = min(g.Lz, nz - zb);
+        const long long begin = (long long)tile * nz + zb;
+        return L3Span{begin, begin + len, nz, 0};
+    }
+    const int zbase = g.nchunks * g.Lz, r = nz - zbase;
+    const long long U = (long long)tiles * r;
+    const long long c = bid - m, gt = (long long)gridDim.x - m;
+    return L3Span{U * c / gt, U * (c + 1) / gt, r, zbase};
+}
+__device__ __forceinline__ L3Seg l3_segment(const L3Geom& g, const L3Span& sp, long long u) {
+    const int tile = (int)(u / sp.r);
+    const int dz = (int)(u - (long long)tile * sp.r);
+    const long long left = sp.end - u;
+    const int len = left < (long long)(sp.r - dz) ? (int)left : sp.r - dz;
+    return L3Seg{(tile % g.tiles_x) * g.TXt, (tile / g.tiles_x) * g.TYt, sp.zbase + dz, len};
+}
+
 // ROT: the accumulators of the open output planes are shifted down one slot after every plane
 // (register moves) instead of being addressed by a compile-time phase J, which needs 2P + 1
 // copies of the plane body: for P = 4 those copies (130 KB of SASS) overflow the instruction
@@ -88,14 +123,8 @@ lat3_kernel(const __grid_constant__ CUtensorMap tm_st, const __grid_constant__ C
     unsigned char* op_ring = st_ring + (size_t)NS * g.st_stride;
 
     const int nx = g.nx, ny = g.ny, nz = g.nz;
-    int bid = blockIdx.x;
-    const int tix = bid % g.tiles_x; bid /= g.tiles_x;
-    const int tiy = bid % g.tiles_y; bid /= g.tiles_y;
-    const int x0 = tix * g.TXt, y0 = tiy * g.TYt;
-    const int z0 = bid * g.Lz;
-    const int z1 = min(nz, z0 + g.Lz);
-    const int nplanes = (z1 - z0) + 2 * P;
     const int tid = threadIdx.x;
+    const L3Span sp = l3_span(g, nz);         // this CTA's share of the (tile, z) space
 
     if (tid == 0) {
         for (int s = 0; s < NB; ++s) { mbar_init(full + s, 1); mbar_init(done + s, (unsigned)g.ncw); }
@@ -110,26 +139,31 @@ lat3_kernel(const __grid_constant__ CUtensorMap tm_st, const __grid_constant__ C
             if (NT >= 1) asm volatile("prefetch.tensormap [%0];" ::"l"(&tm_op0) : "memory");
             if (NT >= 2) asm volatile("prefetch.tensormap [%0];" ::"l"(&tm_op1) : "memory");
             int b = 0, ss = 0;
-            unsigned round = 0;                     // j / NB
-            for (int j = 0; j < nplanes; ++j) {
-                // slot reuse: every consumer warp has finished iteration j - NB (phase round-1 of done[b])
-                if (round > 0) mbar_wait(done + b, (round & 1u) ^ 1u);
-                const bool ops = NT > 0 && j >= 2 * P;
-                mbar_expect_tx(full + b, g.st_bytes + (ops ? NT * g.op_bytes : 0u));
-                int zz = (z0 - P + j) % nz; if (zz < 0) zz += nz;
-                tma_load_3d(st_ring + (size_t)ss * g.st_stride, &tm_st, x0 * U8, y0, zz, full + b);
-                if (ops) {
-                    const int zo = z0 - 2 * P + j;
-                    unsigned char* ob = op_ring + (size_t)b * NT * g.op_stride;
-                    // operands: centre boxes of the padded pair arrays
-                    const int cx = (x0 + HX) * U8, cy = y0 + P;
-                    if (NT >= 1) tma_load_3d(ob, &tm_op0, cx, cy, zo, full + b);
-                    if (NT >= 2) tma_load_3d(ob + g.op_stride, &tm_op1, cx, cy, zo, full + b);
-                    if (NT >= 3) tma_load_3d(ob + 2 * (size_t)g.op_stride, &tm_op2, cx, cy, zo, full + b);
-                    if (NT >= 4) tma_load_3d(ob + 3 * (size_t)g.op_stride, &tm_op3, cx, cy, zo, full + b);
+            unsigned round = 0;                     // iterations so far / NB
+            for (long long s = sp.begin; s < sp.end;) {
+                const L3Seg sg = l3_segment(g, sp, s);
+                const int x0 = sg.x0, y0 = sg.y0, z0 = sg.z0, nplanes = sg.len + 2 * P;
+                for (int j = 0; j < nplanes; ++j) {
+                    // slot reuse: every consumer warp has finished the iteration NB before this one (phase round-1 of done[b])
+                    if (round > 0) mbar_wait(done + b, (round & 1u) ^ 1u);
+                    const bool ops = NT > 0 && j >= 2 * P;
+                    mbar_expect_tx(full + b, g.st_bytes + (ops ? NT * g.op_bytes : 0u));
+                    int zz = (z0 - P + j) % nz; if (zz < 0) zz += nz;
+                    tma_load_3d(st_ring + (size_t)ss * g.st_stride, &tm_st, x0 * U8, y0, zz, full + b);
+                    if (ops) {
+                        const int zo = z0 - 2 * P + j;
+                        unsigned char* ob = op_ring + (size_t)b * NT * g.op_stride;
+                        // operands: centre boxes of the padded pair arrays
+                        const int cx = (x0 + HX) * U8, cy = y0 + P;
+                        if (NT >= 1) tma_load_3d(ob, &tm_op0, cx, cy, zo, full + b);
+                        if (NT >= 2) tma_load_3d(ob + g.op_stride, &tm_op1, cx, cy, zo, full + b);
+                        if (NT >= 3) tma_load_3d(ob + 2 * (size_t)g.op_stride, &tm_op2, cx, cy, zo, full + b);
+                        if (NT >= 4) tma_load_3d(ob + 3 * (size_t)g.op_stride, &tm_op3, cx, cy, zo, full + b);
+                    }
+                    ss = ss + 1 == NS ? 0 : ss + 1;
+                    if (++b == NB) { b = 0; ++round; }
                 }
-                ss = ss + 1 == NS ? 0 : ss + 1;
-                if (++b == NB) { b = 0; ++round; }
+                s += sg.len;
             }
         }
         return;
@@ -138,12 +172,11 @@ lat3_kernel(const __grid_constant__ CUtensorMap tm_st, const __grid_constant__ C
     // ------------------------------------------------------------------ consumer warps
     const int PW = g.PW;
     const int q = tid % g.QX, st = tid / g.QX;
-    const int x = x0 + q * X;
-    const bool owner = st < g.SY && x < nx;
-    const int yrow0 = y0 + st * TY;
     const int nxp = nx + 2 * HX, nyp = ny + 2 * P;
     const int64_t pxy = (int64_t)nxp * nyp;
-    const int gxs = x < HX ? nx : (x >= nx - HX ? -nx : 0);   // periodic image this thread also writes
+    // per segment (set in the loop at the end of the kernel)
+    int z0 = 0, x = 0, yrow0 = 0, gxs = 0;
+    bool owner = false;
 
     Pr acc[NACC][TY][X];
 #pragma unroll
@@ -301,22 +334,35 @@ lat3_kernel(const __grid_constant__ CUtensorMap tm_st, const __grid_constant__ C
         if (++b == NB) { b = 0; phase ^= 1u; }
     };
 
-    if constexpr (ROT) {
+    // The accumulator of an output plane is ASSIGNED by the first plane that reaches it (|dz| = P), so
+    // what the previous segment left in the registers never enters an output of this one.
 #pragma unroll 1
-        for (int i = 0; i < nplanes; ++i) {
-            do_plane(i, std::integral_constant<int, 0>{});
+    for (long long s = sp.begin; s < sp.end;) {
+        const L3Seg sg = l3_segment(g, sp, s);
+        const int nplanes = sg.len + 2 * P;
+        z0 = sg.z0;
+        x = sg.x0 + q * X;
+        owner = st < g.SY && x < nx;
+        yrow0 = sg.y0 + st * TY;
+        gxs = x < HX ? nx : (x >= nx - HX ? -nx : 0);   // periodic image this thread also writes
+        if constexpr (ROT) {
+#pragma unroll 1
+            for (int i = 0; i < nplanes; ++i) {
+                do_plane(i, std::integral_constant<int, 0>{});
 #pragma unroll
-            for (int k = 0; k + 1 < NACC; ++k)
+                for (int k = 0; k + 1 < NACC; ++k)
 #pragma unroll
-                for (int r = 0; r < TY; ++r)
+                    for (int r = 0; r < TY; ++r)
 #pragma unroll
-                    for (int e = 0; e < X; ++e) acc[k][r][e] = acc[k + 1][r][e];
+                        for (int e = 0; e < X; ++e) acc[k][r][e] = acc[k + 1][r][e];
+            }
+        } else {
+            for (int base = 0; base < nplanes; base += NACC)
+                l2_static_for<0, NACC>([&](auto Jc) {
+                    if (base + decltype(Jc)::value < nplanes) do_plane(base + decltype(Jc)::value, Jc);
+                });
         }
-    } else {
-        for (int base = 0; base < nplanes; base += NACC)
-            l2_static_for<0, NACC>([&](auto Jc) {
-                if (base + decltype(Jc)::value < nplanes) do_plane(base + decltype(Jc)::value, Jc);
-            });
+        s += sg.len;
     }
 }
 

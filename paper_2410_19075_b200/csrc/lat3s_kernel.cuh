@@ -49,14 +49,8 @@ lat3s_kernel(const __grid_constant__ CUtensorMap tm_st, const __grid_constant__ 
     unsigned char* op_ring = st_ring + (size_t)NS * g.st_stride;
 
     const int nx = g.nx, ny = g.ny, nz = g.nz;
-    int bid = blockIdx.x;
-    const int tix = bid % g.tiles_x; bid /= g.tiles_x;
-    const int tiy = bid % g.tiles_y; bid /= g.tiles_y;
-    const int x0 = tix * g.TXt, y0 = tiy * g.TYt;
-    const int z0 = bid * g.Lz;
-    const int z1 = min(nz, z0 + g.Lz);
-    const int nplanes = (z1 - z0) + 2 * P;
     const int tid = threadIdx.x;
+    const L3Span sp = l3_span(g, nz);         // this CTA's share of the (tile, z) space (lat3_kernel.cuh)
 
     if (tid == 0) {
         for (int s = 0; s < NB; ++s) { mbar_init(full + s, 1); mbar_init(done + s, (unsigned)g.ncw); }
@@ -72,22 +66,27 @@ lat3s_kernel(const __grid_constant__ CUtensorMap tm_st, const __grid_constant__ 
             if (NT >= 2) asm volatile("prefetch.tensormap [%0];" ::"l"(&tm_op1) : "memory");
             int b = 0, ss = 0;
             unsigned round = 0;
-            for (int j = 0; j < nplanes; ++j) {
-                if (round > 0) mbar_wait(done + b, (round & 1u) ^ 1u);
-                const bool ops = NT > 0 && j >= 2 * P;
-                mbar_expect_tx(full + b, g.st_bytes + (ops ? NT * g.op_bytes : 0u));
-                int zz = (z0 - P + j) % nz; if (zz < 0) zz += nz;
-                tma_load_4d(st_ring + (size_t)ss * g.st_stride, &tm_st, x0, y0, zz, 0, full + b);
-                if (ops) {
-                    const int zo = z0 - 2 * P + j;
-                    unsigned char* ob = op_ring + (size_t)b * NT * g.op_stride;
-                    if (NT >= 1) tma_load_3d(ob, &tm_op0, x0, y0, zo, full + b);
-                    if (NT >= 2) tma_load_3d(ob + g.op_stride, &tm_op1, x0, y0, zo, full + b);
-                    if (NT >= 3) tma_load_3d(ob + 2 * (size_t)g.op_stride, &tm_op2, x0, y0, zo, full + b);
-                    if (NT >= 4) tma_load_3d(ob + 3 * (size_t)g.op_stride, &tm_op3, x0, y0, zo, full + b);
+            for (long long s = sp.begin; s < sp.end;) {
+                const L3Seg sg = l3_segment(g, sp, s);
+                const int x0 = sg.x0, y0 = sg.y0, z0 = sg.z0, nplanes = sg.len + 2 * P;
+                for (int j = 0; j < nplanes; ++j) {
+                    if (round > 0) mbar_wait(done + b, (round & 1u) ^ 1u);
+                    const bool ops = NT > 0 && j >= 2 * P;
+                    mbar_expect_tx(full + b, g.st_bytes + (ops ? NT * g.op_bytes : 0u));
+                    int zz = (z0 - P + j) % nz; if (zz < 0) zz += nz;
+                    tma_load_4d(st_ring + (size_t)ss * g.st_stride, &tm_st, x0, y0, zz, 0, full + b);
+                    if (ops) {
+                        const int zo = z0 - 2 * P + j;
+                        unsigned char* ob = op_ring + (size_t)b * NT * g.op_stride;
+                        if (NT >= 1) tma_load_3d(ob, &tm_op0, x0, y0, zo, full + b);
+                        if (NT >= 2) tma_load_3d(ob + g.op_stride, &tm_op1, x0, y0, zo, full + b);
+                        if (NT >= 3) tma_load_3d(ob + 2 * (size_t)g.op_stride, &tm_op2, x0, y0, zo, full + b);
+                        if (NT >= 4) tma_load_3d(ob + 3 * (size_t)g.op_stride, &tm_op3, x0, y0, zo, full + b);
+                    }
+                    ss = ss + 1 == NS ? 0 : ss + 1;
+                    if (++b == NB) { b = 0; ++round; }
                 }
-                ss = ss + 1 == NS ? 0 : ss + 1;
-                if (++b == NB) { b = 0; ++round; }
+                s += sg.len;
             }
         }
         return;
@@ -100,14 +99,13 @@ lat3s_kernel(const __grid_constant__ CUtensorMap tm_st, const __grid_constant__ 
     const int f = lane >> 4;                              // 0: cos plane, 1: sin plane
     const int unit = (tid >> 5) * 16 + (lane & 15);
     const int q = unit % g.QX, st = unit / g.QX;
-    const int x = x0 + q * X;
-    const bool owner = st < g.SY && x < nx;
-    const int yrow0 = y0 + st * TY;
     const int nxp = nx + 2 * HX, nyp = ny + 2 * P;
     const int64_t nxy = (int64_t)nx * ny;
     const int64_t pxy = (int64_t)nxp * nyp;
-    const int gxs = x < HX ? nx : (x >= nx - HX ? -nx : 0);   // periodic image this thread also writes
     const int splane = PW * g.PH;                             // scalars between the staged cos and sin boxes
+    // per segment (set in the loop at the end of the kernel)
+    int z0 = 0, x = 0, yrow0 = 0, gxs = 0;
+    bool owner = false;
 
     Pr acc[NACC][TY];
 #pragma unroll
@@ -254,20 +252,33 @@ lat3s_kernel(const __grid_constant__ CUtensorMap tm_st, const __grid_constant__ 
         if (++b == NB) { b = 0; phase ^= 1u; }
     };
 
-    if constexpr (ROT) {
+    // The accumulator of an output plane is ASSIGNED by the first plane that reaches it (|dz| = P), so
+    // what the previous segment left in the registers never enters an output of this one.
 #pragma unroll 1
-        for (int i = 0; i < nplanes; ++i) {
-            do_plane(i, std::integral_constant<int, 0>{});
+    for (long long s = sp.begin; s < sp.end;) {
+        const L3Seg sg = l3_segment(g, sp, s);
+        const int nplanes = sg.len + 2 * P;
+        z0 = sg.z0;
+        x = sg.x0 + q * X;
+        owner = st < g.SY && x < nx;
+        yrow0 = sg.y0 + st * TY;
+        gxs = x < HX ? nx : (x >= nx - HX ? -nx : 0);   // periodic image this thread also writes
+        if constexpr (ROT) {
+#pragma unroll 1
+            for (int i = 0; i < nplanes; ++i) {
+                do_plane(i, std::integral_constant<int, 0>{});
 #pragma unroll
-            for (int k = 0; k + 1 < NACC; ++k)
+                for (int k = 0; k + 1 < NACC; ++k)
 #pragma unroll
-                for (int r = 0; r < TY; ++r) acc[k][r] = acc[k + 1][r];
+                    for (int r = 0; r < TY; ++r) acc[k][r] = acc[k + 1][r];
+            }
+        } else {
+            for (int base = 0; base < nplanes; base += NACC)
+                l2_static_for<0, NACC>([&](auto Jc) {
+                    if (base + decltype(Jc)::value < nplanes) do_plane(base + decltype(Jc)::value, Jc);
+                });
         }
-    } else {
-        for (int base = 0; base < nplanes; base += NACC)
-            l2_static_for<0, NACC>([&](auto Jc) {
-                if (base + decltype(Jc)::value < nplanes) do_plane(base + decltype(Jc)::value, Jc);
-            });
+        s += sg.len;
     }
 }
 

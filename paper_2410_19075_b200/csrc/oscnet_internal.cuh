@@ -221,6 +221,7 @@ struct net {
     int32_t cb_es;         // entries staged in shared memory
     size_t cb_smem;
     int32_t l3_force_tx, l3_force_sy, l3_force_ctas;   // FAST_LATTICE3D_V3: tile chosen by the autotuner (0 = by score)
+    int32_t l3_force_tail;   // FAST_LATTICE3D_V3: -1 = chunk-aligned grid only, no tail of spans (autotuner)
     int32_t ks_planar;     // 1 = KS exchange fields E_a / E_b are two planes (cos | sin), not pairs (fp64 on FAST_LATTICE3D_V3)
     int32_t pairs;         // 1 = state arrays are ghost-padded interleaved pairs (FHN on FAST_LATTICE3D_V2)
     char err[512];
