@@ -102,12 +102,18 @@ template <class T, int MODEL, int P, int STAGE>
 static auto l3_kernel_ptr() {
     typedef L3Sh<T, MODEL, P> S;
     if constexpr (S::SPLIT) {
-        // fp64, P = 4: rotating accumulators (small code, no spills); fp32: compile-time phases
-        // measured faster (cfg 3a 2.26e10 vs 1.97e10)
-        // P = 6: rotating accumulators for both dtypes (13 copies of the plane body otherwise)
-        return lat3s_kernel<T, P, STAGE, S::TY, S::MAXT, S::MINB, (P > 4 || (P > 2 && sizeof(T) == 8))>;
+        // accumulator addressing (ROT of lat3_kernel.cuh), measured on a B200 at P = 4:
+        //   fp32 (cfg 3a, e10 osc-steps/s): ROT 0 (nine plane bodies, 146 KB of SASS) 2.26 | 1: 1.97 | 2: 2.42 |
+        //     3: 2.50 | 4: 2.53 | 5: 2.57 | 6: 2.43 | 7: 2.38 -- five bodies (73 KB) still sit in the instruction
+        //     cache, six do not;
+        //   fp64 (cfg 3b): ROT 1: 1.19 | 2: 1.25 | 3: 1.19 (spills at the 168-register cap of two CTAs per SM).
+        //   P = 6, fp64 (cfg 6c, e9): ROT 1: 3.20 | 2: 3.06 | 3: 2.47 (13 open planes: spills grow with the group).
+        constexpr int ROT0 = P > 4 ? 1 : P == 4 ? (sizeof(T) == 4 ? 5 : 2) : 0;
+        return lat3s_kernel<T, P, STAGE, S::TY, S::MAXT, S::MINB, ROT0>;
     } else {
-        return lat3_kernel<T, MODEL, P, STAGE, S::X, S::TY, L3_MAXT, L3_MINB, (P > 2 && sizeof(T) == 4)>;
+        // FHN, P = 2, fp32 (cfg 5, HBM-bound): ROT 0 (five bodies, 53-65 KB) 5.53e10 | 2: 5.60e10 | 3: 5.31e10 -- noise
+        constexpr int ROTF = (P > 2 && sizeof(T) == 4) ? 1 : 0;
+        return lat3_kernel<T, MODEL, P, STAGE, S::X, S::TY, L3_MAXT, L3_MINB, ROTF>;
     }
 }
 

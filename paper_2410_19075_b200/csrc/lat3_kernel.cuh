@@ -96,11 +96,14 @@ __device__ __forceinline__ L3Seg l3_segment(const L3Geom& g, const L3Span& sp, l
     return L3Seg{(tile % g.tiles_x) * g.TXt, (tile / g.tiles_x) * g.TYt, sp.zbase + dz, len};
 }
 
-// ROT: the accumulators of the open output planes are shifted down one slot after every plane
-// (register moves) instead of being addressed by a compile-time phase J, which needs 2P + 1
-// copies of the plane body: for P = 4 those copies (130 KB of SASS) overflow the instruction
-// cache once the decoupled warps drift apart (profiles/r01_lat3_ncu.md, cfg 3a: no_instruction).
-template <class T, int MODEL, int P, int STAGE, int X, int TY, int MAXT, int MINB, bool ROT>
+// ROT = 0: the accumulators of the open output planes are addressed by a compile-time phase J modulo
+// 2P + 1, which needs 2P + 1 copies of the plane body: for P = 4 those copies (130 KB of SASS) overflow
+// the instruction cache once the decoupled warps drift apart (profiles/r01_lat3_ncu.md, cfg 3a:
+// no_instruction).  ROT = 1: one body, the accumulators shifted down one slot after every plane (2P
+// register moves per accumulator row and plane).  ROT = G > 1: G bodies with phases 0 .. G-1 indexing
+// G - 1 slots past 2P + 1, one shift by G slots after every G planes (the moves of ROT = 1 divided by G).
+template <int ROT, int NACC> __host__ __device__ constexpr int l3_slot(int j) { return ROT > 0 ? j : j % NACC; }
+template <class T, int MODEL, int P, int STAGE, int X, int TY, int MAXT, int MINB, int ROT>
 __global__ void __launch_bounds__(MAXT, MINB)
 lat3_kernel(const __grid_constant__ CUtensorMap tm_st, const __grid_constant__ CUtensorMap tm_op0,
             const __grid_constant__ CUtensorMap tm_op1, const __grid_constant__ CUtensorMap tm_op2,
@@ -111,6 +114,7 @@ lat3_kernel(const __grid_constant__ CUtensorMap tm_st, const __grid_constant__ C
     constexpr int NCOL = X + 2 * HX;          // pairs a thread reads per staged row
     constexpr int OFF = HX - P;
     constexpr int NACC = 2 * P + 1;
+    constexpr int NSLOT = NACC + (ROT > 1 ? ROT - 1 : 0);   // accumulator slots (ROT > 1: the group's phases index past NACC)
     constexpr int NT = L3Ops<MODEL, STAGE>::N;
     constexpr int U8 = (int)sizeof(Pr) / 8;   // 8-byte TMA elements per pair
     constexpr int EW = 2 * X;                 // scalars per thread-row of an operand / output tile
@@ -178,9 +182,9 @@ lat3_kernel(const __grid_constant__ CUtensorMap tm_st, const __grid_constant__ C
     int z0 = 0, x = 0, yrow0 = 0, gxs = 0;
     bool owner = false;
 
-    Pr acc[NACC][TY][X];
+    Pr acc[NSLOT][TY][X];
 #pragma unroll
-    for (int k = 0; k < NACC; ++k)
+    for (int k = 0; k < NSLOT; ++k)
 #pragma unroll
         for (int r = 0; r < TY; ++r)
 #pragma unroll
@@ -233,7 +237,7 @@ lat3_kernel(const __grid_constant__ CUtensorMap tm_st, const __grid_constant__ C
                     {   // |dz| = 0: straight into the accumulator of output plane i
                         const int w = l2_run_w(P, 0, ady);
 #pragma unroll
-                        for (int e = 0; e < X; ++e) acc[(J + P) % NACC][r][e] = padd(acc[(J + P) % NACC][r][e], R[w][e]);
+                        for (int e = 0; e < X; ++e) acc[l3_slot<ROT, NACC>(J + P)][r][e] = padd(acc[l3_slot<ROT, NACC>(J + P)][r][e], R[w][e]);
                     }
 #pragma unroll
                     for (int k = 1; k < P; ++k) {    // 0 < |dz| < P: in-plane partial sums
@@ -248,8 +252,8 @@ lat3_kernel(const __grid_constant__ CUtensorMap tm_st, const __grid_constant__ C
                     if (ady == 0) {                  // |dz| = P: the centre alone (first / last contribution)
 #pragma unroll
                         for (int e = 0; e < X; ++e) {
-                            acc[(J + 2 * P) % NACC][r][e] = R[0][e];
-                            acc[J % NACC][r][e] = padd(acc[J % NACC][r][e], R[0][e]);
+                            acc[l3_slot<ROT, NACC>(J + 2 * P)][r][e] = R[0][e];
+                            acc[l3_slot<ROT, NACC>(J)][r][e] = padd(acc[l3_slot<ROT, NACC>(J)][r][e], R[0][e]);
                         }
                     }
                 }
@@ -260,8 +264,8 @@ lat3_kernel(const __grid_constant__ CUtensorMap tm_st, const __grid_constant__ C
                 for (int r = 0; r < TY; ++r)
 #pragma unroll
                     for (int e = 0; e < X; ++e) {
-                        acc[(J + P - k) % NACC][r][e] = padd(acc[(J + P - k) % NACC][r][e], A[k - 1][r][e]);
-                        acc[(J + P + k) % NACC][r][e] = padd(acc[(J + P + k) % NACC][r][e], A[k - 1][r][e]);
+                        acc[l3_slot<ROT, NACC>(J + P - k)][r][e] = padd(acc[l3_slot<ROT, NACC>(J + P - k)][r][e], A[k - 1][r][e]);
+                        acc[l3_slot<ROT, NACC>(J + P + k)][r][e] = padd(acc[l3_slot<ROT, NACC>(J + P + k)][r][e], A[k - 1][r][e]);
                     }
         }
         // ---- finish output plane zo (accumulator J)
@@ -278,7 +282,7 @@ lat3_kernel(const __grid_constant__ CUtensorMap tm_st, const __grid_constant__ C
                     T lo[X];
 #pragma unroll
                     for (int e = 0; e < X; ++e) {
-                        const Pr W = acc[J % NACC][r][e];
+                        const Pr W = acc[l3_slot<ROT, NACC>(J)][r][e];
                         lo[e] = sqrt(W.x * W.x + W.y * W.y) * mp.inv_nb;
                     }
                     stg_vec<X>((T*)a.out + ((int64_t)zo * ny + yy) * nx + x, lo);
@@ -303,7 +307,7 @@ lat3_kernel(const __grid_constant__ CUtensorMap tm_st, const __grid_constant__ C
 #pragma unroll
                 for (int e = 0; e < X; ++e) {
                     const Pr c = cb[r * PW + e];
-                    const Pr W = acc[J % NACC][r][e];
+                    const Pr W = acc[l3_slot<ROT, NACC>(J)][r][e];
                     // sum_j (u_j - u_i) over the ball = W - n_ball c whether or not the centre counts
                     const Pr Cc = pfma(c, Pr{-mp.nb, -mp.nb}, W);
                     const T u = c.x, v = c.y;
@@ -345,22 +349,20 @@ lat3_kernel(const __grid_constant__ CUtensorMap tm_st, const __grid_constant__ C
         owner = st < g.SY && x < nx;
         yrow0 = sg.y0 + st * TY;
         gxs = x < HX ? nx : (x >= nx - HX ? -nx : 0);   // periodic image this thread also writes
-        if constexpr (ROT) {
+        constexpr int GSZ = ROT > 0 ? ROT : NACC;       // plane bodies in the loop
 #pragma unroll 1
-            for (int i = 0; i < nplanes; ++i) {
-                do_plane(i, std::integral_constant<int, 0>{});
+        for (int base = 0; base < nplanes; base += GSZ) {
+            l2_static_for<0, GSZ>([&](auto Jc) {
+                if (base + decltype(Jc)::value < nplanes) do_plane(base + decltype(Jc)::value, Jc);
+            });
+            if constexpr (ROT > 0) {
 #pragma unroll
                 for (int k = 0; k + 1 < NACC; ++k)
 #pragma unroll
                     for (int r = 0; r < TY; ++r)
 #pragma unroll
-                        for (int e = 0; e < X; ++e) acc[k][r][e] = acc[k + 1][r][e];
+                        for (int e = 0; e < X; ++e) acc[k][r][e] = acc[k + ROT][r][e];
             }
-        } else {
-            for (int base = 0; base < nplanes; base += NACC)
-                l2_static_for<0, NACC>([&](auto Jc) {
-                    if (base + decltype(Jc)::value < nplanes) do_plane(base + decltype(Jc)::value, Jc);
-                });
         }
         s += sg.len;
     }

@@ -24,7 +24,7 @@
 
 namespace oscnet {
 
-template <class T, int P, int STAGE, int TY, int MAXT, int MINB, bool ROT>
+template <class T, int P, int STAGE, int TY, int MAXT, int MINB, int ROT>
 __global__ void __launch_bounds__(MAXT, MINB)
 lat3s_kernel(const __grid_constant__ CUtensorMap tm_st, const __grid_constant__ CUtensorMap tm_op0,
              const __grid_constant__ CUtensorMap tm_op1, const __grid_constant__ CUtensorMap tm_op2,
@@ -38,6 +38,7 @@ lat3s_kernel(const __grid_constant__ CUtensorMap tm_st, const __grid_constant__ 
     constexpr int OFF = HX - P;
     constexpr int NCOL = X + 2 * P;           // scalars a thread reads per staged row
     constexpr int NACC = 2 * P + 1;
+    constexpr int NSLOT = NACC + (ROT > 1 ? ROT - 1 : 0);   // accumulator slots (ROT > 1: the group's phases index past NACC)
     constexpr int NT = L3Ops<MODEL, STAGE>::N;
     static_assert(OFF % 2 == 0 && NCOL % 2 == 0, "aligned column pairs");
 
@@ -107,9 +108,9 @@ lat3s_kernel(const __grid_constant__ CUtensorMap tm_st, const __grid_constant__ 
     int z0 = 0, x = 0, yrow0 = 0, gxs = 0;
     bool owner = false;
 
-    Pr acc[NACC][TY];
+    Pr acc[NSLOT][TY];
 #pragma unroll
-    for (int k = 0; k < NACC; ++k)
+    for (int k = 0; k < NSLOT; ++k)
 #pragma unroll
         for (int r = 0; r < TY; ++r) acc[k][r] = Pr{T(0), T(0)};
 
@@ -156,7 +157,7 @@ lat3s_kernel(const __grid_constant__ CUtensorMap tm_st, const __grid_constant__ 
                     if (ady > P) continue;
                     {   // |dz| = 0: straight into the accumulator of output plane i
                         const int w = l2_run_w(P, 0, ady);
-                        acc[(J + P) % NACC][r] = padd(acc[(J + P) % NACC][r], R[w]);
+                        acc[l3_slot<ROT, NACC>(J + P)][r] = padd(acc[l3_slot<ROT, NACC>(J + P)][r], R[w]);
                     }
 #pragma unroll
                     for (int k = 1; k < P; ++k) {    // 0 < |dz| < P: in-plane partial sums
@@ -167,8 +168,8 @@ lat3s_kernel(const __grid_constant__ CUtensorMap tm_st, const __grid_constant__ 
                         }
                     }
                     if (ady == 0) {                  // |dz| = P: the centre alone (first / last contribution)
-                        acc[(J + 2 * P) % NACC][r] = R[0];
-                        acc[J % NACC][r] = padd(acc[J % NACC][r], R[0]);
+                        acc[l3_slot<ROT, NACC>(J + 2 * P)][r] = R[0];
+                        acc[l3_slot<ROT, NACC>(J)][r] = padd(acc[l3_slot<ROT, NACC>(J)][r], R[0]);
                     }
                 }
             }
@@ -176,17 +177,17 @@ lat3s_kernel(const __grid_constant__ CUtensorMap tm_st, const __grid_constant__ 
             for (int k = 1; k < P; ++k)
 #pragma unroll
                 for (int r = 0; r < TY; ++r) {
-                    acc[(J + P - k) % NACC][r] = padd(acc[(J + P - k) % NACC][r], A[k - 1][r]);
-                    acc[(J + P + k) % NACC][r] = padd(acc[(J + P + k) % NACC][r], A[k - 1][r]);
+                    acc[l3_slot<ROT, NACC>(J + P - k)][r] = padd(acc[l3_slot<ROT, NACC>(J + P - k)][r], A[k - 1][r]);
+                    acc[l3_slot<ROT, NACC>(J + P + k)][r] = padd(acc[l3_slot<ROT, NACC>(J + P + k)][r], A[k - 1][r]);
                 }
         }
         // ---- finish output plane zo (accumulator J): lane f takes the output rows 2m + f of the block
         if (zo >= z0) {                                   // uniform over the CTA
 #pragma unroll
           for (int m = 0; m < TY / 2; ++m) {              // rows 2m, 2m + 1: lane f finishes row 2m + f
-            const Pr send = f ? acc[J % NACC][2 * m] : acc[J % NACC][2 * m + 1];    // the row the partner finishes
+            const Pr send = f ? acc[l3_slot<ROT, NACC>(J)][2 * m] : acc[l3_slot<ROT, NACC>(J)][2 * m + 1];    // the row the partner finishes
             const T other[X] = {__shfl_xor_sync(0xffffffffu, send.x, 16), __shfl_xor_sync(0xffffffffu, send.y, 16)};
-            const Pr ownp = f ? acc[J % NACC][2 * m + 1] : acc[J % NACC][2 * m];
+            const Pr ownp = f ? acc[l3_slot<ROT, NACC>(J)][2 * m + 1] : acc[l3_slot<ROT, NACC>(J)][2 * m];
             const T ownv[X] = {ownp.x, ownp.y};
             const int r = 2 * m + f;
             const int yy = yrow0 + r;
@@ -263,20 +264,18 @@ lat3s_kernel(const __grid_constant__ CUtensorMap tm_st, const __grid_constant__ 
         owner = st < g.SY && x < nx;
         yrow0 = sg.y0 + st * TY;
         gxs = x < HX ? nx : (x >= nx - HX ? -nx : 0);   // periodic image this thread also writes
-        if constexpr (ROT) {
+        constexpr int GSZ = ROT > 0 ? ROT : NACC;       // plane bodies in the loop
 #pragma unroll 1
-            for (int i = 0; i < nplanes; ++i) {
-                do_plane(i, std::integral_constant<int, 0>{});
+        for (int base = 0; base < nplanes; base += GSZ) {
+            l2_static_for<0, GSZ>([&](auto Jc) {
+                if (base + decltype(Jc)::value < nplanes) do_plane(base + decltype(Jc)::value, Jc);
+            });
+            if constexpr (ROT > 0) {
 #pragma unroll
                 for (int k = 0; k + 1 < NACC; ++k)
 #pragma unroll
-                    for (int r = 0; r < TY; ++r) acc[k][r] = acc[k + 1][r];
+                    for (int r = 0; r < TY; ++r) acc[k][r] = acc[k + ROT][r];
             }
-        } else {
-            for (int base = 0; base < nplanes; base += NACC)
-                l2_static_for<0, NACC>([&](auto Jc) {
-                    if (base + decltype(Jc)::value < nplanes) do_plane(base + decltype(Jc)::value, Jc);
-                });
         }
         s += sg.len;
     }
