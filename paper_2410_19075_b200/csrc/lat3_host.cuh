@@ -234,12 +234,13 @@ static int32_t l3_configure_stage(net* h) {
     if (occ < 1) return NET_ERR_UNSUPPORTED;
     // Grid (l3_span in lat3_kernel.cuh): chunk-aligned CTAs, tiles x chunks of them, marching in step;
     // where they leave part of a single wave empty, shorter chunks plus a tail of equal spans over the
-    // planes left at the top of the columns.  Cost = waves x planes of the longest CTA, every segment
-    // paying its 2P lead-in planes (+ 4 for the pipeline restart).  l3_force_tail < 0: aligned only.
+    // planes left at the top of the columns.  Cost = waves x planes of the longest CTA, a chunk paying
+    // its 2P lead-in planes (+ 4 for the pipeline restart).  l3_force_tail < 0: aligned only.
     const int64_t slots = (int64_t)occ * sms, tiles = (int64_t)g.tiles_x * g.tiles_y;
     const int64_t SP = tiles * g.nz;                                         // tile-planes of one stage
     const int HZ = 2 * P + 4;
-    int64_t best_cost = -1, grid = tiles;
+    double best_cost = -1.0;
+    int64_t grid = tiles;
     g.Lz = g.nz; g.nchunks = 1;
     const bool allow_tail = h->l3_force_tail >= 0 && want_lz == 0 && !getenv("OSCNET_LAT3_NO_TAIL");
     for (int nch = 1; nch <= g.nz; ++nch) {
@@ -247,16 +248,20 @@ static int32_t l3_configure_stage(net* h) {
         const int chunks = (g.nz + Lz - 1) / Lz;
         const int64_t m = tiles * chunks;
         const int64_t waves = (m + slots - 1) / slots;
-        const int64_t cost = waves * (Lz + HZ);
+        const double cost = (double)(waves * (Lz + HZ));
         if (best_cost < 0 || cost < best_cost) { best_cost = cost; g.Lz = Lz; g.nchunks = chunks; grid = m; }
         if (!allow_tail || m >= slots) continue;
         const int64_t gt = slots - m;                                        // CTAs of the tail
-        for (int a = Lz - 1; a >= 1 && 2 * a >= Lz; --a) {
+        // lead-in planes only accumulate (no finisher): about 3/4 of a plane each; a span of Lt planes
+        // in columns of r planes starts 1 + Lt / r segments on average (fit to A sweeps on cfg 3a / 3b:
+        // optimum at 87-91 of 100 planes)
+        const double lead = 0.75 * (2 * P);
+        for (int a = Lz - 1; a >= 8 * P && 2 * a >= Lz; --a) {    // short chunks: the tail's lead-ins cost more than they fill (cfg 6b: 6.8e9 aligned, 6.2e9 with a tail)
             const int64_t r = g.nz - (int64_t)chunks * a;
             if (r <= 0) continue;
-            const int64_t Lt = (tiles * r + gt - 1) / gt;
-            const int64_t segs = 1 + (Lt + r - 2) / r;
-            const int64_t tail = Lt + segs * HZ, c2 = a + HZ > tail ? a + HZ : tail;
+            const double Lt = (double)(tiles * r) / (double)gt;
+            const double tail = Lt + (1.0 + Lt / (double)r) * lead + (HZ - lead), main = a + HZ;   // same scale as `cost`
+            const double c2 = main > tail ? main : tail;
             if (c2 < best_cost) { best_cost = c2; g.Lz = a; g.nchunks = chunks; grid = slots; }
         }
     }
