@@ -406,6 +406,16 @@ static int32_t l3_configure(net* h) {
     int32_t rc = l3_configure_tile<T, MODEL, P>(h);
     if (rc) return rc;
     if (getenv("OSCNET_LAT3") || getenv("OSCNET_NO_AUTOTUNE") || h->n < (1 << 21)) return NET_OK;
+    // OSCNET_LAT3_PICK = "TXt,SY,CTAS,TAIL": the autotuner's pick of an earlier run (it prints the line
+    // under OSCNET_VERBOSE), so that a profiler pass -- whose replays disturb the timing pass -- captures
+    // the geometry the plain run used
+    if (const char* e = getenv("OSCNET_LAT3_PICK")) {
+        int tx = 0, sy = 0, ctas = 0, tail = 0;
+        if (sscanf(e, "%d,%d,%d,%d", &tx, &sy, &ctas, &tail) == 4 && tx > 0 && sy > 0) {
+            h->l3_force_tx = tx; h->l3_force_sy = sy; h->l3_force_ctas = ctas; h->l3_force_tail = tail;
+            return l3_configure_tile<T, MODEL, P>(h);
+        }
+    }
     struct Cand { int tx, sy; double score; int ctas, tail; };
     constexpr int KMAX = 10;
     Cand cand[KMAX];
@@ -486,6 +496,8 @@ static int32_t l3_configure(net* h) {
     if (cudaGetLastError() != cudaSuccess) best = -1;
     if (best >= 0) { h->l3_force_tx = best_c.tx; h->l3_force_sy = best_c.sy; h->l3_force_ctas = best_c.ctas; h->l3_force_tail = best_c.tail; }
     else h->l3_force_tx = h->l3_force_sy = h->l3_force_ctas = h->l3_force_tail = 0;
+    if (getenv("OSCNET_VERBOSE"))
+        fprintf(stderr, "lat3 autotune pick: OSCNET_LAT3_PICK=%d,%d,%d,%d\n", h->l3_force_tx, h->l3_force_sy, h->l3_force_ctas, h->l3_force_tail);
     return l3_configure_tile<T, MODEL, P>(h);
 }
 
