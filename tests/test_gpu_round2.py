@@ -127,12 +127,14 @@ def _with_env(name, value, fn):
             os.environ[name] = old
 
 
-@pytest.mark.parametrize("cfg,tiles", [("5", ["32,4,16,2,2", "64,2,64,1,3"]),
-                                       ("3a", ["32,4,16,2,2", "64,2,64,1,2"]),
-                                       ("3b", ["32,4,16,2,2", "64,2,64,1,1"])])
+@pytest.mark.parametrize("cfg,tiles", [("5", ["32,4,16,2,2", "64,2,64,1,3", "32,4,32,2,2,27", "32,4,-37,2,2"]),
+                                       ("3a", ["32,4,16,2,2", "64,2,64,1,2", "32,4,32,2,2,25", "16,8,-53,2,2"]),
+                                       ("3b", ["32,4,16,2,2", "64,2,64,1,1", "32,4,32,2,2,20", "64,2,-9,1,1"])])
 def test_lattice_tiles_give_identical_bits(cfg, tiles):
-    """OSCNET_LAT3 = TXt,SY,Lz,D,CTAS forces the tile / z chunk / pipeline depth of the lat3 kernels.
-    Every output's arithmetic is the same for every tile, so the states must agree bit for bit."""
+    """OSCNET_LAT3 = TXt,SY,Lz,D,CTAS[,A] forces the tile / z chunk / pipeline depth of the lat3 kernels
+    (with A: chunks shortened to A planes and a tail of equal spans over the rest, CTAs that run several
+    segments; Lz < 0: -Lz CTAs with equal spans of the whole (tile, z) space, cut anywhere).
+    Every output's arithmetic is the same for every tile and grid, so the states must agree bit for bit."""
     w = configs.get(cfg, n1=64)
     inp = H.make_inputs(w, seed=9)
     states = []
