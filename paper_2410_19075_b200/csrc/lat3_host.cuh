@@ -44,6 +44,16 @@ template <class T> inline int l3s_pad(int TXt, int HX, int TY) {
         if (((TY * (TXt + 2 * HX + pad) - TXt) * (int)sizeof(T)) % 128 == 0) return pad;
     return -1;
 }
+// The same for the pair kernel (elements are (u, v) pairs of 2 sizeof(T) bytes; a thread reads X = 2 of them
+// per 16 or 32 bytes): cfg 5, tile 78 x 16, had 32 % of its shared-memory wavefronts in such conflicts with the
+// shared-memory data pipe the busiest unit of the SM (71 %; profiles/r02_ncu.md).
+template <class T> inline int l3p_pad(int TXt, int HX, int TY) {
+    const int eb = 2 * (int)sizeof(T);
+    const int q = eb >= 16 ? 1 : 16 / eb;
+    for (int pad = 0; pad * eb < 128; pad += q)
+        if (((TY * (TXt + 2 * HX + pad) - TXt) * eb) % 128 == 0) return pad;
+    return -1;
+}
 
 typedef CUresult (*l3_encode_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
@@ -156,8 +166,10 @@ static int32_t l3_enumerate(int nx, int ny, int want_tx, int want_sy, F&& f) {
             constexpr bool PLANAR = S::SPLIT;
             const int row_bytes = (TXt + 2 * HX) * (PLANAR ? (int)sizeof(T) : 2 * (int)sizeof(T));
             const bool straddle = QX % 8 != 0 && SY > 1;
+            const bool ppad = !getenv("OSCNET_L3P_NOPAD");
             const double bank_pen = PLANAR ? (QX % (sizeof(T) == 8 ? 8 : 16) != 0 && l3s_pad<T>(TXt, HX, TY) < 0 ? 0.85 : 1.0)
-                                           : ((straddle && (TY * row_bytes) % 128 == 0) ? 0.85 : 1.0);
+                                  : ppad ? (straddle && QX % (sizeof(T) == 8 ? 4 : 8) != 0 && l3p_pad<T>(TXt, HX, TY) < 0 ? 0.85 : 1.0)
+                                         : ((straddle && (TY * row_bytes) % 128 == 0) ? 0.85 : 1.0);
             f(TXt, SY, lane_eff * cover * size_pen * bank_pen / (1.0 + 0.25 * (halo - 1.0)));
         }
         if (want_tx > 0) break;
@@ -201,6 +213,10 @@ static int32_t l3_configure_stage(net* h) {
     g.PW = g.TXt + 2 * HX;
     if (S::SPLIT && g.QX % (sizeof(T) == 8 ? 8 : 16) != 0 && !getenv("OSCNET_L3S_NOPAD")) {
         const int pad = l3s_pad<T>(g.TXt, HX, TY);
+        if (pad > 0 && (g.PW + pad) * U8 <= 256) g.PW += pad;
+    }
+    if (!S::SPLIT && g.SY > 1 && g.QX % (sizeof(T) == 8 ? 4 : 8) != 0 && !getenv("OSCNET_L3P_NOPAD")) {
+        const int pad = l3p_pad<T>(g.TXt, HX, TY);
         if (pad > 0 && (g.PW + pad) * U8 <= 256) g.PW += pad;
     }
     g.PH = g.TYt + 2 * P;
