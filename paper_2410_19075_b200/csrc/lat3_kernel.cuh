@@ -304,9 +304,20 @@ lat3_kernel(const __grid_constant__ CUtensorMap tm_st, const __grid_constant__ C
                 if (NT >= 2) ldg_vec<EW>(ob + ostride + r * orow, o1);
                 T ov[EW];
                 [[maybe_unused]] T zv[EW];
+                // centre pairs of the row: one 16-byte load for the two f32 pairs of a thread (two 8-byte
+                // loads at a 16-byte lane stride take twice the wavefronts)
+                Pr cpair[X];
+                if constexpr (sizeof(T) == 4 && X == 2) {
+                    const float4 c4 = *reinterpret_cast<const float4*>(cb + r * PW);
+                    cpair[0] = Pr{c4.x, c4.y};
+                    cpair[1] = Pr{c4.z, c4.w};
+                } else {
+#pragma unroll
+                    for (int e = 0; e < X; ++e) cpair[e] = cb[r * PW + e];
+                }
 #pragma unroll
                 for (int e = 0; e < X; ++e) {
-                    const Pr c = cb[r * PW + e];
+                    const Pr c = cpair[e];
                     const Pr W = acc[l3_slot<ROT, NACC>(J)][r][e];
                     // sum_j (u_j - u_i) over the ball = W - n_ball c whether or not the centre counts
                     const Pr Cc = pfma(c, Pr{-mp.nb, -mp.nb}, W);
