@@ -239,7 +239,7 @@ int32_t net_workspace_bytes(const net_desc* desc, size_t* bytes);
  * net_*_params struct of desc->model (params_bytes = its sizeof).  d_workspace: device memory,
  * 256-byte aligned, >= net_workspace_bytes; owned by the caller and must outlive the handle.
  * cuda_stream: a cudaStream_t (NULL = legacy default stream).  On failure *out is NULL.
- * Cost: 3D lattice nets of >= 2^21 elements on the tiled kernels time the ten best-scoring tiles at
+ * Cost: 3D lattice nets of >= 2^19 elements on the tiled kernels time the ten best-scoring tiles at
  * three pipeline depths on one RK4 step each (about 500 launches on zeroed buffers, 0.1 - 1 s) and keep
  * the fastest; the arithmetic of every output is the same for every tile, so results do not depend on
  * the pick (tests/test_gpu_round2.py::test_lattice_tiles_give_identical_bits).  The pick is reported
@@ -346,7 +346,7 @@ int32_t net_get_counters(net_t* net, int64_t* kernel_launches, int32_t* method_i
 int32_t net_get_kernel_family(net_t* net, int32_t* family);
 
 /* Launch geometry of the stage kernel in use (diagnostic; the lattice tile is picked by a timing
- * pass inside net_create for nets of >= 2^21 elements, so a bench line should print it).  out8 =
+ * pass inside net_create for nets of >= 2^19 elements, so a bench line should print it).  out8 =
  * {kernel family, tile x, tile y, z planes per chunk, prefetch depth, grid, threads, dynamic shared
  * memory in bytes} of RK4 stage 1; entries a family does not have are 0. */
 int32_t net_get_launch_config(net_t* net, int32_t* out8);

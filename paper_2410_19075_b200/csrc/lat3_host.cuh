@@ -421,7 +421,7 @@ static int32_t l3_configure(net* h) {
     h->l3_force_tx = h->l3_force_sy = h->l3_force_ctas = h->l3_force_tail = 0;
     int32_t rc = l3_configure_tile<T, MODEL, P>(h);
     if (rc) return rc;
-    if (getenv("OSCNET_LAT3") || getenv("OSCNET_NO_AUTOTUNE") || h->n < (1 << 21)) return NET_OK;
+    if (getenv("OSCNET_LAT3") || getenv("OSCNET_NO_AUTOTUNE") || h->n < (1 << 19)) return NET_OK;
     // OSCNET_LAT3_PICK = "TXt,SY,CTAS,TAIL": the autotuner's pick of an earlier run (it prints the line
     // under OSCNET_VERBOSE), so that a profiler pass -- whose replays disturb the timing pass -- captures
     // the geometry the plain run used
