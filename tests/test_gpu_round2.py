@@ -151,6 +151,27 @@ def test_lattice_tiles_give_identical_bits(cfg, tiles):
         assert np.array_equal(states[0], y)
 
 
+@pytest.mark.parametrize("cfg", ["3a", "3b", "5"])
+def test_tail_grid_on_ragged_tiles(cfg):
+    """Tiles that do not divide the lattice (40 = 32 + 8 in x, 40 = 5 x 8 or 2.5 x 16 in y) under a tail grid
+    and under free spans: segments start in ragged tiles too.  Same bits as the default geometry, and the
+    default agrees with the oracle."""
+    w = configs.get(cfg, n1=40)
+    inp = H.make_inputs(w, seed=12)
+
+    def run():
+        net = H.make_gpu(w, inp)
+        assert net.kernel_family() == 6
+        net.integrate(7, w.dt)
+        y = net.get_state()
+        net.close()
+        return y
+    base = run()
+    assert H.traj_err(w, base, H.make_oracle(w, inp).rk4(inp["y0"], 7, w.dt)) <= H.TOL_TRAJ[w.dtype]
+    for spec in ("32,4,20,2,2,13", "32,4,-41,2,2"):
+        assert np.array_equal(base, _with_env("OSCNET_LAT3", spec, run)), spec
+
+
 # ------------------------------------------------------------------ radius 6 (the paper's largest, PAPER.md:339)
 @pytest.mark.parametrize("cfg,extent", [("3b", (16, 16, 16)), ("3a", (20, 16, 14)), ("3b", (26, 14, 18))])
 def test_ks_lattice_radius_6_on_the_field_split_kernel(cfg, extent):
